@@ -1,0 +1,200 @@
+// api.cu -- context, validation, scratch sizing, the host-buffer frame entry and the FFMA
+// micro-benchmark of libfhgs.so (declared in include/fhgs.h).
+#include <math.h>
+#include <new>
+
+#include "common.cuh"
+#include "layout.cuh"
+
+extern "C" const char* fhgs_version(void) { return "fhgs-b200 0.1 sm_100a"; }
+
+extern "C" fhgs_status fhgs_create(fhgs_ctx** out, int device) {
+    if (!out) return FHGS_ERR_INVALID;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return FHGS_ERR_INTERNAL;
+    fhgs_ctx* c = new (std::nothrow) fhgs_ctx();
+    if (!c) return FHGS_ERR_INTERNAL;
+    c->device = device;
+    c->err[0] = 0;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { delete c; return FHGS_ERR_INTERNAL; }
+    c->num_sms = prop.multiProcessorCount;
+    c->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
+    if (prop.major < 10) {   // sm_100a only: there is no fallback path
+        delete c;
+        return FHGS_ERR_INTERNAL;
+    }
+    if (cudaSetDevice(device) != cudaSuccess) { delete c; return FHGS_ERR_INTERNAL; }
+    *out = c;
+    return FHGS_OK;
+}
+
+extern "C" void fhgs_destroy(fhgs_ctx* ctx) { delete ctx; }
+
+extern "C" const char* fhgs_last_error(const fhgs_ctx* ctx) { return ctx ? ctx->err : "NULL context"; }
+
+extern "C" void fhgs_default_params(fhgs_params* p) {
+    if (!p) return;
+    p->z_near = 0.2f;
+    p->cov_dilation = 0.3f;
+    p->jac_clamp = 1.3f;
+    p->q_cutoff = 9.0f;
+    p->alpha_max = 0.9999f;
+    p->t_min = 1e-4f;
+    p->den_eps = 1e-8f;
+    p->bg[0] = p->bg[1] = p->bg[2] = 0.0f;
+}
+
+extern "C" size_t fhgs_scratch_bytes(int32_t n, int32_t width, int32_t height, uint64_t capacity) {
+    if (n < 0 || width <= 0 || height <= 0) return 0;
+    return make_scratch_layout(n, capacity).total;
+}
+
+fhgs_status validate_camera(fhgs_ctx* ctx, const fhgs_camera* cam) {
+    if (cam->width <= 0 || cam->height <= 0) FHGS_INVALID(ctx, "camera: width/height must be > 0");
+    const long long tiles = (long long)tiles_x(cam->width) * tiles_y(cam->height);
+    if (tiles >= (1LL << 31)) FHGS_INVALID(ctx, "camera: too many tiles for the 32-bit tile id");
+    for (int i = 0; i < 16; ++i)
+        if (!finite_f(cam->view[i]) || !finite_f(cam->proj[i])) FHGS_INVALID(ctx, "camera: non-finite matrix entry");
+    for (int i = 0; i < 3; ++i)
+        if (!finite_f(cam->cam_pos[i])) FHGS_INVALID(ctx, "camera: non-finite cam_pos");
+    if (!(cam->proj[0] != 0.0f) || !(cam->proj[5] != 0.0f)) FHGS_INVALID(ctx, "camera: proj[0]/proj[5] must be non-zero");
+    return FHGS_OK;
+}
+
+fhgs_status validate_params(fhgs_ctx* ctx, const fhgs_params* p) {
+    const float v[10] = {p->z_near, p->cov_dilation, p->jac_clamp, p->q_cutoff, p->alpha_max,
+                         p->t_min, p->den_eps, p->bg[0], p->bg[1], p->bg[2]};
+    for (int i = 0; i < 10; ++i)
+        if (!finite_f(v[i])) FHGS_INVALID(ctx, "params: non-finite value");
+    if (!(p->z_near > 0.0f)) FHGS_INVALID(ctx, "params: z_near must be > 0 (depth bits must order like depth)");
+    if (!(p->q_cutoff >= 0.0f) || !(p->alpha_max > 0.0f && p->alpha_max <= 1.0f) || !(p->t_min >= 0.0f))
+        FHGS_INVALID(ctx, "params: q_cutoff >= 0, 0 < alpha_max <= 1, t_min >= 0 required");
+    return FHGS_OK;
+}
+
+fhgs_status validate_view_state(fhgs_ctx* ctx, const fhgs_view_state* vs, const fhgs_camera* cam) {
+    if (vs->n < 0) FHGS_INVALID(ctx, "view_state: n < 0");
+    if (cam && (vs->width != cam->width || vs->height != cam->height))
+        FHGS_INVALID(ctx, "view_state: width/height differ from the camera's");
+    if (vs->capacity >= (1ull << 30)) FHGS_INVALID(ctx, "view_state: capacity must be < 2^30");
+    if (!vs->xy || !vs->depth || !vs->conic_opacity || !vs->rgb || !vs->radius || !vs->rect ||
+        !vs->tiles_touched || !vs->offsets || !vs->num_instances || !vs->ranges || !vs->scratch)
+        FHGS_INVALID(ctx, "view_state: NULL buffer");
+    if (vs->capacity > 0 && (!vs->keys[0] || !vs->keys[1] || !vs->vals[0] || !vs->vals[1]))
+        FHGS_INVALID(ctx, "view_state: NULL key/value buffer");
+    if (!aligned_to(vs->conic_opacity, 16) || !aligned_to(vs->xy, 8) || !aligned_to(vs->rect, 8) ||
+        !aligned_to(vs->keys[0], 8) || !aligned_to(vs->keys[1], 8) || !aligned_to(vs->ranges, 8) ||
+        !aligned_to(vs->scratch, 256) || !aligned_to(vs->num_instances, 8))
+        FHGS_INVALID(ctx, "view_state: misaligned buffer");
+    if (vs->scratch_bytes < fhgs_scratch_bytes(vs->n, vs->width, vs->height, vs->capacity))
+        FHGS_INVALID(ctx, "view_state: scratch too small (see fhgs_scratch_bytes)");
+    return FHGS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Host-buffer frame: copies in, P -> S -> R -> F, copies out.  No arithmetic here.
+// ------------------------------------------------------------------------------------------------
+extern "C" fhgs_status fhgs_frame_host(fhgs_ctx* ctx, const fhgs_host_frame* host, const fhgs_gaussians* g,
+                                       const fhgs_camera* cam, const fhgs_params* prm, fhgs_view_state* vs,
+                                       const fhgs_frame_workspace* ws, uint64_t* num_instances_host,
+                                       void* stream) {
+    if (!ctx) return FHGS_ERR_INVALID;
+    if (!host || !g || !cam || !prm || !vs || !ws) FHGS_INVALID(ctx, "fhgs_frame_host: NULL argument");
+    if (g->n < 0 || g->sh_degree < 0 || g->sh_degree > 3 || !g->feat || g->feat_dim <= 0)
+        FHGS_INVALID(ctx, "fhgs_frame_host: bad Gaussian description");
+    if (!host->mean || !host->scale || !host->quat || !host->opacity || !host->sh || !host->feat || !host->gt)
+        FHGS_INVALID(ctx, "fhgs_frame_host: NULL host input");
+    if (!ws->out_rgb || !ws->out_feat || !ws->gt || !ws->num || !ws->den || !ws->fused_feat)
+        FHGS_INVALID(ctx, "fhgs_frame_host: NULL workspace buffer");
+    fhgs_status st;
+    if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t n = (size_t)g->n, K = (size_t)(g->sh_degree + 1) * (g->sh_degree + 1);
+    const size_t e = g->feat_dtype == FHGS_F16 ? 2 : 4, D = (size_t)g->feat_dim;
+    const size_t px = (size_t)cam->width * cam->height;
+    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->mean, host->mean, n * 12, cudaMemcpyHostToDevice, s));
+    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->scale, host->scale, n * 12, cudaMemcpyHostToDevice, s));
+    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->quat, host->quat, n * 16, cudaMemcpyHostToDevice, s));
+    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->opacity, host->opacity, n * 4, cudaMemcpyHostToDevice, s));
+    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->sh, host->sh, n * K * 12, cudaMemcpyHostToDevice, s));
+    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->feat, host->feat, n * D * e, cudaMemcpyHostToDevice, s));
+    FHGS_CUDA(ctx, cudaMemcpyAsync(ws->gt, host->gt, px * D * e, cudaMemcpyHostToDevice, s));
+    if ((st = fhgs_project(ctx, g, cam, prm, vs, stream)) != FHGS_OK) return st;
+    if ((st = fhgs_bin_sort(ctx, cam, vs, nullptr, 0, stream)) != FHGS_OK) return st;
+    if ((st = fhgs_render(ctx, g, cam, prm, vs, ws->out_rgb, ws->out_feat, nullptr, nullptr, stream)) != FHGS_OK) return st;
+    if ((st = fhgs_fuse_features(ctx, cam, prm, vs, ws->gt, g->feat_dim, g->feat_dtype, ws->num, ws->den,
+                                 ws->fused_feat, g->feat_dtype, FHGS_FUSE_ZERO | FHGS_FUSE_FINALIZE, stream)) != FHGS_OK)
+        return st;
+    if (host->out_rgb) FHGS_CUDA(ctx, cudaMemcpyAsync(host->out_rgb, ws->out_rgb, px * 12, cudaMemcpyDeviceToHost, s));
+    if (host->out_feat) FHGS_CUDA(ctx, cudaMemcpyAsync(host->out_feat, ws->out_feat, px * D * e, cudaMemcpyDeviceToHost, s));
+    if (host->fused_feat) FHGS_CUDA(ctx, cudaMemcpyAsync(host->fused_feat, ws->fused_feat, n * D * e, cudaMemcpyDeviceToHost, s));
+    uint64_t m = 0;
+    FHGS_CUDA(ctx, cudaMemcpyAsync(&m, vs->num_instances, 8, cudaMemcpyDeviceToHost, s));
+    FHGS_CUDA(ctx, cudaStreamSynchronize(s));
+    if (num_instances_host) *num_instances_host = m;
+    if (m > vs->capacity) return set_err(ctx, FHGS_ERR_CAPACITY, "fhgs_frame_host: %s%lld instances exceed capacity", "", (long long)m);
+    return FHGS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
+// FFMA micro-benchmark: 8 CTAs of 8 warps per SM, 32 independent accumulator chains per thread.
+// ------------------------------------------------------------------------------------------------
+namespace {
+constexpr int FFMA_CHAINS = 32;
+// Outer-product form acc[i][j] += a[i] * b[j] (8 x 4), i.e. the three-register FFMA the compositing
+// kernels issue, not the constant-operand form.
+__global__ void __launch_bounds__(256) ffma_peak_kernel(float* out, int iters, float a0, float b0) {
+    float acc[8][4], a[8], b[4];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) a[i] = a0 * (float)(threadIdx.x + i + 1);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) b[j] = b0 * (float)(threadIdx.x + 3 * j + 1);
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 4; ++r)
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+    }
+    float s = 0.f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) s += acc[i][j];
+    if (s == 123.456f) out[0] = s;   // never true in practice; keeps the chains alive
+}
+}  // namespace
+
+extern "C" fhgs_status fhgs_ffma_peak(fhgs_ctx* ctx, int32_t iters, double* lane_ops_per_s, double* ms, void* stream) {
+    if (!ctx) return FHGS_ERR_INVALID;
+    if (iters <= 0 || !lane_ops_per_s) FHGS_INVALID(ctx, "fhgs_ffma_peak: iters <= 0 or NULL output");
+    cudaStream_t s = (cudaStream_t)stream;
+    float* d = nullptr;
+    FHGS_CUDA(ctx, cudaMalloc(&d, 4));
+    const int grid = ctx->num_sms * 8;
+    cudaEvent_t e0, e1;
+    FHGS_CUDA(ctx, cudaEventCreate(&e0));
+    FHGS_CUDA(ctx, cudaEventCreate(&e1));
+    ffma_peak_kernel<<<grid, 256, 0, s>>>(d, iters / 4 + 1, 1e-6f, 1e-6f);   // warm-up
+    FHGS_CUDA(ctx, cudaEventRecord(e0, s));
+    ffma_peak_kernel<<<grid, 256, 0, s>>>(d, iters, 1e-6f, 1e-6f);
+    FHGS_CUDA(ctx, cudaEventRecord(e1, s));
+    FHGS_CUDA(ctx, cudaStreamSynchronize(s));
+    FHGS_LAUNCH_CHECK(ctx);
+    float t = 0.f;
+    FHGS_CUDA(ctx, cudaEventElapsedTime(&t, e0, e1));
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    const double ops = (double)grid * 256.0 * (double)iters * 4.0 * FFMA_CHAINS;
+    *lane_ops_per_s = ops / ((double)t * 1e-3);
+    if (ms) *ms = (double)t;
+    return FHGS_OK;
+}

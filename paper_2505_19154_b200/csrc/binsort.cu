@@ -1,0 +1,535 @@
+// binsort.cu -- step S (fhgs_bin_sort): prefix sum + key duplication, onesweep radix sort, ranges.
+// PAPER.md:302, 312-314 (DuplicateWithKeys, SortByKeys, IdentifyTileRanges); SURVEY 8(c) C1-S.
+//
+// Kernels
+//   scan_dup_kernel    single-pass prefix sum of tiles_touched with decoupled look-back (one status
+//                      word per CTA), fused with the emission of the (key,val) pairs: the CTA's
+//                      instances are produced cooperatively (binary search of the instance index
+//                      in the CTA-local prefix sums) so that a Gaussian covering thousands of
+//                      tiles does not serialise one thread, and all key/value stores are
+//                      coalesced.  The digit histograms of every later sort pass are accumulated
+//                      here too (the keys are in registers anyway), saving one full read.
+//   onesweep_kernel    one least-significant-digit pass (8-bit digit) of a STABLE radix sort:
+//                      warp-synchronous match-any ranking, per-CTA digit counts published to a
+//                      status array, chained look-back for the cross-CTA prefix, keys and values
+//                      reordered through shared memory so that global stores are coalesced per
+//                      digit run.  CTA ids come from an atomic ticket so that a CTA only ever
+//                      waits on CTAs that already started.
+//   ranges_kernel      tile boundaries of the sorted keys.
+//
+// Two equivalent schedules (both give the unique sorted list of C1-S step 3):
+//   FHGS_SORT_FULL_KEY  LSD passes over all significant bits of the 64-bit keys
+//                       (32 + ceil(log2(GW*GH)) bits -> 6 passes at 1080p).
+//   default             order the Gaussians by (depth bits, index) first -- 4 passes over N
+//                       32-bit keys, ~30x fewer elements than the instance list -- emit the
+//                       instances in that order, then run only the tile-id digit passes (2 at
+//                       1080p) over the 64-bit keys.  LSD radix sort is stable, so the result is
+//                       identical; the instance list is moved 2 times instead of 6.
+#include <algorithm>
+
+#include "common.cuh"
+#include "layout.cuh"
+
+namespace {
+
+constexpr uint32_t FULL = 0xffffffffu;
+
+__device__ __forceinline__ uint32_t lanemask_lt() {
+    uint32_t m;
+    asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+    return m;
+}
+__device__ __forceinline__ uint64_t ld_volatile_u64(const uint64_t* p) { return *reinterpret_cast<const volatile uint64_t*>(p); }
+__device__ __forceinline__ void st_volatile_u64(uint64_t* p, uint64_t v) { *reinterpret_cast<volatile uint64_t*>(p) = v; }
+__device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p) { return *reinterpret_cast<const volatile uint32_t*>(p); }
+__device__ __forceinline__ void st_volatile_u32(uint32_t* p, uint32_t v) { *reinterpret_cast<volatile uint32_t*>(p) = v; }
+
+// ------------------------------------------------------------------------------------------------
+// scan + duplicate
+// ------------------------------------------------------------------------------------------------
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_ITEMS = SCAN_TILE / SCAN_THREADS;   // 4
+constexpr uint64_t ST_AGG = 1ull << 62, ST_INC = 2ull << 62, ST_VAL = (1ull << 62) - 1;
+
+struct ScanDupArgs {
+    int n, GW;
+    const uint32_t* tiles_touched;
+    const uint16_t* rect;
+    const float* depth;
+    const uint32_t* perm;        // NULL = index order
+    uint32_t* offsets;           // NULL = do not write
+    uint64_t* num_instances;     // NULL = do not write
+    uint64_t* status;            // [scan_tiles]
+    uint32_t* ticket;
+    uint64_t capacity;
+    uint64_t* keys;              // NULL = scan only
+    uint32_t* vals;
+    uint32_t* hist;              // [npass][256]
+    int first_bit, npass;
+};
+
+__global__ void __launch_bounds__(SCAN_THREADS) scan_dup_kernel(const ScanDupArgs a) {
+    __shared__ uint32_t s_incl[SCAN_TILE];     // CTA-local inclusive prefix of tiles_touched
+    __shared__ uint32_t s_gid[SCAN_TILE];
+    __shared__ uint32_t s_depth[SCAN_TILE];
+    __shared__ uint2 s_rect[SCAN_TILE];
+    __shared__ uint32_t s_hist[SORT_MAX_PASSES][256];
+    __shared__ uint32_t s_warp[SCAN_THREADS / 32];
+    __shared__ uint32_t s_ticket;
+    __shared__ uint64_t s_prefix;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) s_ticket = atomicAdd(a.ticket, 1u);
+    if (a.keys)
+        for (int j = tid; j < a.npass * 256; j += SCAN_THREADS) (&s_hist[0][0])[j] = 0;
+    __syncthreads();
+    const uint32_t ticket = s_ticket;
+    const int base = (int)ticket * SCAN_TILE;
+
+    // load (blocked: thread t owns items base + 4t .. 4t+3)
+    uint32_t tt[SCAN_ITEMS];
+    uint32_t sum = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        const int j = base + tid * SCAN_ITEMS + k;
+        uint32_t g = 0, t = 0;
+        if (j < a.n) {
+            g = a.perm ? __ldg(a.perm + j) : (uint32_t)j;
+            t = __ldg(a.tiles_touched + g);
+        }
+        tt[k] = t;
+        sum += t;
+        s_gid[tid * SCAN_ITEMS + k] = g;
+    }
+    // CTA-wide inclusive scan of the per-thread sums
+    uint32_t incl = sum;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t o = __shfl_up_sync(FULL, incl, d);
+        if (lane >= d) incl += o;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    uint32_t warp_off = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < SCAN_THREADS / 32; ++w) {
+        const uint32_t v = s_warp[w];
+        if (w < warp) warp_off += v;
+        total += v;
+    }
+    uint32_t run = warp_off + incl - sum;   // exclusive prefix of this thread inside the CTA
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        run += tt[k];
+        s_incl[tid * SCAN_ITEMS + k] = run;
+    }
+    // decoupled look-back for the cross-CTA prefix (one thread; chains are short)
+    if (tid == 0) {
+        uint64_t excl = 0;
+        if (ticket == 0) {
+            st_volatile_u64(a.status, ST_INC | (uint64_t)total);
+        } else {
+            st_volatile_u64(a.status + ticket, ST_AGG | (uint64_t)total);
+            int p = (int)ticket - 1;
+            while (true) {
+                const uint64_t v = ld_volatile_u64(a.status + p);
+                if ((v >> 62) == 0) continue;
+                excl += v & ST_VAL;
+                if ((v >> 62) == 2) break;
+                --p;
+            }
+            st_volatile_u64(a.status + ticket, ST_INC | (excl + total));
+        }
+        s_prefix = excl;
+        if (a.num_instances && base + SCAN_TILE >= a.n) *a.num_instances = excl + total;
+    }
+    __syncthreads();
+    const uint64_t prefix = s_prefix;
+    if (a.offsets) {
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) {
+            const int j = base + tid * SCAN_ITEMS + k;
+            if (j < a.n) a.offsets[s_gid[tid * SCAN_ITEMS + k]] = (uint32_t)(prefix + s_incl[tid * SCAN_ITEMS + k]);
+        }
+    }
+    if (!a.keys) return;
+
+    // stage rect / depth of the Gaussians that emit
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+        const int li = tid * SCAN_ITEMS + k;
+        if (tt[k]) {
+            const uint32_t g = s_gid[li];
+            s_rect[li] = __ldg(reinterpret_cast<const uint2*>(a.rect) + g);
+            const uint32_t zb = __float_as_uint(__ldg(a.depth + g));
+            s_depth[li] = zb;
+            // depth digits are shared by every instance of the Gaussian: count tt[k] at once
+            for (int p = 0; p < a.npass; ++p) {
+                const int bit = a.first_bit + 8 * p;
+                if (bit < 32) atomicAdd(&s_hist[p][(zb >> bit) & 255u], tt[k]);
+            }
+        }
+    }
+    __syncthreads();
+
+    // cooperative emission: instance j of the CTA belongs to the first item with incl > j
+    const int first_tile_pass = a.first_bit >= 32 ? 0 : (32 - a.first_bit) / 8;
+    const uint32_t rounds = (total + SCAN_THREADS - 1) / SCAN_THREADS;
+    for (uint32_t r = 0; r < rounds; ++r) {
+        const uint32_t j = r * SCAN_THREADS + tid;
+        const bool valid = j < total;
+        uint32_t tile_id = 0xffffffffu;
+        if (valid) {
+            int lo = 0, hi = SCAN_TILE - 1;
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (s_incl[mid] > j) hi = mid; else lo = mid + 1;
+            }
+            const uint32_t start = lo ? s_incl[lo - 1] : 0u;
+            const uint32_t local = j - start;
+            const uint2 rc = s_rect[lo];
+            const uint32_t x0 = rc.x & 0xffffu, y0 = rc.x >> 16, x1 = rc.y & 0xffffu;
+            const uint32_t w = x1 - x0;
+            const uint32_t ty = y0 + local / w, tx = x0 + local % w;
+            tile_id = ty * (uint32_t)a.GW + tx;
+            const uint64_t pos = prefix + j;
+            if (pos < a.capacity) {
+                a.keys[pos] = ((uint64_t)tile_id << 32) | (uint64_t)s_depth[lo];
+                a.vals[pos] = s_gid[lo];
+            }
+        }
+        // tile-id digits: consecutive instances mostly share the high digits -> aggregate
+        // equal digits inside the warp before touching shared memory
+        for (int p = first_tile_pass; p < a.npass; ++p) {
+            const int bit = a.first_bit + 8 * p - 32;
+            const uint32_t d = valid ? ((tile_id >> bit) & 255u) : 256u;
+            const uint32_t peers = __match_any_sync(FULL, d);
+            if (valid && (peers & lanemask_lt()) == 0) atomicAdd(&s_hist[p][d], (uint32_t)__popc(peers));
+        }
+    }
+    __syncthreads();
+    for (int j = tid; j < a.npass * 256; j += SCAN_THREADS) {
+        const uint32_t c = (&s_hist[0][0])[j];
+        if (c) atomicAdd(a.hist + j, c);
+    }
+}
+
+// exclusive scan of every 256-bin histogram (one CTA of 256 threads per pass)
+__global__ void __launch_bounds__(256) hist_scan_kernel(uint32_t* hist) {
+    __shared__ uint32_t s_w[8];
+    uint32_t* h = hist + blockIdx.x * 256;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t c = h[tid];
+    uint32_t incl = c;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t o = __shfl_up_sync(FULL, incl, d);
+        if (lane >= d) incl += o;
+    }
+    if (lane == 31) s_w[warp] = incl;
+    __syncthreads();
+    uint32_t off = 0;
+    for (int w = 0; w < warp; ++w) off += s_w[w];
+    h[tid] = off + incl - c;
+}
+
+// ------------------------------------------------------------------------------------------------
+// depth pre-sort input: key = depth bits (0xffffffff for culled Gaussians), val = index;
+// accumulates the four digit histograms of the 32-bit keys.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) presort_init_kernel(int n, const float* depth, const uint32_t* tiles_touched,
+                                                           uint32_t* keys, uint32_t* vals, uint32_t* hist32) {
+    __shared__ uint32_t s_hist[4][256];
+    for (int j = threadIdx.x; j < 1024; j += 256) (&s_hist[0][0])[j] = 0;
+    __syncthreads();
+    for (int i = blockIdx.x * 256 + threadIdx.x; i < n; i += gridDim.x * 256) {
+        const uint32_t k = __ldg(tiles_touched + i) ? __float_as_uint(__ldg(depth + i)) : 0xffffffffu;
+        keys[i] = k;
+        vals[i] = (uint32_t)i;
+#pragma unroll
+        for (int p = 0; p < 4; ++p) atomicAdd(&s_hist[p][(k >> (8 * p)) & 255u], 1u);
+    }
+    __syncthreads();
+    for (int j = threadIdx.x; j < 1024; j += 256) {
+        const uint32_t c = (&s_hist[0][0])[j];
+        if (c) atomicAdd(hist32 + j, c);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// onesweep pass
+// ------------------------------------------------------------------------------------------------
+constexpr int OS_THREADS = 256;
+constexpr int OS_WARPS = OS_THREADS / 32;
+constexpr uint32_t OS_AGG = 1u << 30, OS_INC = 2u << 30, OS_VAL = (1u << 30) - 1;
+
+template <typename KeyT>
+struct OneSweepArgs {
+    const KeyT* keys_in;
+    const uint32_t* vals_in;
+    KeyT* keys_out;
+    uint32_t* vals_out;
+    const uint64_t* count_dev;   // device count (instance sort) or NULL
+    uint64_t count_host;         // used when count_dev == NULL
+    uint64_t capacity;           // count > capacity -> the pass does nothing
+    int shift;
+    const uint32_t* hist_excl;   // [256] exclusive digit offsets of this pass
+    uint32_t* status;            // [tiles][256]
+    uint32_t* ticket;
+};
+
+template <typename KeyT, int ITEMS>
+__global__ void __launch_bounds__(OS_THREADS) onesweep_kernel(const OneSweepArgs<KeyT> a) {
+    constexpr int TILE = OS_THREADS * ITEMS;
+    __shared__ uint32_t s_cnt[OS_WARPS][256];   // per-warp digit counts -> per-warp exclusive offsets
+    __shared__ __align__(16) KeyT s_keys[TILE]; // reused for the values
+    __shared__ uint32_t s_bin_start[256];       // CTA-local start of each digit run
+    __shared__ uint32_t s_goff[256];            // global offset of digit run minus its local start
+    __shared__ uint32_t s_w[OS_WARPS];
+    __shared__ uint32_t s_ticket;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint64_t count = a.count_dev ? *a.count_dev : a.count_host;
+    if (count > a.capacity) return;
+    if (tid == 0) s_ticket = atomicAdd(a.ticket, 1u);
+#pragma unroll
+    for (int w = 0; w < OS_WARPS; ++w) s_cnt[w][tid] = 0;
+    __syncthreads();
+    const uint32_t ticket = s_ticket;
+    const uint64_t tile_base = (uint64_t)ticket * TILE;
+    if (tile_base >= count) return;
+    const uint32_t tile_valid = (uint32_t)min((uint64_t)TILE, count - tile_base);
+
+    // warp-striped load: warp w, item i, lane l <-> element w*ITEMS*32 + i*32 + l (processing order)
+    KeyT key[ITEMS];
+    uint32_t val[ITEMS];
+    uint32_t rank[ITEMS];
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) {
+        const uint32_t e = warp * ITEMS * 32 + i * 32 + lane;
+        if (e < tile_valid) {
+            key[i] = a.keys_in[tile_base + e];
+            val[i] = a.vals_in[tile_base + e];
+        } else {
+            key[i] = ~(KeyT)0;   // sorts last inside the tile; never written out
+            val[i] = 0;
+        }
+    }
+    // stable ranking inside the warp: equal digits are ranked by (item, lane)
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) {
+        const uint32_t d = (uint32_t)(key[i] >> a.shift) & 255u;
+        const uint32_t peers = __match_any_sync(FULL, d);
+        const int leader = __ffs(peers) - 1;
+        uint32_t old = 0;
+        if (lane == leader) {
+            old = s_cnt[warp][d];
+            s_cnt[warp][d] = old + __popc(peers);
+        }
+        old = __shfl_sync(FULL, old, leader);
+        rank[i] = old + __popc(peers & lanemask_lt());
+        __syncwarp();
+    }
+    __syncthreads();
+    // digit `tid`: per-warp exclusive offsets and the CTA count
+    uint32_t cnt = 0;
+#pragma unroll
+    for (int w = 0; w < OS_WARPS; ++w) {
+        const uint32_t c = s_cnt[w][tid];
+        s_cnt[w][tid] = cnt;
+        cnt += c;
+    }
+    if (tid == 255) cnt -= (uint32_t)TILE - tile_valid;   // padding keys all carry digit 255
+    // publish, then look back over the earlier CTAs
+    uint32_t excl = 0;
+    uint32_t* my = a.status + (size_t)ticket * 256 + tid;
+    if (ticket == 0) {
+        st_volatile_u32(my, OS_INC | cnt);
+    } else {
+        st_volatile_u32(my, OS_AGG | cnt);
+        const uint32_t* p = my - 256;
+        while (true) {
+            const uint32_t v = ld_volatile_u32(p);
+            if ((v >> 30) == 0) continue;
+            excl += v & OS_VAL;
+            if ((v >> 30) == 2) break;
+            p -= 256;
+        }
+        st_volatile_u32(my, OS_INC | (excl + cnt));
+    }
+    // CTA-local exclusive scan over digits
+    uint32_t incl = cnt;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t o = __shfl_up_sync(FULL, incl, d);
+        if (lane >= d) incl += o;
+    }
+    if (lane == 31) s_w[warp] = incl;
+    __syncthreads();
+    uint32_t off = 0;
+    for (int w = 0; w < warp; ++w) off += s_w[w];
+    const uint32_t bin_start = off + incl - cnt;
+    s_bin_start[tid] = bin_start;
+    s_goff[tid] = a.hist_excl[tid] + excl - bin_start;
+    __syncthreads();
+    // keys -> shared memory at their CTA-local sorted position
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) {
+        const uint32_t d = (uint32_t)(key[i] >> a.shift) & 255u;
+        rank[i] += s_bin_start[d] + s_cnt[warp][d];
+        s_keys[rank[i]] = key[i];
+    }
+    __syncthreads();
+    uint32_t gpos[ITEMS];
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) {
+        const uint32_t j = i * OS_THREADS + tid;
+        if (j < tile_valid) {
+            const KeyT k = s_keys[j];
+            const uint32_t d = (uint32_t)(k >> a.shift) & 255u;
+            gpos[i] = s_goff[d] + j;
+            a.keys_out[gpos[i]] = k;
+        }
+    }
+    __syncthreads();
+    uint32_t* s_vals = reinterpret_cast<uint32_t*>(s_keys);
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) s_vals[rank[i]] = val[i];
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) {
+        const uint32_t j = i * OS_THREADS + tid;
+        if (j < tile_valid) a.vals_out[gpos[i]] = s_vals[j];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// tile ranges (C1-S step 4)
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) ranges_kernel(const uint64_t* keys, const uint64_t* count_dev, uint64_t capacity,
+                                                     uint32_t* ranges) {
+    const uint64_t count = *count_dev;
+    if (count > capacity) return;
+    for (uint64_t k = (uint64_t)blockIdx.x * 256 + threadIdx.x; k < count; k += (uint64_t)gridDim.x * 256) {
+        const uint32_t t = (uint32_t)(keys[k] >> 32);
+        if (k == 0 || (uint32_t)(keys[k - 1] >> 32) != t) ranges[2 * (size_t)t] = (uint32_t)k;
+        if (k + 1 == count || (uint32_t)(keys[k + 1] >> 32) != t) ranges[2 * (size_t)t + 1] = (uint32_t)(k + 1);
+    }
+}
+
+int ceil_log2(uint64_t v) {
+    int b = 0;
+    while ((1ull << b) < v) ++b;
+    return b;
+}
+
+}  // namespace
+
+extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs_view_state* vs,
+                                     uint64_t* num_instances_host, uint32_t flags, void* stream) {
+    if (!ctx) return FHGS_ERR_INVALID;
+    if (!cam || !vs) FHGS_INVALID(ctx, "fhgs_bin_sort: NULL argument");
+    fhgs_status st;
+    if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
+    if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
+    if (flags & ~(uint32_t)FHGS_SORT_FULL_KEY) FHGS_INVALID(ctx, "fhgs_bin_sort: unknown flag");
+    cudaStream_t s = (cudaStream_t)stream;
+    const int GW = tiles_x(cam->width), GH = tiles_y(cam->height);
+    const size_t ntiles = (size_t)GW * GH;
+    const ScratchLayout L = make_scratch_layout(vs->n, vs->capacity);
+    char* sc = (char*)vs->scratch;
+    uint32_t* ctrl = (uint32_t*)(sc + L.ctrl);
+    uint32_t* hist = (uint32_t*)(sc + L.hist);
+    uint32_t* hist32 = (uint32_t*)(sc + L.hist32);
+    uint64_t* scan_status = (uint64_t*)(sc + L.scan_status);
+    uint32_t* sort_status = (uint32_t*)(sc + L.sort_status);
+
+    FHGS_CUDA(ctx, cudaMemsetAsync(sc, 0, L.zero_bytes, s));
+    FHGS_CUDA(ctx, cudaMemsetAsync(scan_status, 0, 2 * L.scan_tiles * 8, s));
+    FHGS_CUDA(ctx, cudaMemsetAsync(vs->ranges, 0, ntiles * 8, s));
+    FHGS_CUDA(ctx, cudaMemsetAsync(vs->num_instances, 0, 8, s));
+
+    const int tile_bits = ceil_log2(ntiles);
+    const bool full_key = (flags & FHGS_SORT_FULL_KEY) != 0;
+    const int first_bit = full_key ? 0 : 32;
+    const int npass = ((32 + tile_bits) - first_bit + 7) / 8;
+    vs->sorted_buf = npass & 1;
+
+    if (vs->n > 0) {
+        const int scan_grid = (vs->n + SCAN_TILE - 1) / SCAN_TILE;
+        const uint32_t* perm = nullptr;
+        if (!full_key) {
+            // order the Gaussians by (depth bits, index): 4 stable passes over 32-bit keys
+            uint32_t* pk[2] = {(uint32_t*)(sc + L.pre_keys[0]), (uint32_t*)(sc + L.pre_keys[1])};
+            uint32_t* pv[2] = {(uint32_t*)(sc + L.pre_vals[0]), (uint32_t*)(sc + L.pre_vals[1])};
+            const int grid = std::min((vs->n + 255) / 256, ctx->num_sms * 8);
+            presort_init_kernel<<<grid, 256, 0, s>>>(vs->n, vs->depth, vs->tiles_touched, pk[0], pv[0], hist32);
+            FHGS_LAUNCH_CHECK(ctx);
+            hist_scan_kernel<<<4, 256, 0, s>>>(hist32);
+            FHGS_LAUNCH_CHECK(ctx);
+            const int pre_grid = (vs->n + SORT_TILE_K32 - 1) / SORT_TILE_K32;
+            for (int p = 0; p < 4; ++p) {
+                FHGS_CUDA(ctx, cudaMemsetAsync(sort_status, 0, (size_t)pre_grid * 256 * 4, s));
+                OneSweepArgs<uint32_t> oa;
+                oa.keys_in = pk[p & 1]; oa.vals_in = pv[p & 1];
+                oa.keys_out = pk[(p + 1) & 1]; oa.vals_out = pv[(p + 1) & 1];
+                oa.count_dev = nullptr; oa.count_host = (uint64_t)vs->n; oa.capacity = (uint64_t)vs->n;
+                oa.shift = 8 * p; oa.hist_excl = hist32 + 256 * p; oa.status = sort_status;
+                oa.ticket = ctrl + CTRL_PRESORT_TICKET + p;
+                onesweep_kernel<uint32_t, SORT_TILE_K32 / OS_THREADS><<<pre_grid, OS_THREADS, 0, s>>>(oa);
+                FHGS_LAUNCH_CHECK(ctx);
+            }
+            perm = pv[0];   // 4 passes -> back in buffer 0
+            // `offsets` is defined in index order (C1-S step 1): a scan-only launch
+            ScanDupArgs sa0;
+            memset(&sa0, 0, sizeof(sa0));
+            sa0.n = vs->n; sa0.GW = GW; sa0.tiles_touched = vs->tiles_touched;
+            sa0.offsets = vs->offsets; sa0.num_instances = vs->num_instances;
+            sa0.status = scan_status + L.scan_tiles; sa0.ticket = ctrl + CTRL_SCAN2_TICKET;
+            scan_dup_kernel<<<scan_grid, SCAN_THREADS, 0, s>>>(sa0);
+            FHGS_LAUNCH_CHECK(ctx);
+        }
+        ScanDupArgs sa;
+        sa.n = vs->n; sa.GW = GW;
+        sa.tiles_touched = vs->tiles_touched; sa.rect = vs->rect; sa.depth = vs->depth;
+        sa.perm = perm;
+        sa.offsets = full_key ? vs->offsets : nullptr;
+        sa.num_instances = full_key ? vs->num_instances : nullptr;
+        sa.status = scan_status; sa.ticket = ctrl + CTRL_SCAN_TICKET;
+        sa.capacity = vs->capacity;
+        sa.keys = vs->keys[0]; sa.vals = vs->vals[0];
+        sa.hist = hist; sa.first_bit = first_bit; sa.npass = npass;
+        if (vs->capacity == 0) { sa.keys = nullptr; sa.offsets = vs->offsets; sa.num_instances = vs->num_instances; sa.perm = nullptr; }
+        scan_dup_kernel<<<scan_grid, SCAN_THREADS, 0, s>>>(sa);
+        FHGS_LAUNCH_CHECK(ctx);
+
+        if (vs->capacity > 0) {
+            hist_scan_kernel<<<npass, 256, 0, s>>>(hist);
+            FHGS_LAUNCH_CHECK(ctx);
+            const int sort_grid = (int)((vs->capacity + SORT_TILE_K64 - 1) / SORT_TILE_K64);
+            for (int p = 0; p < npass; ++p) {
+                FHGS_CUDA(ctx, cudaMemsetAsync(sort_status, 0, (size_t)sort_grid * 256 * 4, s));
+                OneSweepArgs<uint64_t> oa;
+                oa.keys_in = vs->keys[p & 1]; oa.vals_in = vs->vals[p & 1];
+                oa.keys_out = vs->keys[(p + 1) & 1]; oa.vals_out = vs->vals[(p + 1) & 1];
+                oa.count_dev = vs->num_instances; oa.count_host = 0; oa.capacity = vs->capacity;
+                oa.shift = first_bit + 8 * p; oa.hist_excl = hist + 256 * p; oa.status = sort_status;
+                oa.ticket = ctrl + CTRL_SORT_TICKET + p;
+                onesweep_kernel<uint64_t, SORT_TILE_K64 / OS_THREADS><<<sort_grid, OS_THREADS, 0, s>>>(oa);
+                FHGS_LAUNCH_CHECK(ctx);
+            }
+            uint64_t rg = (vs->capacity + 255) / 256;
+            if (rg > (uint64_t)ctx->num_sms * 16) rg = (uint64_t)ctx->num_sms * 16;
+            const int rgrid = (int)rg;
+            ranges_kernel<<<rgrid, 256, 0, s>>>(vs->keys[vs->sorted_buf], vs->num_instances, vs->capacity, vs->ranges);
+            FHGS_LAUNCH_CHECK(ctx);
+        }
+    }
+    if (num_instances_host) {
+        FHGS_CUDA(ctx, cudaMemcpyAsync(num_instances_host, vs->num_instances, 8, cudaMemcpyDeviceToHost, s));
+        FHGS_CUDA(ctx, cudaStreamSynchronize(s));
+        if (*num_instances_host > vs->capacity)
+            return set_err(ctx, FHGS_ERR_CAPACITY, "fhgs_bin_sort: %s%lld instances exceed capacity", "", (long long)*num_instances_host);
+    }
+    return FHGS_OK;
+}

@@ -1,0 +1,65 @@
+// common.cuh -- shared by the CUDA translation units of libfhgs.so (never by oracle/).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "fhgs.h"
+
+#define FHGS_TILE 16
+#define FHGS_TILE_PX 256
+
+struct fhgs_ctx {
+    int device;
+    int num_sms;
+    int max_smem_optin;
+    char err[512];
+};
+
+// Pinhole intrinsics derived from proj[] (fhgs.h "Conventions"): double, rounded once.
+struct Intrinsics {
+    float fx, fy, cx, cy, tanx, tany;
+};
+
+static inline Intrinsics make_intrinsics(const fhgs_camera* cam) {
+    Intrinsics k;
+    const double W = (double)cam->width, H = (double)cam->height;
+    k.fx = (float)((double)cam->proj[0] * W / 2.0);
+    k.fy = (float)((double)cam->proj[5] * H / 2.0);
+    k.cx = (float)(((double)cam->proj[2] + 1.0) * W / 2.0 - 0.5);
+    k.cy = (float)(((double)cam->proj[6] + 1.0) * H / 2.0 - 0.5);
+    k.tanx = (float)(1.0 / (double)cam->proj[0]);
+    k.tany = (float)(1.0 / (double)cam->proj[5]);
+    return k;
+}
+
+static inline fhgs_status set_err(fhgs_ctx* ctx, fhgs_status st, const char* fmt, const char* a = "",
+                                  long long b = 0) {
+    if (ctx) snprintf(ctx->err, sizeof(ctx->err), fmt, a, b);
+    return st;
+}
+
+#define FHGS_INVALID(ctx, msg) return set_err((ctx), FHGS_ERR_INVALID, "%s", (msg))
+
+#define FHGS_CUDA(ctx, expr)                                                                  \
+    do {                                                                                      \
+        cudaError_t e__ = (expr);                                                             \
+        if (e__ != cudaSuccess) {                                                             \
+            snprintf((ctx)->err, sizeof((ctx)->err), "CUDA error %s at %s:%d (%s)",           \
+                     cudaGetErrorName(e__), __FILE__, __LINE__, cudaGetErrorString(e__));     \
+            return FHGS_ERR_INTERNAL;                                                         \
+        }                                                                                     \
+    } while (0)
+
+#define FHGS_LAUNCH_CHECK(ctx) FHGS_CUDA(ctx, cudaGetLastError())
+
+static inline bool finite_f(float v) { return v == v && v - v == 0.0f; }
+static inline bool aligned_to(const void* p, size_t a) { return ((uintptr_t)p % a) == 0; }
+
+static inline int tiles_x(int w) { return (w + FHGS_TILE - 1) / FHGS_TILE; }
+static inline int tiles_y(int h) { return (h + FHGS_TILE - 1) / FHGS_TILE; }
+
+fhgs_status validate_camera(fhgs_ctx* ctx, const fhgs_camera* cam);
+fhgs_status validate_params(fhgs_ctx* ctx, const fhgs_params* prm);
+fhgs_status validate_view_state(fhgs_ctx* ctx, const fhgs_view_state* vs, const fhgs_camera* cam);

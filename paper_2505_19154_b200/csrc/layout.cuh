@@ -1,0 +1,53 @@
+// layout.cuh -- carve-up of fhgs_view_state::scratch (shared by api.cu and binsort.cu).
+#pragma once
+#include <stddef.h>
+#include <stdint.h>
+
+constexpr int SCAN_TILE = 1024;        // Gaussians per CTA of the scan+duplicate kernel
+constexpr int SORT_TILE_K64 = 4096;    // pairs per CTA of a 64-bit-key onesweep pass
+constexpr int SORT_TILE_K32 = 4096;    // pairs per CTA of a 32-bit-key onesweep pass
+constexpr int SORT_MAX_PASSES = 8;
+
+// ctrl words (uint32_t)
+enum {
+    CTRL_SCAN_TICKET = 0,     // dynamic CTA id of the scan+duplicate kernel
+    CTRL_SCAN2_TICKET = 13,   // same, for the index-order offsets scan of the depth-pre-sorted mode
+    CTRL_SORT_TICKET = 1,     // [1..8]  dynamic CTA ids, one per instance-sort pass
+    CTRL_PRESORT_TICKET = 9,  // [9..12] dynamic CTA ids of the depth pre-sort passes
+    CTRL_TILE_QUEUE = 16,     // render / fuse tile queue heads
+    CTRL_WORDS = 64
+};
+
+struct ScratchLayout {
+    size_t ctrl;          // uint32_t[CTRL_WORDS]
+    size_t hist;          // uint32_t[SORT_MAX_PASSES][256]   instance-sort digit histograms
+    size_t hist32;        // uint32_t[4][256]                 depth pre-sort digit histograms
+    size_t zero_bytes;    // [0, zero_bytes) is cleared at the start of every fhgs_bin_sort
+    size_t scan_status;   // uint64_t[2][scan_tiles]
+    size_t sort_status;   // uint32_t[sort_tiles][256]
+    size_t pre_keys[2];   // uint32_t[n]  depth bits (ping-pong)
+    size_t pre_vals[2];   // uint32_t[n]  Gaussian index (ping-pong)
+    size_t scan_tiles, sort_tiles, pre_tiles;
+    size_t total;
+};
+
+static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+static inline ScratchLayout make_scratch_layout(int32_t n, uint64_t capacity) {
+    ScratchLayout L;
+    size_t off = 0;
+    L.ctrl = off; off += align_up(CTRL_WORDS * 4, 256);
+    L.hist = off; off += (size_t)SORT_MAX_PASSES * 256 * 4;
+    L.hist32 = off; off += (size_t)4 * 256 * 4;
+    L.zero_bytes = off;
+    L.scan_tiles = ((size_t)n + SCAN_TILE - 1) / SCAN_TILE + 1;
+    L.scan_status = off; off += align_up(2 * L.scan_tiles * 8, 256);
+    L.sort_tiles = ((size_t)capacity + SORT_TILE_K64 - 1) / SORT_TILE_K64 + 1;
+    L.pre_tiles = ((size_t)n + SORT_TILE_K32 - 1) / SORT_TILE_K32 + 1;
+    const size_t st = L.sort_tiles > L.pre_tiles ? L.sort_tiles : L.pre_tiles;
+    L.sort_status = off; off += st * 256 * 4;
+    for (int i = 0; i < 2; ++i) { L.pre_keys[i] = off; off += align_up((size_t)n * 4, 256); }
+    for (int i = 0; i < 2; ++i) { L.pre_vals[i] = off; off += align_up((size_t)n * 4, 256); }
+    L.total = align_up(off, 256);
+    return L;
+}

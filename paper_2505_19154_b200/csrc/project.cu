@@ -1,0 +1,284 @@
+// project.cu -- step P (fhgs_project): EWA projection, culling, tile rectangle, SH colour.
+// PAPER.md:302 (CullGaussian), PAPER.md:309-310 (2DScreenGaussians); SURVEY 8(c) C1-P.
+//
+// Arithmetic rule of this step: every +,-,*,/,sqrt is ONE IEEE binary32 operation, round to
+// nearest even, in the written order, never contracted into an FMA.  This file therefore uses
+// the __f*_rn intrinsics throughout, which ptxas never fuses, so the result does not depend on
+// compiler flags.  The step is HBM-bound (236 B read + 56 B written per visible Gaussian at SH
+// degree 3), so the un-fused arithmetic costs nothing.
+//
+// Layout: one thread per Gaussian.  The SH block of a CTA (256 Gaussians x K x 3 floats, one
+// contiguous span of global memory) is staged through shared memory with coalesced 16-byte
+// loads; every thread then reads its own row with a conflict-free padded stride.
+#include "common.cuh"
+
+namespace {
+
+__device__ __forceinline__ float mul(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ float add(float a, float b) { return __fadd_rn(a, b); }
+__device__ __forceinline__ float sub(float a, float b) { return __fsub_rn(a, b); }
+__device__ __forceinline__ float dvd(float a, float b) { return __fdiv_rn(a, b); }
+__device__ __forceinline__ float sq(float a) { return __fsqrt_rn(a); }
+__device__ __forceinline__ float clampf(float v, float lo, float hi) { return fminf(fmaxf(v, lo), hi); }
+__device__ __forceinline__ bool finite_dev(float v) { return fabsf(v) <= 3.402823466e38f; }
+
+struct ProjectArgs {
+    int n, sh_degree, W, H, GW, GH;
+    const float *mean, *scale, *quat, *opacity, *sh;
+    float V[16];
+    float cam_pos[3];
+    float fx, fy, cx, cy, Lx, Ly;
+    float z_near, dil;
+    float *xy, *depth, *conic_opacity, *rgb;
+    int32_t* radius;
+    uint16_t* rect;
+    uint32_t* tiles_touched;
+};
+
+constexpr int PROJ_THREADS = 256;
+
+// Real orthonormal spherical harmonics up to degree 3 (C1-P step 10).
+__device__ __forceinline__ void sh_basis(int degree, float x, float y, float z, float* Y) {
+    const float C0 = 0.28209479177387814f, C1 = 0.4886025119029199f;
+    Y[0] = C0;
+    if (degree < 1) return;
+    Y[1] = -mul(C1, y);
+    Y[2] = mul(C1, z);
+    Y[3] = -mul(C1, x);
+    if (degree < 2) return;
+    const float xx = mul(x, x), yy = mul(y, y), zz = mul(z, z);
+    const float xy = mul(x, y), yz = mul(y, z), xz = mul(x, z);
+    Y[4] = mul(1.0925484305920792f, xy);
+    Y[5] = mul(-1.0925484305920792f, yz);
+    Y[6] = mul(0.31539156525252005f, sub(sub(mul(2.0f, zz), xx), yy));
+    Y[7] = mul(-1.0925484305920792f, xz);
+    Y[8] = mul(0.5462742152960396f, sub(xx, yy));
+    if (degree < 3) return;
+    Y[9] = mul(mul(-0.5900435899266435f, y), sub(mul(3.0f, xx), yy));
+    Y[10] = mul(mul(2.890611442640554f, xy), z);
+    Y[11] = mul(mul(-0.4570457994644658f, y), sub(sub(mul(4.0f, zz), xx), yy));
+    Y[12] = mul(mul(0.3731763325901154f, z), sub(sub(mul(2.0f, zz), mul(3.0f, xx)), mul(3.0f, yy)));
+    Y[13] = mul(mul(-0.4570457994644658f, x), sub(sub(mul(4.0f, zz), xx), yy));
+    Y[14] = mul(mul(1.445305721320277f, z), sub(xx, yy));
+    Y[15] = mul(mul(-0.5900435899266435f, x), sub(xx, mul(3.0f, yy)));
+}
+
+template <int DEG>
+__global__ void __launch_bounds__(PROJ_THREADS) project_kernel(const ProjectArgs a) {
+    constexpr int K = (DEG + 1) * (DEG + 1);
+    constexpr int ROW = 3 * K;                 // floats per Gaussian
+    constexpr int PAD = (ROW % 2 == 0) ? ROW + 1 : ROW;  // odd stride -> conflict-free rows
+    extern __shared__ float s_sh[];            // [PROJ_THREADS][PAD]
+
+    const int base = blockIdx.x * PROJ_THREADS;
+    const int i = base + threadIdx.x;
+    const int cnt = min(PROJ_THREADS, a.n - base);
+
+    // Stage this CTA's SH rows: contiguous span [base*ROW, (base+cnt)*ROW), coalesced.
+    {
+        const float* src = a.sh + (size_t)base * ROW;
+        const int total = cnt * ROW;
+        if ((((uintptr_t)src) & 15) == 0) {
+            const int total4 = total >> 2;
+            const float4* src4 = reinterpret_cast<const float4*>(src);
+            for (int j = threadIdx.x; j < total4; j += PROJ_THREADS) {
+                const float4 v = __ldg(src4 + j);
+                const int e = j * 4;
+                s_sh[((e + 0) / ROW) * PAD + (e + 0) % ROW] = v.x;
+                s_sh[((e + 1) / ROW) * PAD + (e + 1) % ROW] = v.y;
+                s_sh[((e + 2) / ROW) * PAD + (e + 2) % ROW] = v.z;
+                s_sh[((e + 3) / ROW) * PAD + (e + 3) % ROW] = v.w;
+            }
+            for (int e = (total4 << 2) + threadIdx.x; e < total; e += PROJ_THREADS)
+                s_sh[(e / ROW) * PAD + e % ROW] = __ldg(src + e);
+        } else {
+            for (int e = threadIdx.x; e < total; e += PROJ_THREADS)
+                s_sh[(e / ROW) * PAD + e % ROW] = __ldg(src + e);
+        }
+    }
+    __syncthreads();
+    if (i >= a.n) return;
+
+    float o_xy0 = 0.f, o_xy1 = 0.f, o_depth = 0.f;
+    float4 o_co = make_float4(0.f, 0.f, 0.f, 0.f);
+    float o_rgb[3] = {0.f, 0.f, 0.f};
+    int o_radius = 0;
+    uint32_t o_tt = 0;
+    ushort4 o_rect = make_ushort4(0, 0, 0, 0);
+
+    do {
+        const float p0 = __ldg(a.mean + 3 * (size_t)i), p1 = __ldg(a.mean + 3 * (size_t)i + 1),
+                    p2 = __ldg(a.mean + 3 * (size_t)i + 2);
+        const float* V = a.V;
+        // 1. camera-space position
+        float t[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k)
+            t[k] = add(add(add(mul(V[4 * k], p0), mul(V[4 * k + 1], p1)), mul(V[4 * k + 2], p2)), V[4 * k + 3]);
+        const float z = t[2];
+        if (!(z >= a.z_near)) break;
+        // 2. pixel position
+        const float u = dvd(t[0], z), v = dvd(t[1], z);
+        const float px = add(mul(a.fx, u), a.cx), py = add(mul(a.fy, v), a.cy);
+        // 3. clamp for the Jacobian only
+        const float uc = fminf(fmaxf(u, -a.Lx), a.Lx), vc = fminf(fmaxf(v, -a.Ly), a.Ly);
+        const float X = mul(uc, z), Y = mul(vc, z);
+        // 4. rotation from the (normalised) quaternion
+        const float4 qv = __ldg(reinterpret_cast<const float4*>(a.quat) + i);
+        float qw = qv.x, qx = qv.y, qy = qv.z, qz = qv.w;
+        const float qn = sq(add(add(add(mul(qw, qw), mul(qx, qx)), mul(qy, qy)), mul(qz, qz)));
+        qw = dvd(qw, qn); qx = dvd(qx, qn); qy = dvd(qy, qn); qz = dvd(qz, qn);
+        float R[9];
+        R[0] = sub(1.0f, mul(2.0f, add(mul(qy, qy), mul(qz, qz))));
+        R[1] = mul(2.0f, sub(mul(qx, qy), mul(qw, qz)));
+        R[2] = mul(2.0f, add(mul(qx, qz), mul(qw, qy)));
+        R[3] = mul(2.0f, add(mul(qx, qy), mul(qw, qz)));
+        R[4] = sub(1.0f, mul(2.0f, add(mul(qx, qx), mul(qz, qz))));
+        R[5] = mul(2.0f, sub(mul(qy, qz), mul(qw, qx)));
+        R[6] = mul(2.0f, sub(mul(qx, qz), mul(qw, qy)));
+        R[7] = mul(2.0f, add(mul(qy, qz), mul(qw, qx)));
+        R[8] = sub(1.0f, mul(2.0f, add(mul(qx, qx), mul(qy, qy))));
+        // 5. Sigma3D = (R S)(R S)^T
+        const float s0 = __ldg(a.scale + 3 * (size_t)i), s1 = __ldg(a.scale + 3 * (size_t)i + 1),
+                    s2 = __ldg(a.scale + 3 * (size_t)i + 2);
+        float M[9];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            M[3 * k] = mul(R[3 * k], s0);
+            M[3 * k + 1] = mul(R[3 * k + 1], s1);
+            M[3 * k + 2] = mul(R[3 * k + 2], s2);
+        }
+        float S[9];
+#pragma unroll
+        for (int r = 0; r < 3; ++r)
+#pragma unroll
+            for (int c = r; c < 3; ++c) {
+                const float s = add(add(mul(M[3 * r], M[3 * c]), mul(M[3 * r + 1], M[3 * c + 1])),
+                                    mul(M[3 * r + 2], M[3 * c + 2]));
+                S[3 * r + c] = s;
+                S[3 * c + r] = s;
+            }
+        // 6. A = J R_v  (2x3)
+        const float J00 = dvd(a.fx, z), J02 = -dvd(mul(a.fx, X), mul(z, z));
+        const float J11 = dvd(a.fy, z), J12 = -dvd(mul(a.fy, Y), mul(z, z));
+        float A[6];
+#pragma unroll
+        for (int j = 0; j < 3; ++j) {
+            A[j] = add(mul(J00, V[j]), mul(J02, V[8 + j]));
+            A[3 + j] = add(mul(J11, V[4 + j]), mul(J12, V[8 + j]));
+        }
+        // 7. Sigma2D = A Sigma3D A^T + dil I
+        float U[6];
+#pragma unroll
+        for (int r = 0; r < 2; ++r)
+#pragma unroll
+            for (int j = 0; j < 3; ++j)
+                U[3 * r + j] = add(add(mul(A[3 * r], S[j]), mul(A[3 * r + 1], S[3 + j])), mul(A[3 * r + 2], S[6 + j]));
+        const float ca = add(add(add(mul(U[0], A[0]), mul(U[1], A[1])), mul(U[2], A[2])), a.dil);
+        const float cb = add(add(mul(U[0], A[3]), mul(U[1], A[4])), mul(U[2], A[5]));
+        const float cc = add(add(add(mul(U[3], A[3]), mul(U[4], A[4])), mul(U[5], A[5])), a.dil);
+        const float det = sub(mul(ca, cc), mul(cb, cb));
+        if (!(det > 0.0f)) break;
+        const float inv = dvd(1.0f, det);
+        const float conA = mul(cc, inv), conB = -mul(cb, inv), conC = mul(ca, inv);
+        // 8. radius
+        const float mid = mul(0.5f, add(ca, cc));
+        const float disc = fmaxf(sub(mul(mid, mid), det), 0.0f);
+        const float lam = add(mid, sq(disc));
+        const float r = ceilf(mul(3.0f, sq(lam)));
+        // 9. tile rectangle
+        if (!(finite_dev(px) && finite_dev(py) && finite_dev(r))) break;
+        const float x0 = clampf(floorf(dvd(sub(px, r), 16.0f)), 0.0f, (float)a.GW);
+        const float x1 = clampf(add(floorf(dvd(add(px, r), 16.0f)), 1.0f), 0.0f, (float)a.GW);
+        const float y0 = clampf(floorf(dvd(sub(py, r), 16.0f)), 0.0f, (float)a.GH);
+        const float y1 = clampf(add(floorf(dvd(add(py, r), 16.0f)), 1.0f), 0.0f, (float)a.GH);
+        const int ix0 = (int)x0, ix1 = (int)x1, iy0 = (int)y0, iy1 = (int)y1;
+        if (ix1 <= ix0 || iy1 <= iy0) break;
+        // 10. SH colour
+        float dx = sub(p0, a.cam_pos[0]), dy = sub(p1, a.cam_pos[1]), dz = sub(p2, a.cam_pos[2]);
+        const float dn = sq(add(add(mul(dx, dx), mul(dy, dy)), mul(dz, dz)));
+        dx = dvd(dx, dn); dy = dvd(dy, dn); dz = dvd(dz, dn);
+        float Yb[K];
+        sh_basis(DEG, dx, dy, dz, Yb);
+        const float* row = s_sh + threadIdx.x * PAD;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            float c = 0.5f;
+#pragma unroll
+            for (int l = 0; l < K; ++l) c = add(c, mul(Yb[l], row[3 * l + k]));
+            o_rgb[k] = fmaxf(c, 0.0f);
+        }
+        o_xy0 = px; o_xy1 = py; o_depth = z;
+        o_co = make_float4(conA, conB, conC, __ldg(a.opacity + i));
+        o_radius = (int)r;
+        o_rect = make_ushort4((unsigned short)ix0, (unsigned short)iy0, (unsigned short)ix1, (unsigned short)iy1);
+        o_tt = (uint32_t)((ix1 - ix0) * (iy1 - iy0));
+    } while (0);
+
+    reinterpret_cast<float2*>(a.xy)[i] = make_float2(o_xy0, o_xy1);
+    a.depth[i] = o_depth;
+    reinterpret_cast<float4*>(a.conic_opacity)[i] = o_co;
+    a.rgb[3 * (size_t)i] = o_rgb[0];
+    a.rgb[3 * (size_t)i + 1] = o_rgb[1];
+    a.rgb[3 * (size_t)i + 2] = o_rgb[2];
+    a.radius[i] = o_radius;
+    reinterpret_cast<ushort4*>(a.rect)[i] = o_rect;
+    a.tiles_touched[i] = o_tt;
+}
+
+template <int DEG>
+cudaError_t launch_project(const ProjectArgs& a, cudaStream_t st) {
+    constexpr int K = (DEG + 1) * (DEG + 1);
+    constexpr int ROW = 3 * K;
+    constexpr int PAD = (ROW % 2 == 0) ? ROW + 1 : ROW;
+    const size_t smem = (size_t)PROJ_THREADS * PAD * sizeof(float);
+    cudaError_t e = cudaFuncSetAttribute(project_kernel<DEG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const int grid = (a.n + PROJ_THREADS - 1) / PROJ_THREADS;
+    project_kernel<DEG><<<grid, PROJ_THREADS, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+extern "C" fhgs_status fhgs_project(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam,
+                                    const fhgs_params* prm, fhgs_view_state* vs, void* stream) {
+    if (!ctx) return FHGS_ERR_INVALID;
+    if (!g || !cam || !prm || !vs) FHGS_INVALID(ctx, "fhgs_project: NULL argument");
+    fhgs_status st;
+    if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
+    if ((st = validate_params(ctx, prm)) != FHGS_OK) return st;
+    if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
+    if (g->n < 0 || g->n != vs->n) FHGS_INVALID(ctx, "fhgs_project: g->n < 0 or != vs->n");
+    if (g->sh_degree < 0 || g->sh_degree > 3) FHGS_INVALID(ctx, "fhgs_project: sh_degree not in [0,3]");
+    if (g->n == 0) return FHGS_OK;
+    if (!g->mean || !g->scale || !g->quat || !g->opacity || !g->sh)
+        FHGS_INVALID(ctx, "fhgs_project: NULL Gaussian array");
+    if (!aligned_to(g->quat, 16) || !aligned_to(g->mean, 4) || !aligned_to(g->scale, 4) || !aligned_to(g->sh, 4))
+        FHGS_INVALID(ctx, "fhgs_project: quat must be 16-byte aligned");
+
+    ProjectArgs a;
+    a.n = g->n; a.sh_degree = g->sh_degree; a.W = cam->width; a.H = cam->height;
+    a.GW = tiles_x(cam->width); a.GH = tiles_y(cam->height);
+    a.mean = g->mean; a.scale = g->scale; a.quat = g->quat; a.opacity = g->opacity; a.sh = g->sh;
+    memcpy(a.V, cam->view, sizeof(a.V));
+    memcpy(a.cam_pos, cam->cam_pos, sizeof(a.cam_pos));
+    const Intrinsics k = make_intrinsics(cam);
+    a.fx = k.fx; a.fy = k.fy; a.cx = k.cx; a.cy = k.cy;
+    a.Lx = prm->jac_clamp * k.tanx;   // single binary32 multiply, as C1-P step 3
+    a.Ly = prm->jac_clamp * k.tany;
+    a.z_near = prm->z_near; a.dil = prm->cov_dilation;
+    a.xy = vs->xy; a.depth = vs->depth; a.conic_opacity = vs->conic_opacity; a.rgb = vs->rgb;
+    a.radius = vs->radius; a.rect = vs->rect; a.tiles_touched = vs->tiles_touched;
+
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e;
+    switch (g->sh_degree) {
+        case 0: e = launch_project<0>(a, s); break;
+        case 1: e = launch_project<1>(a, s); break;
+        case 2: e = launch_project<2>(a, s); break;
+        default: e = launch_project<3>(a, s); break;
+    }
+    FHGS_CUDA(ctx, e);
+    return FHGS_OK;
+}

@@ -1,0 +1,354 @@
+// render.cu -- step R (fhgs_render): per-tile front-to-back compositing of RGB + D feature channels.
+// PAPER.md:90-95 (Eq. 4); SURVEY 8(c) C1-R.
+//
+// One CTA (256 threads) per 16x16 tile.  The feature work of a tile is the product
+//     F[256 px, D] += W[256 px, K] * f[K, D]
+// over the K instances that survive the tile cull (traverse.cuh).  It is evaluated in sub-batches of
+// KB staged instances:
+//   phase B  thread = pixel: weights w = alpha*T for the KB instances (sequential in T), RGB
+//            accumulation, w parked in shared memory W[kk][slot]; each warp records which
+//            instances gave any of its 32 pixels a weight.
+//   phase C  register-tiled outer products: thread = 8 pixels x (DC/8) channels, accumulators in
+//            registers (128 for DC = 128); one broadcast LDS.128 pair of W and DC/32 LDS.128 of f
+//            feed 8*DC/8 FFMAs.  Instances with no weight inside the warp are skipped (warp-uniform).
+// The feature rows of a sub-batch are fetched with cp.async while phase B runs.
+// D > DC is handled by channel passes (the traversal is repeated per pass; RGB/T/n are written by
+// pass 0).  Small D (not a multiple of 64) uses the per-pixel variant: CH accumulators per thread,
+// updated inside phase B from broadcast shared-memory reads.
+#include "traverse.cuh"
+
+namespace {
+
+struct RenderArgs {
+    TraverseArgs t;
+    const float* rgb_g;   // [n,3]
+    const void* feat;     // [n,D] or NULL
+    int D;
+    float bg[3];
+    float* out_rgb;
+    void* out_feat;
+    float* out_T;
+    uint32_t* out_n;
+};
+
+constexpr int R_KB = 64;   // staged instances per sub-batch
+
+template <typename FT> struct FeatIO;
+template <> struct FeatIO<float> {
+    static __device__ __forceinline__ float4 load4(const float* p) { return *reinterpret_cast<const float4*>(p); }
+    static __device__ __forceinline__ void store4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
+};
+template <> struct FeatIO<__half> {
+    static __device__ __forceinline__ float4 load4(const __half* p) {
+        const uint2 r = *reinterpret_cast<const uint2*>(p);
+        const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
+        const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
+        return make_float4(a.x, a.y, b.x, b.y);
+    }
+    static __device__ __forceinline__ void store4(__half* p, float4 v) {
+        const __half2 a = __floats2half2_rn(v.x, v.y), b = __floats2half2_rn(v.z, v.w);
+        uint2 r;
+        r.x = *reinterpret_cast<const uint32_t*>(&a);
+        r.y = *reinterpret_cast<const uint32_t*>(&b);
+        *reinterpret_cast<uint2*>(p) = r;
+    }
+};
+
+// ---------------------------------------------------------------------------------------------
+// TILED variant: DC in {64,128}
+// ---------------------------------------------------------------------------------------------
+template <int DC, typename FT>
+struct TiledSmem {
+    TileQueue q;
+    float4 rgb[TR_QCAP];                       // staged colours (xyz used)
+    __align__(16) float W[R_KB * TR_THREADS];  // W[kk][slot]
+    __align__(16) FT F[R_KB * DC];             // feature rows of the sub-batch
+};
+
+template <int DC, typename FT>
+__global__ void __launch_bounds__(TR_THREADS, 1) render_tiled_kernel(const RenderArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    TiledSmem<DC, FT>& sm = *reinterpret_cast<TiledSmem<DC, FT>*>(smem_raw);
+    constexpr int NJ = DC / 32;                // float4 groups of channels per thread
+    constexpr int CPR = DC * (int)sizeof(FT) / 16;   // 16-byte chunks per feature row
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tile = blockIdx.x;
+    const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
+    int sx, sy;
+    slot_to_xy(tid, sx, sy);
+    const int px = tx0 + sx, py = ty0 + sy;
+    const bool inside = px < a.t.W && py < a.t.H;
+    const float fx = (float)px, fy = (float)py;
+    const float bx0 = (float)tx0, by0 = (float)ty0;
+    const float bx1 = (float)min(tx0 + FHGS_TILE - 1, a.t.W - 1), by1 = (float)min(ty0 + FHGS_TILE - 1, a.t.H - 1);
+    const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
+    const FT* feat = reinterpret_cast<const FT*>(a.feat);
+    FT* out_feat = reinterpret_cast<FT*>(a.out_feat);
+
+    // phase-C coordinates: 8 pixels (one row run) x NJ*4 channels
+    const int pgl = lane >> 3, cg = lane & 7;
+    const int pg = warp * 4 + pgl;
+
+    for (int c0 = 0; c0 < a.D; c0 += DC) {
+        float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
+        uint32_t n = 0;
+        bool done = !inside;
+        float acc[8][NJ * 4];
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < NJ * 4; ++j) acc[i][j] = 0.f;
+        uint32_t pos = range.x;
+        int q_head = 0, q_count = 0;
+
+        while (true) {
+            while (q_count < R_KB && pos < range.y) {
+                const int tail = q_head + q_count;
+                const int added = stage_chunk(a.t, sm.q, pos, range.y, tail, bx0, by0, bx1, by1);
+                // colours of the survivors just appended (slots tail .. tail+added)
+                for (int k = tid; k < added; k += TR_THREADS) {
+                    const int s = (tail + k) & (TR_QCAP - 1);
+                    const uint32_t id = sm.q.id[s];
+                    sm.rgb[s] = make_float4(__ldg(a.rgb_g + 3 * (size_t)id), __ldg(a.rgb_g + 3 * (size_t)id + 1),
+                                            __ldg(a.rgb_g + 3 * (size_t)id + 2), 0.f);
+                }
+                q_count += added;
+                pos += TR_THREADS;
+            }
+            const int nb = min(R_KB, q_count);
+            if (nb == 0) break;
+            __syncthreads();   // staged colours visible; previous phase C finished with W/F
+            // async fetch of the sub-batch's feature rows
+            for (int c = tid; c < nb * CPR; c += TR_THREADS) {
+                const int row = c / CPR, ch = c % CPR;
+                const uint32_t id = sm.q.id[(q_head + row) & (TR_QCAP - 1)];
+                cp_async16(reinterpret_cast<unsigned char*>(sm.F) + (size_t)row * DC * sizeof(FT) + ch * 16,
+                           reinterpret_cast<const unsigned char*>(feat + (size_t)id * a.D + c0) + ch * 16);
+            }
+            // phase B
+            unsigned long long any_mask = 0ull;
+            for (int kk = 0; kk < nb; ++kk) {
+                const int s = (q_head + kk) & (TR_QCAP - 1);
+                const float w = eval_weight(sm.q.xy[s], sm.q.co[s], fx, fy, a.t, T, done, n);
+                if (w != 0.f) {
+                    const float4 c = sm.rgb[s];
+                    C0 = fmaf(w, c.x, C0); C1 = fmaf(w, c.y, C1); C2 = fmaf(w, c.z, C2);
+                }
+                sm.W[kk * TR_THREADS + tid] = w;
+                if (__any_sync(TR_FULL, w != 0.f)) any_mask |= 1ull << kk;
+            }
+            cp_async_wait_all();
+            __syncthreads();
+            // phase C
+            for (int kk = 0; kk < nb; ++kk) {
+                if (!((any_mask >> kk) & 1ull)) continue;
+                const float4 wa = *reinterpret_cast<const float4*>(&sm.W[kk * TR_THREADS + pg * 8]);
+                const float4 wb = *reinterpret_cast<const float4*>(&sm.W[kk * TR_THREADS + pg * 8 + 4]);
+                const float wv[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
+                float fv[NJ * 4];
+#pragma unroll
+                for (int j = 0; j < NJ; ++j) {
+                    const float4 f = FeatIO<FT>::load4(&sm.F[kk * DC + j * 32 + cg * 4]);
+                    fv[4 * j] = f.x; fv[4 * j + 1] = f.y; fv[4 * j + 2] = f.z; fv[4 * j + 3] = f.w;
+                }
+#pragma unroll
+                for (int i = 0; i < 8; ++i)
+#pragma unroll
+                    for (int j = 0; j < NJ * 4; ++j) acc[i][j] = fmaf(wv[i], fv[j], acc[i][j]);
+            }
+            q_head = (q_head + nb) & (TR_QCAP - 1);
+            q_count -= nb;
+            if (__syncthreads_and(done)) break;
+        }
+
+        if (c0 == 0 && inside) {
+            const size_t p = (size_t)py * a.t.W + px;
+            a.out_rgb[3 * p] = fmaf(T, a.bg[0], C0);
+            a.out_rgb[3 * p + 1] = fmaf(T, a.bg[1], C1);
+            a.out_rgb[3 * p + 2] = fmaf(T, a.bg[2], C2);
+            if (a.out_T) a.out_T[p] = T;
+            if (a.out_n) a.out_n[p] = n;
+        }
+        // feature output: this thread's 8 pixels are slots pg*8 .. pg*8+7 = one row run of 8
+        {
+            const int oy = ty0 + ((warp >> 1) << 2) + pgl;
+            const int ox0 = tx0 + ((warp & 1) << 3);
+            if (oy < a.t.H) {
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    const int ox = ox0 + i;
+                    if (ox < a.t.W) {
+                        FT* dst = out_feat + ((size_t)oy * a.t.W + ox) * a.D + c0;
+#pragma unroll
+                        for (int j = 0; j < NJ; ++j)
+                            FeatIO<FT>::store4(dst + j * 32 + cg * 4, make_float4(acc[i][4 * j], acc[i][4 * j + 1],
+                                                                                  acc[i][4 * j + 2], acc[i][4 * j + 3]));
+                    }
+                }
+            }
+        }
+        __syncthreads();   // ring and W/F are reused by the next channel pass
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// PIXEL variant: CH in {0,4,8,16} feature channels per pass, accumulated by the pixel's own thread
+// ---------------------------------------------------------------------------------------------
+template <int CH>
+struct PixelSmem {
+    TileQueue q;
+    float4 rgb[TR_QCAP];
+    __align__(16) float F[TR_QCAP * (CH > 0 ? CH : 1)];
+};
+
+template <int CH, typename FT>
+__global__ void __launch_bounds__(TR_THREADS) render_pixel_kernel(const RenderArgs a) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    PixelSmem<CH>& sm = *reinterpret_cast<PixelSmem<CH>*>(smem_raw);
+
+    const int tid = threadIdx.x;
+    const int tile = blockIdx.x;
+    const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
+    int sx, sy;
+    slot_to_xy(tid, sx, sy);
+    const int px = tx0 + sx, py = ty0 + sy;
+    const bool inside = px < a.t.W && py < a.t.H;
+    const float fx = (float)px, fy = (float)py;
+    const float bx0 = (float)tx0, by0 = (float)ty0;
+    const float bx1 = (float)min(tx0 + FHGS_TILE - 1, a.t.W - 1), by1 = (float)min(ty0 + FHGS_TILE - 1, a.t.H - 1);
+    const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
+    const FT* feat = reinterpret_cast<const FT*>(a.feat);
+    FT* out_feat = reinterpret_cast<FT*>(a.out_feat);
+    const int D = CH > 0 ? a.D : 1;
+
+    for (int c0 = 0; c0 < D; c0 += (CH > 0 ? CH : 1)) {
+        float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
+        uint32_t n = 0;
+        bool done = !inside;
+        float acc[CH > 0 ? CH : 1];
+#pragma unroll
+        for (int j = 0; j < (CH > 0 ? CH : 1); ++j) acc[j] = 0.f;
+        uint32_t pos = range.x;
+        int q_head = 0, q_count = 0;
+        while (true) {
+            while (q_count < R_KB && pos < range.y) {
+                const int tail = q_head + q_count;
+                const int added = stage_chunk(a.t, sm.q, pos, range.y, tail, bx0, by0, bx1, by1);
+                for (int k = tid; k < added; k += TR_THREADS) {
+                    const int s = (tail + k) & (TR_QCAP - 1);
+                    const uint32_t id = sm.q.id[s];
+                    sm.rgb[s] = make_float4(__ldg(a.rgb_g + 3 * (size_t)id), __ldg(a.rgb_g + 3 * (size_t)id + 1),
+                                            __ldg(a.rgb_g + 3 * (size_t)id + 2), 0.f);
+                }
+                if constexpr (CH > 0) {
+                    for (int k = tid; k < added * (CH / 4); k += TR_THREADS) {
+                        const int r = k / (CH / 4), c = k % (CH / 4);
+                        const int s = (tail + r) & (TR_QCAP - 1);
+                        const uint32_t id = sm.q.id[s];
+                        *reinterpret_cast<float4*>(&sm.F[s * CH + 4 * c]) = FeatIO<FT>::load4(feat + (size_t)id * a.D + c0 + 4 * c);
+                    }
+                }
+                q_count += added;
+                pos += TR_THREADS;
+            }
+            const int nb = q_count;   // drain everything staged
+            if (nb == 0) break;
+            __syncthreads();
+            for (int kk = 0; kk < nb; ++kk) {
+                const int s = (q_head + kk) & (TR_QCAP - 1);
+                const float w = eval_weight(sm.q.xy[s], sm.q.co[s], fx, fy, a.t, T, done, n);
+                if (w != 0.f) {
+                    const float4 c = sm.rgb[s];
+                    C0 = fmaf(w, c.x, C0); C1 = fmaf(w, c.y, C1); C2 = fmaf(w, c.z, C2);
+                    if constexpr (CH > 0) {
+#pragma unroll
+                        for (int j = 0; j < CH / 4; ++j) {
+                            const float4 f = *reinterpret_cast<const float4*>(&sm.F[s * CH + 4 * j]);
+                            acc[4 * j] = fmaf(w, f.x, acc[4 * j]);
+                            acc[4 * j + 1] = fmaf(w, f.y, acc[4 * j + 1]);
+                            acc[4 * j + 2] = fmaf(w, f.z, acc[4 * j + 2]);
+                            acc[4 * j + 3] = fmaf(w, f.w, acc[4 * j + 3]);
+                        }
+                    }
+                }
+            }
+            q_head = (q_head + nb) & (TR_QCAP - 1);
+            q_count = 0;
+            if (__syncthreads_and(done)) break;
+        }
+        if (inside) {
+            const size_t p = (size_t)py * a.t.W + px;
+            if (c0 == 0) {
+                a.out_rgb[3 * p] = fmaf(T, a.bg[0], C0);
+                a.out_rgb[3 * p + 1] = fmaf(T, a.bg[1], C1);
+                a.out_rgb[3 * p + 2] = fmaf(T, a.bg[2], C2);
+                if (a.out_T) a.out_T[p] = T;
+                if (a.out_n) a.out_n[p] = n;
+            }
+            if constexpr (CH > 0) {
+#pragma unroll
+                for (int j = 0; j < CH / 4; ++j)
+                    FeatIO<FT>::store4(out_feat + p * a.D + c0 + 4 * j,
+                                       make_float4(acc[4 * j], acc[4 * j + 1], acc[4 * j + 2], acc[4 * j + 3]));
+            }
+        }
+        __syncthreads();
+    }
+}
+
+template <typename K>
+cudaError_t launch(K kernel, size_t smem, int grid, cudaStream_t st, const RenderArgs& a) {
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kernel<<<grid, TR_THREADS, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <typename FT>
+cudaError_t dispatch(const RenderArgs& a, int grid, cudaStream_t st, bool has_feat) {
+    if (!has_feat) return launch(render_pixel_kernel<0, FT>, sizeof(PixelSmem<0>), grid, st, a);
+    if (a.D % 128 == 0) return launch(render_tiled_kernel<128, FT>, sizeof(TiledSmem<128, FT>), grid, st, a);
+    if (a.D % 64 == 0) return launch(render_tiled_kernel<64, FT>, sizeof(TiledSmem<64, FT>), grid, st, a);
+    if (a.D % 16 == 0) return launch(render_pixel_kernel<16, FT>, sizeof(PixelSmem<16>), grid, st, a);
+    if (a.D % 8 == 0) return launch(render_pixel_kernel<8, FT>, sizeof(PixelSmem<8>), grid, st, a);
+    return launch(render_pixel_kernel<4, FT>, sizeof(PixelSmem<4>), grid, st, a);
+}
+
+}  // namespace
+
+extern "C" fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam,
+                                   const fhgs_params* prm, const fhgs_view_state* vs, float* out_rgb,
+                                   void* out_feat, float* out_T, uint32_t* out_ncontrib, void* stream) {
+    if (!ctx) return FHGS_ERR_INVALID;
+    if (!g || !cam || !prm || !vs) FHGS_INVALID(ctx, "fhgs_render: NULL argument");
+    fhgs_status st;
+    if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
+    if ((st = validate_params(ctx, prm)) != FHGS_OK) return st;
+    if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
+    if (!out_rgb) FHGS_INVALID(ctx, "fhgs_render: out_rgb is required");
+    const bool has_feat = out_feat != nullptr;
+    if (has_feat) {
+        if (!g->feat) FHGS_INVALID(ctx, "fhgs_render: out_feat given but g->feat is NULL");
+        if (g->feat_dtype != FHGS_F32 && g->feat_dtype != FHGS_F16) FHGS_INVALID(ctx, "fhgs_render: unknown feat_dtype");
+        const int mult = g->feat_dtype == FHGS_F16 ? 8 : 4;
+        if (g->feat_dim <= 0 || g->feat_dim % mult) FHGS_INVALID(ctx, "fhgs_render: feat_dim must be a positive multiple of 4 (f32) / 8 (f16)");
+        if (!aligned_to(g->feat, 16) || !aligned_to(out_feat, 16)) FHGS_INVALID(ctx, "fhgs_render: feat/out_feat must be 16-byte aligned");
+        if (g->n != vs->n) FHGS_INVALID(ctx, "fhgs_render: g->n != vs->n");
+    }
+    RenderArgs a;
+    a.t.W = cam->width; a.t.H = cam->height; a.t.GW = tiles_x(cam->width);
+    a.t.ranges = vs->ranges; a.t.vals = vs->vals[vs->sorted_buf & 1];
+    a.t.xy = reinterpret_cast<const float2*>(vs->xy);
+    a.t.conic_opacity = reinterpret_cast<const float4*>(vs->conic_opacity);
+    a.t.q_cutoff = prm->q_cutoff; a.t.alpha_max = prm->alpha_max; a.t.t_min = prm->t_min;
+    a.rgb_g = vs->rgb; a.feat = g->feat; a.D = has_feat ? g->feat_dim : 0;
+    a.bg[0] = prm->bg[0]; a.bg[1] = prm->bg[1]; a.bg[2] = prm->bg[2];
+    a.out_rgb = out_rgb; a.out_feat = out_feat; a.out_T = out_T; a.out_n = out_ncontrib;
+    const int grid = tiles_x(cam->width) * tiles_y(cam->height);
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e = (has_feat && g->feat_dtype == FHGS_F16) ? dispatch<__half>(a, grid, s, has_feat)
+                                                            : dispatch<float>(a, grid, s, has_feat);
+    FHGS_CUDA(ctx, e);
+    return FHGS_OK;
+}

@@ -1,0 +1,187 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Bars (north_star / SURVEY 8(c)): integers bit-exact (radius, rect,
+tiles_touched, M, offsets, sorted keys AND values, ranges, n_contrib off fragile pixels); fp32
+RGB / features / T / fused vectors within 1e-4 max abs; 2e-3 where features are stored fp16."""
+import numpy as np
+import pytest
+
+from oracle import fhgs_oracle as fo
+from paper_2505_19154_b200 import inputs
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+
+
+def run_case(cfg, views, tol, literal_pixels=None, sort_flags=(0, 1), capacity_slack=1.25, check_finalize=True):
+    """Full P -> S -> R -> F parity of one config over `views`; returns worst errors."""
+    scene = inputs.make_scene(cfg)
+    cams = [inputs.make_camera(cfg, v) for v in views]
+    prs = [pu.oracle_view(scene, cam) for cam in cams]
+    bins = [fo.bins(pr, cfg.width, cfg.height) for pr in prs]
+    cap = int(max(b["M"] for b in bins) * capacity_slack) + 16
+    gp = pu.GpuPath(scene, cfg.width, cfg.height, cap)
+    feat32 = scene.feat.astype(np.float32)
+    fabs = float(np.abs(feat32).max())
+    worst = {}
+    num_o = np.zeros((scene.n, cfg.feat_dim)); den_o = np.zeros(scene.n)
+    num_g = den_g = None
+    frag_touch = np.zeros(scene.n, np.int64)
+    for vi, (v, cam, pr, bo) in enumerate(zip(views, cams, prs, bins)):
+        for fl in sort_flags:
+            c, m = gp.project_sort(cam, flags=fl)
+            pu.check_projection(pr, gp.vs.projected())
+            pu.check_bins(bo, gp.vs, m)
+        order = fo.global_order(pr)
+        g = gp.render(c)
+        if literal_pixels is None:
+            o = fo.render_scatter(pr, order, feat32, cfg.width, cfg.height)
+            pix = None
+        else:
+            rng = np.random.default_rng(7 + v)
+            pix = np.unique(rng.integers(0, cfg.width * cfg.height, size=literal_pixels)).astype(np.int32)
+            o = fo.render_literal(pr, order, feat32, cfg.width, cfg.height, pix=pix)
+        w = pu.check_render(o, g, fabs, tol, pix=pix)
+        for k, val in w.items():
+            worst[k] = max(worst.get(k, 0), val)
+        # fusion, accumulated over the views
+        gt = inputs.make_gt_map(cfg, v, cam)
+        gabs = float(np.abs(gt.astype(np.float32)).max())
+        if literal_pixels is None:
+            fo.fuse(pr, order, gt, cfg.width, cfg.height, num=num_o, den=den_o)
+            fpix = np.nonzero(o["fragile"])[0]
+            frag_touch += pu.gaussians_touching(pr, fpix, cfg.width)
+            fl = None if vi == 0 else 0
+            num_g, den_g = gp.fuse(c, gt, num_g, den_g, flags=fl)
+    if num_g is not None:
+        w = pu.check_fuse(num_o, den_o, num_g, den_g, gabs, tol, frag_touch)
+        worst.update({"fuse_" + k: val for k, val in w.items()})
+        if check_finalize:
+            f_o = fo.finalize(num_o, den_o, feat32)
+            f_g = gp.finalize(num_g, den_g, scene.feat)
+            worst["fused"], worst["fused_rows"] = pu.check_finalized(f_o, f_g, den_o, tol, fragile_mask=frag_touch > 0)
+            # rows with den <= eps keep their previous value exactly
+            keep = den_o <= 1e-8
+            assert np.array_equal(f_g[keep], scene.feat[keep])
+    return worst
+
+
+def test_tiny_all_views():
+    """configs[0]: N=1000, D=8, 64x64, 4 views (per-pixel kernels, CH=8)."""
+    w = run_case(inputs.CONFIGS["tiny"], range(4), pu.TOL_F32)
+    print(w)
+
+
+def test_small_reduced():
+    """configs[1] at N=20,000 (oracle in seconds), 2 of the 8 views, D=16, SH degree 1, 256x256."""
+    cfg = pu.reduced_config("small", n=20_000)
+    w = run_case(cfg, [0, 3], pu.TOL_F32)
+    print(w)
+
+
+def test_mid_shape_ragged_tiles_d128():
+    """configs[2] shape at reduced size: D=128 unit features (tiled kernels, DC=128), SH degree 3,
+    328x200 px: 20.5 x 12.5 tiles -> ragged right column and bottom row."""
+    cfg = pu.reduced_config("mid", n=60_000, width=328, height=200, log_scale_mu=-3.3)
+    w = run_case(cfg, [0], pu.TOL_F32)
+    print(w)
+
+
+def test_d64_and_d192_paths():
+    """DC=64 kernels: D=64 (one pass) and D=192 (three passes)."""
+    for d in (64, 192):
+        cfg = pu.reduced_config("mid", n=15_000, width=160, height=96, log_scale_mu=-3.0, feat_dim=d)
+        print(d, run_case(cfg, [0], pu.TOL_F32, sort_flags=(0,)))
+
+
+def test_multiview_shape_d256():
+    """configs[4] shape at reduced size: blobs, D=256 (two channel passes), 3 orbit views accumulated."""
+    cfg = pu.reduced_config("multiview", n=40_000, width=216, height=168, n_views=200, log_scale_mu=-3.0)
+    w = run_case(cfg, [0, 67, 133], pu.TOL_F32, sort_flags=(0,))
+    print(w)
+
+
+def test_large_shape_fp16_d512():
+    """configs[3] shape at reduced size: D=512 stored fp16, accumulated fp32, fp16 image / fused output."""
+    cfg = pu.reduced_config("large", n=30_000, width=200, height=120, log_scale_mu=-3.3)
+    w = run_case(cfg, [0], pu.TOL_F16, sort_flags=(0,))
+    print(w)
+
+
+def test_odd_d_paths():
+    """D=4 and D=24 (CH=4 / CH=8 per-pixel kernels)."""
+    for d in (4, 24):
+        cfg = pu.reduced_config("tiny", n=3000, feat_dim=d, width=80, height=48)
+        print(d, run_case(cfg, [1], pu.TOL_F32, sort_flags=(0,)))
+
+
+def test_edge_cases():
+    import torch
+    from paper_2505_19154_b200 import binding as fb
+    cfg = inputs.CONFIGS["tiny"]
+    scene = inputs.make_scene(cfg)
+    cam = inputs.make_camera(cfg, 0)
+    # (a) nothing visible: every Gaussian behind the camera -> M = 0, background image, num/den untouched
+    behind = inputs.Scene(scene.mean + np.array([0, 0, -100], np.float32), scene.scale, scene.quat, scene.opacity,
+                          scene.sh, scene.feat, scene.sh_degree)
+    gp = pu.GpuPath(behind, 64, 64, 1024)
+    gp.prm = fb.default_params(bg=(0.25, 0.5, 0.75))
+    c, m = gp.project_sort(cam)
+    assert m == 0 and int(gp.vs.ranges.abs().sum()) == 0
+    g = gp.render(c)
+    assert np.all(g["n"] == 0) and np.all(g["T"] == 1.0) and np.all(g["feat"] == 0)
+    assert np.allclose(g["rgb"], np.array([0.25, 0.5, 0.75], np.float32))
+    num, den = gp.fuse(c, inputs.make_gt_map(cfg, 0))
+    assert float(num.abs().sum()) == 0 and float(den.abs().sum()) == 0
+    # (b) capacity overflow: synchronous bin_sort reports it, M is still exact, ranges stay empty
+    pr = pu.oracle_view(scene, cam)
+    m_true = fo.bins(pr, 64, 64)["M"]
+    gp2 = pu.GpuPath(scene, 64, 64, m_true - 1)
+    cc = gp2.camera(cam)
+    fb.project(gp2.ctx, gp2.g, cc, gp2.prm, gp2.vs)
+    with pytest.raises(fb.FhgsError) as ei:
+        fb.bin_sort(gp2.ctx, cc, gp2.vs, sync=True)
+    assert ei.value.status == fb.FHGS_ERR_CAPACITY
+    assert int(gp2.vs.num_instances.item()) == m_true and int(gp2.vs.ranges.abs().sum()) == 0
+    # exactly enough capacity works
+    gp3 = pu.GpuPath(scene, 64, 64, m_true)
+    c3, m3 = gp3.project_sort(cam)
+    assert m3 == m_true
+    # (c) invalid arguments are rejected before anything is enqueued
+    bad = fb.make_camera(cam.view, cam.proj, cam.cam_pos, 0, 64)
+    with pytest.raises(fb.FhgsError) as ei:
+        fb.project(gp3.ctx, gp3.g, bad, gp3.prm, gp3.vs)
+    assert ei.value.status == fb.FHGS_ERR_INVALID
+    with pytest.raises(fb.FhgsError):
+        fb.render(gp3.ctx, gp3.g, c3, gp3.prm, gp3.vs, None)
+    # (d) n = 0
+    empty = inputs.Scene(scene.mean[:0], scene.scale[:0], scene.quat[:0], scene.opacity[:0], scene.sh[:0],
+                         scene.feat[:0], scene.sh_degree)
+    gp4 = pu.GpuPath(empty, 64, 64, 16)
+    c4, m4 = gp4.project_sort(cam)
+    assert m4 == 0
+    # (e) RGB-only render (no features) equals the RGB of the feature render
+    g_full = gp3.render(c3)
+    g_rgb = gp3.render(c3, with_feat=False)
+    assert np.array_equal(g_full["rgb"], g_rgb["rgb"]) and np.array_equal(g_full["n"], g_rgb["n"])
+    # (f) determinism of P, S, R
+    g_again = gp3.render(c3)
+    for k in ("rgb", "feat", "T", "n"):
+        assert np.array_equal(g_full[k], g_again[k])
+
+
+def test_constant_map_and_l2norm():
+    """north_star pin on the GPU path: a constant GT map fuses to that constant; L2NORM normalises."""
+    cfg = inputs.CONFIGS["tiny"]
+    scene = inputs.make_scene(cfg)
+    cam = inputs.make_camera(cfg, 2)
+    gp = pu.GpuPath(scene, 64, 64, 8192)
+    c, m = gp.project_sort(cam)
+    v = np.linspace(-2.0, 3.0, cfg.feat_dim).astype(np.float32)
+    gt = np.broadcast_to(v, (64, 64, cfg.feat_dim)).copy()
+    num, den = gp.fuse(c, gt)
+    f = gp.finalize(num, den, scene.feat)
+    seen = den.cpu().numpy() > 1e-6
+    assert seen.sum() > 100
+    assert np.abs(f[seen] - v).max() <= 1e-4
+    fn = gp.finalize(num, den, scene.feat, l2norm=True)
+    assert np.abs(fn[seen] - v / np.linalg.norm(v)).max() <= 1e-4
