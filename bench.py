@@ -1,0 +1,386 @@
+#!/usr/bin/env python
+"""bench.py -- rendered+fused frames/s of the FHGS hot path on the Mid workload (BASELINE.json
+configs[2]: N = 10^6 Gaussians, SH degree 3, D = 128 fp32 unit features, one 1920x1080 view, one
+1920x1080x128 fp32 GT feature map; seeded synthetic inputs, recipe in DESIGN.md).
+
+A "step" = one frame = fhgs_project -> fhgs_bin_sort -> fhgs_render (RGB + D features) ->
+fhgs_fuse_features (clear, accumulate one GT map, finalise), all through the C ABI.
+
+    python bench.py --gpus N --steps K --warmup W            # the CUDA path (one rank per GPU)
+    python bench.py --impl reference --steps K --warmup W    # the CPU oracle on host cores
+
+Prints ONE JSON line (see DESIGN.md "Measurement" for every field).  N > 1 (torchrun): frames are
+independent units, each rank renders and fuses its own frame (camera k = rank of an 8-camera
+circle), no data-path collective; `value` = frames of all ranks / max-over-ranks time ("weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "rendered+fused frames/s at 1080p D=128"
+UNIT = "frames/s"
+FP32_LANES_PER_SM = 128
+L2_BYTES = 126 * 2 ** 20
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+# --------------------------------------------------------------------------------------------------
+# clocks: nvidia-smi sampled DURING the timed region
+# --------------------------------------------------------------------------------------------------
+class ClockSampler:
+    QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+             "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+             "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.proc = None
+        self.gpu = gpu_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu), f"--query-gpu={self.QUERY}",
+                                          "--format=csv,noheader,nounits", "-lms", "50"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.06)
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------------------------------
+# the oracle arm (cpu_baseline and --impl reference): a bounded sample = a centred, tile-aligned
+# crop of the Mid frame (same scene, same camera, principal point shifted)
+# --------------------------------------------------------------------------------------------------
+class OracleSample:
+    def __init__(self, scene, cfg, cam, crop_w, crop_h):
+        from oracle import fhgs_oracle as fo
+        from paper_2505_19154_b200 import inputs
+        self.fo, self.scene, self.cfg = fo, scene, cfg
+        fo.lib()
+        x0 = (cfg.width - crop_w) // 2 // 16 * 16
+        y0 = (cfg.height - crop_h) // 2 // 16 * 16
+        self.cam = inputs.crop_camera(cam, x0, y0, crop_w, crop_h)
+        self.w, self.h = crop_w, crop_h
+        self.frac = (crop_w * crop_h) / float(cfg.width * cfg.height)
+        self.feat32 = np.ascontiguousarray(scene.feat, dtype=np.float32)
+        rng = np.random.default_rng(cfg.seed * 1000 + 999)
+        g = rng.standard_normal((crop_h, crop_w, cfg.feat_dim), dtype=np.float32)
+        g /= np.maximum(np.sqrt((g * g).sum(axis=-1, keepdims=True)), 1e-30)
+        self.gt = g
+        self.desc = (f"oracle P+S+R+F on the centred {crop_w}x{crop_h} crop of the 1920x1080 Mid frame (all N=10^6 "
+                     f"Gaussians projected, {self.frac:.4f} of the pixels); frames/s = 1 / (t_P + (t_S+t_R+t_F)/{self.frac:.4f})")
+
+    def step(self) -> float:
+        """One sample; returns the extrapolated seconds per FULL frame."""
+        fo, s, c = self.fo, self.scene, self.cam
+        t0 = time.perf_counter()
+        pr = fo.project(s.mean, s.scale, s.quat, s.opacity, s.sh, s.sh_degree, fo.cam_array(c.view, c.proj, c.cam_pos),
+                        c.width, c.height)
+        t1 = time.perf_counter()
+        fo.bins(pr, c.width, c.height)
+        order = fo.global_order(pr)
+        fo.render_scatter(pr, order, self.feat32, c.width, c.height)
+        num, den = fo.fuse(pr, order, self.gt, c.width, c.height)
+        fo.finalize(num, den, self.feat32)
+        t2 = time.perf_counter()
+        return (t1 - t0) + (t2 - t1) / self.frac
+
+
+def run_reference(args, rank: int):
+    """--impl reference: the oracle, as it stands, on the host cores; rank 0 only."""
+    if rank != 0:
+        return
+    from oracle import fhgs_oracle as fo
+    from paper_2505_19154_b200 import inputs
+    fo.build()
+    cfg = inputs.CONFIGS["mid"]
+    scene = inputs.make_scene(cfg)
+    cam = inputs.make_camera(cfg, 0)
+    smp = OracleSample(scene, cfg, cam, 480, 272)
+    for _ in range(args.warmup):
+        smp.step()
+    t0 = time.perf_counter()
+    per_frame = [smp.step() for _ in range(args.steps)]
+    wall = time.perf_counter() - t0
+    sec = sum(per_frame) / len(per_frame)
+    val = 1.0 / sec
+    cores = fo.num_threads()
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": 0, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * wall / args.steps, "ms_per_frame_extrapolated": 1e3 * sec,
+            "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "mid: N=1e6 SH3 D=128 f32, 1 view 1920x1080 + one 1920x1080x128 GT map",
+                       "sample": smp.desc},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": smp.desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# --------------------------------------------------------------------------------------------------
+# the CUDA arm
+# --------------------------------------------------------------------------------------------------
+def launches_per_frame(width: int, height: int) -> int:
+    """Kernels of libfhgs.so launched per frame (default sort schedule): project 1; bin_sort =
+    presort_init 1 + hist_scan 1 + 4 depth onesweep passes + offsets scan 1 + scan_dup 1 +
+    hist_scan 1 + ceil(tile_bits/8) tile-id onesweep passes + ranges 1; render 1; fuse 1 + finalise 1."""
+    tiles = ((width + 15) // 16) * ((height + 15) // 16)
+    tile_bits = max(1, (tiles - 1).bit_length())
+    return 1 + (1 + 1 + 4 + 1 + 1 + 1 + (tile_bits + 7) // 8 + 1) + 1 + 2
+
+
+def run_cuda(args, rank: int, world: int, local_rank: int):
+    import torch
+    import torch.distributed as dist
+    from paper_2505_19154_b200 import binding as fb   # fails loudly without libfhgs.so
+    from paper_2505_19154_b200 import inputs
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the FHGS path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    peaks = load_peaks()
+
+    cfg = inputs.CONFIGS["mid"]
+    if args.small:   # debugging aid only; never a bench line
+        cfg = inputs.scaled(cfg, n=100_000, width=640, height=368, log_scale_mu=-3.5)
+    scene = inputs.make_scene(cfg)
+    cam_np = inputs.make_camera(cfg, 0) if rank == 0 else inputs.circle_camera(rank % 8, 8, cfg.width, cfg.height)
+    gt_np = inputs.make_gt_map(cfg, rank, cam_np)
+    W, H, D, n = cfg.width, cfg.height, cfg.feat_dim, scene.n
+    capacity = int(40e6) if not args.small else int(8e6)
+
+    ctx = fb.Context(local_rank)
+    g = fb.Gaussians(scene.mean, scene.scale, scene.quat, scene.opacity, scene.sh, scene.feat, scene.sh_degree, device=dev)
+    vs = fb.ViewState(n, W, H, capacity, device=dev)
+    prm = fb.default_params()
+    cam = fb.make_camera(cam_np.view, cam_np.proj, cam_np.cam_pos, W, H)
+    f32 = torch.float32
+    gt = torch.from_numpy(gt_np).to(dev)
+    out_rgb = torch.empty((H, W, 3), dtype=f32, device=dev)
+    out_feat = torch.empty((H, W, D), dtype=f32, device=dev)
+    out_T = torch.empty((H, W), dtype=f32, device=dev)
+    out_n = torch.empty((H, W), dtype=torch.int32, device=dev)
+    num = torch.zeros((n, D), dtype=f32, device=dev)
+    den = torch.zeros((n,), dtype=f32, device=dev)
+    fused = g.feat.clone()
+    stream = torch.cuda.current_stream()
+
+    NAMES = ["project", "bin_sort", "render", "fuse_zero", "fuse_accumulate", "fuse_finalize"]
+
+    def frame(evs=None):
+        def mark(i):
+            if evs is not None:
+                evs[i].record(stream)
+        mark(0)
+        fb.project(ctx, g, cam, prm, vs)
+        mark(1)
+        fb.bin_sort(ctx, cam, vs, sync=False)
+        mark(2)
+        fb.render(ctx, g, cam, prm, vs, out_rgb, out_feat, out_T, out_n)
+        mark(3)
+        fb.fuse_features(ctx, None, prm, vs, None, num, den, None, fb.FHGS_FUSE_ZERO_ONLY)
+        mark(4)
+        fb.fuse_features(ctx, cam, prm, vs, gt, num, den, None, 0)
+        mark(5)
+        fb.fuse_features(ctx, None, prm, vs, None, num, den, fused, fb.FHGS_FUSE_FINALIZE_ONLY)
+        mark(6)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # capacity check once, outside the timed region
+    fb.project(ctx, g, cam, prm, vs)
+    M = fb.bin_sort(ctx, cam, vs, sync=True)
+
+    for _ in range(max(args.warmup, 3)):
+        frame()
+    barrier()
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(7)] for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    barrier()
+    for k in range(args.steps):
+        frame(evs[k])
+    barrier()
+    clocks = sampler.stop()
+    total_ms = evs[0][0].elapsed_time(evs[-1][6])
+    if world > 1:
+        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * args.steps / (total_ms * 1e-3)
+    parts = {nm: statistics.mean(evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(args.steps))
+             for i, nm in enumerate(NAMES)}
+
+    # ---- algorithmic work of this frame, from the path's integer outputs
+    n_contrib_total = int(out_n.view(torch.int32).to(torch.int64).sum().item())
+    n_vis = int((vs.tiles_touched.view(torch.int32) != 0).sum().item())
+    K = (scene.sh_degree + 1) ** 2
+    tiles = ((W + 15) // 16) * ((H + 15) // 16)
+    tile_bits = max(1, (tiles - 1).bit_length())
+    p_full = (32 + tile_bits + 7) // 8
+    work = {
+        # contributor-only lane-ops: 7 (q) + 8 (alpha, w, T, RGB) + D feature FMAs per (pixel, contributor)
+        "render_lane_ops": (7 + 8 + D) * n_contrib_total,
+        "fuse_lane_ops": (7 + 6 + D) * n_contrib_total,
+        "fuse_bytes": W * H * D * 4,                                      # the GT map, read once
+        "project_bytes": 44 * n + 12 * K * n_vis + 16 * n + 40 * n_vis,
+        "bin_sort_bytes": (4 * n + 12 * n_vis + 4 * n + 12 * M) + (8 * M + p_full * 24 * M) + (8 * M + 8 * tiles),
+        "finalize_bytes": n * 4 + 2 * n_vis * D * 4,
+    }
+    ffma_ops, _ = ctx.ffma_peak(2048)
+    alu_nominal = 148 * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6       # lane-ops/s at max clock
+    steps_roof = {}
+    for nm, ops in (("render", work["render_lane_ops"]), ("fuse_accumulate", work["fuse_lane_ops"])):
+        ach = 2.0 * ops / (parts[nm] * 1e-3) / 1e12
+        steps_roof[nm] = {"bound": "alu", "achieved": ach, "peak": 2.0 * alu_nominal / 1e12, "unit": "TFLOP/s",
+                          "frac": ach / (2.0 * alu_nominal / 1e12), "ms": parts[nm],
+                          "frac_of_measured_ffma": 2.0 * ops / (parts[nm] * 1e-3) / (2.0 * ffma_ops)}
+    for nm, by in (("project", work["project_bytes"]), ("bin_sort", work["bin_sort_bytes"]),
+                   ("fuse_finalize", work["finalize_bytes"])):
+        ach = by / (parts[nm] * 1e-3) / 1e9
+        steps_roof[nm] = {"bound": "hbm", "achieved": ach, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                          "frac": ach / peaks["hbm_gbs"], "ms": parts[nm]}
+    steps_roof["fuse_accumulate"]["hbm_gbs_gt_map"] = work["fuse_bytes"] / (parts["fuse_accumulate"] * 1e-3) / 1e9
+    dominant = max(("render", "fuse_accumulate", "bin_sort", "project", "fuse_finalize"), key=lambda k: parts[k])
+    roofline = dict(steps_roof[dominant])
+    roofline["kernel"] = {"render": "render_tiled_kernel<128,float>", "fuse_accumulate": "fuse_tiled_kernel<128,float>",
+                          "bin_sort": "fhgs_bin_sort (13 launches)", "project": "project_kernel",
+                          "fuse_finalize": "finalize_kernel<float>"}[dominant]
+    roofline["peak_source"] = ("148 SMs x 128 FP32 lanes x sm_max_mhz (MEASURED_PEAKS.json), FMA = 2 flop"
+                               if roofline["bound"] == "alu" else f"hbm_gbs of MEASURED_PEAKS.json ({peaks['source']})")
+    roofline["traffic"] = None
+
+    # ---- end to end through fhgs_frame_host: host (pinned) buffers, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        host = dict(mean=pin(scene.mean), scale=pin(scene.scale), quat=pin(scene.quat), opacity=pin(scene.opacity),
+                    sh=pin(scene.sh), feat=pin(scene.feat), gt=pin(gt_np),
+                    out_rgb=torch.empty((H, W, 3), dtype=f32).pin_memory(),
+                    out_feat=torch.empty((H, W, D), dtype=f32).pin_memory(),
+                    fused_feat=torch.empty((n, D), dtype=f32).pin_memory())
+        ws = dict(out_rgb=out_rgb, out_feat=out_feat, gt=gt, num=num, den=den, fused_feat=fused)
+        h2d = sum(host[k].numel() * host[k].element_size() for k in ("mean", "scale", "quat", "opacity", "sh", "feat", "gt"))
+        d2h = sum(host[k].numel() * host[k].element_size() for k in ("out_rgb", "out_feat", "fused_feat")) + 8
+        e_steps = max(3, min(args.steps, 10))
+        for _ in range(2):
+            fb.frame_host(ctx, host, g, cam, prm, vs, ws)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e_steps):
+            fb.frame_host(ctx, host, g, cam, prm, vs, ws)   # synchronises the stream before returning
+        barrier()
+        e_s = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([e_s], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e_s = float(t.item())
+        e2e = {"value": world * e_steps / e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+               "steps": e_steps, "ms_per_step": 1e3 * e_s / e_steps}
+        del host
+
+    cpu_baseline = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import fhgs_oracle as fo   # the one place bench.py's CUDA arm runs the oracle
+        fo.build()
+        smp = OracleSample(scene, cfg, cam_np, min(960, W), min(544, H))
+        sec = smp.step()
+        cpu_baseline = {"value": 1.0 / sec, "unit": UNIT, "cores": fo.num_threads(), "kind": "oracle", "sample": smp.desc,
+                        "seconds_per_frame_extrapolated": sec}
+
+    if rank == 0:
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": f"mid: N={n} SH{scene.sh_degree} D={D} f32, 1 view {W}x{H} + one {W}x{H}x{D} GT map"
+                                       + (" [--small debug size, not a bench line]" if args.small else ""),
+                           "instances_M": M, "visible": n_vis, "contributors_per_px": n_contrib_total / (W * H),
+                           "l2": "no flush: inputs larger than L2 (GT map %.2f GB, feat %.2f GB, pairs %.2f GB vs 126 MB)"
+                                 % (gt.numel() * 4 / 1e9, g.feat.numel() * 4 / 1e9, 12 * M / 1e9),
+                           "parallelism": f"{world} independent frame(s), one per GPU"},
+                "ms": parts, "roofline": roofline, "roofline_steps": steps_roof,
+                "ffma_peak_measured_tflops": 2.0 * ffma_ops / 1e12,
+                "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches_per_frame(W, H) * args.steps,
+                "clocks": clocks}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--small", action="store_true", help="debug-size workload (not a bench line)")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    if world == 1 and args.gpus > 1:
+        sys.stderr.write("bench.py: --gpus N > 1 must be launched with torch.distributed.run (one rank per GPU); "
+                         "running rank 0 only\n")
+    run_cuda(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -174,14 +174,17 @@ FHGS_API fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const f
  * out_feat[i,:] = num[i,:]/den[i] for every i with den[i] > den_eps and leaves other rows of
  * out_feat untouched; FHGS_FUSE_L2NORM additionally divides finalised rows by their L2 norm
  * (PAPER.md:136 unit-norm features; off by default).  FHGS_FUSE_FINALIZE_ONLY skips the
- * accumulation of a view (gt, cam may then be NULL) and only finalises.
+ * accumulation of a view (gt, cam may then be NULL) and only finalises.  FHGS_FUSE_ZERO_ONLY
+ * clears num,den and returns (cam, gt, out_feat may be NULL) -- lets a caller time the three
+ * parts of a fused frame separately.
  * gt [H,W,D] gt_dtype, 16-byte aligned; num [n,D] f32 16-byte aligned; den [n] f32;
  * out_feat [n,D] out_dtype or NULL. */
 enum {
     FHGS_FUSE_ZERO = 1,
     FHGS_FUSE_FINALIZE = 2,
     FHGS_FUSE_L2NORM = 4,
-    FHGS_FUSE_FINALIZE_ONLY = 8
+    FHGS_FUSE_FINALIZE_ONLY = 8,
+    FHGS_FUSE_ZERO_ONLY = 16
 };
 FHGS_API fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam, const fhgs_params* prm,
                                const fhgs_view_state* vs, const void* gt, int32_t feat_dim,

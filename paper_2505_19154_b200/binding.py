@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libfhgs.so")
 FHGS_OK, FHGS_ERR_INTERNAL, FHGS_ERR_INVALID, FHGS_ERR_CAPACITY = 0, 1, 2, 3
 FHGS_F32, FHGS_F16 = 0, 1
 FHGS_SORT_FULL_KEY = 1
-FHGS_FUSE_ZERO, FHGS_FUSE_FINALIZE, FHGS_FUSE_L2NORM, FHGS_FUSE_FINALIZE_ONLY = 1, 2, 4, 8
+FHGS_FUSE_ZERO, FHGS_FUSE_FINALIZE, FHGS_FUSE_L2NORM, FHGS_FUSE_FINALIZE_ONLY, FHGS_FUSE_ZERO_ONLY = 1, 2, 4, 8, 16
 
 EXPORTS = ["fhgs_create", "fhgs_destroy", "fhgs_last_error", "fhgs_version", "fhgs_default_params",
            "fhgs_scratch_bytes", "fhgs_project", "fhgs_bin_sort", "fhgs_render", "fhgs_fuse_features",

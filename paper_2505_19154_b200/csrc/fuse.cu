@@ -321,9 +321,11 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
                                           int32_t out_dtype, uint32_t flags, void* stream) {
     if (!ctx) return FHGS_ERR_INVALID;
     if (!prm || !vs || !num || !den) FHGS_INVALID(ctx, "fhgs_fuse_features: NULL argument");
-    if (flags & ~(uint32_t)(FHGS_FUSE_ZERO | FHGS_FUSE_FINALIZE | FHGS_FUSE_L2NORM | FHGS_FUSE_FINALIZE_ONLY))
+    if (flags & ~(uint32_t)(FHGS_FUSE_ZERO | FHGS_FUSE_FINALIZE | FHGS_FUSE_L2NORM | FHGS_FUSE_FINALIZE_ONLY | FHGS_FUSE_ZERO_ONLY))
         FHGS_INVALID(ctx, "fhgs_fuse_features: unknown flag");
-    const bool accumulate = !(flags & FHGS_FUSE_FINALIZE_ONLY);
+    const bool zero_only = (flags & FHGS_FUSE_ZERO_ONLY) != 0;
+    if (zero_only && (flags & ~(uint32_t)FHGS_FUSE_ZERO_ONLY)) FHGS_INVALID(ctx, "fhgs_fuse_features: ZERO_ONLY excludes other flags");
+    const bool accumulate = !(flags & (FHGS_FUSE_FINALIZE_ONLY | FHGS_FUSE_ZERO_ONLY));
     const bool finalize = (flags & (FHGS_FUSE_FINALIZE | FHGS_FUSE_FINALIZE_ONLY)) != 0;
     fhgs_status st;
     if ((st = validate_params(ctx, prm)) != FHGS_OK) return st;
@@ -345,7 +347,7 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
     }
     cudaStream_t s = (cudaStream_t)stream;
     const size_t n = (size_t)vs->n;
-    if (flags & FHGS_FUSE_ZERO) {
+    if (flags & (FHGS_FUSE_ZERO | FHGS_FUSE_ZERO_ONLY)) {
         FHGS_CUDA(ctx, cudaMemsetAsync(num, 0, n * feat_dim * sizeof(float), s));
         FHGS_CUDA(ctx, cudaMemsetAsync(den, 0, n * sizeof(float), s));
     }

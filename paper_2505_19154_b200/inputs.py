@@ -132,6 +132,23 @@ def orbit_camera(v: int, cfg: Config) -> Camera:
     return look_at_camera(pos, target, cfg.width, cfg.height)
 
 
+def crop_camera(cam: Camera, x0: int, y0: int, width: int, height: int) -> Camera:
+    """The same pinhole camera restricted to the pixel window [x0,x0+width) x [y0,y0+height): fx, fy
+    and the view matrix are unchanged, the principal point moves by (-x0,-y0).  Pure camera
+    bookkeeping (used for bounded oracle samples of a large frame)."""
+    w, h = cam.width, cam.height
+    proj = cam.proj.astype(np.float64).reshape(4, 4).copy()
+    fx = proj[0, 0] * w / 2.0
+    fy = proj[1, 1] * h / 2.0
+    cx = (proj[0, 2] + 1.0) * w / 2.0 - 0.5 - x0
+    cy = (proj[1, 2] + 1.0) * h / 2.0 - 0.5 - y0
+    proj[0, 0] = 2.0 * fx / width
+    proj[1, 1] = 2.0 * fy / height
+    proj[0, 2] = 2.0 * (cx + 0.5) / width - 1.0
+    proj[1, 2] = 2.0 * (cy + 0.5) / height - 1.0
+    return Camera(cam.view.copy(), proj.astype(np.float32).reshape(16), cam.cam_pos.copy(), int(width), int(height))
+
+
 def make_camera(cfg: Config, view_idx: int) -> Camera:
     if cfg.gt_kind == "blobs":
         return orbit_camera(view_idx, cfg)
