@@ -15,7 +15,8 @@
 // D > DC is handled by channel passes (the traversal is repeated per pass; RGB/T/n are written by
 // pass 0).  Small D (not a multiple of 64) uses the per-pixel variant: CH accumulators per thread,
 // updated inside phase B from broadcast shared-memory reads.
-#include "traverse.cuh"
+#include "layout.cuh"
+#include "ws.cuh"
 
 namespace {
 
@@ -31,7 +32,7 @@ struct RenderArgs {
     uint32_t* out_n;
 };
 
-constexpr int R_KB = 64;   // staged instances per sub-batch
+constexpr int R_KB = 64;   // staged instances per drain of the per-pixel variant
 
 template <typename FT> struct FeatIO;
 template <> struct FeatIO<float> {
@@ -55,140 +56,206 @@ template <> struct FeatIO<__half> {
 };
 
 // ---------------------------------------------------------------------------------------------
-// TILED variant: DC in {64,128}
+// TILED variant (DC in {64,128}): warp-specialised persistent pipeline (ws.cuh)
 // ---------------------------------------------------------------------------------------------
+constexpr int R_STAGES = 3;
+
 template <int DC, typename FT>
-struct TiledSmem {
-    TileQueue q;
-    float4 rgb[TR_QCAP];                       // staged colours (xyz used)
-    __align__(16) float W[R_KB * TR_THREADS];  // W[kk][slot]
-    __align__(16) FT F[R_KB * DC];             // feature rows of the sub-batch
+struct RenderWsSmem {
+    WsCtrl<R_STAGES> ct;
+    float4 rgb[WS_QCAP];                                   // staged colours (xyz used)
+    __align__(128) float W[R_STAGES][WS_KB * WS_CONS];     // W[s][kk][slot]
+    __align__(128) FT F[R_STAGES][WS_KB * DC];             // feature rows of the batch
 };
 
 template <int DC, typename FT>
-__global__ void __launch_bounds__(TR_THREADS, 1) render_tiled_kernel(const RenderArgs a) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    TiledSmem<DC, FT>& sm = *reinterpret_cast<TiledSmem<DC, FT>*>(smem_raw);
-    constexpr int NJ = DC / 32;                // float4 groups of channels per thread
-    constexpr int CPR = DC * (int)sizeof(FT) / 16;   // 16-byte chunks per feature row
-
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int tile = blockIdx.x;
-    const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
-    int sx, sy;
-    slot_to_xy(tid, sx, sy);
-    const int px = tx0 + sx, py = ty0 + sy;
-    const bool inside = px < a.t.W && py < a.t.H;
-    const float fx = (float)px, fy = (float)py;
-    const float bx0 = (float)tx0, by0 = (float)ty0;
-    const float bx1 = (float)min(tx0 + FHGS_TILE - 1, a.t.W - 1), by1 = (float)min(ty0 + FHGS_TILE - 1, a.t.H - 1);
-    const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
+__device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, const RenderArgs& a, const WsWork& wk) {
+    const int p = threadIdx.x - WS_CONS, lane = p & 31, pw = p >> 5;
+    const int slot0 = (2 * pw) * 32 + lane, slot1 = slot0 + 32;
     const FT* feat = reinterpret_cast<const FT*>(a.feat);
-    FT* out_feat = reinterpret_cast<FT*>(a.out_feat);
-
-    // phase-C coordinates: 8 pixels (one row run) x NJ*4 channels
-    const int pgl = lane >> 3, cg = lane & 7;
-    const int pg = warp * 4 + pgl;
-
-    for (int c0 = 0; c0 < a.D; c0 += DC) {
-        float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
-        uint32_t n = 0;
-        bool done = !inside;
-        float acc[8][NJ * 4];
-#pragma unroll
-        for (int i = 0; i < 8; ++i)
-#pragma unroll
-            for (int j = 0; j < NJ * 4; ++j) acc[i][j] = 0.f;
+    const float q_cutoff = a.t.q_cutoff, alpha_max = a.t.alpha_max, t_min = a.t.t_min;
+    int stage = 0;
+    uint32_t phase = 0;
+    while (true) {
+        const int item = ws_next_item(sm.ct, wk, p);
+        if (item >= wk.n_items) {
+            mbar_wait(&sm.ct.empty[stage], phase ^ 1u);
+            if (p == 0) sm.ct.meta[stage] = WsMeta{0, -1, 0, WS_FLAG_EXIT};
+            mbar_arrive(&sm.ct.full[stage]);
+            break;
+        }
+        const int tile = item / wk.n_chunks, c0 = (item % wk.n_chunks) * DC;
+        const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
+        int sx, sy;
+        slot_to_xy(slot0, sx, sy);
+        const int px0 = tx0 + sx, py0 = ty0 + sy;
+        slot_to_xy(slot1, sx, sy);
+        const int px1 = tx0 + sx, py1 = ty0 + sy;
+        const bool in0 = px0 < a.t.W && py0 < a.t.H, in1 = px1 < a.t.W && py1 < a.t.H;
+        WsPixel P0{(float)px0, (float)py0, 1.f, 0u, !in0}, P1{(float)px1, (float)py1, 1.f, 0u, !in1};
+        float C00 = 0.f, C01 = 0.f, C02 = 0.f, C10 = 0.f, C11 = 0.f, C12 = 0.f;
+        const float bx0 = (float)tx0, by0 = (float)ty0;
+        const float bx1 = (float)min(tx0 + FHGS_TILE - 1, a.t.W - 1), by1 = (float)min(ty0 + FHGS_TILE - 1, a.t.H - 1);
+        const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
         uint32_t pos = range.x;
-        int q_head = 0, q_count = 0;
-
-        while (true) {
-            while (q_count < R_KB && pos < range.y) {
-                const int tail = q_head + q_count;
-                const int added = stage_chunk(a.t, sm.q, pos, range.y, tail, bx0, by0, bx1, by1);
-                // colours of the survivors just appended (slots tail .. tail+added)
-                for (int k = tid; k < added; k += TR_THREADS) {
-                    const int s = (tail + k) & (TR_QCAP - 1);
-                    const uint32_t id = sm.q.id[s];
-                    sm.rgb[s] = make_float4(__ldg(a.rgb_g + 3 * (size_t)id), __ldg(a.rgb_g + 3 * (size_t)id + 1),
-                                            __ldg(a.rgb_g + 3 * (size_t)id + 2), 0.f);
+        int qh = 0, qt = 0;
+        WsChunk ch;
+        ws_chunk_prefetch_id(a.t, pos, range.y, p, ch);
+        ws_chunk_issue(a.t, a.rgb_g, ch);
+        ws_chunk_prefetch_id(a.t, pos + WS_PROD, range.y, p, ch);
+        bool last = false;
+        do {
+            while (qt - qh < WS_KB && pos < range.y) {
+                qt += ws_chunk_append(sm.ct, ch, qt, bx0, by0, bx1, by1, q_cutoff, p,
+                                      [&](int s, const WsChunk& c) { sm.rgb[s] = make_float4(c.r, c.gr, c.b, 0.f); });
+                pos += WS_PROD;
+                ws_chunk_issue(a.t, a.rgb_g, ch);
+                ws_chunk_prefetch_id(a.t, pos + WS_PROD, range.y, p, ch);
+            }
+            const int nb = min(WS_KB, qt - qh);
+            mbar_wait(&sm.ct.empty[stage], phase ^ 1u);
+            // feature rows of the batch: one bulk async copy each, counted on full[stage]
+            if (pw == 0 && lane < nb) {
+                const uint32_t id = __float_as_uint(sm.ct.rec1[(qh + lane) & (WS_QCAP - 1)].z);
+                mbar_expect_tx(&sm.ct.full[stage], (uint32_t)(DC * sizeof(FT)));
+                bulk_g2s(&sm.F[stage][lane * DC], feat + (size_t)id * a.D + c0, (uint32_t)(DC * sizeof(FT)), &sm.ct.full[stage]);
+            }
+            // weights of the batch for this thread's two pixels
+            uint32_t m0 = 0u, m1 = 0u;
+            float* Wd = sm.W[stage];
+            if (!__all_sync(TR_FULL, P0.done && P1.done)) {
+#pragma unroll 2
+                for (int kk = 0; kk < nb; ++kk) {
+                    const int s = (qh + kk) & (WS_QCAP - 1);
+                    const float4 r0 = sm.ct.rec0[s];
+                    const float4 r1 = sm.ct.rec1[s];
+                    const float w0 = ws_weight(r0, r1.x, r1.y, P0, q_cutoff, alpha_max, t_min);
+                    const float w1 = ws_weight(r0, r1.x, r1.y, P1, q_cutoff, alpha_max, t_min);
+                    Wd[kk * WS_CONS + slot0] = w0;
+                    Wd[kk * WS_CONS + slot1] = w1;
+                    const bool nz0 = w0 != 0.f, nz1 = w1 != 0.f;
+                    if (nz0 || nz1) {
+                        const float4 c = sm.rgb[s];
+                        C00 = fmaf(w0, c.x, C00); C01 = fmaf(w0, c.y, C01); C02 = fmaf(w0, c.z, C02);
+                        C10 = fmaf(w1, c.x, C10); C11 = fmaf(w1, c.y, C11); C12 = fmaf(w1, c.z, C12);
+                    }
+                    if (__any_sync(TR_FULL, nz0)) m0 |= 1u << kk;
+                    if (__any_sync(TR_FULL, nz1)) m1 |= 1u << kk;
                 }
-                q_count += added;
-                pos += TR_THREADS;
             }
-            const int nb = min(R_KB, q_count);
-            if (nb == 0) break;
-            __syncthreads();   // staged colours visible; previous phase C finished with W/F
-            // async fetch of the sub-batch's feature rows
-            for (int c = tid; c < nb * CPR; c += TR_THREADS) {
-                const int row = c / CPR, ch = c % CPR;
-                const uint32_t id = sm.q.id[(q_head + row) & (TR_QCAP - 1)];
-                cp_async16(reinterpret_cast<unsigned char*>(sm.F) + (size_t)row * DC * sizeof(FT) + ch * 16,
-                           reinterpret_cast<const unsigned char*>(feat + (size_t)id * a.D + c0) + ch * 16);
+            if (lane == 0) {
+                sm.ct.mask[stage][2 * pw] = m0;
+                sm.ct.mask[stage][2 * pw + 1] = m1;
             }
-            // phase B
-            unsigned long long any_mask = 0ull;
-            for (int kk = 0; kk < nb; ++kk) {
-                const int s = (q_head + kk) & (TR_QCAP - 1);
-                const float w = eval_weight(sm.q.xy[s], sm.q.co[s], fx, fy, a.t, T, done, n);
-                if (w != 0.f) {
-                    const float4 c = sm.rgb[s];
-                    C0 = fmaf(w, c.x, C0); C1 = fmaf(w, c.y, C1); C2 = fmaf(w, c.z, C2);
-                }
-                sm.W[kk * TR_THREADS + tid] = w;
-                if (__any_sync(TR_FULL, w != 0.f)) any_mask |= 1ull << kk;
+            qh += nb;
+            const bool all_done = named_bar_and(WS_BAR_PROD_RED, WS_PROD, P0.done && P1.done);
+            last = all_done || (pos >= range.y && qt == qh);
+            if (p == 0) sm.ct.meta[stage] = WsMeta{nb, tile, c0, last ? WS_FLAG_LAST : 0};
+            mbar_arrive(&sm.ct.full[stage]);
+            if (++stage == R_STAGES) { stage = 0; phase ^= 1u; }
+        } while (!last);
+        if (c0 == 0) {
+            if (in0) {
+                const size_t o = (size_t)py0 * a.t.W + px0;
+                a.out_rgb[3 * o] = fmaf(P0.T, a.bg[0], C00);
+                a.out_rgb[3 * o + 1] = fmaf(P0.T, a.bg[1], C01);
+                a.out_rgb[3 * o + 2] = fmaf(P0.T, a.bg[2], C02);
+                if (a.out_T) a.out_T[o] = P0.T;
+                if (a.out_n) a.out_n[o] = P0.n;
             }
-            cp_async_wait_all();
-            __syncthreads();
-            // phase C
-            for (int kk = 0; kk < nb; ++kk) {
-                if (!((any_mask >> kk) & 1ull)) continue;
-                const float4 wa = *reinterpret_cast<const float4*>(&sm.W[kk * TR_THREADS + pg * 8]);
-                const float4 wb = *reinterpret_cast<const float4*>(&sm.W[kk * TR_THREADS + pg * 8 + 4]);
-                const float wv[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
-                float fv[NJ * 4];
-#pragma unroll
-                for (int j = 0; j < NJ; ++j) {
-                    const float4 f = FeatIO<FT>::load4(&sm.F[kk * DC + j * 32 + cg * 4]);
-                    fv[4 * j] = f.x; fv[4 * j + 1] = f.y; fv[4 * j + 2] = f.z; fv[4 * j + 3] = f.w;
-                }
-#pragma unroll
-                for (int i = 0; i < 8; ++i)
-#pragma unroll
-                    for (int j = 0; j < NJ * 4; ++j) acc[i][j] = fmaf(wv[i], fv[j], acc[i][j]);
+            if (in1) {
+                const size_t o = (size_t)py1 * a.t.W + px1;
+                a.out_rgb[3 * o] = fmaf(P1.T, a.bg[0], C10);
+                a.out_rgb[3 * o + 1] = fmaf(P1.T, a.bg[1], C11);
+                a.out_rgb[3 * o + 2] = fmaf(P1.T, a.bg[2], C12);
+                if (a.out_T) a.out_T[o] = P1.T;
+                if (a.out_n) a.out_n[o] = P1.n;
             }
-            q_head = (q_head + nb) & (TR_QCAP - 1);
-            q_count -= nb;
-            if (__syncthreads_and(done)) break;
         }
+    }
+}
 
-        if (c0 == 0 && inside) {
-            const size_t p = (size_t)py * a.t.W + px;
-            a.out_rgb[3 * p] = fmaf(T, a.bg[0], C0);
-            a.out_rgb[3 * p + 1] = fmaf(T, a.bg[1], C1);
-            a.out_rgb[3 * p + 2] = fmaf(T, a.bg[2], C2);
-            if (a.out_T) a.out_T[p] = T;
-            if (a.out_n) a.out_n[p] = n;
+template <int DC, typename FT>
+__device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT>& sm, const RenderArgs& a) {
+    constexpr int NJ = DC / 32;   // float4 channel groups per thread
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int pgl = lane >> 3, cg = lane & 7;
+    const int pg = warp * 4 + pgl;   // 8-pixel row run: slots pg*8 .. pg*8+7
+    FT* out_feat = reinterpret_cast<FT*>(a.out_feat);
+    float acc[8][NJ * 4];
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+#pragma unroll
+        for (int j = 0; j < NJ * 4; ++j) acc[i][j] = 0.f;
+    int stage = 0;
+    uint32_t phase = 0;
+    while (true) {
+        mbar_wait(&sm.ct.full[stage], phase);
+        const WsMeta m = sm.ct.meta[stage];
+        if (m.flags & WS_FLAG_EXIT) break;
+        uint32_t mk = sm.ct.mask[stage][warp];
+        const float* Ws = sm.W[stage] + pg * 8;
+        const FT* Fs = sm.F[stage] + cg * 4;
+        while (mk) {
+            const int kk = __ffs(mk) - 1;
+            mk &= mk - 1u;
+            const float4 wa = *reinterpret_cast<const float4*>(Ws + kk * WS_CONS);
+            const float4 wb = *reinterpret_cast<const float4*>(Ws + kk * WS_CONS + 4);
+            const float wv[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
+            float fv[NJ * 4];
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) {
+                const float4 f = FeatIO<FT>::load4(Fs + kk * DC + j * 32);
+                fv[4 * j] = f.x; fv[4 * j + 1] = f.y; fv[4 * j + 2] = f.z; fv[4 * j + 3] = f.w;
+            }
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < NJ * 4; ++j) acc[i][j] = fmaf(wv[i], fv[j], acc[i][j]);
         }
-        // feature output: this thread's 8 pixels are slots pg*8 .. pg*8+7 = one row run of 8
-        {
+        mbar_arrive(&sm.ct.empty[stage]);
+        if (++stage == R_STAGES) { stage = 0; phase ^= 1u; }
+        if (m.flags & WS_FLAG_LAST) {
+            const int tx0 = (m.tile % a.t.GW) * FHGS_TILE, ty0 = (m.tile / a.t.GW) * FHGS_TILE;
             const int oy = ty0 + ((warp >> 1) << 2) + pgl;
             const int ox0 = tx0 + ((warp & 1) << 3);
-            if (oy < a.t.H) {
 #pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    const int ox = ox0 + i;
-                    if (ox < a.t.W) {
-                        FT* dst = out_feat + ((size_t)oy * a.t.W + ox) * a.D + c0;
+            for (int i = 0; i < 8; ++i) {
+                const int ox = ox0 + i;
+                if (oy < a.t.H && ox < a.t.W) {
+                    FT* dst = out_feat + ((size_t)oy * a.t.W + ox) * a.D + m.c0 + cg * 4;
 #pragma unroll
-                        for (int j = 0; j < NJ; ++j)
-                            FeatIO<FT>::store4(dst + j * 32 + cg * 4, make_float4(acc[i][4 * j], acc[i][4 * j + 1],
-                                                                                  acc[i][4 * j + 2], acc[i][4 * j + 3]));
-                    }
+                    for (int j = 0; j < NJ; ++j)
+                        FeatIO<FT>::store4(dst + j * 32, make_float4(acc[i][4 * j], acc[i][4 * j + 1], acc[i][4 * j + 2], acc[i][4 * j + 3]));
                 }
+#pragma unroll
+                for (int j = 0; j < NJ * 4; ++j) acc[i][j] = 0.f;
             }
         }
-        __syncthreads();   // ring and W/F are reused by the next channel pass
+    }
+}
+
+template <int DC, typename FT>
+__global__ void __launch_bounds__(WS_THREADS, 1) render_ws_kernel(const RenderArgs a, const WsWork wk) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    RenderWsSmem<DC, FT>& sm = *reinterpret_cast<RenderWsSmem<DC, FT>*>(smem_raw);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < R_STAGES; ++s) {
+            mbar_init(&sm.ct.full[s], WS_PROD);
+            mbar_init(&sm.ct.empty[s], WS_CONS);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+    if (threadIdx.x >= WS_CONS) {
+        setmaxnreg_dec<88>();
+        render_ws_producer<DC, FT>(sm, a, wk);
+    } else {
+        setmaxnreg_inc<200>();
+        render_ws_consumer<DC, FT>(sm, a);
+        if (threadIdx.x == 0) ws_queue_release(wk);
     }
 }
 
@@ -204,7 +271,7 @@ struct PixelSmem {
 
 template <int CH, typename FT>
 __global__ void __launch_bounds__(TR_THREADS) render_pixel_kernel(const RenderArgs a) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     PixelSmem<CH>& sm = *reinterpret_cast<PixelSmem<CH>*>(smem_raw);
 
     const int tid = threadIdx.x;
@@ -305,11 +372,25 @@ cudaError_t launch(K kernel, size_t smem, int grid, cudaStream_t st, const Rende
     return cudaGetLastError();
 }
 
+template <int DC, typename FT>
+cudaError_t launch_ws(const RenderArgs& a, int tiles, int num_sms, uint32_t* queue, cudaStream_t st) {
+    const size_t smem = sizeof(RenderWsSmem<DC, FT>);
+    cudaError_t e = cudaFuncSetAttribute(render_ws_kernel<DC, FT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    WsWork wk;
+    wk.queue = queue;
+    wk.n_chunks = a.D / DC;
+    wk.n_items = tiles * wk.n_chunks;
+    const int grid = wk.n_items < num_sms ? wk.n_items : num_sms;
+    render_ws_kernel<DC, FT><<<grid, WS_THREADS, smem, st>>>(a, wk);
+    return cudaGetLastError();
+}
+
 template <typename FT>
-cudaError_t dispatch(const RenderArgs& a, int grid, cudaStream_t st, bool has_feat) {
+cudaError_t dispatch(const RenderArgs& a, int grid, int num_sms, uint32_t* queue, cudaStream_t st, bool has_feat) {
     if (!has_feat) return launch(render_pixel_kernel<0, FT>, sizeof(PixelSmem<0>), grid, st, a);
-    if (a.D % 128 == 0) return launch(render_tiled_kernel<128, FT>, sizeof(TiledSmem<128, FT>), grid, st, a);
-    if (a.D % 64 == 0) return launch(render_tiled_kernel<64, FT>, sizeof(TiledSmem<64, FT>), grid, st, a);
+    if (a.D % 128 == 0) return launch_ws<128, FT>(a, grid, num_sms, queue, st);
+    if (a.D % 64 == 0) return launch_ws<64, FT>(a, grid, num_sms, queue, st);
     if (a.D % 16 == 0) return launch(render_pixel_kernel<16, FT>, sizeof(PixelSmem<16>), grid, st, a);
     if (a.D % 8 == 0) return launch(render_pixel_kernel<8, FT>, sizeof(PixelSmem<8>), grid, st, a);
     return launch(render_pixel_kernel<4, FT>, sizeof(PixelSmem<4>), grid, st, a);
@@ -347,8 +428,9 @@ extern "C" fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const
     a.out_rgb = out_rgb; a.out_feat = out_feat; a.out_T = out_T; a.out_n = out_ncontrib;
     const int grid = tiles_x(cam->width) * tiles_y(cam->height);
     cudaStream_t s = (cudaStream_t)stream;
-    cudaError_t e = (has_feat && g->feat_dtype == FHGS_F16) ? dispatch<__half>(a, grid, s, has_feat)
-                                                            : dispatch<float>(a, grid, s, has_feat);
+    uint32_t* queue = reinterpret_cast<uint32_t*>((char*)vs->scratch + make_scratch_layout(vs->n, vs->capacity).ctrl) + CTRL_TILE_QUEUE;
+    cudaError_t e = (has_feat && g->feat_dtype == FHGS_F16) ? dispatch<__half>(a, grid, ctx->num_sms, queue, s, has_feat)
+                                                            : dispatch<float>(a, grid, ctx->num_sms, queue, s, has_feat);
     FHGS_CUDA(ctx, e);
     return FHGS_OK;
 }

@@ -1,0 +1,219 @@
+// ws.cuh -- the warp-specialised, persistent tile pipeline shared by the tiled render and fuse kernels.
+//
+// One CTA per SM, 384 threads: warps 0-7 are CONSUMERS (the D-channel product of the step), warps
+// 8-11 are PRODUCERS (tile traversal: fetch, tile cull, blend weights w = alpha*T of PAPER.md:95).
+// The CTA pulls work items (tile, channel chunk) from an atomic queue until it is empty.
+//
+// Producer (128 threads, 2 pixels each; slot s of the 16x16 tile: warp-block = s/32 covers 8x4 px):
+//   stage   128 instances of the tile's sorted range are examined by one thread each (one chunk
+//           ahead is prefetched into registers): exact ellipse-vs-tile-box test (traverse.cuh),
+//           survivors appended in order to a shared-memory ring {xy, conic, opacity, id, rgb}.
+//   batch   up to WS_KB ring entries form a batch in pipeline stage s: one bulk async copy
+//           (cp.async.bulk, completion counted on the stage's `full` mbarrier) per feature row
+//           (render) is issued first; then every producer thread evaluates the normative q, the
+//           cut-off, alpha, w, T for its 2 pixels and parks w in W[s][kk][slot]; per warp-block
+//           bit masks say which instances gave the block any weight.
+//   signal  meta[s] = {nb, tile, chunk, flags}; all 128 producers arrive on full[s].
+// Consumer (256 threads): waits full[s], multiplies, arrives on empty[s]; on the LAST batch of an
+// item it writes its accumulators out.  Producers run ahead by up to WS_STAGES batches, across
+// tile boundaries, so global-load latency, the sequential weight phase and the FFMA-bound product
+// overlap instead of alternating.
+#pragma once
+#include "traverse.cuh"
+
+constexpr int WS_CONS = 256;
+constexpr int WS_PROD = 128;
+constexpr int WS_THREADS = WS_CONS + WS_PROD;
+constexpr int WS_KB = 32;      // instances per batch (one bit each in the 32-bit block masks)
+constexpr int WS_QCAP = 256;   // survivor ring capacity (power of two) >= WS_KB - 1 + WS_PROD
+
+enum { WS_FLAG_LAST = 1, WS_FLAG_EXIT = 2 };
+enum { WS_BAR_PROD = 1, WS_BAR_PROD_RED = 2 };   // named barriers (0 = __syncthreads)
+
+struct WsMeta {
+    int nb, tile, c0, flags;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.shared::cta.b64 st, [%0];\n\t}" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                 : "=r"(ok)
+                 : "r"(smem_u32(bar)), "r"(parity)
+                 : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) {
+    }
+}
+// 1-D bulk async copy global -> shared, completion (bytes) counted on `bar`.
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+// barrier + AND-reduction of a predicate over the participating threads
+__device__ __forceinline__ bool named_bar_and(int id, int nthreads, bool pred) {
+    uint32_t r;
+    asm volatile(
+        "{\n\t.reg .pred p, q;\n\tsetp.ne.u32 p, %1, 0;\n\tbarrier.red.and.pred q, %2, %3, p;\n\tselp.u32 %0, 1, 0, q;\n\t}"
+        : "=r"(r)
+        : "r"((uint32_t)pred), "r"(id), "r"(nthreads)
+        : "memory");
+    return r != 0;
+}
+template <int N>
+__device__ __forceinline__ void setmaxnreg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N>
+__device__ __forceinline__ void setmaxnreg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// Control block of the pipeline (lives at the front of dynamic shared memory).
+template <int STAGES>
+struct WsCtrl {
+    uint64_t full[STAGES];
+    uint64_t empty[STAGES];
+    WsMeta meta[STAGES];
+    uint32_t mask[STAGES][8];     // per warp-block: bit kk set <=> instance kk gave the block a weight
+    uint32_t wcount[WS_PROD / 32];
+    int item;                     // work item broadcast among the producers
+    float4 rec0[WS_QCAP];         // gx, gy, A, 2B
+    float4 rec1[WS_QCAP];         // C, opacity, id (bits), unused
+};
+
+struct WsWork {
+    uint32_t* queue;      // [0] next item, [1] finished CTAs (self-resetting; zero between launches)
+    int n_items;          // tiles * chunks
+    int n_chunks;
+};
+
+// Per-pixel blend state of a producer thread.
+struct WsPixel {
+    float fx, fy, T;
+    uint32_t n;
+    bool done;
+};
+
+// C1-R steps 1-4 for one (pixel, Gaussian); q is the normative binary32 expression
+// fmaf(dx, fmaf(2B, dy, A dx), (C dy) dy).  Returns w (0 when the Gaussian does not contribute).
+__device__ __forceinline__ float ws_weight(const float4 r0, const float C, const float op, WsPixel& p, const float q_cutoff,
+                                           const float alpha_max, const float t_min) {
+    const float dx = __fsub_rn(r0.x, p.fx), dy = __fsub_rn(r0.y, p.fy);
+    const float q = __fmaf_rn(dx, __fmaf_rn(r0.w, dy, __fmul_rn(r0.z, dx)), __fmul_rn(__fmul_rn(C, dy), dy));
+    float w = 0.f;
+    if (!p.done && q <= q_cutoff) {
+        const float G = ex2_approx(-0.72134752044448170368f * fmaxf(q, 0.f));   // exp(-q/2)
+        const float alpha = fminf(alpha_max, op * G);
+        w = alpha * p.T;
+        p.T = fmaf(-alpha, p.T, p.T);
+        ++p.n;
+        p.done = p.T < t_min;
+    }
+    return w;
+}
+
+// Chunk of 128 instances held in registers (one per producer thread), software-pipelined two deep:
+// `id_next` (the sorted-list entry of the chunk after this one) is in flight while this chunk's
+// projected Gaussian (xy, conic, opacity, colour) is in flight, so neither dependent global load is
+// waited for at its issue point.
+struct WsChunk {
+    uint32_t id;
+    float2 g;
+    float4 co;
+    float r, gr, b;
+    bool valid;
+    uint32_t id_next;
+    bool valid_next;
+};
+
+__device__ __forceinline__ void ws_chunk_issue(const TraverseArgs& a, const float* rgb_g, WsChunk& c) {
+    // consume id_next -> issue this chunk's gathers
+    c.id = c.id_next;
+    c.valid = c.valid_next;
+    c.g = make_float2(0.f, 0.f);
+    c.co = make_float4(0.f, 0.f, 0.f, 0.f);
+    c.r = c.gr = c.b = 0.f;
+    if (c.valid) {
+        c.g = __ldg(a.xy + c.id);
+        c.co = __ldg(a.conic_opacity + c.id);
+        if (rgb_g) {
+            c.r = __ldg(rgb_g + 3 * (size_t)c.id);
+            c.gr = __ldg(rgb_g + 3 * (size_t)c.id + 1);
+            c.b = __ldg(rgb_g + 3 * (size_t)c.id + 2);
+        }
+    }
+}
+__device__ __forceinline__ void ws_chunk_prefetch_id(const TraverseArgs& a, uint32_t pos, uint32_t end, int p, WsChunk& c) {
+    const uint32_t idx = pos + (uint32_t)p;
+    c.valid_next = idx < end;
+    c.id_next = c.valid_next ? __ldg(a.vals + idx) : 0u;
+}
+
+// Tile-cull the chunk and append the survivors, in order, to the ring at q_tail.  Returns the number
+// appended (same in all producer threads).  Two producer-wide barriers.
+template <typename CTRL, typename EXTRA>
+__device__ __forceinline__ int ws_chunk_append(CTRL& ct, const WsChunk& c, int q_tail, float bx0, float by0, float bx1,
+                                               float by1, float q_cutoff, int p, EXTRA&& extra) {
+    const int lane = p & 31, pw = p >> 5;
+    float4 co = c.co;
+    co.y = 2.0f * co.y;   // exact
+    const bool keep = c.valid && tile_may_contribute(c.g, co, bx0, by0, bx1, by1, q_cutoff);
+    const uint32_t ballot = __ballot_sync(TR_FULL, keep);
+    if (lane == 0) ct.wcount[pw] = __popc(ballot);
+    named_bar_sync(WS_BAR_PROD, WS_PROD);
+    int off = 0, total = 0;
+#pragma unroll
+    for (int w = 0; w < WS_PROD / 32; ++w) {
+        const int cnt = (int)ct.wcount[w];
+        if (w < pw) off += cnt;
+        total += cnt;
+    }
+    if (keep) {
+        const int s = (q_tail + off + __popc(ballot & ((1u << lane) - 1u))) & (WS_QCAP - 1);
+        ct.rec0[s] = make_float4(c.g.x, c.g.y, co.x, co.y);
+        ct.rec1[s] = make_float4(co.z, co.w, __uint_as_float(c.id), 0.f);
+        extra(s, c);
+    }
+    named_bar_sync(WS_BAR_PROD, WS_PROD);
+    return total;
+}
+
+// Fetch the next work item for the producers (thread p == 0 pops the queue).
+template <typename CTRL>
+__device__ __forceinline__ int ws_next_item(CTRL& ct, const WsWork& wk, int p) {
+    if (p == 0) ct.item = (int)atomicAdd(wk.queue, 1u);
+    named_bar_sync(WS_BAR_PROD, WS_PROD);
+    const int item = ct.item;
+    named_bar_sync(WS_BAR_PROD, WS_PROD);
+    return item;
+}
+
+// Last CTA out resets the queue so that the next launch on this view state starts from zero.
+__device__ __forceinline__ void ws_queue_release(const WsWork& wk) {
+    __threadfence();
+    const uint32_t fin = atomicAdd(wk.queue + 1, 1u);
+    if (fin == gridDim.x - 1) {
+        wk.queue[0] = 0u;
+        wk.queue[1] = 0u;
+        __threadfence();
+    }
+}
