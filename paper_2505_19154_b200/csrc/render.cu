@@ -76,14 +76,15 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
     const float q_cutoff = a.t.q_cutoff, alpha_max = a.t.alpha_max, t_min = a.t.t_min;
     int stage = 0;
     uint32_t phase = 0;
+    int item = ws_pop_end(sm.ct, ws_pop_begin(wk, p), p);
     while (true) {
-        const int item = ws_next_item(sm.ct, wk, p);
         if (item >= wk.n_items) {
             mbar_wait(&sm.ct.empty[stage], phase ^ 1u);
             if (p == 0) sm.ct.meta[stage] = WsMeta{0, -1, 0, WS_FLAG_EXIT};
             mbar_arrive(&sm.ct.full[stage]);
             break;
         }
+        const uint32_t popped = ws_pop_begin(wk, p);   // next item, consumed at the end of this one
         const int tile = item / wk.n_chunks, c0 = (item % wk.n_chunks) * DC;
         const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
         int sx, sy;
@@ -124,24 +125,23 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
             uint32_t m0 = 0u, m1 = 0u;
             float* Wd = sm.W[stage];
             if (!__all_sync(TR_FULL, P0.done && P1.done)) {
-#pragma unroll 2
+#pragma unroll 4
                 for (int kk = 0; kk < nb; ++kk) {
                     const int s = (qh + kk) & (WS_QCAP - 1);
                     const float4 r0 = sm.ct.rec0[s];
                     const float4 r1 = sm.ct.rec1[s];
+                    const float4 c = sm.rgb[s];
                     const float w0 = ws_weight(r0, r1.x, r1.y, P0, q_cutoff, alpha_max, t_min);
                     const float w1 = ws_weight(r0, r1.x, r1.y, P1, q_cutoff, alpha_max, t_min);
                     Wd[kk * WS_CONS + slot0] = w0;
                     Wd[kk * WS_CONS + slot1] = w1;
-                    const bool nz0 = w0 != 0.f, nz1 = w1 != 0.f;
-                    if (nz0 || nz1) {
-                        const float4 c = sm.rgb[s];
-                        C00 = fmaf(w0, c.x, C00); C01 = fmaf(w0, c.y, C01); C02 = fmaf(w0, c.z, C02);
-                        C10 = fmaf(w1, c.x, C10); C11 = fmaf(w1, c.y, C11); C12 = fmaf(w1, c.z, C12);
-                    }
-                    if (__any_sync(TR_FULL, nz0)) m0 |= 1u << kk;
-                    if (__any_sync(TR_FULL, nz1)) m1 |= 1u << kk;
+                    C00 = fmaf(w0, c.x, C00); C01 = fmaf(w0, c.y, C01); C02 = fmaf(w0, c.z, C02);
+                    C10 = fmaf(w1, c.x, C10); C11 = fmaf(w1, c.y, C11); C12 = fmaf(w1, c.z, C12);
+                    m0 |= (w0 != 0.f ? 1u : 0u) << kk;
+                    m1 |= (w1 != 0.f ? 1u : 0u) << kk;
                 }
+                m0 = __reduce_or_sync(TR_FULL, m0);
+                m1 = __reduce_or_sync(TR_FULL, m1);
             }
             if (lane == 0) {
                 sm.ct.mask[stage][2 * pw] = m0;
@@ -172,6 +172,7 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
                 if (a.out_n) a.out_n[o] = P1.n;
             }
         }
+        item = ws_pop_end(sm.ct, popped, p);
     }
 }
 

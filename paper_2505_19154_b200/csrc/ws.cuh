@@ -117,17 +117,17 @@ struct WsPixel {
 // fmaf(dx, fmaf(2B, dy, A dx), (C dy) dy).  Returns w (0 when the Gaussian does not contribute).
 __device__ __forceinline__ float ws_weight(const float4 r0, const float C, const float op, WsPixel& p, const float q_cutoff,
                                            const float alpha_max, const float t_min) {
+    // branch-free: the only loop-carried chain is w = a*T; T = T - a*T (everything else pipelines)
     const float dx = __fsub_rn(r0.x, p.fx), dy = __fsub_rn(r0.y, p.fy);
     const float q = __fmaf_rn(dx, __fmaf_rn(r0.w, dy, __fmul_rn(r0.z, dx)), __fmul_rn(__fmul_rn(C, dy), dy));
-    float w = 0.f;
-    if (!p.done && q <= q_cutoff) {
-        const float G = ex2_approx(-0.72134752044448170368f * fmaxf(q, 0.f));   // exp(-q/2)
-        const float alpha = fminf(alpha_max, op * G);
-        w = alpha * p.T;
-        p.T = fmaf(-alpha, p.T, p.T);
-        ++p.n;
-        p.done = p.T < t_min;
-    }
+    const float G = ex2_approx(-0.72134752044448170368f * fmaxf(q, 0.f));   // exp(-q/2)
+    const float alpha = fminf(alpha_max, op * G);
+    const bool c = (q <= q_cutoff) && !p.done;
+    const float a = c ? alpha : 0.f;
+    const float w = a * p.T;
+    p.T = fmaf(-a, p.T, p.T);
+    p.n += c ? 1u : 0u;
+    p.done = p.done || (p.T < t_min);
     return w;
 }
 
@@ -197,10 +197,14 @@ __device__ __forceinline__ int ws_chunk_append(CTRL& ct, const WsChunk& c, int q
     return total;
 }
 
-// Fetch the next work item for the producers (thread p == 0 pops the queue).
+// Work-item queue: thread p == 0 pops; the pop for the NEXT item is issued at the start of the current
+// one (ws_pop_begin) and only consumed at its end (ws_pop_end), so its latency is hidden.
+__device__ __forceinline__ uint32_t ws_pop_begin(const WsWork& wk, int p) {
+    return p == 0 ? atomicAdd(wk.queue, 1u) : 0u;
+}
 template <typename CTRL>
-__device__ __forceinline__ int ws_next_item(CTRL& ct, const WsWork& wk, int p) {
-    if (p == 0) ct.item = (int)atomicAdd(wk.queue, 1u);
+__device__ __forceinline__ int ws_pop_end(CTRL& ct, uint32_t popped, int p) {
+    if (p == 0) ct.item = (int)popped;
     named_bar_sync(WS_BAR_PROD, WS_PROD);
     const int item = ct.item;
     named_bar_sync(WS_BAR_PROD, WS_PROD);
