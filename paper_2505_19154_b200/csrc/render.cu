@@ -70,12 +70,13 @@ struct RenderWsSmem {
 
 template <int DC, typename FT>
 __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, const RenderArgs& a, const WsWork& wk) {
-    const int p = threadIdx.x - WS_CONS, lane = p & 31, pw = p >> 5;
-    const int slot0 = (2 * pw) * 32 + lane, slot1 = slot0 + 32;
+    const int p = threadIdx.x - WS_CONS, lane = p & 31, pw = p >> 5;   // p = pixel slot, pw = warp-block
     const FT* feat = reinterpret_cast<const FT*>(a.feat);
     const float q_cutoff = a.t.q_cutoff, alpha_max = a.t.alpha_max, t_min = a.t.t_min;
     int stage = 0;
     uint32_t phase = 0;
+    int sx, sy;
+    slot_to_xy(p, sx, sy);
     int item = ws_pop_end(sm.ct, ws_pop_begin(wk, p), p);
     while (true) {
         if (item >= wk.n_items) {
@@ -87,14 +88,10 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
         const uint32_t popped = ws_pop_begin(wk, p);   // next item, consumed at the end of this one
         const int tile = item / wk.n_chunks, c0 = (item % wk.n_chunks) * DC;
         const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
-        int sx, sy;
-        slot_to_xy(slot0, sx, sy);
-        const int px0 = tx0 + sx, py0 = ty0 + sy;
-        slot_to_xy(slot1, sx, sy);
-        const int px1 = tx0 + sx, py1 = ty0 + sy;
-        const bool in0 = px0 < a.t.W && py0 < a.t.H, in1 = px1 < a.t.W && py1 < a.t.H;
-        WsPixel P0{(float)px0, (float)py0, 1.f, 0u, !in0}, P1{(float)px1, (float)py1, 1.f, 0u, !in1};
-        float C00 = 0.f, C01 = 0.f, C02 = 0.f, C10 = 0.f, C11 = 0.f, C12 = 0.f;
+        const int px = tx0 + sx, py = ty0 + sy;
+        const bool inside = px < a.t.W && py < a.t.H;
+        WsPixel P{(float)px, (float)py, 1.f, 0u, !inside};
+        float C0 = 0.f, C1 = 0.f, C2 = 0.f;
         const float bx0 = (float)tx0, by0 = (float)ty0;
         const float bx1 = (float)min(tx0 + FHGS_TILE - 1, a.t.W - 1), by1 = (float)min(ty0 + FHGS_TILE - 1, a.t.H - 1);
         const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
@@ -114,63 +111,45 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
                 ws_chunk_prefetch_id(a.t, pos + WS_PROD, range.y, p, ch);
             }
             const int nb = min(WS_KB, qt - qh);
-            mbar_wait(&sm.ct.empty[stage], phase ^ 1u);
+            mbar_wait_backoff(&sm.ct.empty[stage], phase ^ 1u);
             // feature rows of the batch: one bulk async copy each, counted on full[stage]
             if (pw == 0 && lane < nb) {
                 const uint32_t id = __float_as_uint(sm.ct.rec1[(qh + lane) & (WS_QCAP - 1)].z);
                 mbar_expect_tx(&sm.ct.full[stage], (uint32_t)(DC * sizeof(FT)));
                 bulk_g2s(&sm.F[stage][lane * DC], feat + (size_t)id * a.D + c0, (uint32_t)(DC * sizeof(FT)), &sm.ct.full[stage]);
             }
-            // weights of the batch for this thread's two pixels
-            uint32_t m0 = 0u, m1 = 0u;
-            float* Wd = sm.W[stage];
-            if (!__all_sync(TR_FULL, P0.done && P1.done)) {
+            // weights of the batch for this thread's pixel
+            uint32_t m = 0u;
+            float* Wd = sm.W[stage] + p;
+            if (!__all_sync(TR_FULL, P.done)) {
 #pragma unroll 4
                 for (int kk = 0; kk < nb; ++kk) {
                     const int s = (qh + kk) & (WS_QCAP - 1);
                     const float4 r0 = sm.ct.rec0[s];
                     const float4 r1 = sm.ct.rec1[s];
                     const float4 c = sm.rgb[s];
-                    const float w0 = ws_weight(r0, r1.x, r1.y, P0, q_cutoff, alpha_max, t_min);
-                    const float w1 = ws_weight(r0, r1.x, r1.y, P1, q_cutoff, alpha_max, t_min);
-                    Wd[kk * WS_CONS + slot0] = w0;
-                    Wd[kk * WS_CONS + slot1] = w1;
-                    C00 = fmaf(w0, c.x, C00); C01 = fmaf(w0, c.y, C01); C02 = fmaf(w0, c.z, C02);
-                    C10 = fmaf(w1, c.x, C10); C11 = fmaf(w1, c.y, C11); C12 = fmaf(w1, c.z, C12);
-                    m0 |= (w0 != 0.f ? 1u : 0u) << kk;
-                    m1 |= (w1 != 0.f ? 1u : 0u) << kk;
+                    const float w = ws_weight(r0, r1.x, r1.y, P, q_cutoff, alpha_max, t_min);
+                    Wd[kk * WS_CONS] = w;
+                    C0 = fmaf(w, c.x, C0); C1 = fmaf(w, c.y, C1); C2 = fmaf(w, c.z, C2);
+                    m |= (w != 0.f ? 1u : 0u) << kk;
                 }
-                m0 = __reduce_or_sync(TR_FULL, m0);
-                m1 = __reduce_or_sync(TR_FULL, m1);
+                m = __reduce_or_sync(TR_FULL, m);
             }
-            if (lane == 0) {
-                sm.ct.mask[stage][2 * pw] = m0;
-                sm.ct.mask[stage][2 * pw + 1] = m1;
-            }
+            if (lane == 0) sm.ct.mask[stage][pw] = m;
             qh += nb;
-            const bool all_done = named_bar_and(WS_BAR_PROD_RED, WS_PROD, P0.done && P1.done);
+            const bool all_done = named_bar_and(WS_BAR_PROD_RED, WS_PROD, P.done);
             last = all_done || (pos >= range.y && qt == qh);
             if (p == 0) sm.ct.meta[stage] = WsMeta{nb, tile, c0, last ? WS_FLAG_LAST : 0};
             mbar_arrive(&sm.ct.full[stage]);
             if (++stage == R_STAGES) { stage = 0; phase ^= 1u; }
         } while (!last);
-        if (c0 == 0) {
-            if (in0) {
-                const size_t o = (size_t)py0 * a.t.W + px0;
-                a.out_rgb[3 * o] = fmaf(P0.T, a.bg[0], C00);
-                a.out_rgb[3 * o + 1] = fmaf(P0.T, a.bg[1], C01);
-                a.out_rgb[3 * o + 2] = fmaf(P0.T, a.bg[2], C02);
-                if (a.out_T) a.out_T[o] = P0.T;
-                if (a.out_n) a.out_n[o] = P0.n;
-            }
-            if (in1) {
-                const size_t o = (size_t)py1 * a.t.W + px1;
-                a.out_rgb[3 * o] = fmaf(P1.T, a.bg[0], C10);
-                a.out_rgb[3 * o + 1] = fmaf(P1.T, a.bg[1], C11);
-                a.out_rgb[3 * o + 2] = fmaf(P1.T, a.bg[2], C12);
-                if (a.out_T) a.out_T[o] = P1.T;
-                if (a.out_n) a.out_n[o] = P1.n;
-            }
+        if (c0 == 0 && inside) {
+            const size_t o = (size_t)py * a.t.W + px;
+            a.out_rgb[3 * o] = fmaf(P.T, a.bg[0], C0);
+            a.out_rgb[3 * o + 1] = fmaf(P.T, a.bg[1], C1);
+            a.out_rgb[3 * o + 2] = fmaf(P.T, a.bg[2], C2);
+            if (a.out_T) a.out_T[o] = P.T;
+            if (a.out_n) a.out_n[o] = P.n;
         }
         item = ws_pop_end(sm.ct, popped, p);
     }
@@ -183,11 +162,11 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT>& sm, con
     const int pgl = lane >> 3, cg = lane & 7;
     const int pg = warp * 4 + pgl;   // 8-pixel row run: slots pg*8 .. pg*8+7
     FT* out_feat = reinterpret_cast<FT*>(a.out_feat);
-    float acc[8][NJ * 4];
+    unsigned long long acc[8][NJ * 2];   // packed channel pairs (fma.rn.f32x2)
 #pragma unroll
     for (int i = 0; i < 8; ++i)
 #pragma unroll
-        for (int j = 0; j < NJ * 4; ++j) acc[i][j] = 0.f;
+        for (int j = 0; j < NJ * 2; ++j) acc[i][j] = 0ull;
     int stage = 0;
     uint32_t phase = 0;
     while (true) {
@@ -203,16 +182,19 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT>& sm, con
             const float4 wa = *reinterpret_cast<const float4*>(Ws + kk * WS_CONS);
             const float4 wb = *reinterpret_cast<const float4*>(Ws + kk * WS_CONS + 4);
             const float wv[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
-            float fv[NJ * 4];
+            unsigned long long fv[NJ * 2];
 #pragma unroll
             for (int j = 0; j < NJ; ++j) {
                 const float4 f = FeatIO<FT>::load4(Fs + kk * DC + j * 32);
-                fv[4 * j] = f.x; fv[4 * j + 1] = f.y; fv[4 * j + 2] = f.z; fv[4 * j + 3] = f.w;
+                fv[2 * j] = pack2(f.x, f.y);
+                fv[2 * j + 1] = pack2(f.z, f.w);
             }
 #pragma unroll
-            for (int i = 0; i < 8; ++i)
+            for (int i = 0; i < 8; ++i) {
+                const unsigned long long w2 = pack2(wv[i], wv[i]);
 #pragma unroll
-                for (int j = 0; j < NJ * 4; ++j) acc[i][j] = fmaf(wv[i], fv[j], acc[i][j]);
+                for (int j = 0; j < NJ * 2; ++j) acc[i][j] = fma2(w2, fv[j], acc[i][j]);
+            }
         }
         mbar_arrive(&sm.ct.empty[stage]);
         if (++stage == R_STAGES) { stage = 0; phase ^= 1u; }
@@ -226,11 +208,13 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT>& sm, con
                 if (oy < a.t.H && ox < a.t.W) {
                     FT* dst = out_feat + ((size_t)oy * a.t.W + ox) * a.D + m.c0 + cg * 4;
 #pragma unroll
-                    for (int j = 0; j < NJ; ++j)
-                        FeatIO<FT>::store4(dst + j * 32, make_float4(acc[i][4 * j], acc[i][4 * j + 1], acc[i][4 * j + 2], acc[i][4 * j + 3]));
+                    for (int j = 0; j < NJ; ++j) {
+                        const float2 lo = unpack2(acc[i][2 * j]), hi = unpack2(acc[i][2 * j + 1]);
+                        FeatIO<FT>::store4(dst + j * 32, make_float4(lo.x, lo.y, hi.x, hi.y));
+                    }
                 }
 #pragma unroll
-                for (int j = 0; j < NJ * 4; ++j) acc[i][j] = 0.f;
+                for (int j = 0; j < NJ * 2; ++j) acc[i][j] = 0ull;
             }
         }
     }
@@ -251,10 +235,10 @@ __global__ void __launch_bounds__(WS_THREADS, 1) render_ws_kernel(const RenderAr
     }
     __syncthreads();
     if (threadIdx.x >= WS_CONS) {
-        setmaxnreg_dec<88>();
+        setmaxnreg_dec<72>();
         render_ws_producer<DC, FT>(sm, a, wk);
     } else {
-        setmaxnreg_inc<200>();
+        setmaxnreg_inc<184>();
         render_ws_consumer<DC, FT>(sm, a);
         if (threadIdx.x == 0) ws_queue_release(wk);
     }

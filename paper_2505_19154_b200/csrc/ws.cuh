@@ -1,19 +1,19 @@
 // ws.cuh -- the warp-specialised, persistent tile pipeline shared by the tiled render and fuse kernels.
 //
-// One CTA per SM, 384 threads: warps 0-7 are CONSUMERS (the D-channel product of the step), warps
-// 8-11 are PRODUCERS (tile traversal: fetch, tile cull, blend weights w = alpha*T of PAPER.md:95).
+// One CTA per SM, 512 threads: warps 0-7 are CONSUMERS (the D-channel product of the step), warps
+// 8-15 are PRODUCERS (tile traversal: fetch, tile cull, blend weights w = alpha*T of PAPER.md:95).
 // The CTA pulls work items (tile, channel chunk) from an atomic queue until it is empty.
 //
-// Producer (128 threads, 2 pixels each; slot s of the 16x16 tile: warp-block = s/32 covers 8x4 px):
-//   stage   128 instances of the tile's sorted range are examined by one thread each (one chunk
+// Producer (256 threads, one pixel each; slot s of the 16x16 tile: warp-block = s/32 covers 8x4 px):
+//   stage   256 instances of the tile's sorted range are examined by one thread each (one chunk
 //           ahead is prefetched into registers): exact ellipse-vs-tile-box test (traverse.cuh),
 //           survivors appended in order to a shared-memory ring {xy, conic, opacity, id, rgb}.
 //   batch   up to WS_KB ring entries form a batch in pipeline stage s: one bulk async copy
 //           (cp.async.bulk, completion counted on the stage's `full` mbarrier) per feature row
 //           (render) is issued first; then every producer thread evaluates the normative q, the
-//           cut-off, alpha, w, T for its 2 pixels and parks w in W[s][kk][slot]; per warp-block
+//           cut-off, alpha, w, T for its pixel and parks w in W[s][kk][slot]; per warp-block
 //           bit masks say which instances gave the block any weight.
-//   signal  meta[s] = {nb, tile, chunk, flags}; all 128 producers arrive on full[s].
+//   signal  meta[s] = {nb, tile, chunk, flags}; all 256 producers arrive on full[s].
 // Consumer (256 threads): waits full[s], multiplies, arrives on empty[s]; on the LAST batch of an
 // item it writes its accumulators out.  Producers run ahead by up to WS_STAGES batches, across
 // tile boundaries, so global-load latency, the sequential weight phase and the FFMA-bound product
@@ -22,10 +22,10 @@
 #include "traverse.cuh"
 
 constexpr int WS_CONS = 256;
-constexpr int WS_PROD = 128;
+constexpr int WS_PROD = 256;
 constexpr int WS_THREADS = WS_CONS + WS_PROD;
 constexpr int WS_KB = 32;      // instances per batch (one bit each in the 32-bit block masks)
-constexpr int WS_QCAP = 256;   // survivor ring capacity (power of two) >= WS_KB - 1 + WS_PROD
+constexpr int WS_QCAP = 512;   // survivor ring capacity (power of two) >= WS_KB - 1 + WS_PROD
 
 enum { WS_FLAG_LAST = 1, WS_FLAG_EXIT = 2 };
 enum { WS_BAR_PROD = 1, WS_BAR_PROD_RED = 2 };   // named barriers (0 = __syncthreads)
@@ -56,6 +56,29 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     while (!mbar_try_wait(bar, parity)) {
     }
+}
+// same, with a short sleep between probes (for the side that is normally ahead: it should not
+// burn issue slots the other side needs)
+__device__ __forceinline__ void mbar_wait_backoff(uint64_t* bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) __nanosleep(100);
+}
+
+// Packed FP32 FMA (sm_100+ fma.rn.f32x2): acc.{lo,hi} += w * f.{lo,hi}, each lane an IEEE fma.
+// One issue slot for two FMAs -- the consumer loops are issue-bound next to the producer warps.
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ float2 unpack2(unsigned long long v) {
+    float2 r;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(r.x), "=f"(r.y) : "l"(v));
+    return r;
+}
+__device__ __forceinline__ unsigned long long fma2(unsigned long long a, unsigned long long b, unsigned long long c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
 }
 // 1-D bulk async copy global -> shared, completion (bytes) counted on `bar`.
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
@@ -131,7 +154,7 @@ __device__ __forceinline__ float ws_weight(const float4 r0, const float C, const
     return w;
 }
 
-// Chunk of 128 instances held in registers (one per producer thread), software-pipelined two deep:
+// Chunk of WS_PROD instances held in registers (one per producer thread), software-pipelined two deep:
 // `id_next` (the sorted-list entry of the chunk after this one) is in flight while this chunk's
 // projected Gaussian (xy, conic, opacity, colour) is in flight, so neither dependent global load is
 // waited for at its issue point.
