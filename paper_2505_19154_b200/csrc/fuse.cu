@@ -14,7 +14,8 @@
 // PIXEL variant (small D): thread = pixel holds its G row in registers; each (warp, Gaussian)
 // segment is reduced with shuffles and leaves as one atomic per channel from lane 0.
 // The finalise kernel divides (one warp per Gaussian row) and optionally L2-normalises.
-#include "traverse.cuh"
+#include "layout.cuh"
+#include "ws.cuh"
 
 namespace {
 
@@ -104,7 +105,7 @@ __device__ __forceinline__ void fuse_gemm(const float* __restrict__ W, const flo
 
 template <int DC, typename GT>
 __global__ void __launch_bounds__(TR_THREADS, 1) fuse_tiled_kernel(const FuseArgs a) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_raw[];
     FuseTiledSmem<DC>& sm = *reinterpret_cast<FuseTiledSmem<DC>*>(smem_raw);
 
     const int tid = threadIdx.x;
@@ -179,6 +180,289 @@ __global__ void __launch_bounds__(TR_THREADS, 1) fuse_tiled_kernel(const FuseArg
             q_count -= nb;
             if (__syncthreads_and(done)) break;
         }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// WS variant (fp32 map, D multiple of 128): warp-specialised persistent pipeline (ws.cuh)
+//   warps 0-7   consumers: num[32 inst, 128 ch] += W^T G for one batch.  Thread = 8 instances x 4
+//               channels over one HALF of the tile's pixels (warps 0-3: pixels 0-127, warps 4-7:
+//               128-255); per pixel 1 LDS.128 of G + 2 LDS.128 of W (each one wavefront) feed 16
+//               packed FMAs (fma.rn.f32x2, instance pairs packed).  The two halves are combined
+//               through shared memory (roles alternate per batch) and leave as one
+//               red.global.add.v4.f32 per (tile, Gaussian, 4 channels).
+//   warps 8-15  producers: traversal, tile cull, blend weights -> W[stage][pixel][kk] (swizzled
+//               float4 quads so that both sides are bank-conflict free).
+//   warp 16     scheduler: pops (tile, chunk) items from the global queue, hands them to the
+//               producers through a 2-deep ring, and -- once the consumers released the GT tile
+//               of the previous item -- issues the bulk async copies of the next GT tile
+//               (16 rows x 8 KB when D == 128) onto the g_full mbarrier.
+// ---------------------------------------------------------------------------------------------
+constexpr int FW_STAGES = 2;
+constexpr int FW_DC = 128;
+constexpr int FW_THREADS = WS_THREADS + 32;
+constexpr int FW_BAR_CONS = 3;
+enum { FW_FLAG_FIRST = 4 };
+
+struct FuseWsSmem {
+    WsCtrl<FW_STAGES> ct;
+    uint64_t g_full, g_free;
+    uint64_t item_full[2], item_empty[2];
+    int items[2];
+    __align__(16) uint32_t ids[FW_STAGES][WS_KB];
+    __align__(16) float den_s[2][WS_KB];
+    __align__(128) float W[FW_STAGES][WS_CONS * WS_KB];   // [pixel][quad ^ (pixel & 7)][4]
+    __align__(128) float P[WS_KB * FW_DC];                // partial sums of the writing half
+    __align__(128) float G[WS_CONS * FW_DC];              // [pixel][channel], pixel = y*16 + x
+};
+
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)), "r"(bytes)
+                 : "memory");
+}
+
+__device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem& sm, const FuseArgs& a, const WsWork& wk) {
+    const int lane = threadIdx.x & 31;
+    const float* gt = reinterpret_cast<const float*>(a.gt);
+    int islot = 0;
+    uint32_t iphase = 0, gphase = 0;
+    while (true) {
+        int item = 0;
+        if (lane == 0) {
+            item = (int)atomicAdd(wk.queue, 1u);
+            mbar_wait_backoff(&sm.item_empty[islot], iphase ^ 1u);
+            sm.items[islot] = item;
+            mbar_arrive(&sm.item_full[islot]);
+        }
+        item = __shfl_sync(TR_FULL, item, 0);
+        if (++islot == 2) { islot = 0; iphase ^= 1u; }
+        if (item >= wk.n_items) break;
+        const int tile = item / wk.n_chunks, c0 = (item % wk.n_chunks) * FW_DC;
+        {
+            const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
+            if (range.x >= range.y) continue;   // empty tile: the producers skip it too
+        }
+        const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
+        const int nx = min(FHGS_TILE, a.t.W - tx0), ny = min(FHGS_TILE, a.t.H - ty0);
+        if (lane == 0) {
+            mbar_wait_backoff(&sm.g_free, gphase ^ 1u);
+            mbar_arrive_expect_tx(&sm.g_full, (uint32_t)(nx * ny * FW_DC * 4));
+        }
+        __syncwarp();
+        if (a.D == FW_DC) {   // a tile row is one contiguous span
+            if (lane < ny)
+                bulk_g2s(&sm.G[lane * FHGS_TILE * FW_DC], gt + ((size_t)(ty0 + lane) * a.t.W + tx0) * FW_DC,
+                         (uint32_t)(nx * FW_DC * 4), &sm.g_full);
+        } else {
+            for (int pix = lane; pix < FHGS_TILE_PX; pix += 32) {
+                const int x = pix & 15, y = pix >> 4;
+                if (x < nx && y < ny)
+                    bulk_g2s(&sm.G[pix * FW_DC], gt + ((size_t)(ty0 + y) * a.t.W + tx0 + x) * a.D + c0, (uint32_t)(FW_DC * 4),
+                             &sm.g_full);
+            }
+        }
+        gphase ^= 1u;
+    }
+}
+
+__device__ __forceinline__ void fuse_ws_producer(FuseWsSmem& sm, const FuseArgs& a, const WsWork& wk) {
+    const int p = threadIdx.x - WS_CONS, lane = p & 31;
+    const float q_cutoff = a.t.q_cutoff, alpha_max = a.t.alpha_max, t_min = a.t.t_min;
+    const int sx = p & 15, sy = p >> 4;   // row-major pixel slot (matches the GT tile rows)
+    int stage = 0, islot = 0;
+    uint32_t phase = 0, iphase = 0;
+    while (true) {
+        mbar_wait(&sm.item_full[islot], iphase);
+        const int item = sm.items[islot];
+        mbar_arrive(&sm.item_empty[islot]);
+        if (++islot == 2) { islot = 0; iphase ^= 1u; }
+        if (item >= wk.n_items) {
+            mbar_wait(&sm.ct.empty[stage], phase ^ 1u);
+            if (p == 0) sm.ct.meta[stage] = WsMeta{0, -1, 0, WS_FLAG_EXIT};
+            mbar_arrive(&sm.ct.full[stage]);
+            break;
+        }
+        const int tile = item / wk.n_chunks, c0 = (item % wk.n_chunks) * FW_DC;
+        const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
+        const int px = tx0 + sx, py = ty0 + sy;
+        const bool inside = px < a.t.W && py < a.t.H;
+        WsPixel P{(float)px, (float)py, 1.f, 0u, !inside};
+        const float bx0 = (float)tx0, by0 = (float)ty0;
+        const float bx1 = (float)min(tx0 + FHGS_TILE - 1, a.t.W - 1), by1 = (float)min(ty0 + FHGS_TILE - 1, a.t.H - 1);
+        const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
+        if (range.x >= range.y) continue;   // empty tile (the scheduler loads no GT tile for it)
+        uint32_t pos = range.x;
+        int qh = 0, qt = 0;
+        WsChunk ch;
+        ws_chunk_prefetch_id(a.t, pos, range.y, p, ch);
+        ws_chunk_issue(a.t, nullptr, ch);
+        ws_chunk_prefetch_id(a.t, pos + WS_PROD, range.y, p, ch);
+        bool last = false, first = true;
+        do {
+            while (qt - qh < WS_KB && pos < range.y) {
+                qt += ws_chunk_append(sm.ct, ch, qt, bx0, by0, bx1, by1, q_cutoff, p, [](int, const WsChunk&) {});
+                pos += WS_PROD;
+                ws_chunk_issue(a.t, nullptr, ch);
+                ws_chunk_prefetch_id(a.t, pos + WS_PROD, range.y, p, ch);
+            }
+            const int nb = min(WS_KB, qt - qh);
+            mbar_wait_backoff(&sm.ct.empty[stage], phase ^ 1u);
+            if (p < WS_KB) sm.ids[stage][p] = p < nb ? __float_as_uint(sm.ct.rec1[(qh + p) & (WS_QCAP - 1)].z) : 0u;
+            float* Wd = sm.W[stage] + p * WS_KB;
+            const bool warp_done = __all_sync(TR_FULL, P.done);
+#pragma unroll 2
+            for (int kq = 0; kq < WS_KB / 4; ++kq) {
+                float w4[4] = {0.f, 0.f, 0.f, 0.f};
+                if (!warp_done && kq * 4 < nb) {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const int kk = kq * 4 + j;
+                        const int s = (qh + kk) & (WS_QCAP - 1);
+                        const float4 r0 = sm.ct.rec0[s];
+                        const float4 r1 = sm.ct.rec1[s];
+                        WsPixel Q = P;
+                        const float w = ws_weight(r0, r1.x, r1.y, Q, q_cutoff, alpha_max, t_min);
+                        if (kk < nb) { P = Q; w4[j] = w; }
+                    }
+                }
+                *reinterpret_cast<float4*>(Wd + ((kq ^ (p & 7)) << 2)) = make_float4(w4[0], w4[1], w4[2], w4[3]);
+            }
+            qh += nb;
+            const bool all_done = named_bar_and(WS_BAR_PROD_RED, WS_PROD, P.done);
+            last = all_done || (pos >= range.y && qt == qh);
+            if (p == 0) sm.ct.meta[stage] = WsMeta{nb, tile, c0, (last ? WS_FLAG_LAST : 0) | (first ? FW_FLAG_FIRST : 0)};
+            first = false;
+            mbar_arrive(&sm.ct.full[stage]);
+            if (++stage == FW_STAGES) { stage = 0; phase ^= 1u; }
+        } while (!last);
+    }
+    (void)lane;
+}
+
+__device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem& sm, const FuseArgs& a) {
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int half = warp >> 2, cw = warp & 3;
+    const int kg = lane >> 3, cg = lane & 7;
+    const int ch = cw * 32 + cg * 4;          // this thread's 4 channels inside the chunk
+    const float* Gs = sm.G + half * 128 * FW_DC + ch;
+    int stage = 0;
+    uint32_t phase = 0, gphase = 0, batch = 0;
+    while (true) {
+        mbar_wait(&sm.ct.full[stage], phase);
+        const WsMeta m = sm.ct.meta[stage];
+        if (m.flags & WS_FLAG_EXIT) break;
+        if (m.flags & FW_FLAG_FIRST) {
+            mbar_wait(&sm.g_full, gphase);
+            gphase ^= 1u;
+        }
+        uint32_t id[8];
+        {
+            const uint4 i0 = *reinterpret_cast<const uint4*>(&sm.ids[stage][kg * 8]);
+            const uint4 i1 = *reinterpret_cast<const uint4*>(&sm.ids[stage][kg * 8 + 4]);
+            id[0] = i0.x; id[1] = i0.y; id[2] = i0.z; id[3] = i0.w;
+            id[4] = i1.x; id[5] = i1.y; id[6] = i1.z; id[7] = i1.w;
+        }
+        unsigned long long acc[4][4];   // [instance pair][channel], packed (inst 2i, inst 2i+1)
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int c = 0; c < 4; ++c) acc[i][c] = 0ull;
+        const float* Ws = sm.W[stage] + half * 128 * WS_KB;
+#pragma unroll 1
+        for (int s0 = 0; s0 < 128; s0 += 8) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int s = s0 + u;   // (s & 7) == u
+                const ulonglong2 wa = *reinterpret_cast<const ulonglong2*>(Ws + s * WS_KB + (((2 * kg) ^ u) << 2));
+                const ulonglong2 wb = *reinterpret_cast<const ulonglong2*>(Ws + s * WS_KB + (((2 * kg + 1) ^ u) << 2));
+                const float4 g = *reinterpret_cast<const float4*>(Gs + s * FW_DC);
+                const unsigned long long g2[4] = {pack2(g.x, g.x), pack2(g.y, g.y), pack2(g.z, g.z), pack2(g.w, g.w)};
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    acc[0][c] = fma2(wa.x, g2[c], acc[0][c]);
+                    acc[1][c] = fma2(wa.y, g2[c], acc[1][c]);
+                    acc[2][c] = fma2(wb.x, g2[c], acc[2][c]);
+                    acc[3][c] = fma2(wb.y, g2[c], acc[3][c]);
+                }
+            }
+        }
+        // den partial: warp (half, cw) sums pixels [128 half + 32 cw, +32) for instance kk = lane
+        {
+            const float* Wp = Ws + cw * 32 * WS_KB;
+            float dsum = 0.f;
+#pragma unroll 8
+            for (int j = 0; j < 32; ++j) dsum += Wp[j * WS_KB + ((((lane >> 2) ^ (j & 7)) << 2) | (lane & 3))];
+            atomicAdd(&sm.den_s[batch & 1][lane], dsum);
+        }
+        mbar_arrive(&sm.ct.empty[stage]);
+        if (m.flags & WS_FLAG_LAST) mbar_arrive(&sm.g_free);
+        if (++stage == FW_STAGES) { stage = 0; phase ^= 1u; }
+        const bool writer = ((batch & 1u) != 0u) == (half != 0);
+        if (writer) {
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float2 v0 = unpack2(acc[i][0]), v1 = unpack2(acc[i][1]), v2 = unpack2(acc[i][2]), v3 = unpack2(acc[i][3]);
+                *reinterpret_cast<float4*>(&sm.P[(kg * 8 + 2 * i) * FW_DC + ch]) = make_float4(v0.x, v1.x, v2.x, v3.x);
+                *reinterpret_cast<float4*>(&sm.P[(kg * 8 + 2 * i + 1) * FW_DC + ch]) = make_float4(v0.y, v1.y, v2.y, v3.y);
+            }
+        }
+        named_bar_sync(FW_BAR_CONS, WS_CONS);
+        if (!writer) {
+            const float4 d0 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][kg * 8]);
+            const float4 d1 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][kg * 8 + 4]);
+            const float dv[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const float2 v0 = unpack2(acc[i][0]), v1 = unpack2(acc[i][1]), v2 = unpack2(acc[i][2]), v3 = unpack2(acc[i][3]);
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int k8 = 2 * i + e, kk = kg * 8 + k8;
+                    if (kk < m.nb && dv[k8] != 0.f) {
+                        const float4 pp = *reinterpret_cast<const float4*>(&sm.P[kk * FW_DC + ch]);
+                        const float4 mine = e ? make_float4(v0.y, v1.y, v2.y, v3.y) : make_float4(v0.x, v1.x, v2.x, v3.x);
+                        red_add_v4(a.num + (size_t)id[k8] * a.D + m.c0 + ch,
+                                   make_float4(mine.x + pp.x, mine.y + pp.y, mine.z + pp.z, mine.w + pp.w));
+                        if (m.c0 == 0 && ch == 0) red_add(a.den + id[k8], dv[k8]);
+                    }
+                }
+            }
+            // all four channel warps of this half must have read den_s before it is cleared
+            asm volatile("bar.sync %0, %1;" ::"r"(4 + half), "r"(128) : "memory");
+            if (cw == 0) sm.den_s[batch & 1][lane] = 0.f;
+        }
+        ++batch;
+    }
+}
+
+__global__ void __launch_bounds__(FW_THREADS, 1) fuse_ws_kernel(const FuseArgs a, const WsWork wk) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    FuseWsSmem& sm = *reinterpret_cast<FuseWsSmem*>(smem_raw);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < FW_STAGES; ++s) {
+            mbar_init(&sm.ct.full[s], WS_PROD);
+            mbar_init(&sm.ct.empty[s], WS_CONS);
+        }
+        mbar_init(&sm.g_full, 1);
+        mbar_init(&sm.g_free, WS_CONS);
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(&sm.item_full[s], 1);
+            mbar_init(&sm.item_empty[s], WS_PROD);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    // the GT tile buffer must never hold non-finite garbage (pixels outside the image keep stale data, weight 0)
+    for (int i = threadIdx.x; i < WS_CONS * FW_DC / 4; i += FW_THREADS) reinterpret_cast<float4*>(sm.G)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (threadIdx.x < 2 * WS_KB) (&sm.den_s[0][0])[threadIdx.x] = 0.f;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+    if (threadIdx.x >= WS_THREADS) {
+        fuse_ws_scheduler(sm, a, wk);
+    } else if (threadIdx.x >= WS_CONS) {
+        fuse_ws_producer(sm, a, wk);
+    } else {
+        fuse_ws_consumer(sm, a);
+        if (threadIdx.x == 0) ws_queue_release(wk);
     }
 }
 
@@ -304,8 +588,22 @@ cudaError_t launch(K kernel, size_t smem, int grid, cudaStream_t st, const FuseA
     return cudaGetLastError();
 }
 
+cudaError_t launch_fuse_ws(const FuseArgs& a, int tiles, int num_sms, uint32_t* queue, cudaStream_t st) {
+    const size_t smem = sizeof(FuseWsSmem);
+    cudaError_t e = cudaFuncSetAttribute(fuse_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    WsWork wk;
+    wk.queue = queue;
+    wk.n_chunks = a.D / FW_DC;
+    wk.n_items = tiles * wk.n_chunks;
+    const int grid = wk.n_items < num_sms ? wk.n_items : num_sms;
+    fuse_ws_kernel<<<grid, FW_THREADS, smem, st>>>(a, wk);
+    return cudaGetLastError();
+}
+
 template <typename GT>
-cudaError_t dispatch(const FuseArgs& a, int grid, cudaStream_t st) {
+cudaError_t dispatch(const FuseArgs& a, int grid, int num_sms, uint32_t* queue, cudaStream_t st) {
+    if (sizeof(GT) == 4 && a.D % FW_DC == 0) return launch_fuse_ws(a, grid, num_sms, queue, st);
     if (a.D % 128 == 0) return launch(fuse_tiled_kernel<128, GT>, sizeof(FuseTiledSmem<128>), grid, st, a);
     if (a.D % 64 == 0) return launch(fuse_tiled_kernel<64, GT>, sizeof(FuseTiledSmem<64>), grid, st, a);
     if (a.D % 16 == 0) return launch(fuse_pixel_kernel<16, GT>, 0, grid, st, a);
@@ -360,7 +658,9 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
         a.t.q_cutoff = prm->q_cutoff; a.t.alpha_max = prm->alpha_max; a.t.t_min = prm->t_min;
         a.gt = gt; a.D = feat_dim; a.num = num; a.den = den;
         const int grid = tiles_x(cam->width) * tiles_y(cam->height);
-        cudaError_t e = gt_dtype == FHGS_F16 ? dispatch<__half>(a, grid, s) : dispatch<float>(a, grid, s);
+        uint32_t* queue = reinterpret_cast<uint32_t*>((char*)vs->scratch + make_scratch_layout(vs->n, vs->capacity).ctrl) + CTRL_TILE_QUEUE;
+        cudaError_t e = gt_dtype == FHGS_F16 ? dispatch<__half>(a, grid, ctx->num_sms, queue, s)
+                                             : dispatch<float>(a, grid, ctx->num_sms, queue, s);
         FHGS_CUDA(ctx, e);
     }
     if (finalize && n > 0) {
