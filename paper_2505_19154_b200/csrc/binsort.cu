@@ -57,7 +57,8 @@ struct ScanDupArgs {
     const uint16_t* rect;
     const float* depth;
     const uint32_t* perm;        // NULL = index order
-    uint32_t* offsets;           // NULL = do not write
+    uint32_t* offsets;           // NULL = do not write; indexed by Gaussian
+    uint32_t* incl_pos;          // NULL = do not write; indexed by scan position (perm order)
     uint64_t* num_instances;     // NULL = do not write
     uint64_t* status;            // [scan_tiles]
     uint32_t* ticket;
@@ -152,6 +153,13 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_dup_kernel(const ScanDupArg
             if (j < a.n) a.offsets[s_gid[tid * SCAN_ITEMS + k]] = (uint32_t)(prefix + s_incl[tid * SCAN_ITEMS + k]);
         }
     }
+    if (a.incl_pos) {
+#pragma unroll
+        for (int k = 0; k < SCAN_ITEMS; ++k) {
+            const int j = base + tid * SCAN_ITEMS + k;
+            if (j < a.n) a.incl_pos[j] = (uint32_t)(prefix + s_incl[tid * SCAN_ITEMS + k]);
+        }
+    }
     if (!a.keys) return;
 
     // stage rect / depth of the Gaussians that emit
@@ -209,6 +217,110 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_dup_kernel(const ScanDupArg
     }
     __syncthreads();
     for (int j = tid; j < a.npass * 256; j += SCAN_THREADS) {
+        const uint32_t c = (&s_hist[0][0])[j];
+        if (c) atomicAdd(a.hist + j, c);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// balanced emission (default schedule).  In depth order the nearest Gaussians -- the ones with the
+// largest footprints -- are consecutive, so a CTA-per-1024-Gaussians emission is badly unbalanced
+// (one CTA may own millions of instances).  Here the work unit is EMIT_TILE consecutive INSTANCES:
+//   emit_partition_kernel  starts[b] = first depth-ordered Gaussian g with incl[g] > min(b*EMIT_TILE, M-1)
+//   emit_kernel            persistent CTAs; per unit the covering Gaussians (at most EMIT_TILE + 1,
+//                          all visible: culled ones sort last) are staged in shared memory, every
+//                          instance finds its owner by binary search; stores are coalesced.
+// ------------------------------------------------------------------------------------------------
+struct EmitArgs {
+    int n, GW;
+    const uint32_t* perm;      // [n] depth-ordered Gaussian indices, visible first
+    const uint32_t* incl;      // [n] inclusive prefix of tiles_touched in that order
+    const uint16_t* rect;
+    const float* depth;
+    const uint64_t* num_instances;
+    uint64_t capacity;
+    uint32_t* starts;          // [units + 1]
+    int units;                 // ceil(capacity / EMIT_TILE)
+    uint64_t* keys;
+    uint32_t* vals;
+    uint32_t* hist;            // [npass][256] tile-id digit histograms
+    int npass;
+};
+
+__global__ void __launch_bounds__(256) emit_partition_kernel(const EmitArgs a) {
+    const int b = blockIdx.x * 256 + threadIdx.x;
+    if (b > a.units) return;
+    const uint64_t M = *a.num_instances;
+    if (M == 0 || M > a.capacity) return;
+    uint64_t j = (uint64_t)b * EMIT_TILE;
+    if (j > M - 1) j = M - 1;
+    int lo = 0, hi = a.n - 1;   // incl[n-1] = M > j
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if ((uint64_t)__ldg(a.incl + mid) > j) hi = mid; else lo = mid + 1;
+    }
+    a.starts[b] = (uint32_t)lo;
+}
+
+constexpr int EMIT_THREADS = 256;
+
+__global__ void __launch_bounds__(EMIT_THREADS) emit_kernel(const EmitArgs a) {
+    __shared__ uint32_t s_incl[EMIT_TILE + 1];
+    __shared__ uint32_t s_gid[EMIT_TILE + 1];
+    __shared__ uint32_t s_depth[EMIT_TILE + 1];
+    __shared__ uint2 s_rect[EMIT_TILE + 1];
+    __shared__ uint32_t s_hist[SORT_MAX_PASSES][256];
+    const int tid = threadIdx.x;
+    const uint64_t M = *a.num_instances;
+    if (M == 0 || M > a.capacity) return;
+    for (int j = tid; j < a.npass * 256; j += EMIT_THREADS) (&s_hist[0][0])[j] = 0;
+    const uint32_t units = (uint32_t)((M + EMIT_TILE - 1) / EMIT_TILE);
+    for (uint32_t b = blockIdx.x; b < units; b += gridDim.x) {
+        const uint32_t j0 = b * EMIT_TILE;
+        const uint32_t cnt = (uint32_t)min((uint64_t)EMIT_TILE, M - j0);
+        const uint32_t g_lo = __ldg(a.starts + b), g_hi = __ldg(a.starts + b + 1);
+        const int span = (int)(g_hi - g_lo) + 1;   // <= EMIT_TILE + 1
+        __syncthreads();   // previous unit done with the staging arrays (and s_hist zeroed)
+        for (int i = tid; i < span; i += EMIT_THREADS) {
+            const uint32_t g = __ldg(a.perm + g_lo + i);
+            s_incl[i] = __ldg(a.incl + g_lo + i);
+            s_gid[i] = g;
+            s_depth[i] = __float_as_uint(__ldg(a.depth + g));
+            s_rect[i] = __ldg(reinterpret_cast<const uint2*>(a.rect) + g);
+        }
+        const uint32_t before = g_lo ? __ldg(a.incl + g_lo - 1) : 0u;
+        __syncthreads();
+#pragma unroll
+        for (int r = 0; r < EMIT_TILE / EMIT_THREADS; ++r) {
+            const uint32_t jl = r * EMIT_THREADS + tid;
+            const bool valid = jl < cnt;
+            uint32_t tile_id = 0xffffffffu;
+            if (valid) {
+                const uint32_t j = j0 + jl;
+                int lo = 0, hi = span - 1;
+                while (lo < hi) {
+                    const int mid = (lo + hi) >> 1;
+                    if (s_incl[mid] > j) hi = mid; else lo = mid + 1;
+                }
+                const uint32_t start = lo ? s_incl[lo - 1] : before;
+                const uint32_t local = j - start;
+                const uint2 rc = s_rect[lo];
+                const uint32_t x0 = rc.x & 0xffffu, y0 = rc.x >> 16, x1 = rc.y & 0xffffu;
+                const uint32_t w = x1 - x0;
+                const uint32_t ry = local / w;
+                tile_id = (y0 + ry) * (uint32_t)a.GW + x0 + (local - ry * w);
+                a.keys[j] = ((uint64_t)tile_id << 32) | (uint64_t)s_depth[lo];
+                a.vals[j] = s_gid[lo];
+            }
+            for (int p = 0; p < a.npass; ++p) {
+                const uint32_t d = valid ? ((tile_id >> (8 * p)) & 255u) : 256u;
+                const uint32_t peers = __match_any_sync(FULL, d);
+                if (valid && (peers & lanemask_lt()) == 0) atomicAdd(&s_hist[p][d], (uint32_t)__popc(peers));
+            }
+        }
+    }
+    __syncthreads();
+    for (int j = tid; j < a.npass * 256; j += EMIT_THREADS) {
         const uint32_t c = (&s_hist[0][0])[j];
         if (c) atomicAdd(a.hist + j, c);
     }
@@ -489,19 +601,40 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
             scan_dup_kernel<<<scan_grid, SCAN_THREADS, 0, s>>>(sa0);
             FHGS_LAUNCH_CHECK(ctx);
         }
-        ScanDupArgs sa;
-        sa.n = vs->n; sa.GW = GW;
-        sa.tiles_touched = vs->tiles_touched; sa.rect = vs->rect; sa.depth = vs->depth;
-        sa.perm = perm;
-        sa.offsets = full_key ? vs->offsets : nullptr;
-        sa.num_instances = full_key ? vs->num_instances : nullptr;
-        sa.status = scan_status; sa.ticket = ctrl + CTRL_SCAN_TICKET;
-        sa.capacity = vs->capacity;
-        sa.keys = vs->keys[0]; sa.vals = vs->vals[0];
-        sa.hist = hist; sa.first_bit = first_bit; sa.npass = npass;
-        if (vs->capacity == 0) { sa.keys = nullptr; sa.offsets = vs->offsets; sa.num_instances = vs->num_instances; sa.perm = nullptr; }
-        scan_dup_kernel<<<scan_grid, SCAN_THREADS, 0, s>>>(sa);
-        FHGS_LAUNCH_CHECK(ctx);
+        if (full_key || vs->capacity == 0) {
+            ScanDupArgs sa;
+            memset(&sa, 0, sizeof(sa));
+            sa.n = vs->n; sa.GW = GW;
+            sa.tiles_touched = vs->tiles_touched; sa.rect = vs->rect; sa.depth = vs->depth;
+            sa.offsets = vs->offsets; sa.num_instances = vs->num_instances;
+            sa.status = scan_status; sa.ticket = ctrl + CTRL_SCAN_TICKET;
+            sa.capacity = vs->capacity;
+            if (vs->capacity > 0) { sa.keys = vs->keys[0]; sa.vals = vs->vals[0]; }
+            sa.hist = hist; sa.first_bit = first_bit; sa.npass = npass;
+            if (full_key || perm == nullptr) {
+                scan_dup_kernel<<<scan_grid, SCAN_THREADS, 0, s>>>(sa);
+                FHGS_LAUNCH_CHECK(ctx);
+            }
+        } else {
+            // prefix sums in depth order, then instance-balanced emission
+            uint32_t* incl = (uint32_t*)(sc + L.pre_incl);
+            ScanDupArgs sa;
+            memset(&sa, 0, sizeof(sa));
+            sa.n = vs->n; sa.GW = GW; sa.tiles_touched = vs->tiles_touched; sa.perm = perm;
+            sa.incl_pos = incl; sa.status = scan_status; sa.ticket = ctrl + CTRL_SCAN_TICKET;
+            scan_dup_kernel<<<scan_grid, SCAN_THREADS, 0, s>>>(sa);
+            FHGS_LAUNCH_CHECK(ctx);
+            EmitArgs ea;
+            ea.n = vs->n; ea.GW = GW; ea.perm = perm; ea.incl = incl; ea.rect = vs->rect; ea.depth = vs->depth;
+            ea.num_instances = vs->num_instances; ea.capacity = vs->capacity;
+            ea.starts = (uint32_t*)(sc + L.emit_starts); ea.units = (int)L.emit_tiles;
+            ea.keys = vs->keys[0]; ea.vals = vs->vals[0]; ea.hist = hist; ea.npass = npass;
+            emit_partition_kernel<<<(ea.units + 1 + 255) / 256, 256, 0, s>>>(ea);
+            FHGS_LAUNCH_CHECK(ctx);
+            const int egrid = std::min(ea.units, ctx->num_sms * 8);
+            emit_kernel<<<egrid, EMIT_THREADS, 0, s>>>(ea);
+            FHGS_LAUNCH_CHECK(ctx);
+        }
 
         if (vs->capacity > 0) {
             hist_scan_kernel<<<npass, 256, 0, s>>>(hist);

@@ -7,6 +7,7 @@ constexpr int SCAN_TILE = 1024;        // Gaussians per CTA of the scan+duplicat
 constexpr int SORT_TILE_K64 = 4096;    // pairs per CTA of a 64-bit-key onesweep pass
 constexpr int SORT_TILE_K32 = 4096;    // pairs per CTA of a 32-bit-key onesweep pass
 constexpr int SORT_MAX_PASSES = 8;
+constexpr int EMIT_TILE = 1024;        // instances per work unit of the balanced emission kernel
 
 // ctrl words (uint32_t)
 enum {
@@ -27,7 +28,9 @@ struct ScratchLayout {
     size_t sort_status;   // uint32_t[sort_tiles][256]
     size_t pre_keys[2];   // uint32_t[n]  depth bits (ping-pong)
     size_t pre_vals[2];   // uint32_t[n]  Gaussian index (ping-pong)
-    size_t scan_tiles, sort_tiles, pre_tiles;
+    size_t pre_incl;      // uint32_t[n]  inclusive prefix of tiles_touched in depth order
+    size_t emit_starts;   // uint32_t[emit_tiles + 1]  first depth-ordered Gaussian of every EMIT_TILE instances
+    size_t scan_tiles, sort_tiles, pre_tiles, emit_tiles;
     size_t total;
 };
 
@@ -48,6 +51,9 @@ static inline ScratchLayout make_scratch_layout(int32_t n, uint64_t capacity) {
     L.sort_status = off; off += st * 256 * 4;
     for (int i = 0; i < 2; ++i) { L.pre_keys[i] = off; off += align_up((size_t)n * 4, 256); }
     for (int i = 0; i < 2; ++i) { L.pre_vals[i] = off; off += align_up((size_t)n * 4, 256); }
+    L.pre_incl = off; off += align_up((size_t)n * 4, 256);
+    L.emit_tiles = ((size_t)capacity + EMIT_TILE - 1) / EMIT_TILE;
+    L.emit_starts = off; off += align_up((L.emit_tiles + 1) * 4, 256);
     L.total = align_up(off, 256);
     return L;
 }
