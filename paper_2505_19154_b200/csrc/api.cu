@@ -48,7 +48,7 @@ extern "C" void fhgs_default_params(fhgs_params* p) {
 
 extern "C" size_t fhgs_scratch_bytes(int32_t n, int32_t width, int32_t height, uint64_t capacity) {
     if (n < 0 || width <= 0 || height <= 0) return 0;
-    return make_scratch_layout(n, capacity).total;
+    return make_scratch_layout(n, capacity, width, height).total;
 }
 
 fhgs_status validate_camera(fhgs_ctx* ctx, const fhgs_camera* cam) {
@@ -85,7 +85,7 @@ fhgs_status validate_view_state(fhgs_ctx* ctx, const fhgs_view_state* vs, const 
     if (vs->capacity > 0 && (!vs->keys[0] || !vs->keys[1] || !vs->vals[0] || !vs->vals[1]))
         FHGS_INVALID(ctx, "view_state: NULL key/value buffer");
     if (!aligned_to(vs->conic_opacity, 16) || !aligned_to(vs->xy, 8) || !aligned_to(vs->rect, 8) ||
-        !aligned_to(vs->keys[0], 8) || !aligned_to(vs->keys[1], 8) || !aligned_to(vs->ranges, 8) ||
+        !aligned_to(vs->keys[0], 16) || !aligned_to(vs->keys[1], 16) || !aligned_to(vs->vals[0], 16) || !aligned_to(vs->vals[1], 16) || !aligned_to(vs->ranges, 8) ||
         !aligned_to(vs->scratch, 256) || !aligned_to(vs->num_instances, 8))
         FHGS_INVALID(ctx, "view_state: misaligned buffer");
     if (vs->scratch_bytes < fhgs_scratch_bytes(vs->n, vs->width, vs->height, vs->capacity))

@@ -263,6 +263,7 @@ __global__ void __launch_bounds__(256) emit_partition_kernel(const EmitArgs a) {
 }
 
 constexpr int EMIT_THREADS = 256;
+constexpr int EMIT_ITEMS = EMIT_TILE / EMIT_THREADS;   // 4 consecutive instances per thread
 
 __global__ void __launch_bounds__(EMIT_THREADS) emit_kernel(const EmitArgs a) {
     __shared__ uint32_t s_incl[EMIT_TILE + 1];
@@ -270,6 +271,7 @@ __global__ void __launch_bounds__(EMIT_THREADS) emit_kernel(const EmitArgs a) {
     __shared__ uint32_t s_depth[EMIT_TILE + 1];
     __shared__ uint2 s_rect[EMIT_TILE + 1];
     __shared__ uint32_t s_hist[SORT_MAX_PASSES][256];
+    static_assert(EMIT_ITEMS == 4, "vector stores below assume 4 instances per thread");
     const int tid = threadIdx.x;
     const uint64_t M = *a.num_instances;
     if (M == 0 || M > a.capacity) return;
@@ -290,33 +292,52 @@ __global__ void __launch_bounds__(EMIT_THREADS) emit_kernel(const EmitArgs a) {
         }
         const uint32_t before = g_lo ? __ldg(a.incl + g_lo - 1) : 0u;
         __syncthreads();
+        const uint32_t jl = tid * EMIT_ITEMS;
+        if (jl < cnt) {
+            const uint32_t j = j0 + jl;
+            int lo = 0, hi = span - 1;
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (s_incl[mid] > j) hi = mid; else lo = mid + 1;
+            }
+            // walk the (up to) 4 consecutive instances: position inside the owner's rect advances in row-major order
+            uint32_t end = s_incl[lo];
+            uint32_t local = j - (lo ? s_incl[lo - 1] : before);
+            uint2 rc = s_rect[lo];
+            uint32_t x0 = rc.x & 0xffffu, x1 = rc.y & 0xffffu, w = x1 - x0;
+            uint32_t ty = (rc.x >> 16) + local / w, tx = x0 + local % w;
+            uint32_t zb = s_depth[lo], gid = s_gid[lo];
+            uint64_t k[EMIT_ITEMS];
+            uint32_t v[EMIT_ITEMS], tl[EMIT_ITEMS];
 #pragma unroll
-        for (int r = 0; r < EMIT_TILE / EMIT_THREADS; ++r) {
-            const uint32_t jl = r * EMIT_THREADS + tid;
-            const bool valid = jl < cnt;
-            uint32_t tile_id = 0xffffffffu;
-            if (valid) {
-                const uint32_t j = j0 + jl;
-                int lo = 0, hi = span - 1;
-                while (lo < hi) {
-                    const int mid = (lo + hi) >> 1;
-                    if (s_incl[mid] > j) hi = mid; else lo = mid + 1;
+            for (int e = 0; e < EMIT_ITEMS; ++e) {
+                tl[e] = ty * (uint32_t)a.GW + tx;
+                k[e] = ((uint64_t)tl[e] << 32) | (uint64_t)zb;
+                v[e] = gid;
+                if (e + 1 < EMIT_ITEMS && jl + e + 1 < cnt) {
+                    if (j + e + 1 == end) {   // next owner (every staged Gaussian has >= 1 instance)
+                        ++lo;
+                        end = s_incl[lo];
+                        rc = s_rect[lo];
+                        x0 = rc.x & 0xffffu; x1 = rc.y & 0xffffu;
+                        ty = rc.x >> 16; tx = x0;
+                        zb = s_depth[lo]; gid = s_gid[lo];
+                    } else if (++tx == x1) {
+                        tx = x0; ++ty;
+                    }
                 }
-                const uint32_t start = lo ? s_incl[lo - 1] : before;
-                const uint32_t local = j - start;
-                const uint2 rc = s_rect[lo];
-                const uint32_t x0 = rc.x & 0xffffu, y0 = rc.x >> 16, x1 = rc.y & 0xffffu;
-                const uint32_t w = x1 - x0;
-                const uint32_t ry = local / w;
-                tile_id = (y0 + ry) * (uint32_t)a.GW + x0 + (local - ry * w);
-                a.keys[j] = ((uint64_t)tile_id << 32) | (uint64_t)s_depth[lo];
-                a.vals[j] = s_gid[lo];
             }
-            for (int p = 0; p < a.npass; ++p) {
-                const uint32_t d = valid ? ((tile_id >> (8 * p)) & 255u) : 256u;
-                const uint32_t peers = __match_any_sync(FULL, d);
-                if (valid && (peers & lanemask_lt()) == 0) atomicAdd(&s_hist[p][d], (uint32_t)__popc(peers));
+            if (jl + EMIT_ITEMS <= cnt) {
+                *reinterpret_cast<ulonglong2*>(a.keys + j) = make_ulonglong2(k[0], k[1]);
+                *reinterpret_cast<ulonglong2*>(a.keys + j + 2) = make_ulonglong2(k[2], k[3]);
+                *reinterpret_cast<uint4*>(a.vals + j) = make_uint4(v[0], v[1], v[2], v[3]);
+            } else {
+                for (int e = 0; e < EMIT_ITEMS; ++e)
+                    if (jl + e < cnt) { a.keys[j + e] = k[e]; a.vals[j + e] = v[e]; }
             }
+            for (int p = 0; p < a.npass; ++p)
+                for (int e = 0; e < EMIT_ITEMS; ++e)
+                    if (jl + e < cnt) atomicAdd(&s_hist[p][(tl[e] >> (8 * p)) & 255u], 1u);
         }
     }
     __syncthreads();
@@ -349,22 +370,114 @@ __global__ void __launch_bounds__(256) hist_scan_kernel(uint32_t* hist) {
 // depth pre-sort input: key = depth bits (0xffffffff for culled Gaussians), val = index;
 // accumulates the four digit histograms of the 32-bit keys.
 // ------------------------------------------------------------------------------------------------
+// When `diff` is given (tile grid small enough for shared memory) the kernel also accumulates the 2-D
+// difference array of the per-tile instance counts: +1 at (y0,x0), -1 at (y0,x1), -1 at (y1,x0),
+// +1 at (y1,x1) for every visible Gaussian; its 2-D prefix sum (tile_scan_kernel) is the number of
+// instances of every tile, from which the tile ranges and the tile-digit histograms follow without
+// touching the instance list.
 __global__ void __launch_bounds__(256) presort_init_kernel(int n, const float* depth, const uint32_t* tiles_touched,
-                                                           uint32_t* keys, uint32_t* vals, uint32_t* hist32) {
+                                                           uint32_t* keys, uint32_t* vals, uint32_t* hist32,
+                                                           const uint16_t* rect, int gw1, int gh1, int* diff) {
+    extern __shared__ int s_diff[];
     __shared__ uint32_t s_hist[4][256];
     for (int j = threadIdx.x; j < 1024; j += 256) (&s_hist[0][0])[j] = 0;
+    const int cells = diff ? gw1 * gh1 : 0;
+    for (int j = threadIdx.x; j < cells; j += 256) s_diff[j] = 0;
     __syncthreads();
     for (int i = blockIdx.x * 256 + threadIdx.x; i < n; i += gridDim.x * 256) {
-        const uint32_t k = __ldg(tiles_touched + i) ? __float_as_uint(__ldg(depth + i)) : 0xffffffffu;
+        const bool vis = __ldg(tiles_touched + i) != 0;
+        const uint32_t k = vis ? __float_as_uint(__ldg(depth + i)) : 0xffffffffu;
         keys[i] = k;
         vals[i] = (uint32_t)i;
 #pragma unroll
         for (int p = 0; p < 4; ++p) atomicAdd(&s_hist[p][(k >> (8 * p)) & 255u], 1u);
+        if (diff && vis) {
+            const uint2 rc = __ldg(reinterpret_cast<const uint2*>(rect) + i);
+            const int x0 = rc.x & 0xffffu, y0 = rc.x >> 16, x1 = rc.y & 0xffffu, y1 = rc.y >> 16;
+            atomicAdd(&s_diff[y0 * gw1 + x0], 1);
+            atomicAdd(&s_diff[y0 * gw1 + x1], -1);
+            atomicAdd(&s_diff[y1 * gw1 + x0], -1);
+            atomicAdd(&s_diff[y1 * gw1 + x1], 1);
+        }
     }
     __syncthreads();
     for (int j = threadIdx.x; j < 1024; j += 256) {
         const uint32_t c = (&s_hist[0][0])[j];
         if (c) atomicAdd(hist32 + j, c);
+    }
+    for (int j = threadIdx.x; j < cells; j += 256) {
+        const int c = s_diff[j];
+        if (c) atomicAdd(diff + j, c);
+    }
+}
+
+// One CTA: 2-D prefix sum of the difference grid -> per-tile instance counts -> tile ranges
+// (C1-S step 4: exclusive prefix over tile ids, (0,0) for empty tiles) and the exclusive digit
+// histograms of the tile-id sort passes.  Nothing is written when M > capacity.
+constexpr int TS_THREADS = 1024;
+__global__ void __launch_bounds__(TS_THREADS) tile_scan_kernel(const int* diff, int gw1, int gh1, const uint64_t* num_instances,
+                                                               uint64_t capacity, uint32_t* ranges, uint32_t* hist, int npass) {
+    extern __shared__ int s_g[];                 // [gh1][gw1]
+    __shared__ uint32_t s_h[SORT_MAX_PASSES][256];
+    __shared__ uint32_t s_part[TS_THREADS / 32];
+    __shared__ uint32_t s_carry;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint64_t M = *num_instances;
+    if (M > capacity) return;
+    const int GW = gw1 - 1, GH = gh1 - 1, cells = gw1 * gh1, ntiles = GW * GH;
+    for (int j = tid; j < cells; j += TS_THREADS) s_g[j] = diff[j];
+    for (int j = tid; j < npass * 256; j += TS_THREADS) (&s_h[0][0])[j] = 0;
+    if (tid == 0) s_carry = 0;
+    __syncthreads();
+    for (int y = tid; y < gh1; y += TS_THREADS) {      // prefix along x
+        int run = 0;
+        for (int x = 0; x < gw1; ++x) { run += s_g[y * gw1 + x]; s_g[y * gw1 + x] = run; }
+    }
+    __syncthreads();
+    for (int x = tid; x < gw1; x += TS_THREADS) {      // prefix along y
+        int run = 0;
+        for (int y = 0; y < gh1; ++y) { run += s_g[y * gw1 + x]; s_g[y * gw1 + x] = run; }
+    }
+    __syncthreads();
+    // exclusive scan over tile ids, TS_THREADS tiles per round
+    for (int base = 0; base < ntiles; base += TS_THREADS) {
+        const int t = base + tid;
+        uint32_t c = 0;
+        if (t < ntiles) c = (uint32_t)s_g[(t / GW) * gw1 + (t % GW)];
+        uint32_t incl = c;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const uint32_t o = __shfl_up_sync(FULL, incl, d);
+            if (lane >= d) incl += o;
+        }
+        if (lane == 31) s_part[warp] = incl;
+        __syncthreads();
+        uint32_t off = s_carry;
+        for (int w = 0; w < warp; ++w) off += s_part[w];
+        const uint32_t excl = off + incl - c;
+        if (t < ntiles && c) {
+            ranges[2 * (size_t)t] = excl;
+            ranges[2 * (size_t)t + 1] = excl + c;
+            for (int p = 0; p < npass; ++p) atomicAdd(&s_h[p][((uint32_t)t >> (8 * p)) & 255u], c);
+        }
+        __syncthreads();
+        if (tid == TS_THREADS - 1) s_carry = excl + c;
+        __syncthreads();
+    }
+    // exclusive scan of every digit histogram (warp w handles pass w)
+    if (warp < npass) {
+        uint32_t run = 0;
+        for (int b = 0; b < 256; b += 32) {
+            const uint32_t c = s_h[warp][b + lane];
+            uint32_t incl = c;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const uint32_t o = __shfl_up_sync(FULL, incl, d);
+                if (lane >= d) incl += o;
+            }
+            hist[warp * 256 + b + lane] = run + incl - c;
+            run += __shfl_sync(FULL, incl, 31);
+        }
     }
 }
 
@@ -548,7 +661,7 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
     cudaStream_t s = (cudaStream_t)stream;
     const int GW = tiles_x(cam->width), GH = tiles_y(cam->height);
     const size_t ntiles = (size_t)GW * GH;
-    const ScratchLayout L = make_scratch_layout(vs->n, vs->capacity);
+    const ScratchLayout L = make_scratch_layout(vs->n, vs->capacity, cam->width, cam->height);
     char* sc = (char*)vs->scratch;
     uint32_t* ctrl = (uint32_t*)(sc + L.ctrl);
     uint32_t* hist = (uint32_t*)(sc + L.hist);
@@ -563,6 +676,12 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
 
     const int tile_bits = ceil_log2(ntiles);
     const bool full_key = (flags & FHGS_SORT_FULL_KEY) != 0;
+    // per-tile counts through the 2-D difference grid (default schedule, grid small enough for shared memory)
+    const int gw1 = GW + 1, gh1 = GH + 1;
+    const bool grid_counts = !full_key && vs->capacity > 0 && (size_t)gw1 * gh1 <= (size_t)TILE_GRID_MAX;
+    int* tile_diff = (int*)(sc + L.tile_diff);
+    const size_t diff_bytes = (size_t)gw1 * gh1 * 4;
+    if (grid_counts) FHGS_CUDA(ctx, cudaMemsetAsync(tile_diff, 0, diff_bytes, s));
     const int first_bit = full_key ? 0 : 32;
     const int npass = ((32 + tile_bits) - first_bit + 7) / 8;
     vs->sorted_buf = npass & 1;
@@ -574,8 +693,11 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
             // order the Gaussians by (depth bits, index): 4 stable passes over 32-bit keys
             uint32_t* pk[2] = {(uint32_t*)(sc + L.pre_keys[0]), (uint32_t*)(sc + L.pre_keys[1])};
             uint32_t* pv[2] = {(uint32_t*)(sc + L.pre_vals[0]), (uint32_t*)(sc + L.pre_vals[1])};
-            const int grid = std::min((vs->n + 255) / 256, ctx->num_sms * 8);
-            presort_init_kernel<<<grid, 256, 0, s>>>(vs->n, vs->depth, vs->tiles_touched, pk[0], pv[0], hist32);
+            const int grid = std::min((vs->n + 255) / 256, ctx->num_sms * (grid_counts ? 4 : 8));
+            if (grid_counts)
+                FHGS_CUDA(ctx, cudaFuncSetAttribute(presort_init_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)diff_bytes));
+            presort_init_kernel<<<grid, 256, grid_counts ? diff_bytes : 0, s>>>(vs->n, vs->depth, vs->tiles_touched, pk[0], pv[0], hist32,
+                                                                               vs->rect, gw1, gh1, grid_counts ? tile_diff : nullptr);
             FHGS_LAUNCH_CHECK(ctx);
             hist_scan_kernel<<<4, 256, 0, s>>>(hist32);
             FHGS_LAUNCH_CHECK(ctx);
@@ -628,7 +750,12 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
             ea.n = vs->n; ea.GW = GW; ea.perm = perm; ea.incl = incl; ea.rect = vs->rect; ea.depth = vs->depth;
             ea.num_instances = vs->num_instances; ea.capacity = vs->capacity;
             ea.starts = (uint32_t*)(sc + L.emit_starts); ea.units = (int)L.emit_tiles;
-            ea.keys = vs->keys[0]; ea.vals = vs->vals[0]; ea.hist = hist; ea.npass = npass;
+            ea.keys = vs->keys[0]; ea.vals = vs->vals[0]; ea.hist = hist; ea.npass = grid_counts ? 0 : npass;
+            if (grid_counts) {   // ranges and digit offsets from the per-tile counts
+                FHGS_CUDA(ctx, cudaFuncSetAttribute(tile_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)diff_bytes));
+                tile_scan_kernel<<<1, TS_THREADS, diff_bytes, s>>>(tile_diff, gw1, gh1, vs->num_instances, vs->capacity, vs->ranges, hist, npass);
+                FHGS_LAUNCH_CHECK(ctx);
+            }
             emit_partition_kernel<<<(ea.units + 1 + 255) / 256, 256, 0, s>>>(ea);
             FHGS_LAUNCH_CHECK(ctx);
             const int egrid = std::min(ea.units, ctx->num_sms * 8);
@@ -637,8 +764,10 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
         }
 
         if (vs->capacity > 0) {
-            hist_scan_kernel<<<npass, 256, 0, s>>>(hist);
-            FHGS_LAUNCH_CHECK(ctx);
+            if (!grid_counts) {
+                hist_scan_kernel<<<npass, 256, 0, s>>>(hist);
+                FHGS_LAUNCH_CHECK(ctx);
+            }
             const int sort_grid = (int)((vs->capacity + SORT_TILE_K64 - 1) / SORT_TILE_K64);
             for (int p = 0; p < npass; ++p) {
                 FHGS_CUDA(ctx, cudaMemsetAsync(sort_status, 0, (size_t)sort_grid * 256 * 4, s));
@@ -651,11 +780,13 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
                 onesweep_kernel<uint64_t, SORT_TILE_K64 / OS_THREADS><<<sort_grid, OS_THREADS, 0, s>>>(oa);
                 FHGS_LAUNCH_CHECK(ctx);
             }
-            uint64_t rg = (vs->capacity + 255) / 256;
-            if (rg > (uint64_t)ctx->num_sms * 16) rg = (uint64_t)ctx->num_sms * 16;
-            const int rgrid = (int)rg;
-            ranges_kernel<<<rgrid, 256, 0, s>>>(vs->keys[vs->sorted_buf], vs->num_instances, vs->capacity, vs->ranges);
-            FHGS_LAUNCH_CHECK(ctx);
+            if (!grid_counts) {
+                uint64_t rg = (vs->capacity + 255) / 256;
+                if (rg > (uint64_t)ctx->num_sms * 16) rg = (uint64_t)ctx->num_sms * 16;
+                const int rgrid = (int)rg;
+                ranges_kernel<<<rgrid, 256, 0, s>>>(vs->keys[vs->sorted_buf], vs->num_instances, vs->capacity, vs->ranges);
+                FHGS_LAUNCH_CHECK(ctx);
+            }
         }
     }
     if (num_instances_host) {

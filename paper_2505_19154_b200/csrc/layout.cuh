@@ -7,6 +7,7 @@ constexpr int SCAN_TILE = 1024;        // Gaussians per CTA of the scan+duplicat
 constexpr int SORT_TILE_K64 = 4096;    // pairs per CTA of a 64-bit-key onesweep pass
 constexpr int SORT_TILE_K32 = 4096;    // pairs per CTA of a 32-bit-key onesweep pass
 constexpr int SORT_MAX_PASSES = 8;
+constexpr int TILE_GRID_MAX = 12288;   // (GW+1)*(GH+1) limit of the shared-memory tile-count path (48 KB)
 constexpr int EMIT_TILE = 1024;        // instances per work unit of the balanced emission kernel
 
 // ctrl words (uint32_t)
@@ -30,13 +31,14 @@ struct ScratchLayout {
     size_t pre_vals[2];   // uint32_t[n]  Gaussian index (ping-pong)
     size_t pre_incl;      // uint32_t[n]  inclusive prefix of tiles_touched in depth order
     size_t emit_starts;   // uint32_t[emit_tiles + 1]  first depth-ordered Gaussian of every EMIT_TILE instances
+    size_t tile_diff;     // int32_t[(GW+1)*(GH+1)]  2-D difference array of the per-tile instance counts
     size_t scan_tiles, sort_tiles, pre_tiles, emit_tiles;
     size_t total;
 };
 
 static inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-static inline ScratchLayout make_scratch_layout(int32_t n, uint64_t capacity) {
+static inline ScratchLayout make_scratch_layout(int32_t n, uint64_t capacity, int32_t width = 0, int32_t height = 0) {
     ScratchLayout L;
     size_t off = 0;
     L.ctrl = off; off += align_up(CTRL_WORDS * 4, 256);
@@ -54,6 +56,8 @@ static inline ScratchLayout make_scratch_layout(int32_t n, uint64_t capacity) {
     L.pre_incl = off; off += align_up((size_t)n * 4, 256);
     L.emit_tiles = ((size_t)capacity + EMIT_TILE - 1) / EMIT_TILE;
     L.emit_starts = off; off += align_up((L.emit_tiles + 1) * 4, 256);
+    const size_t gw1 = (size_t)((width + 15) / 16 + 1), gh1 = (size_t)((height + 15) / 16 + 1);
+    L.tile_diff = off; off += align_up(gw1 * gh1 * 4, 256);   // last: the regions above do not depend on width/height
     L.total = align_up(off, 256);
     return L;
 }

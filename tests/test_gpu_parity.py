@@ -114,6 +114,22 @@ def test_odd_d_paths():
         print(d, run_case(cfg, [1], pu.TOL_F32, sort_flags=(0,)))
 
 
+def test_large_tile_grid_fallback_sort():
+    """2064x1616 px -> (GW+1)*(GH+1) = 130*102 > 12288: fhgs_bin_sort leaves the shared-memory tile-count
+    path and derives histograms / ranges from the instance list; both schedules, integers bit-exact."""
+    cfg = pu.reduced_config("tiny", n=4000, width=2064, height=1616, log_scale_mu=-2.2)
+    scene = inputs.make_scene(cfg)
+    cam = inputs.make_camera(cfg, 1)
+    pr = pu.oracle_view(scene, cam)
+    bo = fo.bins(pr, cfg.width, cfg.height)
+    gp = pu.GpuPath(scene, cfg.width, cfg.height, bo["M"] + 7)
+    for fl in (0, 1):
+        c, m = gp.project_sort(cam, flags=fl)
+        pu.check_projection(pr, gp.vs.projected())
+        pu.check_bins(bo, gp.vs, m)
+    print("M =", bo["M"])
+
+
 def test_edge_cases():
     import torch
     from paper_2505_19154_b200 import binding as fb
