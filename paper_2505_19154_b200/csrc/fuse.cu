@@ -202,6 +202,7 @@ constexpr int FW_STAGES = 2;
 constexpr int FW_DC = 128;
 constexpr int FW_THREADS = WS_THREADS + 32;
 constexpr int FW_BAR_CONS = 3;
+constexpr int FW_WQ = (WS_CONS + 1) * 4;   // floats per quad row: 256 pixels x float4 + 16 B pad (bank spread over quads)
 enum { FW_FLAG_FIRST = 4 };
 
 struct FuseWsSmem {
@@ -211,9 +212,10 @@ struct FuseWsSmem {
     int items[2];
     __align__(16) uint32_t ids[FW_STAGES][WS_KB];
     __align__(16) float den_s[2][WS_KB];
-    __align__(128) float W[FW_STAGES][WS_CONS * WS_KB];   // [pixel][quad ^ (pixel & 7)][4]
+    __align__(128) float W[FW_STAGES][FW_WQ * WS_KB / 4];  // [quad kk/4][pixel][4], quad stride padded by one float4
     __align__(128) float P[WS_KB * FW_DC];                // partial sums of the writing half
     __align__(128) float G[WS_CONS * FW_DC];              // [pixel][channel], pixel = y*16 + x
+    float G_pad[FW_DC];                                   // target of the consumers' one-past-the-end prefetch
 };
 
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
@@ -308,7 +310,7 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem& sm, const FuseArgs&
             const int nb = min(WS_KB, qt - qh);
             mbar_wait_backoff(&sm.ct.empty[stage], phase ^ 1u);
             if (p < WS_KB) sm.ids[stage][p] = p < nb ? __float_as_uint(sm.ct.rec1[(qh + p) & (WS_QCAP - 1)].z) : 0u;
-            float* Wd = sm.W[stage] + p * WS_KB;
+            float* Wd = sm.W[stage] + p * 4;
             const bool warp_done = __all_sync(TR_FULL, P.done);
 #pragma unroll 2
             for (int kq = 0; kq < WS_KB / 4; ++kq) {
@@ -325,7 +327,7 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem& sm, const FuseArgs&
                         if (kk < nb) { P = Q; w4[j] = w; }
                     }
                 }
-                *reinterpret_cast<float4*>(Wd + ((kq ^ (p & 7)) << 2)) = make_float4(w4[0], w4[1], w4[2], w4[3]);
+                *reinterpret_cast<float4*>(Wd + kq * FW_WQ) = make_float4(w4[0], w4[1], w4[2], w4[3]);
             }
             qh += nb;
             const bool all_done = named_bar_and(WS_BAR_PROD_RED, WS_PROD, P.done);
@@ -367,15 +369,22 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem& sm, const FuseArgs&
         for (int i = 0; i < 4; ++i)
 #pragma unroll
             for (int c = 0; c < 4; ++c) acc[i][c] = 0ull;
-        const float* Ws = sm.W[stage] + half * 128 * WS_KB;
+        // W for pixel s, instances 8 kg .. 8 kg + 7: two float4 at fixed offsets from one base -> no address arithmetic
+        const float* Ws = sm.W[stage] + (2 * kg) * FW_WQ + half * 128 * 4;
+        // software-pipelined over pixels: the operands of pixel s+1 are in flight while pixel s is multiplied
+        ulonglong2 wa = *reinterpret_cast<const ulonglong2*>(Ws);
+        ulonglong2 wb = *reinterpret_cast<const ulonglong2*>(Ws + FW_WQ);
+        float4 g = *reinterpret_cast<const float4*>(Gs);
 #pragma unroll 1
-        for (int s0 = 0; s0 < 128; s0 += 8) {
+        for (int s0 = 0; s0 < 128; s0 += 16) {
+            const float* Wb = Ws + s0 * 4;
+            const float* Gb = Gs + s0 * FW_DC;
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const int s = s0 + u;   // (s & 7) == u
-                const ulonglong2 wa = *reinterpret_cast<const ulonglong2*>(Ws + s * WS_KB + (((2 * kg) ^ u) << 2));
-                const ulonglong2 wb = *reinterpret_cast<const ulonglong2*>(Ws + s * WS_KB + (((2 * kg + 1) ^ u) << 2));
-                const float4 g = *reinterpret_cast<const float4*>(Gs + s * FW_DC);
+            for (int u = 0; u < 16; ++u) {
+                const int un = u + 1;   // the prefetch past the last pixel lands in the row pad / G_pad (never used)
+                const ulonglong2 wa_n = *reinterpret_cast<const ulonglong2*>(Wb + un * 4);
+                const ulonglong2 wb_n = *reinterpret_cast<const ulonglong2*>(Wb + FW_WQ + un * 4);
+                const float4 g_n = *reinterpret_cast<const float4*>(Gb + un * FW_DC);
                 const unsigned long long g2[4] = {pack2(g.x, g.x), pack2(g.y, g.y), pack2(g.z, g.z), pack2(g.w, g.w)};
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
@@ -384,15 +393,16 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem& sm, const FuseArgs&
                     acc[2][c] = fma2(wb.x, g2[c], acc[2][c]);
                     acc[3][c] = fma2(wb.y, g2[c], acc[3][c]);
                 }
+                wa = wa_n; wb = wb_n; g = g_n;
             }
         }
         // den partial: warp (half, cw) sums pixels [128 half + 32 cw, +32) for instance kk = lane
         {
-            const float* Wp = Ws + cw * 32 * WS_KB;
-            float dsum = 0.f;
-#pragma unroll 8
-            for (int j = 0; j < 32; ++j) dsum += Wp[j * WS_KB + ((((lane >> 2) ^ (j & 7)) << 2) | (lane & 3))];
-            atomicAdd(&sm.den_s[batch & 1][lane], dsum);
+            const float* Wp = sm.W[stage] + (lane >> 2) * FW_WQ + (half * 128 + cw * 32) * 4 + (lane & 3);
+            float d0 = 0.f, d1 = 0.f;
+#pragma unroll
+            for (int j = 0; j < 32; j += 2) { d0 += Wp[j * 4]; d1 += Wp[j * 4 + 4]; }
+            atomicAdd(&sm.den_s[batch & 1][lane], d0 + d1);
         }
         mbar_arrive(&sm.ct.empty[stage]);
         if (m.flags & WS_FLAG_LAST) mbar_arrive(&sm.g_free);
@@ -452,7 +462,7 @@ __global__ void __launch_bounds__(FW_THREADS, 1) fuse_ws_kernel(const FuseArgs a
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     // the GT tile buffer must never hold non-finite garbage (pixels outside the image keep stale data, weight 0)
-    for (int i = threadIdx.x; i < WS_CONS * FW_DC / 4; i += FW_THREADS) reinterpret_cast<float4*>(sm.G)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int i = threadIdx.x; i < (WS_CONS + 1) * FW_DC / 4; i += FW_THREADS) reinterpret_cast<float4*>(sm.G)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (threadIdx.x < 2 * WS_KB) (&sm.den_s[0][0])[threadIdx.x] = 0.f;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
