@@ -12,13 +12,16 @@ import parity_util as pu
 pytestmark = pytest.mark.gpu
 
 
-def run_case(cfg, views, tol, literal_pixels=None, sort_flags=(0, 1), capacity_slack=1.25, check_finalize=True):
+def run_case(cfg, views, tol, literal_pixels=None, sort_flags=(0, 1), capacity_slack=1.25, check_finalize=True,
+             fixed_capacity=None):
     """Full P -> S -> R -> F parity of one config over `views`; returns worst errors."""
     scene = inputs.make_scene(cfg)
     cams = [inputs.make_camera(cfg, v) for v in views]
     prs = [pu.oracle_view(scene, cam) for cam in cams]
     bins = [fo.bins(pr, cfg.width, cfg.height) for pr in prs]
     cap = int(max(b["M"] for b in bins) * capacity_slack) + 16
+    if fixed_capacity is not None:
+        cap = fixed_capacity
     gp = pu.GpuPath(scene, cfg.width, cfg.height, cap)
     feat32 = scene.feat.astype(np.float32)
     fabs = float(np.abs(feat32).max())
@@ -112,6 +115,31 @@ def test_odd_d_paths():
     for d in (4, 24):
         cfg = pu.reduced_config("tiny", n=3000, feat_dim=d, width=80, height=48)
         print(d, run_case(cfg, [1], pu.TOL_F32, sort_flags=(0,)))
+
+
+def test_mid_full_size_bench_configuration():
+    """configs[2] at FULL size, exactly as bench.py launches it (N=10^6, SH3, D=128 fp32, 1920x1080, default sort
+    schedule, capacity 40e6): every integer output bit-exact (radius, rect, tiles_touched, M, offsets, all 3.2e7 sorted
+    keys and values, ranges, n_contrib), every float of the image / feature image / fused vectors within 1e-4."""
+    cfg = inputs.CONFIGS["mid"]
+    w = run_case(cfg, [0], pu.TOL_F32, sort_flags=(0,), capacity_slack=1.0, fixed_capacity=int(40e6))
+    print(w)
+
+
+def test_large_full_size_sampled_pixels():
+    """configs[3] at FULL size (N=3*10^6, D=512 fp16, 1920x1080): projection and the whole sorted instance list
+    (9.5e7 pairs) bit-exact; the rendered image on 300 random pixels against the literal per-pixel oracle."""
+    cfg = inputs.CONFIGS["large"]
+    w = run_case(cfg, [0], pu.TOL_F16, literal_pixels=300, sort_flags=(0,), capacity_slack=1.02)
+    print(w)
+
+
+def test_multiview_full_size_two_views():
+    """configs[4] at FULL size (N=2*10^6 in 64 blobs, D=256 fp32, 1296x968), views 0 and 100 of the 200-camera orbit
+    fused into one accumulator: full element-by-element parity of P, S, R, F."""
+    cfg = inputs.CONFIGS["multiview"]
+    w = run_case(cfg, [0, 100], pu.TOL_F32, sort_flags=(0,), capacity_slack=1.02)
+    print(w)
 
 
 def test_large_tile_grid_fallback_sort():
