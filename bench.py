@@ -167,19 +167,31 @@ def run_reference(args, rank: int):
 # the CUDA arm
 # --------------------------------------------------------------------------------------------------
 def launches_per_frame(width: int, height: int) -> int:
-    """Kernels of libfhgs.so launched per frame (default sort schedule): project 1; bin_sort =
-    presort_init 1 + hist_scan 1 + 4 depth onesweep passes + offsets scan 1 + scan_dup 1 +
-    hist_scan 1 + ceil(tile_bits/8) tile-id onesweep passes + ranges 1; render 1; fuse 1 + finalise 1."""
-    tiles = ((width + 15) // 16) * ((height + 15) // 16)
-    tile_bits = max(1, (tiles - 1).bit_length())
-    return 1 + (1 + 1 + 4 + 1 + 1 + 1 + (tile_bits + 7) // 8 + 1) + 1 + 2
+    """Kernels of libfhgs.so launched per frame (default sort schedule; memsets are not kernels): project 1;
+    bin_sort = presort_init 1 + hist_scan 1 + 4 depth onesweep passes + offsets scan 1 + depth-order scan 1 +
+    [tile_scan 1 | hist_scan 1 + ranges 1] + emit_partition 1 + emit 1 + ceil(tile_bits/8) tile-id onesweep passes;
+    render 1; fuse 1 + finalise 1."""
+    gw, gh = (width + 15) // 16, (height + 15) // 16
+    tile_bits = max(1, (gw * gh - 1).bit_length())
+    grid_counts = (gw + 1) * (gh + 1) <= 12288
+    return 1 + (1 + 1 + 4 + 1 + 1 + (1 if grid_counts else 2) + 1 + 1 + (tile_bits + 7) // 8) + 1 + 2
+
+
+def load_traffic() -> dict:
+    """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the hot kernels, from the committed
+    `ncu --set full` capture summarised in profiles/ (bench.py never runs under a profiler)."""
+    path = os.path.join(ROOT, "profiles", "r01_traffic.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f)
+    return {}
 
 
 def run_cuda(args, rank: int, world: int, local_rank: int):
     import torch
     import torch.distributed as dist
     from paper_2505_19154_b200 import binding as fb   # fails loudly without libfhgs.so
-    from paper_2505_19154_b200 import inputs
+    from paper_2505_19154_b200 import inputs, parallel
 
     if not torch.cuda.is_available():
         raise RuntimeError("bench.py needs a CUDA device: the FHGS path has no CPU fallback")
@@ -254,11 +266,7 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
         frame(evs[k])
     barrier()
     clocks = sampler.stop()
-    total_ms = evs[0][0].elapsed_time(evs[-1][6])
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = parallel.max_over_ranks(evs[0][0].elapsed_time(evs[-1][6]), dev)
     ms_per_step = total_ms / args.steps
     value = world * args.steps / (total_ms * 1e-3)
     parts = {nm: statistics.mean(evs[k][i].elapsed_time(evs[k][i + 1]) for k in range(args.steps))
@@ -296,12 +304,15 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     steps_roof["fuse_accumulate"]["hbm_gbs_gt_map"] = work["fuse_bytes"] / (parts["fuse_accumulate"] * 1e-3) / 1e9
     dominant = max(("render", "fuse_accumulate", "bin_sort", "project", "fuse_finalize"), key=lambda k: parts[k])
     roofline = dict(steps_roof[dominant])
-    roofline["kernel"] = {"render": "render_tiled_kernel<128,float>", "fuse_accumulate": "fuse_tiled_kernel<128,float>",
-                          "bin_sort": "fhgs_bin_sort (13 launches)", "project": "project_kernel",
+    roofline["kernel"] = {"render": "render_ws_kernel<128,float>", "fuse_accumulate": "fuse_ws_kernel",
+                          "bin_sort": "fhgs_bin_sort (14 launches)", "project": "project_kernel<3>",
                           "fuse_finalize": "finalize_kernel<float>"}[dominant]
     roofline["peak_source"] = ("148 SMs x 128 FP32 lanes x sm_max_mhz (MEASURED_PEAKS.json), FMA = 2 flop"
                                if roofline["bound"] == "alu" else f"hbm_gbs of MEASURED_PEAKS.json ({peaks['source']})")
-    roofline["traffic"] = None
+    traffic = load_traffic().get(roofline["kernel"])
+    roofline["traffic"] = traffic["dram_bytes_per_launch"] if traffic else None
+    if traffic:
+        roofline["traffic_source"] = traffic["source"]
 
     # ---- end to end through fhgs_frame_host: host (pinned) buffers, copies inside the timed region
     e2e = None
@@ -324,10 +335,7 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
             fb.frame_host(ctx, host, g, cam, prm, vs, ws)   # synchronises the stream before returning
         barrier()
         e_s = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([e_s], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e_s = float(t.item())
+        e_s = parallel.max_over_ranks(e_s, dev)
         e2e = {"value": world * e_steps / e_s, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                "steps": e_steps, "ms_per_step": 1e3 * e_s / e_steps}
         del host
