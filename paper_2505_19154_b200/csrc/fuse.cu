@@ -388,10 +388,10 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem& sm, const FuseArgs&
                 const unsigned long long g2[4] = {pack2(g.x, g.x), pack2(g.y, g.y), pack2(g.z, g.z), pack2(g.w, g.w)};
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
-                    acc[0][c] = fma2(wa.x, g2[c], acc[0][c]);
-                    acc[1][c] = fma2(wa.y, g2[c], acc[1][c]);
-                    acc[2][c] = fma2(wb.x, g2[c], acc[2][c]);
-                    acc[3][c] = fma2(wb.y, g2[c], acc[3][c]);
+                    fma2_acc(acc[0][c], wa.x, g2[c]);
+                    fma2_acc(acc[1][c], wa.y, g2[c]);
+                    fma2_acc(acc[2][c], wb.x, g2[c]);
+                    fma2_acc(acc[3][c], wb.y, g2[c]);
                 }
                 wa = wa_n; wb = wb_n; g = g_n;
             }

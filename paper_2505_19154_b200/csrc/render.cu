@@ -38,6 +38,8 @@ template <typename FT> struct FeatIO;
 template <> struct FeatIO<float> {
     static __device__ __forceinline__ float4 load4(const float* p) { return *reinterpret_cast<const float4*>(p); }
     static __device__ __forceinline__ void store4(float* p, float4 v) { *reinterpret_cast<float4*>(p) = v; }
+    // 4 consecutive channels as two packed pairs, straight from the 16-byte load (no repacking moves)
+    static __device__ __forceinline__ ulonglong2 load_pairs(const float* p) { return *reinterpret_cast<const ulonglong2*>(p); }
 };
 template <> struct FeatIO<__half> {
     static __device__ __forceinline__ float4 load4(const __half* p) {
@@ -52,6 +54,10 @@ template <> struct FeatIO<__half> {
         r.x = *reinterpret_cast<const uint32_t*>(&a);
         r.y = *reinterpret_cast<const uint32_t*>(&b);
         *reinterpret_cast<uint2*>(p) = r;
+    }
+    static __device__ __forceinline__ ulonglong2 load_pairs(const __half* p) {
+        const float4 f = load4(p);
+        return make_ulonglong2(pack2(f.x, f.y), pack2(f.z, f.w));
     }
 };
 
@@ -162,59 +168,59 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT>& sm, con
     const int pgl = lane >> 3, cg = lane & 7;
     const int pg = warp * 4 + pgl;   // 8-pixel row run: slots pg*8 .. pg*8+7
     FT* out_feat = reinterpret_cast<FT*>(a.out_feat);
-    unsigned long long acc[8][NJ * 2];   // packed channel pairs (fma.rn.f32x2)
-#pragma unroll
-    for (int i = 0; i < 8; ++i)
-#pragma unroll
-        for (int j = 0; j < NJ * 2; ++j) acc[i][j] = 0ull;
     int stage = 0;
     uint32_t phase = 0;
-    while (true) {
-        mbar_wait(&sm.ct.full[stage], phase);
-        const WsMeta m = sm.ct.meta[stage];
-        if (m.flags & WS_FLAG_EXIT) break;
-        uint32_t mk = sm.ct.mask[stage][warp];
-        const float* Ws = sm.W[stage] + pg * 8;
-        const FT* Fs = sm.F[stage] + cg * 4;
-        while (mk) {
-            const int kk = __ffs(mk) - 1;
-            mk &= mk - 1u;
-            const float4 wa = *reinterpret_cast<const float4*>(Ws + kk * WS_CONS);
-            const float4 wb = *reinterpret_cast<const float4*>(Ws + kk * WS_CONS + 4);
-            const float wv[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
-            unsigned long long fv[NJ * 2];
+    while (true) {   // one iteration per work item: accumulators live exactly one item
+        unsigned long long acc[8][NJ * 2];   // packed channel pairs (fma.rn.f32x2)
 #pragma unroll
-            for (int j = 0; j < NJ; ++j) {
-                const float4 f = FeatIO<FT>::load4(Fs + kk * DC + j * 32);
-                fv[2 * j] = pack2(f.x, f.y);
-                fv[2 * j + 1] = pack2(f.z, f.w);
-            }
+        for (int i = 0; i < 8; ++i)
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const unsigned long long w2 = pack2(wv[i], wv[i]);
+            for (int j = 0; j < NJ * 2; ++j) acc[i][j] = 0ull;
+        WsMeta m;
+        while (true) {   // batches of the item
+            mbar_wait(&sm.ct.full[stage], phase);
+            m = sm.ct.meta[stage];
+            if (m.flags & WS_FLAG_EXIT) return;
+            uint32_t mk = sm.ct.mask[stage][warp];
+            const float* Ws = sm.W[stage] + pg * 8;
+            const FT* Fs = sm.F[stage] + cg * 4;
+            while (mk) {
+                const int kk = __ffs(mk) - 1;
+                mk &= mk - 1u;
+                const float4 wa = *reinterpret_cast<const float4*>(Ws + kk * WS_CONS);
+                const float4 wb = *reinterpret_cast<const float4*>(Ws + kk * WS_CONS + 4);
+                const float wv[8] = {wa.x, wa.y, wa.z, wa.w, wb.x, wb.y, wb.z, wb.w};
+                unsigned long long fv[NJ * 2];
 #pragma unroll
-                for (int j = 0; j < NJ * 2; ++j) acc[i][j] = fma2(w2, fv[j], acc[i][j]);
-            }
-        }
-        mbar_arrive(&sm.ct.empty[stage]);
-        if (++stage == R_STAGES) { stage = 0; phase ^= 1u; }
-        if (m.flags & WS_FLAG_LAST) {
-            const int tx0 = (m.tile % a.t.GW) * FHGS_TILE, ty0 = (m.tile / a.t.GW) * FHGS_TILE;
-            const int oy = ty0 + ((warp >> 1) << 2) + pgl;
-            const int ox0 = tx0 + ((warp & 1) << 3);
-#pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                const int ox = ox0 + i;
-                if (oy < a.t.H && ox < a.t.W) {
-                    FT* dst = out_feat + ((size_t)oy * a.t.W + ox) * a.D + m.c0 + cg * 4;
-#pragma unroll
-                    for (int j = 0; j < NJ; ++j) {
-                        const float2 lo = unpack2(acc[i][2 * j]), hi = unpack2(acc[i][2 * j + 1]);
-                        FeatIO<FT>::store4(dst + j * 32, make_float4(lo.x, lo.y, hi.x, hi.y));
-                    }
+                for (int j = 0; j < NJ; ++j) {
+                    const ulonglong2 f = FeatIO<FT>::load_pairs(Fs + kk * DC + j * 32);
+                    fv[2 * j] = f.x;
+                    fv[2 * j + 1] = f.y;
                 }
 #pragma unroll
-                for (int j = 0; j < NJ * 2; ++j) acc[i][j] = 0ull;
+                for (int i = 0; i < 8; ++i) {
+                    const unsigned long long w2 = pack2(wv[i], wv[i]);
+#pragma unroll
+                    for (int j = 0; j < NJ * 2; ++j) fma2_acc(acc[i][j], w2, fv[j]);
+                }
+            }
+            mbar_arrive(&sm.ct.empty[stage]);
+            if (++stage == R_STAGES) { stage = 0; phase ^= 1u; }
+            if (m.flags & WS_FLAG_LAST) break;
+        }
+        const int tx0 = (m.tile % a.t.GW) * FHGS_TILE, ty0 = (m.tile / a.t.GW) * FHGS_TILE;
+        const int oy = ty0 + ((warp >> 1) << 2) + pgl;
+        const int ox0 = tx0 + ((warp & 1) << 3);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const int ox = ox0 + i;
+            if (oy < a.t.H && ox < a.t.W) {
+                FT* dst = out_feat + ((size_t)oy * a.t.W + ox) * a.D + m.c0 + cg * 4;
+#pragma unroll
+                for (int j = 0; j < NJ; ++j) {
+                    const float2 lo = unpack2(acc[i][2 * j]), hi = unpack2(acc[i][2 * j + 1]);
+                    FeatIO<FT>::store4(dst + j * 32, make_float4(lo.x, lo.y, hi.x, hi.y));
+                }
             }
         }
     }
