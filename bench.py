@@ -368,6 +368,129 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
         dist.destroy_process_group()
 
 
+
+# --------------------------------------------------------------------------------------------------
+# the other BASELINE.json configs (parity-test cases; timed for DESIGN.md / BASELINE.md, never the bench line)
+# --------------------------------------------------------------------------------------------------
+def run_cuda_workload(args, local_rank: int):
+    """`--workload tiny|small|large|multiview`: device-timed frames of another config, one GPU.
+    tiny/small/large: step = P + S + R + F(zero, one map, finalise) of view 0.
+    multiview: step = the fusion sweep over `--views` evenly spaced cameras of the 200-camera orbit
+    (P + S + F per view into one accumulator, finalise once); no rendering, as BASELINE.json describes it."""
+    import torch
+    from paper_2505_19154_b200 import binding as fb
+    from paper_2505_19154_b200 import inputs
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the FHGS path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    peaks = load_peaks()
+    cfg = inputs.CONFIGS[args.workload]
+    scene = inputs.make_scene(cfg)
+    W, H, D, n = cfg.width, cfg.height, cfg.feat_dim, scene.n
+    multiview = args.workload == "multiview"
+    views = [int(round(k * cfg.n_views / args.views)) % cfg.n_views for k in range(args.views)] if multiview else [0]
+    cams_np = [inputs.make_camera(cfg, v) for v in views]
+    cams = [fb.make_camera(c.view, c.proj, c.cam_pos, W, H) for c in cams_np]
+    ctx = fb.Context(local_rank)
+    g = fb.Gaussians(scene.mean, scene.scale, scene.quat, scene.opacity, scene.sh, scene.feat, scene.sh_degree, device=dev)
+    prm = fb.default_params()
+    fdt = g.feat.dtype
+    # instance counts (capacity) from a capacity-0 pass per view
+    vs0 = fb.ViewState(n, W, H, 0, device=dev)
+    Ms = []
+    for cam in cams:
+        fb.project(ctx, g, cam, prm, vs0)
+        try:
+            Ms.append(fb.bin_sort(ctx, cam, vs0, sync=True))
+        except fb.FhgsError:
+            Ms.append(int(vs0.num_instances.item()))
+    del vs0
+    vs = fb.ViewState(n, W, H, int(max(Ms) * 1.02) + 1024, device=dev)
+    if multiview:   # map values do not change the timing: one seeded unit-norm map stands in for every view's map
+        gen = torch.Generator(device=dev).manual_seed(cfg.seed)
+        gt = torch.randn((H, W, D), generator=gen, device=dev, dtype=torch.float32)
+        gt /= gt.norm(dim=-1, keepdim=True)
+    else:
+        gt = torch.from_numpy(inputs.make_gt_map(cfg, 0, cams_np[0])).to(dev)
+    f32 = torch.float32
+    out_rgb = torch.empty((H, W, 3), dtype=f32, device=dev)
+    out_feat = None if multiview else torch.empty((H, W, D), dtype=fdt, device=dev)
+    out_n = torch.empty((H, W), dtype=torch.int32, device=dev)
+    num = torch.zeros((n, D), dtype=f32, device=dev)
+    den = torch.zeros((n,), dtype=f32, device=dev)
+    fused = g.feat.clone()
+    stream = torch.cuda.current_stream()
+    NAMES = ["project", "bin_sort", "render", "fuse"]
+    acc = {k: 0.0 for k in NAMES}
+
+    def step(evs=None):
+        for vi, cam in enumerate(cams):
+            e = [torch.cuda.Event(enable_timing=True) for _ in range(5)] if evs is not None else None
+            def mark(i):
+                if e is not None:
+                    e[i].record(stream)
+            mark(0)
+            fb.project(ctx, g, cam, prm, vs)
+            mark(1)
+            fb.bin_sort(ctx, cam, vs, sync=False)
+            mark(2)
+            if not multiview:
+                fb.render(ctx, g, cam, prm, vs, out_rgb, out_feat, None, out_n)
+            mark(3)
+            flags = (fb.FHGS_FUSE_ZERO if vi == 0 else 0) | (fb.FHGS_FUSE_FINALIZE if vi == len(cams) - 1 else 0)
+            fb.fuse_features(ctx, cam, prm, vs, gt, num, den, fused, flags)
+            mark(4)
+            if evs is not None:
+                evs.append(e)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    evs = []
+    e0.record(stream)
+    for _ in range(args.steps):
+        step(evs)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    total_ms = e0.elapsed_time(e1)
+    for e in evs:
+        for i, nm in enumerate(NAMES):
+            acc[nm] += e[i].elapsed_time(e[i + 1]) / args.steps
+    # contributor counts (RGB-only render per view, outside the timed region) for the FP32 accounting
+    n_contrib = 0
+    for cam in cams:
+        fb.project(ctx, g, cam, prm, vs)
+        fb.bin_sort(ctx, cam, vs, sync=False)
+        fb.render(ctx, g, cam, prm, vs, out_rgb, None, None, out_n)
+        n_contrib += int(out_n.to(torch.int64).sum().item())
+    alu_nominal = 148 * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6
+    roof = {}
+    if not multiview:
+        roof["render"] = {"bound": "alu", "ms": acc["render"],
+                          "frac": (15 + D) * n_contrib / (acc["render"] * 1e-3) / alu_nominal}
+    roof["fuse"] = {"bound": "alu", "ms": acc["fuse"], "frac": (13 + D) * n_contrib / (acc["fuse"] * 1e-3) / alu_nominal,
+                    "hbm_gbs_gt_maps": len(cams) * W * H * D * gt.element_size() / (acc["fuse"] * 1e-3) / 1e9,
+                    "note": "includes zeroing num/den and the finalise pass"}
+    unit = "view-sweeps/s" if multiview else UNIT
+    line = {"metric": f"[{args.workload}] " + ("multi-view fusion sweeps/s" if multiview else "rendered+fused frames/s"),
+            "value": args.steps / (total_ms * 1e-3), "unit": unit, "n_gpus": 1, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+            "config": {"workload": f"{args.workload}: N={n} SH{scene.sh_degree} D={D} {cfg.feat_dtype}, {len(cams)} view(s) {W}x{H}"
+                                   " [parity-test config, not the bench line]",
+                       "views": views, "instances_M": Ms, "contributors_per_px": n_contrib / (W * H * len(cams)),
+                       "gt": "one seeded unit-norm map reused for every view (values do not affect timing)" if multiview
+                             else "inputs.make_gt_map"},
+            "ms": acc, "ms_per_view": total_ms / args.steps / len(cams), "roofline_steps": roof, "cpu_baseline": None,
+            "e2e": None, "gpu_launches": None, "clocks": clocks}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -377,12 +500,19 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--small", action="store_true", help="debug-size workload (not a bench line)")
+    ap.add_argument("--workload", default="mid", choices=["mid", "tiny", "small", "large", "multiview"],
+                    help="mid = the bench line (BASELINE.json metric); the others are timed for the record only")
+    ap.add_argument("--views", type=int, default=8, help="multiview: number of evenly spaced orbit cameras per sweep")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.workload != "mid":
+        if rank == 0:
+            run_cuda_workload(args, local_rank)
         return
     if world == 1 and args.gpus > 1:
         sys.stderr.write("bench.py: --gpus N > 1 must be launched with torch.distributed.run (one rank per GPU); "

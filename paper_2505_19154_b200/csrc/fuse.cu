@@ -205,6 +205,7 @@ constexpr int FW_BAR_CONS = 3;
 constexpr int FW_WQ = (WS_CONS + 1) * 4;   // floats per quad row: 256 pixels x float4 + 16 B pad (bank spread over quads)
 enum { FW_FLAG_FIRST = 4 };
 
+template <typename GT>
 struct FuseWsSmem {
     WsCtrl<FW_STAGES> ct;
     uint64_t g_full, g_free;
@@ -214,18 +215,28 @@ struct FuseWsSmem {
     __align__(16) float den_s[2][WS_KB];
     __align__(128) float W[FW_STAGES][FW_WQ * WS_KB / 4];  // [quad kk/4][pixel][4], quad stride padded by one float4
     __align__(128) float P[WS_KB * FW_DC];                // partial sums of the writing half
-    __align__(128) float G[WS_CONS * FW_DC];              // [pixel][channel], pixel = y*16 + x
-    float G_pad[FW_DC];                                   // target of the consumers' one-past-the-end prefetch
+    __align__(128) GT G[WS_CONS * FW_DC];                 // [pixel][channel], pixel = y*16 + x (storage type of the map)
+    GT G_pad[FW_DC];                                      // target of the consumers' one-past-the-end prefetch
 };
+
+// 4 consecutive channels of the staged GT tile -> fp32 (exact for fp16 storage)
+__device__ __forceinline__ float4 ld_g4(const float* p) { return *reinterpret_cast<const float4*>(p); }
+__device__ __forceinline__ float4 ld_g4(const __half* p) {
+    const uint2 r = *reinterpret_cast<const uint2*>(p);
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
+    const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
+    return make_float4(a.x, a.y, b.x, b.y);
+}
 
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)), "r"(bytes)
                  : "memory");
 }
 
-__device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem& sm, const FuseArgs& a, const WsWork& wk) {
+template <typename GT>
+__device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem<GT>& sm, const FuseArgs& a, const WsWork& wk) {
     const int lane = threadIdx.x & 31;
-    const float* gt = reinterpret_cast<const float*>(a.gt);
+    const GT* gt = reinterpret_cast<const GT*>(a.gt);
     int islot = 0;
     uint32_t iphase = 0, gphase = 0;
     while (true) {
@@ -248,18 +259,18 @@ __device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem& sm, const FuseArgs
         const int nx = min(FHGS_TILE, a.t.W - tx0), ny = min(FHGS_TILE, a.t.H - ty0);
         if (lane == 0) {
             mbar_wait_backoff(&sm.g_free, gphase ^ 1u);
-            mbar_arrive_expect_tx(&sm.g_full, (uint32_t)(nx * ny * FW_DC * 4));
+            mbar_arrive_expect_tx(&sm.g_full, (uint32_t)(nx * ny * FW_DC * sizeof(GT)));
         }
         __syncwarp();
         if (a.D == FW_DC) {   // a tile row is one contiguous span
             if (lane < ny)
                 bulk_g2s(&sm.G[lane * FHGS_TILE * FW_DC], gt + ((size_t)(ty0 + lane) * a.t.W + tx0) * FW_DC,
-                         (uint32_t)(nx * FW_DC * 4), &sm.g_full);
+                         (uint32_t)(nx * FW_DC * sizeof(GT)), &sm.g_full);
         } else {
             for (int pix = lane; pix < FHGS_TILE_PX; pix += 32) {
                 const int x = pix & 15, y = pix >> 4;
                 if (x < nx && y < ny)
-                    bulk_g2s(&sm.G[pix * FW_DC], gt + ((size_t)(ty0 + y) * a.t.W + tx0 + x) * a.D + c0, (uint32_t)(FW_DC * 4),
+                    bulk_g2s(&sm.G[pix * FW_DC], gt + ((size_t)(ty0 + y) * a.t.W + tx0 + x) * a.D + c0, (uint32_t)(FW_DC * sizeof(GT)),
                              &sm.g_full);
             }
         }
@@ -267,7 +278,8 @@ __device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem& sm, const FuseArgs
     }
 }
 
-__device__ __forceinline__ void fuse_ws_producer(FuseWsSmem& sm, const FuseArgs& a, const WsWork& wk) {
+template <typename GT>
+__device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseArgs& a, const WsWork& wk) {
     const int p = threadIdx.x - WS_CONS, lane = p & 31;
     const float q_cutoff = a.t.q_cutoff, alpha_max = a.t.alpha_max, t_min = a.t.t_min;
     const int sx = p & 15, sy = p >> 4;   // row-major pixel slot (matches the GT tile rows)
@@ -341,12 +353,13 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem& sm, const FuseArgs&
     (void)lane;
 }
 
-__device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem& sm, const FuseArgs& a) {
+template <typename GT>
+__device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT>& sm, const FuseArgs& a) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int half = warp >> 2, cw = warp & 3;
     const int kg = lane >> 3, cg = lane & 7;
     const int ch = cw * 32 + cg * 4;          // this thread's 4 channels inside the chunk
-    const float* Gs = sm.G + half * 128 * FW_DC + ch;
+    const GT* Gs = sm.G + half * 128 * FW_DC + ch;
     int stage = 0;
     uint32_t phase = 0, gphase = 0, batch = 0;
     while (true) {
@@ -374,17 +387,17 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem& sm, const FuseArgs&
         // software-pipelined over pixels: the operands of pixel s+1 are in flight while pixel s is multiplied
         ulonglong2 wa = *reinterpret_cast<const ulonglong2*>(Ws);
         ulonglong2 wb = *reinterpret_cast<const ulonglong2*>(Ws + FW_WQ);
-        float4 g = *reinterpret_cast<const float4*>(Gs);
+        float4 g = ld_g4(Gs);
 #pragma unroll 1
         for (int s0 = 0; s0 < 128; s0 += 16) {
             const float* Wb = Ws + s0 * 4;
-            const float* Gb = Gs + s0 * FW_DC;
+            const GT* Gb = Gs + s0 * FW_DC;
 #pragma unroll
             for (int u = 0; u < 16; ++u) {
                 const int un = u + 1;   // the prefetch past the last pixel lands in the row pad / G_pad (never used)
                 const ulonglong2 wa_n = *reinterpret_cast<const ulonglong2*>(Wb + un * 4);
                 const ulonglong2 wb_n = *reinterpret_cast<const ulonglong2*>(Wb + FW_WQ + un * 4);
-                const float4 g_n = *reinterpret_cast<const float4*>(Gb + un * FW_DC);
+                const float4 g_n = ld_g4(Gb + un * FW_DC);
                 const unsigned long long g2[4] = {pack2(g.x, g.x), pack2(g.y, g.y), pack2(g.z, g.z), pack2(g.w, g.w)};
 #pragma unroll
                 for (int c = 0; c < 4; ++c) {
@@ -444,9 +457,10 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem& sm, const FuseArgs&
     }
 }
 
+template <typename GT>
 __global__ void __launch_bounds__(FW_THREADS, 1) fuse_ws_kernel(const FuseArgs a, const WsWork wk) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    FuseWsSmem& sm = *reinterpret_cast<FuseWsSmem*>(smem_raw);
+    FuseWsSmem<GT>& sm = *reinterpret_cast<FuseWsSmem<GT>*>(smem_raw);
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int s = 0; s < FW_STAGES; ++s) {
@@ -462,7 +476,8 @@ __global__ void __launch_bounds__(FW_THREADS, 1) fuse_ws_kernel(const FuseArgs a
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     // the GT tile buffer must never hold non-finite garbage (pixels outside the image keep stale data, weight 0)
-    for (int i = threadIdx.x; i < (WS_CONS + 1) * FW_DC / 4; i += FW_THREADS) reinterpret_cast<float4*>(sm.G)[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int i = threadIdx.x; i < (int)((WS_CONS + 1) * FW_DC * sizeof(GT) / 16); i += FW_THREADS)
+        reinterpret_cast<uint4*>(sm.G)[i] = make_uint4(0u, 0u, 0u, 0u);
     if (threadIdx.x < 2 * WS_KB) (&sm.den_s[0][0])[threadIdx.x] = 0.f;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
@@ -598,22 +613,23 @@ cudaError_t launch(K kernel, size_t smem, int grid, cudaStream_t st, const FuseA
     return cudaGetLastError();
 }
 
+template <typename GT>
 cudaError_t launch_fuse_ws(const FuseArgs& a, int tiles, int num_sms, uint32_t* queue, cudaStream_t st) {
-    const size_t smem = sizeof(FuseWsSmem);
-    cudaError_t e = cudaFuncSetAttribute(fuse_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const size_t smem = sizeof(FuseWsSmem<GT>);
+    cudaError_t e = cudaFuncSetAttribute(fuse_ws_kernel<GT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     WsWork wk;
     wk.queue = queue;
     wk.n_chunks = a.D / FW_DC;
     wk.n_items = tiles * wk.n_chunks;
     const int grid = wk.n_items < num_sms ? wk.n_items : num_sms;
-    fuse_ws_kernel<<<grid, FW_THREADS, smem, st>>>(a, wk);
+    fuse_ws_kernel<GT><<<grid, FW_THREADS, smem, st>>>(a, wk);
     return cudaGetLastError();
 }
 
 template <typename GT>
 cudaError_t dispatch(const FuseArgs& a, int grid, int num_sms, uint32_t* queue, cudaStream_t st) {
-    if (sizeof(GT) == 4 && a.D % FW_DC == 0) return launch_fuse_ws(a, grid, num_sms, queue, st);
+    if (a.D % FW_DC == 0) return launch_fuse_ws<GT>(a, grid, num_sms, queue, st);
     if (a.D % 128 == 0) return launch(fuse_tiled_kernel<128, GT>, sizeof(FuseTiledSmem<128>), grid, st, a);
     if (a.D % 64 == 0) return launch(fuse_tiled_kernel<64, GT>, sizeof(FuseTiledSmem<64>), grid, st, a);
     if (a.D % 16 == 0) return launch(fuse_pixel_kernel<16, GT>, 0, grid, st, a);
