@@ -416,8 +416,10 @@ __global__ void __launch_bounds__(256) presort_init_kernel(int n, const float* d
 // histograms of the tile-id sort passes.  Nothing is written when M > capacity.
 constexpr int TS_THREADS = 1024;
 __global__ void __launch_bounds__(TS_THREADS) tile_scan_kernel(const int* diff, int gw1, int gh1, const uint64_t* num_instances,
-                                                               uint64_t capacity, uint32_t* ranges, uint32_t* hist, int npass) {
+                                                               uint64_t capacity, uint32_t* ranges, uint32_t* hist, int npass,
+                                                               uint32_t* order, uint32_t* order_valid) {
     extern __shared__ int s_g[];                 // [gh1][gw1]
+    __shared__ uint32_t s_bucket[34];            // tiles per log2(count) bucket (descending), then their start offsets
     __shared__ uint32_t s_h[SORT_MAX_PASSES][256];
     __shared__ uint32_t s_part[TS_THREADS / 32];
     __shared__ uint32_t s_carry;
@@ -464,6 +466,24 @@ __global__ void __launch_bounds__(TS_THREADS) tile_scan_kernel(const int* diff, 
         if (tid == TS_THREADS - 1) s_carry = excl + c;
         __syncthreads();
     }
+    // work order of render / fuse: tiles by descending floor(log2(count)) (counting sort; empty tiles last)
+    for (int j = tid; j < 34; j += TS_THREADS) s_bucket[j] = 0;
+    __syncthreads();
+    for (int t = tid; t < ntiles; t += TS_THREADS) {
+        const uint32_t c = (uint32_t)s_g[(t / GW) * gw1 + (t % GW)];
+        atomicAdd(&s_bucket[c ? __clz(c) : 32], 1u);   // clz small = long list = early bucket
+    }
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t run = 0;
+        for (int b = 0; b < 33; ++b) { const uint32_t c = s_bucket[b]; s_bucket[b] = run; run += c; }
+    }
+    __syncthreads();
+    for (int t = tid; t < ntiles; t += TS_THREADS) {
+        const uint32_t c = (uint32_t)s_g[(t / GW) * gw1 + (t % GW)];
+        order[atomicAdd(&s_bucket[c ? __clz(c) : 32], 1u)] = (uint32_t)t;
+    }
+    if (tid == 0) *order_valid = 1u;
     // exclusive scan of every digit histogram (warp w handles pass w)
     if (warp < npass) {
         uint32_t run = 0;
@@ -504,7 +524,7 @@ struct OneSweepArgs {
 };
 
 template <typename KeyT, int ITEMS>
-__global__ void __launch_bounds__(OS_THREADS) onesweep_kernel(const OneSweepArgs<KeyT> a) {
+__global__ void __launch_bounds__(OS_THREADS, 3) onesweep_kernel(const OneSweepArgs<KeyT> a) {
     constexpr int TILE = OS_THREADS * ITEMS;
     __shared__ uint32_t s_cnt[OS_WARPS][256];   // per-warp digit counts -> per-warp exclusive offsets
     __shared__ __align__(16) KeyT s_keys[TILE]; // reused for the values
@@ -526,19 +546,13 @@ __global__ void __launch_bounds__(OS_THREADS) onesweep_kernel(const OneSweepArgs
     const uint32_t tile_valid = (uint32_t)min((uint64_t)TILE, count - tile_base);
 
     // warp-striped load: warp w, item i, lane l <-> element w*ITEMS*32 + i*32 + l (processing order)
+    // (the values are fetched only when they are scattered: 16 fewer live registers during the ranking -> 3 CTAs/SM)
     KeyT key[ITEMS];
-    uint32_t val[ITEMS];
     uint32_t rank[ITEMS];
 #pragma unroll
     for (int i = 0; i < ITEMS; ++i) {
         const uint32_t e = warp * ITEMS * 32 + i * 32 + lane;
-        if (e < tile_valid) {
-            key[i] = a.keys_in[tile_base + e];
-            val[i] = a.vals_in[tile_base + e];
-        } else {
-            key[i] = ~(KeyT)0;   // sorts last inside the tile; never written out
-            val[i] = 0;
-        }
+        key[i] = e < tile_valid ? a.keys_in[tile_base + e] : ~(KeyT)0;   // padding sorts last inside the tile; never written out
     }
     // stable ranking inside the warp: equal digits are ranked by (item, lane)
 #pragma unroll
@@ -618,8 +632,16 @@ __global__ void __launch_bounds__(OS_THREADS) onesweep_kernel(const OneSweepArgs
     }
     __syncthreads();
     uint32_t* s_vals = reinterpret_cast<uint32_t*>(s_keys);
+    {
+        uint32_t val[ITEMS];
 #pragma unroll
-    for (int i = 0; i < ITEMS; ++i) s_vals[rank[i]] = val[i];
+        for (int i = 0; i < ITEMS; ++i) {
+            const uint32_t e = warp * ITEMS * 32 + i * 32 + lane;
+            val[i] = e < tile_valid ? a.vals_in[tile_base + e] : 0u;
+        }
+#pragma unroll
+        for (int i = 0; i < ITEMS; ++i) s_vals[rank[i]] = val[i];
+    }
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < ITEMS; ++i) {
@@ -701,6 +723,8 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
             FHGS_LAUNCH_CHECK(ctx);
             hist_scan_kernel<<<4, 256, 0, s>>>(hist32);
             FHGS_LAUNCH_CHECK(ctx);
+            FHGS_CUDA(ctx, cudaFuncSetAttribute(onesweep_kernel<uint32_t, SORT_TILE_K32 / OS_THREADS>,
+                                                cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
             const int pre_grid = (vs->n + SORT_TILE_K32 - 1) / SORT_TILE_K32;
             for (int p = 0; p < 4; ++p) {
                 FHGS_CUDA(ctx, cudaMemsetAsync(sort_status, 0, (size_t)pre_grid * 256 * 4, s));
@@ -753,7 +777,8 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
             ea.keys = vs->keys[0]; ea.vals = vs->vals[0]; ea.hist = hist; ea.npass = grid_counts ? 0 : npass;
             if (grid_counts) {   // ranges and digit offsets from the per-tile counts
                 FHGS_CUDA(ctx, cudaFuncSetAttribute(tile_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)diff_bytes));
-                tile_scan_kernel<<<1, TS_THREADS, diff_bytes, s>>>(tile_diff, gw1, gh1, vs->num_instances, vs->capacity, vs->ranges, hist, npass);
+                tile_scan_kernel<<<1, TS_THREADS, diff_bytes, s>>>(tile_diff, gw1, gh1, vs->num_instances, vs->capacity, vs->ranges, hist, npass,
+                                                                 (uint32_t*)(sc + L.tile_order), ctrl + CTRL_ORDER_VALID);
                 FHGS_LAUNCH_CHECK(ctx);
             }
             emit_partition_kernel<<<(ea.units + 1 + 255) / 256, 256, 0, s>>>(ea);
@@ -768,6 +793,8 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
                 hist_scan_kernel<<<npass, 256, 0, s>>>(hist);
                 FHGS_LAUNCH_CHECK(ctx);
             }
+            FHGS_CUDA(ctx, cudaFuncSetAttribute(onesweep_kernel<uint64_t, SORT_TILE_K64 / OS_THREADS>,
+                                                cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
             const int sort_grid = (int)((vs->capacity + SORT_TILE_K64 - 1) / SORT_TILE_K64);
             for (int p = 0; p < npass; ++p) {
                 FHGS_CUDA(ctx, cudaMemsetAsync(sort_status, 0, (size_t)sort_grid * 256 * 4, s));

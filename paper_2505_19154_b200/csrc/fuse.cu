@@ -250,7 +250,7 @@ __device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem<GT>& sm, const Fuse
         item = __shfl_sync(TR_FULL, item, 0);
         if (++islot == 2) { islot = 0; iphase ^= 1u; }
         if (item >= wk.n_items) break;
-        const int tile = item / wk.n_chunks, c0 = (item % wk.n_chunks) * FW_DC;
+        const int tile = ws_item_tile(wk, item), c0 = (item % wk.n_chunks) * FW_DC;
         {
             const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
             if (range.x >= range.y) continue;   // empty tile: the producers skip it too
@@ -296,7 +296,7 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseA
             mbar_arrive(&sm.ct.full[stage]);
             break;
         }
-        const int tile = item / wk.n_chunks, c0 = (item % wk.n_chunks) * FW_DC;
+        const int tile = ws_item_tile(wk, item), c0 = (item % wk.n_chunks) * FW_DC;
         const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
         const int px = tx0 + sx, py = ty0 + sy;
         const bool inside = px < a.t.W && py < a.t.H;
@@ -614,7 +614,7 @@ cudaError_t launch(K kernel, size_t smem, int grid, cudaStream_t st, const FuseA
 }
 
 template <typename GT>
-cudaError_t launch_fuse_ws(const FuseArgs& a, int tiles, int num_sms, uint32_t* queue, cudaStream_t st) {
+cudaError_t launch_fuse_ws(const FuseArgs& a, int tiles, int num_sms, uint32_t* queue, const uint32_t* order, cudaStream_t st) {
     const size_t smem = sizeof(FuseWsSmem<GT>);
     cudaError_t e = cudaFuncSetAttribute(fuse_ws_kernel<GT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -622,14 +622,16 @@ cudaError_t launch_fuse_ws(const FuseArgs& a, int tiles, int num_sms, uint32_t* 
     wk.queue = queue;
     wk.n_chunks = a.D / FW_DC;
     wk.n_items = tiles * wk.n_chunks;
+    wk.order = order;
+    wk.order_valid = queue - CTRL_TILE_QUEUE + CTRL_ORDER_VALID;
     const int grid = wk.n_items < num_sms ? wk.n_items : num_sms;
     fuse_ws_kernel<GT><<<grid, FW_THREADS, smem, st>>>(a, wk);
     return cudaGetLastError();
 }
 
 template <typename GT>
-cudaError_t dispatch(const FuseArgs& a, int grid, int num_sms, uint32_t* queue, cudaStream_t st) {
-    if (a.D % FW_DC == 0) return launch_fuse_ws<GT>(a, grid, num_sms, queue, st);
+cudaError_t dispatch(const FuseArgs& a, int grid, int num_sms, uint32_t* queue, const uint32_t* order, cudaStream_t st) {
+    if (a.D % FW_DC == 0) return launch_fuse_ws<GT>(a, grid, num_sms, queue, order, st);
     if (a.D % 128 == 0) return launch(fuse_tiled_kernel<128, GT>, sizeof(FuseTiledSmem<128>), grid, st, a);
     if (a.D % 64 == 0) return launch(fuse_tiled_kernel<64, GT>, sizeof(FuseTiledSmem<64>), grid, st, a);
     if (a.D % 16 == 0) return launch(fuse_pixel_kernel<16, GT>, 0, grid, st, a);
@@ -684,9 +686,11 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
         a.t.q_cutoff = prm->q_cutoff; a.t.alpha_max = prm->alpha_max; a.t.t_min = prm->t_min;
         a.gt = gt; a.D = feat_dim; a.num = num; a.den = den;
         const int grid = tiles_x(cam->width) * tiles_y(cam->height);
-        uint32_t* queue = reinterpret_cast<uint32_t*>((char*)vs->scratch + make_scratch_layout(vs->n, vs->capacity).ctrl) + CTRL_TILE_QUEUE;
-        cudaError_t e = gt_dtype == FHGS_F16 ? dispatch<__half>(a, grid, ctx->num_sms, queue, s)
-                                             : dispatch<float>(a, grid, ctx->num_sms, queue, s);
+        const ScratchLayout L = make_scratch_layout(vs->n, vs->capacity, cam->width, cam->height);
+        uint32_t* queue = reinterpret_cast<uint32_t*>((char*)vs->scratch + L.ctrl) + CTRL_TILE_QUEUE;
+        const uint32_t* order = reinterpret_cast<const uint32_t*>((char*)vs->scratch + L.tile_order);
+        cudaError_t e = gt_dtype == FHGS_F16 ? dispatch<__half>(a, grid, ctx->num_sms, queue, order, s)
+                                             : dispatch<float>(a, grid, ctx->num_sms, queue, order, s);
         FHGS_CUDA(ctx, e);
     }
     if (finalize && n > 0) {

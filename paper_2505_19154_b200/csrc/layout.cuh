@@ -17,6 +17,7 @@ enum {
     CTRL_SORT_TICKET = 1,     // [1..8]  dynamic CTA ids, one per instance-sort pass
     CTRL_PRESORT_TICKET = 9,  // [9..12] dynamic CTA ids of the depth pre-sort passes
     CTRL_TILE_QUEUE = 16,     // render / fuse tile queue heads
+    CTRL_ORDER_VALID = 20,    // 1 when tile_order holds the longest-first tile permutation of this view
     CTRL_WORDS = 64
 };
 
@@ -32,6 +33,7 @@ struct ScratchLayout {
     size_t pre_incl;      // uint32_t[n]  inclusive prefix of tiles_touched in depth order
     size_t emit_starts;   // uint32_t[emit_tiles + 1]  first depth-ordered Gaussian of every EMIT_TILE instances
     size_t tile_diff;     // int32_t[(GW+1)*(GH+1)]  2-D difference array of the per-tile instance counts
+    size_t tile_order;    // uint32_t[GW*GH]  tiles by descending instance count (work order of render / fuse)
     size_t scan_tiles, sort_tiles, pre_tiles, emit_tiles;
     size_t total;
 };
@@ -58,6 +60,7 @@ static inline ScratchLayout make_scratch_layout(int32_t n, uint64_t capacity, in
     L.emit_starts = off; off += align_up((L.emit_tiles + 1) * 4, 256);
     const size_t gw1 = (size_t)((width + 15) / 16 + 1), gh1 = (size_t)((height + 15) / 16 + 1);
     L.tile_diff = off; off += align_up(gw1 * gh1 * 4, 256);   // last: the regions above do not depend on width/height
+    L.tile_order = off; off += align_up((gw1 - 1) * (gh1 - 1) * 4, 256);
     L.total = align_up(off, 256);
     return L;
 }

@@ -92,7 +92,7 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
             break;
         }
         const uint32_t popped = ws_pop_begin(wk, p);   // next item, consumed at the end of this one
-        const int tile = item / wk.n_chunks, c0 = (item % wk.n_chunks) * DC;
+        const int tile = ws_item_tile(wk, item), c0 = (item % wk.n_chunks) * DC;
         const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
         const int px = tx0 + sx, py = ty0 + sy;
         const bool inside = px < a.t.W && py < a.t.H;
@@ -364,7 +364,7 @@ cudaError_t launch(K kernel, size_t smem, int grid, cudaStream_t st, const Rende
 }
 
 template <int DC, typename FT>
-cudaError_t launch_ws(const RenderArgs& a, int tiles, int num_sms, uint32_t* queue, cudaStream_t st) {
+cudaError_t launch_ws(const RenderArgs& a, int tiles, int num_sms, uint32_t* queue, const uint32_t* order, cudaStream_t st) {
     const size_t smem = sizeof(RenderWsSmem<DC, FT>);
     cudaError_t e = cudaFuncSetAttribute(render_ws_kernel<DC, FT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -372,16 +372,18 @@ cudaError_t launch_ws(const RenderArgs& a, int tiles, int num_sms, uint32_t* que
     wk.queue = queue;
     wk.n_chunks = a.D / DC;
     wk.n_items = tiles * wk.n_chunks;
+    wk.order = order;
+    wk.order_valid = queue - CTRL_TILE_QUEUE + CTRL_ORDER_VALID;
     const int grid = wk.n_items < num_sms ? wk.n_items : num_sms;
     render_ws_kernel<DC, FT><<<grid, WS_THREADS, smem, st>>>(a, wk);
     return cudaGetLastError();
 }
 
 template <typename FT>
-cudaError_t dispatch(const RenderArgs& a, int grid, int num_sms, uint32_t* queue, cudaStream_t st, bool has_feat) {
+cudaError_t dispatch(const RenderArgs& a, int grid, int num_sms, uint32_t* queue, const uint32_t* order, cudaStream_t st, bool has_feat) {
     if (!has_feat) return launch(render_pixel_kernel<0, FT>, sizeof(PixelSmem<0>), grid, st, a);
-    if (a.D % 128 == 0) return launch_ws<128, FT>(a, grid, num_sms, queue, st);
-    if (a.D % 64 == 0) return launch_ws<64, FT>(a, grid, num_sms, queue, st);
+    if (a.D % 128 == 0) return launch_ws<128, FT>(a, grid, num_sms, queue, order, st);
+    if (a.D % 64 == 0) return launch_ws<64, FT>(a, grid, num_sms, queue, order, st);
     if (a.D % 16 == 0) return launch(render_pixel_kernel<16, FT>, sizeof(PixelSmem<16>), grid, st, a);
     if (a.D % 8 == 0) return launch(render_pixel_kernel<8, FT>, sizeof(PixelSmem<8>), grid, st, a);
     return launch(render_pixel_kernel<4, FT>, sizeof(PixelSmem<4>), grid, st, a);
@@ -419,9 +421,11 @@ extern "C" fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const
     a.out_rgb = out_rgb; a.out_feat = out_feat; a.out_T = out_T; a.out_n = out_ncontrib;
     const int grid = tiles_x(cam->width) * tiles_y(cam->height);
     cudaStream_t s = (cudaStream_t)stream;
-    uint32_t* queue = reinterpret_cast<uint32_t*>((char*)vs->scratch + make_scratch_layout(vs->n, vs->capacity).ctrl) + CTRL_TILE_QUEUE;
-    cudaError_t e = (has_feat && g->feat_dtype == FHGS_F16) ? dispatch<__half>(a, grid, ctx->num_sms, queue, s, has_feat)
-                                                            : dispatch<float>(a, grid, ctx->num_sms, queue, s, has_feat);
+    const ScratchLayout L = make_scratch_layout(vs->n, vs->capacity, cam->width, cam->height);
+    uint32_t* queue = reinterpret_cast<uint32_t*>((char*)vs->scratch + L.ctrl) + CTRL_TILE_QUEUE;
+    const uint32_t* order = reinterpret_cast<const uint32_t*>((char*)vs->scratch + L.tile_order);
+    cudaError_t e = (has_feat && g->feat_dtype == FHGS_F16) ? dispatch<__half>(a, grid, ctx->num_sms, queue, order, s, has_feat)
+                                                            : dispatch<float>(a, grid, ctx->num_sms, queue, order, s, has_feat);
     FHGS_CUDA(ctx, e);
     return FHGS_OK;
 }

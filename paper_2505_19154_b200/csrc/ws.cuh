@@ -131,7 +131,16 @@ struct WsWork {
     uint32_t* queue;      // [0] next item, [1] finished CTAs (self-resetting; zero between launches)
     int n_items;          // tiles * chunks
     int n_chunks;
+    const uint32_t* order;        // tile permutation, longest instance list first (written by fhgs_bin_sort)
+    const uint32_t* order_valid;  // device flag: 0 -> identity order
 };
+
+// Work item -> tile.  The queue hands out items in increasing order; with the longest-first permutation the heavy
+// tiles start early and the tail of the persistent loop is made of short ones.
+__device__ __forceinline__ int ws_item_tile(const WsWork& wk, int item) {
+    const int t = item / wk.n_chunks;
+    return __ldg(wk.order_valid) ? (int)__ldg(wk.order + t) : t;
+}
 
 // Per-pixel blend state of a producer thread.
 struct WsPixel {
