@@ -279,10 +279,20 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     tiles = ((W + 15) // 16) * ((H + 15) // 16)
     tile_bits = max(1, (tiles - 1).bit_length())
     p_full = (32 + tile_bits + 7) // 8
+    # n_eval of SURVEY 8(d): instances of a tile's list walked before the whole tile stopped (fhgs_render's
+    # tile_visited diagnostics of the last timed frame) x the tile's valid pixels
+    gw, gh = (W + 15) // 16, (H + 15) // 16
+    tv = vs.tile_visited().to(torch.int64).view(gh, gw)
+    px_x = torch.clamp(W - 16 * torch.arange(gw, device=dev), max=16)
+    px_y = torch.clamp(H - 16 * torch.arange(gh, device=dev), max=16)
+    n_eval_total = int((tv * (px_y[:, None] * px_x[None, :])).sum().item())
     work = {
-        # contributor-only lane-ops: 7 (q) + 8 (alpha, w, T, RGB) + D feature FMAs per (pixel, contributor)
-        "render_lane_ops": (7 + 8 + D) * n_contrib_total,
-        "fuse_lane_ops": (7 + 6 + D) * n_contrib_total,
+        # lane-ops = sum_x [7 n_eval(x) + (D + 8) n_c(x)] (render), [7 n_eval + (D + 6) n_c] (fuse)
+        "render_lane_ops": 7 * n_eval_total + (8 + D) * n_contrib_total,
+        "fuse_lane_ops": 7 * n_eval_total + (6 + D) * n_contrib_total,
+        # stricter count: only the (pixel, contributor) pairs, nothing for the evaluations that are cut off
+        "render_lane_ops_contrib_only": (7 + 8 + D) * n_contrib_total,
+        "fuse_lane_ops_contrib_only": (7 + 6 + D) * n_contrib_total,
         "fuse_bytes": W * H * D * 4,                                      # the GT map, read once
         "project_bytes": 44 * n + 12 * K * n_vis + 16 * n + 40 * n_vis,
         "bin_sort_bytes": (4 * n + 12 * n_vis + 4 * n + 12 * M) + (8 * M + p_full * 24 * M) + (8 * M + 8 * tiles),
@@ -293,9 +303,12 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     steps_roof = {}
     for nm, ops in (("render", work["render_lane_ops"]), ("fuse_accumulate", work["fuse_lane_ops"])):
         ach = 2.0 * ops / (parts[nm] * 1e-3) / 1e12
+        ops_c = work[("render" if nm == "render" else "fuse") + "_lane_ops_contrib_only"]
         steps_roof[nm] = {"bound": "alu", "achieved": ach, "peak": 2.0 * alu_nominal / 1e12, "unit": "TFLOP/s",
                           "frac": ach / (2.0 * alu_nominal / 1e12), "ms": parts[nm],
-                          "frac_of_measured_ffma": 2.0 * ops / (parts[nm] * 1e-3) / (2.0 * ffma_ops)}
+                          "frac_of_measured_ffma": 2.0 * ops / (parts[nm] * 1e-3) / (2.0 * ffma_ops),
+                          "frac_contributors_only": ops_c / (parts[nm] * 1e-3) / alu_nominal,
+                          "work": "lane-ops = 7 n_eval + (D+%d) n_contrib (SURVEY 8(d)); FMA = 2 flop" % (8 if nm == "render" else 6)}
     for nm, by in (("project", work["project_bytes"]), ("bin_sort", work["bin_sort_bytes"]),
                    ("fuse_finalize", work["finalize_bytes"])):
         ach = by / (parts[nm] * 1e-3) / 1e9
@@ -356,6 +369,7 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
                 "config": {"workload": f"mid: N={n} SH{scene.sh_degree} D={D} f32, 1 view {W}x{H} + one {W}x{H}x{D} GT map"
                                        + (" [--small debug size, not a bench line]" if args.small else ""),
                            "instances_M": M, "visible": n_vis, "contributors_per_px": n_contrib_total / (W * H),
+                           "evaluated_per_px": n_eval_total / (W * H),
                            "l2": "no flush: inputs larger than L2 (GT map %.2f GB, feat %.2f GB, pairs %.2f GB vs 126 MB)"
                                  % (gt.numel() * 4 / 1e9, g.feat.numel() * 4 / 1e9, 12 * M / 1e9),
                            "parallelism": f"{world} independent frame(s), one per GPU"},

@@ -20,7 +20,7 @@ FHGS_SORT_FULL_KEY = 1
 FHGS_FUSE_ZERO, FHGS_FUSE_FINALIZE, FHGS_FUSE_L2NORM, FHGS_FUSE_FINALIZE_ONLY, FHGS_FUSE_ZERO_ONLY = 1, 2, 4, 8, 16
 
 EXPORTS = ["fhgs_create", "fhgs_destroy", "fhgs_last_error", "fhgs_version", "fhgs_default_params",
-           "fhgs_scratch_bytes", "fhgs_project", "fhgs_bin_sort", "fhgs_render", "fhgs_fuse_features",
+           "fhgs_scratch_bytes", "fhgs_scratch_tile_visited", "fhgs_project", "fhgs_bin_sort", "fhgs_render", "fhgs_fuse_features",
            "fhgs_frame_host", "fhgs_ffma_peak"]
 
 
@@ -84,6 +84,8 @@ def _load():
     lib.fhgs_default_params.restype = None
     lib.fhgs_scratch_bytes.restype = C.c_size_t
     lib.fhgs_scratch_bytes.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_uint64]
+    lib.fhgs_scratch_tile_visited.restype = C.c_size_t
+    lib.fhgs_scratch_tile_visited.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_uint64]
     lib.fhgs_project.argtypes = [vp, C.POINTER(CGaussians), C.POINTER(CCamera), C.POINTER(CParams),
                                  C.POINTER(CViewState), vp]
     lib.fhgs_bin_sort.argtypes = [vp, C.POINTER(CCamera), C.POINTER(CViewState), C.POINTER(C.c_uint64),
@@ -247,6 +249,13 @@ class ViewState:
         sp = self.scratch.data_ptr()
         c.scratch = (sp + 255) // 256 * 256
         c.scratch_bytes = sb
+
+    def tile_visited(self) -> torch.Tensor:
+        """Diagnostics written by fhgs_render (see fhgs_scratch_tile_visited): int32 tensor [GW*GH] (device)."""
+        off = int(lib.fhgs_scratch_tile_visited(self.n, self.width, self.height, self.capacity))
+        base = self.c.scratch - self.scratch.data_ptr()
+        gw, gh = (self.width + 15) // 16, (self.height + 15) // 16
+        return self.scratch[base + off: base + off + 4 * gw * gh].view(torch.int32)
 
     # views of the results with the library's integer types (numpy, host)
     def sorted_keys(self, m: int) -> np.ndarray:

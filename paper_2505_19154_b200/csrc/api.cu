@@ -51,6 +51,11 @@ extern "C" size_t fhgs_scratch_bytes(int32_t n, int32_t width, int32_t height, u
     return make_scratch_layout(n, capacity, width, height).total;
 }
 
+extern "C" size_t fhgs_scratch_tile_visited(int32_t n, int32_t width, int32_t height, uint64_t capacity) {
+    if (n < 0 || width <= 0 || height <= 0) return 0;
+    return make_scratch_layout(n, capacity, width, height).tile_visited;
+}
+
 fhgs_status validate_camera(fhgs_ctx* ctx, const fhgs_camera* cam) {
     if (cam->width <= 0 || cam->height <= 0) FHGS_INVALID(ctx, "camera: width/height must be > 0");
     const long long tiles = (long long)tiles_x(cam->width) * tiles_y(cam->height);

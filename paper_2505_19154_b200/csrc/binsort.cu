@@ -554,11 +554,15 @@ __global__ void __launch_bounds__(OS_THREADS, 3) onesweep_kernel(const OneSweepA
         const uint32_t e = warp * ITEMS * 32 + i * 32 + lane;
         key[i] = e < tile_valid ? a.keys_in[tile_base + e] : ~(KeyT)0;   // padding sorts last inside the tile; never written out
     }
-    // stable ranking inside the warp: equal digits are ranked by (item, lane)
+    // stable ranking inside the warp: equal digits are ranked by (item, lane).  The 16 match_any are independent
+    // of one another and are issued back to back (their latency overlaps); only the shared-memory counter update
+    // forms a chain over the items.
+#pragma unroll
+    for (int i = 0; i < ITEMS; ++i) rank[i] = __match_any_sync(FULL, (uint32_t)(key[i] >> a.shift) & 255u);
 #pragma unroll
     for (int i = 0; i < ITEMS; ++i) {
         const uint32_t d = (uint32_t)(key[i] >> a.shift) & 255u;
-        const uint32_t peers = __match_any_sync(FULL, d);
+        const uint32_t peers = rank[i];
         const int leader = __ffs(peers) - 1;
         uint32_t old = 0;
         if (lane == leader) {

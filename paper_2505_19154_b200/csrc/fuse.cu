@@ -314,7 +314,7 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseA
         bool last = false, first = true;
         do {
             while (qt - qh < WS_KB && pos < range.y) {
-                qt += ws_chunk_append(sm.ct, ch, qt, bx0, by0, bx1, by1, q_cutoff, p, [](int, const WsChunk&) {});
+                qt += ws_chunk_append(sm.ct, ch, pos, qt, bx0, by0, bx1, by1, q_cutoff, p, [](int, const WsChunk&) {});
                 pos += WS_PROD;
                 ws_chunk_issue(a.t, nullptr, ch);
                 ws_chunk_prefetch_id(a.t, pos + WS_PROD, range.y, p, ch);

@@ -34,6 +34,7 @@ struct ScratchLayout {
     size_t emit_starts;   // uint32_t[emit_tiles + 1]  first depth-ordered Gaussian of every EMIT_TILE instances
     size_t tile_diff;     // int32_t[(GW+1)*(GH+1)]  2-D difference array of the per-tile instance counts
     size_t tile_order;    // uint32_t[GW*GH]  tiles by descending instance count (work order of render / fuse)
+    size_t tile_visited;  // uint32_t[GW*GH]  diagnostics of fhgs_render: instances of each tile's list walked before it stopped
     size_t scan_tiles, sort_tiles, pre_tiles, emit_tiles;
     size_t total;
 };
@@ -61,6 +62,7 @@ static inline ScratchLayout make_scratch_layout(int32_t n, uint64_t capacity, in
     const size_t gw1 = (size_t)((width + 15) / 16 + 1), gh1 = (size_t)((height + 15) / 16 + 1);
     L.tile_diff = off; off += align_up(gw1 * gh1 * 4, 256);   // last: the regions above do not depend on width/height
     L.tile_order = off; off += align_up((gw1 - 1) * (gh1 - 1) * 4, 256);
+    L.tile_visited = off; off += align_up((gw1 - 1) * (gh1 - 1) * 4, 256);
     L.total = align_up(off, 256);
     return L;
 }

@@ -30,6 +30,7 @@ struct RenderArgs {
     void* out_feat;
     float* out_T;
     uint32_t* out_n;
+    uint32_t* tile_visited;   // [tiles] diagnostics: length of the prefix of the tile's list that was walked
 };
 
 constexpr int R_KB = 64;   // staged instances per drain of the per-pixel variant
@@ -108,9 +109,10 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
         ws_chunk_issue(a.t, a.rgb_g, ch);
         ws_chunk_prefetch_id(a.t, pos + WS_PROD, range.y, p, ch);
         bool last = false;
+        uint32_t last_used = 0u;
         do {
             while (qt - qh < WS_KB && pos < range.y) {
-                qt += ws_chunk_append(sm.ct, ch, qt, bx0, by0, bx1, by1, q_cutoff, p,
+                qt += ws_chunk_append(sm.ct, ch, pos, qt, bx0, by0, bx1, by1, q_cutoff, p,
                                       [&](int s, const WsChunk& c) { sm.rgb[s] = make_float4(c.r, c.gr, c.b, 0.f); });
                 pos += WS_PROD;
                 ws_chunk_issue(a.t, a.rgb_g, ch);
@@ -147,6 +149,13 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
             last = all_done || (pos >= range.y && qt == qh);
             if (p == 0) sm.ct.meta[stage] = WsMeta{nb, tile, c0, last ? WS_FLAG_LAST : 0};
             mbar_arrive(&sm.ct.full[stage]);
+            if (p == 32 && c0 == 0) {   // diagnostics, off the critical path: list position of the last blended instance
+                uint32_t any = 0u;
+#pragma unroll
+                for (int w8 = 0; w8 < 8; ++w8) any |= sm.ct.mask[stage][w8];
+                if (any) last_used = __float_as_uint(sm.ct.rec1[(qh - nb + 31 - __clz(any)) & (WS_QCAP - 1)].w) + 1u - range.x;
+                if (last) a.tile_visited[tile] = all_done ? last_used : range.y - range.x;
+            }
             if (++stage == R_STAGES) { stage = 0; phase ^= 1u; }
         } while (!last);
         if (c0 == 0 && inside) {
@@ -335,6 +344,7 @@ __global__ void __launch_bounds__(TR_THREADS) render_pixel_kernel(const RenderAr
             q_count = 0;
             if (__syncthreads_and(done)) break;
         }
+        if (c0 == 0 && tid == 0) a.tile_visited[tile] = min(pos, range.y) - range.x;   // chunk granular (256 instances)
         if (inside) {
             const size_t p = (size_t)py * a.t.W + px;
             if (c0 == 0) {
@@ -424,6 +434,7 @@ extern "C" fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const
     const ScratchLayout L = make_scratch_layout(vs->n, vs->capacity, cam->width, cam->height);
     uint32_t* queue = reinterpret_cast<uint32_t*>((char*)vs->scratch + L.ctrl) + CTRL_TILE_QUEUE;
     const uint32_t* order = reinterpret_cast<const uint32_t*>((char*)vs->scratch + L.tile_order);
+    a.tile_visited = reinterpret_cast<uint32_t*>((char*)vs->scratch + L.tile_visited);
     cudaError_t e = (has_feat && g->feat_dtype == FHGS_F16) ? dispatch<__half>(a, grid, ctx->num_sms, queue, order, s, has_feat)
                                                             : dispatch<float>(a, grid, ctx->num_sms, queue, order, s, has_feat);
     FHGS_CUDA(ctx, e);

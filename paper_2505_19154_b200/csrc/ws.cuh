@@ -124,7 +124,7 @@ struct WsCtrl {
     uint32_t wcount[WS_PROD / 32];
     int item;                     // work item broadcast among the producers
     float4 rec0[WS_QCAP];         // gx, gy, A, 2B
-    float4 rec1[WS_QCAP];         // C, opacity, id (bits), unused
+    float4 rec1[WS_QCAP];         // C, opacity, id (bits), position in the sorted list (bits)
 };
 
 struct WsWork {
@@ -207,8 +207,8 @@ __device__ __forceinline__ void ws_chunk_prefetch_id(const TraverseArgs& a, uint
 // Tile-cull the chunk and append the survivors, in order, to the ring at q_tail.  Returns the number
 // appended (same in all producer threads).  Two producer-wide barriers.
 template <typename CTRL, typename EXTRA>
-__device__ __forceinline__ int ws_chunk_append(CTRL& ct, const WsChunk& c, int q_tail, float bx0, float by0, float bx1,
-                                               float by1, float q_cutoff, int p, EXTRA&& extra) {
+__device__ __forceinline__ int ws_chunk_append(CTRL& ct, const WsChunk& c, uint32_t chunk_pos, int q_tail, float bx0, float by0,
+                                               float bx1, float by1, float q_cutoff, int p, EXTRA&& extra) {
     const int lane = p & 31, pw = p >> 5;
     float4 co = c.co;
     co.y = 2.0f * co.y;   // exact
@@ -226,7 +226,7 @@ __device__ __forceinline__ int ws_chunk_append(CTRL& ct, const WsChunk& c, int q
     if (keep) {
         const int s = (q_tail + off + __popc(ballot & ((1u << lane) - 1u))) & (WS_QCAP - 1);
         ct.rec0[s] = make_float4(c.g.x, c.g.y, co.x, co.y);
-        ct.rec1[s] = make_float4(co.z, co.w, __uint_as_float(c.id), 0.f);
+        ct.rec1[s] = make_float4(co.z, co.w, __uint_as_float(c.id), __uint_as_float(chunk_pos + (uint32_t)p));
         extra(s, c);
     }
     named_bar_sync(WS_BAR_PROD, WS_PROD);

@@ -213,6 +213,26 @@ def test_edge_cases():
         assert np.array_equal(g_full[k], g_again[k])
 
 
+def test_tile_visited_diagnostics():
+    """fhgs_render's per-tile 'visited' diagnostics (work accounting only): never longer than the tile's list; the
+    Tiny scene never saturates, so every tile walks its whole list; a saturating scene stops early somewhere."""
+    for name, kw, saturates in (("tiny", {}, False), ("mid", dict(n=60_000, width=328, height=200, log_scale_mu=-3.3), True)):
+        cfg = pu.reduced_config(name, **kw) if kw else inputs.CONFIGS[name]
+        scene = inputs.make_scene(cfg)
+        cam = inputs.make_camera(cfg, 0)
+        gp = pu.GpuPath(scene, cfg.width, cfg.height, 4_000_000)
+        c, m = gp.project_sort(cam)
+        gp.render(c)
+        tv = gp.vs.tile_visited().cpu().numpy().astype(np.int64)
+        rg = gp.vs.ranges.cpu().numpy().view(np.uint32).astype(np.int64)
+        ln = rg[:, 1] - rg[:, 0]
+        assert np.all(tv <= ln) and np.all(tv[ln > 0] > 0)
+        if saturates:
+            assert np.any(tv < ln)
+        else:
+            assert np.array_equal(tv, ln)
+
+
 def test_constant_map_and_l2norm():
     """north_star pin on the GPU path: a constant GT map fuses to that constant; L2NORM normalises."""
     cfg = inputs.CONFIGS["tiny"]
