@@ -524,7 +524,7 @@ struct OneSweepArgs {
 };
 
 template <typename KeyT, int ITEMS>
-__global__ void __launch_bounds__(OS_THREADS, 3) onesweep_kernel(const OneSweepArgs<KeyT> a) {
+__global__ void __launch_bounds__(OS_THREADS, ITEMS >= 16 ? 3 : 5) onesweep_kernel(const OneSweepArgs<KeyT> a) {
     constexpr int TILE = OS_THREADS * ITEMS;
     __shared__ uint32_t s_cnt[OS_WARPS][256];   // per-warp digit counts -> per-warp exclusive offsets
     __shared__ __align__(16) KeyT s_keys[TILE]; // reused for the values
@@ -583,23 +583,10 @@ __global__ void __launch_bounds__(OS_THREADS, 3) onesweep_kernel(const OneSweepA
         cnt += c;
     }
     if (tid == 255) cnt -= (uint32_t)TILE - tile_valid;   // padding keys all carry digit 255
-    // publish, then look back over the earlier CTAs
-    uint32_t excl = 0;
+    // publish the CTA's digit counts at once; the look-back itself is deferred until the keys are staged, so that
+    // the wait for the predecessors overlaps the local scan and the shared-memory scatter
     uint32_t* my = a.status + (size_t)ticket * 256 + tid;
-    if (ticket == 0) {
-        st_volatile_u32(my, OS_INC | cnt);
-    } else {
-        st_volatile_u32(my, OS_AGG | cnt);
-        const uint32_t* p = my - 256;
-        while (true) {
-            const uint32_t v = ld_volatile_u32(p);
-            if ((v >> 30) == 0) continue;
-            excl += v & OS_VAL;
-            if ((v >> 30) == 2) break;
-            p -= 256;
-        }
-        st_volatile_u32(my, OS_INC | (excl + cnt));
-    }
+    st_volatile_u32(my, (ticket == 0 ? OS_INC : OS_AGG) | cnt);
     // CTA-local exclusive scan over digits
     uint32_t incl = cnt;
 #pragma unroll
@@ -613,7 +600,6 @@ __global__ void __launch_bounds__(OS_THREADS, 3) onesweep_kernel(const OneSweepA
     for (int w = 0; w < warp; ++w) off += s_w[w];
     const uint32_t bin_start = off + incl - cnt;
     s_bin_start[tid] = bin_start;
-    s_goff[tid] = a.hist_excl[tid] + excl - bin_start;
     __syncthreads();
     // keys -> shared memory at their CTA-local sorted position
 #pragma unroll
@@ -622,6 +608,20 @@ __global__ void __launch_bounds__(OS_THREADS, 3) onesweep_kernel(const OneSweepA
         rank[i] += s_bin_start[d] + s_cnt[warp][d];
         s_keys[rank[i]] = key[i];
     }
+    // look back over the earlier CTAs (digit `tid`)
+    uint32_t excl = 0;
+    if (ticket != 0) {
+        const uint32_t* p = my - 256;
+        while (true) {
+            const uint32_t v = ld_volatile_u32(p);
+            if ((v >> 30) == 0) continue;
+            excl += v & OS_VAL;
+            if ((v >> 30) == 2) break;
+            p -= 256;
+        }
+        st_volatile_u32(my, OS_INC | (excl + cnt));
+    }
+    s_goff[tid] = a.hist_excl[tid] + excl - bin_start;
     __syncthreads();
     uint32_t gpos[ITEMS];
 #pragma unroll
