@@ -50,7 +50,8 @@ typedef enum {
 
 typedef enum { FHGS_F32 = 0, FHGS_F16 = 1 } fhgs_dtype;
 
-/* Opaque context: device ordinal, SM count, last-error text.  Owns nothing on the device. */
+/* Opaque context: device ordinal, SM count, last-error text, and two copy streams + events used only
+ * by fhgs_frame_host.  Owns no device memory. */
 typedef struct fhgs_ctx fhgs_ctx;
 
 FHGS_API fhgs_status fhgs_create(fhgs_ctx** out, int device);
@@ -202,6 +203,9 @@ FHGS_API fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam, c
  * caller, same shapes), runs the four steps on `stream`, copies out_rgb / out_feat /
  * fused_feat device->host and synchronises.  Every *_host pointer is HOST memory (pinned memory
  * makes the copies asynchronous); dev_* are DEVICE pointers.  NULL host outputs are skipped.
+ * The copies run on the context's own copy streams, ordered against `stream` with events, so that
+ * host->device, device->host and the steps overlap (feature table behind P/S, GT map and the image
+ * read-back behind R/F); on return everything has completed.
  * This is the end-to-end entry bench.py times; it performs no arithmetic of its own. */
 typedef struct {
     const float *mean, *scale, *quat, *opacity, *sh; /* HOST, shapes as fhgs_gaussians */

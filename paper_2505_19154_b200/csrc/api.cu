@@ -26,11 +26,22 @@ extern "C" fhgs_status fhgs_create(fhgs_ctx** out, int device) {
         return FHGS_ERR_INTERNAL;
     }
     if (cudaSetDevice(device) != cudaSuccess) { delete c; return FHGS_ERR_INTERNAL; }
+    bool ok = cudaStreamCreateWithFlags(&c->copy_in, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&c->copy_out, cudaStreamNonBlocking) == cudaSuccess;
+    for (cudaEvent_t* e : {&c->ev_start, &c->ev_feat, &c->ev_gt, &c->ev_render, &c->ev_out})
+        ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) { delete c; return FHGS_ERR_INTERNAL; }
     *out = c;
     return FHGS_OK;
 }
 
-extern "C" void fhgs_destroy(fhgs_ctx* ctx) { delete ctx; }
+extern "C" void fhgs_destroy(fhgs_ctx* ctx) {
+    if (!ctx) return;
+    cudaStreamDestroy(ctx->copy_in);
+    cudaStreamDestroy(ctx->copy_out);
+    for (cudaEvent_t e : {ctx->ev_start, ctx->ev_feat, ctx->ev_gt, ctx->ev_render, ctx->ev_out}) cudaEventDestroy(e);
+    delete ctx;
+}
 
 extern "C" const char* fhgs_last_error(const fhgs_ctx* ctx) { return ctx ? ctx->err : "NULL context"; }
 
@@ -119,22 +130,37 @@ extern "C" fhgs_status fhgs_frame_host(fhgs_ctx* ctx, const fhgs_host_frame* hos
     const size_t n = (size_t)g->n, K = (size_t)(g->sh_degree + 1) * (g->sh_degree + 1);
     const size_t e = g->feat_dtype == FHGS_F16 ? 2 : 4, D = (size_t)g->feat_dim;
     const size_t px = (size_t)cam->width * cam->height;
+    // Schedule (three streams, so that PCIe runs in both directions while the steps execute):
+    //   s        : H2D geometry -> P -> S -> [wait feat] R -> [wait gt] F -> D2H fused -> [wait image copies]
+    //   copy_in  : H2D feat -> H2D gt                      (behind everything already enqueued on s)
+    //   copy_out : [wait R] D2H rgb, feature image         (overlaps H2D gt and F)
+    FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_start, s));
+    FHGS_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_in, ctx->ev_start, 0));
+    FHGS_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_out, ctx->ev_start, 0));
     FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->mean, host->mean, n * 12, cudaMemcpyHostToDevice, s));
     FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->scale, host->scale, n * 12, cudaMemcpyHostToDevice, s));
     FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->quat, host->quat, n * 16, cudaMemcpyHostToDevice, s));
     FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->opacity, host->opacity, n * 4, cudaMemcpyHostToDevice, s));
     FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->sh, host->sh, n * K * 12, cudaMemcpyHostToDevice, s));
-    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->feat, host->feat, n * D * e, cudaMemcpyHostToDevice, s));
-    FHGS_CUDA(ctx, cudaMemcpyAsync(ws->gt, host->gt, px * D * e, cudaMemcpyHostToDevice, s));
+    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->feat, host->feat, n * D * e, cudaMemcpyHostToDevice, ctx->copy_in));
+    FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_feat, ctx->copy_in));
+    FHGS_CUDA(ctx, cudaMemcpyAsync(ws->gt, host->gt, px * D * e, cudaMemcpyHostToDevice, ctx->copy_in));
+    FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_gt, ctx->copy_in));
     if ((st = fhgs_project(ctx, g, cam, prm, vs, stream)) != FHGS_OK) return st;
     if ((st = fhgs_bin_sort(ctx, cam, vs, nullptr, 0, stream)) != FHGS_OK) return st;
+    FHGS_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_feat, 0));
     if ((st = fhgs_render(ctx, g, cam, prm, vs, ws->out_rgb, ws->out_feat, nullptr, nullptr, stream)) != FHGS_OK) return st;
+    FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_render, s));
+    FHGS_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_out, ctx->ev_render, 0));
+    if (host->out_rgb) FHGS_CUDA(ctx, cudaMemcpyAsync(host->out_rgb, ws->out_rgb, px * 12, cudaMemcpyDeviceToHost, ctx->copy_out));
+    if (host->out_feat) FHGS_CUDA(ctx, cudaMemcpyAsync(host->out_feat, ws->out_feat, px * D * e, cudaMemcpyDeviceToHost, ctx->copy_out));
+    FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_out, ctx->copy_out));
+    FHGS_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_gt, 0));
     if ((st = fhgs_fuse_features(ctx, cam, prm, vs, ws->gt, g->feat_dim, g->feat_dtype, ws->num, ws->den,
                                  ws->fused_feat, g->feat_dtype, FHGS_FUSE_ZERO | FHGS_FUSE_FINALIZE, stream)) != FHGS_OK)
         return st;
-    if (host->out_rgb) FHGS_CUDA(ctx, cudaMemcpyAsync(host->out_rgb, ws->out_rgb, px * 12, cudaMemcpyDeviceToHost, s));
-    if (host->out_feat) FHGS_CUDA(ctx, cudaMemcpyAsync(host->out_feat, ws->out_feat, px * D * e, cudaMemcpyDeviceToHost, s));
     if (host->fused_feat) FHGS_CUDA(ctx, cudaMemcpyAsync(host->fused_feat, ws->fused_feat, n * D * e, cudaMemcpyDeviceToHost, s));
+    FHGS_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_out, 0));
     uint64_t m = 0;
     FHGS_CUDA(ctx, cudaMemcpyAsync(&m, vs->num_instances, 8, cudaMemcpyDeviceToHost, s));
     FHGS_CUDA(ctx, cudaStreamSynchronize(s));

@@ -213,6 +213,47 @@ def test_edge_cases():
         assert np.array_equal(g_full[k], g_again[k])
 
 
+def test_frame_host_equals_stepwise_calls():
+    """fhgs_frame_host (HOST buffers, copies overlapped with the steps on the context's copy streams) returns exactly
+    what the four calls return when issued one by one (P, S, R are deterministic; fused vectors up to atomic order).
+    Run twice with different host data to catch a copy racing a kernel of the previous frame."""
+    import torch
+    from paper_2505_19154_b200 import binding as fb
+    cfg = pu.reduced_config("mid", n=50_000, width=328, height=200, log_scale_mu=-3.3)
+    for seed_shift in (0, 1):
+        cfg_i = inputs.scaled(cfg, seed=cfg.seed + seed_shift)
+        scene = inputs.make_scene(cfg_i)
+        cam = inputs.make_camera(cfg_i, 0)
+        gt = inputs.make_gt_map(cfg_i, 0, cam)
+        if seed_shift == 0:
+            gp = pu.GpuPath(scene, cfg.width, cfg.height, 3_000_000)
+            dev = gp.g.mean.device
+        W, H, D, n = cfg.width, cfg.height, cfg.feat_dim, scene.n
+        c = gp.camera(cam)
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        host = dict(mean=pin(scene.mean), scale=pin(scene.scale), quat=pin(scene.quat), opacity=pin(scene.opacity),
+                    sh=pin(scene.sh), feat=pin(scene.feat), gt=pin(gt),
+                    out_rgb=torch.zeros((H, W, 3)).pin_memory(), out_feat=torch.zeros((H, W, D)).pin_memory(),
+                    fused_feat=torch.zeros((n, D)).pin_memory())
+        f32 = torch.float32
+        ws = dict(out_rgb=torch.empty((H, W, 3), dtype=f32, device=dev), out_feat=torch.empty((H, W, D), dtype=f32, device=dev),
+                  gt=torch.empty((H, W, D), dtype=f32, device=dev), num=torch.empty((n, D), dtype=f32, device=dev),
+                  den=torch.empty((n,), dtype=f32, device=dev), fused_feat=torch.from_numpy(scene.feat).to(dev))
+        m = fb.frame_host(gp.ctx, host, gp.g, c, gp.prm, gp.vs, ws)
+        # the same frame, step by step, from the device copies frame_host left in gp.g
+        c2, m2 = gp.project_sort(cam)
+        assert m == m2
+        g = gp.render(c2)
+        num, den = gp.fuse(c2, gt)
+        fused = gp.finalize(num, den, scene.feat)
+        assert np.array_equal(host["out_rgb"].numpy(), g["rgb"])
+        assert np.array_equal(host["out_feat"].numpy(), g["feat"])
+        seen = den.cpu().numpy() > 1e-3
+        assert np.abs(host["fused_feat"].numpy()[seen] - fused[seen]).max() <= 1e-5
+        assert np.array_equal(host["fused_feat"].numpy()[~seen & (den.cpu().numpy() <= 1e-8)],
+                              scene.feat[~seen & (den.cpu().numpy() <= 1e-8)])
+
+
 def test_tile_visited_diagnostics():
     """fhgs_render's per-tile 'visited' diagnostics (work accounting only): never longer than the tile's list; the
     Tiny scene never saturates, so every tile walks its whole list; a saturating scene stops early somewhere."""
