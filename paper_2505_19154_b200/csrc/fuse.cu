@@ -357,8 +357,8 @@ template <typename GT>
 __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT>& sm, const FuseArgs& a) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int half = warp >> 2, cw = warp & 3;
-    const int kg = lane >> 3, cg = lane & 7;
-    const int ch = cw * 32 + cg * 4;          // this thread's 4 channels inside the chunk
+    const int kg = warp & 3;                  // the warp's 8 instances of the batch (a short batch idles whole warps)
+    const int ch = lane * 4;                  // this thread's 4 channels inside the chunk
     const GT* Gs = sm.G + half * 128 * FW_DC + ch;
     int stage = 0;
     uint32_t phase = 0, gphase = 0, batch = 0;
@@ -389,7 +389,7 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT>& sm, const FuseA
         ulonglong2 wb = *reinterpret_cast<const ulonglong2*>(Ws + FW_WQ);
         float4 g = ld_g4(Gs);
 #pragma unroll 1
-        for (int s0 = 0; s0 < 128; s0 += 16) {
+        for (int s0 = 0; s0 < (kg * 8 < m.nb ? 128 : 0); s0 += 16) {
             const float* Wb = Ws + s0 * 4;
             const GT* Gb = Gs + s0 * FW_DC;
 #pragma unroll
