@@ -529,3 +529,117 @@ void fo_fuse_finalize(int n, int D, const double *num, const double *den, double
         if (l2norm && ss > 0.0) { const double inv = 1.0 / sqrt(ss); for (int c = 0; c < D; ++c) f[c] *= inv; }
     }
 }
+
+/* ------------------------------------------------------------------------------------------
+ * NDFD forward (Eq. 5-6, Alg. 2).
+ * Per pixel x with ground-truth feature f_gt = gt[x,:], over the fragments of the ray in the
+ * front-to-back blend order of C1-R (same q cut-off, alpha clamp, w_i = alpha_i T_i, stop at
+ * T < t_min):
+ *     phi_i   = f_i . f_gt                      (features are unit-norm, so the
+ *                                                cosine is the dot product)
+ *     sigma_i = 1 / (1 + exp(k (phi_i - lambda)))
+ *     L_gt(x) = sum_i w_i sigma_i                            (Eq. 5)
+ *     L_cf(x) = sum_i sigma_i w_i (W_{i-1} - F_{i-1} . f_i)  (Eq. 6)
+ * with W_n = sum_{i<=n} w_i and F_n = sum_{i<=n} w_i f_i accumulated
+ *   mode 0: in blend order, front to back ("updated one time in each step during the
+ *           front-to-back blend") -- the form the CUDA path builds;
+ *   mode 1: from far to near ("along the ray from far to near"): the fragment list
+ *           of the pixel is collected first and the recurrence runs over it reversed.
+ * The two differ (sigma_i multiplies a different partner set); DESIGN.md lists the reading.
+ * fo_ndfd_pairwise evaluates the explicit O(N^2) double sum of Eq. 6's first line over the same
+ * fragment list (partners j = fragments BEFORE i in the accumulation order) -- the pin of the
+ * O(N) recurrence.
+ * pix: int32 linear pixel ids (y*W+x) or NULL for all pixels.  Outputs double [npix].
+ * ------------------------------------------------------------------------------------------ */
+typedef struct { double w; uint32_t g; } fo_frag;
+
+static int collect_fragments(int n_order, const uint32_t *order, const float *xy, const float *co,
+                             int x, int y, float q_cut, float alpha_max, double t_min,
+                             fo_frag **buf, int *cap) {
+    int cnt = 0;
+    double T = 1.0;
+    for (int k = 0; k < n_order; ++k) {
+        if (T < t_min) break;
+        const uint32_t g = order[k];
+        double alpha;
+        if (!eval_alpha(xy, co, g, x, y, q_cut, alpha_max, &alpha)) continue;
+        if (cnt == *cap) { *cap = *cap ? 2 * *cap : 256; *buf = (fo_frag *)realloc(*buf, (size_t)*cap * sizeof(fo_frag)); }
+        (*buf)[cnt].w = alpha * T; (*buf)[cnt].g = g; ++cnt;
+        T = T * (1.0 - alpha);
+    }
+    return cnt;
+}
+
+static double dotf(const float *a, const float *b, int D) {
+    double s = 0.0;
+    for (int c = 0; c < D; ++c) s += (double)a[c] * (double)b[c];
+    return s;
+}
+
+void fo_ndfd_literal(int n_order, const uint32_t *order, int D, const float *xy,
+                     const float *conic_opacity, const float *feat, const float *gt, int W, int H,
+                     const float *prm, double k_sig, double lambda, int mode, int64_t npix,
+                     const int32_t *pix, double *out_lgt, double *out_lcf) {
+    const float q_cut = prm[P_QCUT], alpha_max = prm[P_AMAX];
+    const double t_min = (double)prm[P_TMIN];
+    if (!pix) npix = (int64_t)W * H;
+#pragma omp parallel
+    {
+        fo_frag *fr = NULL; int cap = 0;
+        double *F = (double *)malloc((size_t)D * sizeof(double));
+#pragma omp for schedule(dynamic, 16)
+        for (int64_t p = 0; p < npix; ++p) {
+            const int id = pix ? pix[p] : (int)p;
+            const int x = id % W, y = id / W;
+            const float *fgt = gt + (size_t)id * D;
+            const int cnt = collect_fragments(n_order, order, xy, conic_opacity, x, y, q_cut, alpha_max, t_min, &fr, &cap);
+            double lgt = 0.0, lcf = 0.0, Wc = 0.0;
+            for (int c = 0; c < D; ++c) F[c] = 0.0;
+            for (int s = 0; s < cnt; ++s) {
+                const fo_frag *e = &fr[mode ? cnt - 1 - s : s];
+                const float *f = feat + (size_t)e->g * D;
+                const double phi = dotf(f, fgt, D);
+                const double sigma = 1.0 / (1.0 + exp(k_sig * (phi - lambda)));
+                double Ff = 0.0;
+                for (int c = 0; c < D; ++c) Ff += F[c] * (double)f[c];
+                lgt += e->w * sigma;
+                lcf += sigma * e->w * (Wc - Ff);
+                Wc += e->w;
+                for (int c = 0; c < D; ++c) F[c] += e->w * (double)f[c];
+            }
+            out_lgt[p] = lgt; out_lcf[p] = lcf;
+        }
+        free(F); free(fr);
+    }
+}
+
+void fo_ndfd_pairwise(int n_order, const uint32_t *order, int D, const float *xy,
+                      const float *conic_opacity, const float *feat, const float *gt, int W, int H,
+                      const float *prm, double k_sig, double lambda, int mode, int64_t npix,
+                      const int32_t *pix, double *out_lcf) {
+    const float q_cut = prm[P_QCUT], alpha_max = prm[P_AMAX];
+    const double t_min = (double)prm[P_TMIN];
+    if (!pix) npix = (int64_t)W * H;
+#pragma omp parallel
+    {
+        fo_frag *fr = NULL; int cap = 0;
+#pragma omp for schedule(dynamic, 16)
+        for (int64_t p = 0; p < npix; ++p) {
+            const int id = pix ? pix[p] : (int)p;
+            const float *fgt = gt + (size_t)id * D;
+            const int cnt = collect_fragments(n_order, order, xy, conic_opacity, id % W, id / W, q_cut, alpha_max, t_min, &fr, &cap);
+            double lcf = 0.0;
+            for (int s = 0; s < cnt; ++s) {
+                const fo_frag *ei = &fr[mode ? cnt - 1 - s : s];
+                const float *fi = feat + (size_t)ei->g * D;
+                const double sigma = 1.0 / (1.0 + exp(k_sig * (dotf(fi, fgt, D) - lambda)));
+                for (int t = 0; t < s; ++t) {
+                    const fo_frag *ej = &fr[mode ? cnt - 1 - t : t];
+                    lcf += sigma * ei->w * ej->w * (1.0 - dotf(fi, feat + (size_t)ej->g * D, D));
+                }
+            }
+            out_lcf[p] = lcf;
+        }
+        free(fr);
+    }
+}

@@ -177,3 +177,23 @@ def finalize(num, den, feat_prev, den_eps=1e-8, l2norm=False) -> np.ndarray:
     lib().fo_fuse_finalize(C.c_int(n), C.c_int(D), _p(num), _p(den), C.c_double(den_eps),
                            C.c_int(1 if l2norm else 0), _p(out))
     return out
+
+
+def ndfd(pr, order, feat, gt, W, H, k=20.0, lam=0.5, mode=0, params=DEFAULT_PARAMS, pix=None, pairwise=False):
+    """NDFD forward: per-pixel L_gt, L_cf (float64) over `pix` (int32 linear ids; None = all).
+    mode 0: W, F accumulated in blend order (front to back); mode 1: from far to near.  pairwise=True also returns
+    the explicit O(N^2) double sum of Eq. 6 (third array)."""
+    feat32, gt32 = _f32(feat), _f32(gt)
+    D = feat32.shape[1]
+    if pix is not None:
+        pix = np.ascontiguousarray(pix, dtype=np.int32)
+    npix = W * H if pix is None else pix.shape[0]
+    lgt, lcf = np.zeros(npix, np.float64), np.zeros(npix, np.float64)
+    args = (C.c_int(order.shape[0]), _p(order), C.c_int(D), _p(pr["xy"]), _p(pr["conic_opacity"]), _p(feat32), _p(gt32),
+            C.c_int(W), C.c_int(H), _p(_f32(params)), C.c_double(k), C.c_double(lam), C.c_int(mode), C.c_int64(npix), _p(pix))
+    lib().fo_ndfd_literal(*args, _p(lgt), _p(lcf))
+    if not pairwise:
+        return lgt, lcf
+    pw = np.zeros(npix, np.float64)
+    lib().fo_ndfd_pairwise(*args, _p(pw))
+    return lgt, lcf, pw
