@@ -198,6 +198,23 @@ FHGS_API fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam, c
                                int32_t gt_dtype, float* num, float* den, void* out_feat,
                                int32_t out_dtype, uint32_t flags, void* stream);
 
+/* NDFD forward -- the paper's non-differentiable feature driving losses
+ * (Eq. 5-6) and PAPER.md:305-335 (Alg. 2), evaluated per pixel x in the SAME front-to-back traversal as
+ * step R (same q cut-off, alpha clamp, w_i = alpha_i T_i, stop once T < t_min), with f_gt = gt[x,:]:
+ *     phi_i = f_i . f_gt (features unit-norm),  sigma_i = 1 / (1 + exp(k (phi_i - lambda)))
+ *     out_lgt[x] = sum_i w_i sigma_i                                   (Eq. 5)
+ *     out_lcf[x] = sum_i sigma_i w_i (W_{i-1} - F_{i-1} . f_i)          (Eq. 6)
+ * where W_n = sum_{i<=n} w_i, F_n = sum_{i<=n} w_i f_i are accumulated in blend order, front to back
+ * (the far-to-near wording of PAPER.md:136 is the other reading).  No feature image
+ * is rendered.  Paper defaults: k = 20, lambda = 0.5.
+ * g->feat [n,D] f32/f16 and gt [H,W,D] f32/f16, both 16-byte aligned; D in {32,64,128,256,512};
+ * out_lgt, out_lcf [H,W] f32 (every pixel is written; pixels no Gaussian reaches get 0).
+ * Uses vs->{xy,conic_opacity,ranges,vals[sorted_buf]} as fhgs_render does. */
+FHGS_API fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam,
+                              const fhgs_params* prm, const fhgs_view_state* vs, const void* gt,
+                              int32_t gt_dtype, float k_sigmoid, float lambda, float* out_lgt,
+                              float* out_lcf, void* stream);
+
 /* One whole frame (P -> S -> R -> F with ZERO|FINALIZE) from HOST buffers: copies the Gaussian
  * arrays and the GT map host->device into `dev_g` / `dev_gt` (device staging owned by the
  * caller, same shapes), runs the four steps on `stream`, copies out_rgb / out_feat /

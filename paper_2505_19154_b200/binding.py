@@ -20,7 +20,7 @@ FHGS_SORT_FULL_KEY = 1
 FHGS_FUSE_ZERO, FHGS_FUSE_FINALIZE, FHGS_FUSE_L2NORM, FHGS_FUSE_FINALIZE_ONLY, FHGS_FUSE_ZERO_ONLY = 1, 2, 4, 8, 16
 
 EXPORTS = ["fhgs_create", "fhgs_destroy", "fhgs_last_error", "fhgs_version", "fhgs_default_params",
-           "fhgs_scratch_bytes", "fhgs_scratch_tile_visited", "fhgs_project", "fhgs_bin_sort", "fhgs_render", "fhgs_fuse_features",
+           "fhgs_scratch_bytes", "fhgs_scratch_tile_visited", "fhgs_project", "fhgs_bin_sort", "fhgs_render", "fhgs_fuse_features", "fhgs_ndfd_forward",
            "fhgs_frame_host", "fhgs_ffma_peak"]
 
 
@@ -97,6 +97,8 @@ def _load():
     lib.fhgs_frame_host.argtypes = [vp, C.POINTER(CHostFrame), C.POINTER(CGaussians), C.POINTER(CCamera),
                                     C.POINTER(CParams), C.POINTER(CViewState), C.POINTER(CFrameWorkspace),
                                     C.POINTER(C.c_uint64), vp]
+    lib.fhgs_ndfd_forward.argtypes = [vp, C.POINTER(CGaussians), C.POINTER(CCamera), C.POINTER(CParams), C.POINTER(CViewState),
+                                      vp, C.c_int32, C.c_float, C.c_float, vp, vp, vp]
     lib.fhgs_ffma_peak.argtypes = [vp, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
     return lib
 
@@ -302,6 +304,14 @@ def fuse_features(ctx: Context, cam, prm: CParams, vs: ViewState, gt, num, den, 
     ctx.check(lib.fhgs_fuse_features(ctx.handle, None if cam is None else C.byref(cam), C.byref(prm), C.byref(vs.c),
                                      _ptr(gt), d, gt_code, _ptr(num), _ptr(den), _ptr(out_feat), out_code,
                                      C.c_uint32(flags), _stream(stream)))
+
+
+def ndfd_forward(ctx: Context, g: Gaussians, cam: CCamera, prm: CParams, vs: ViewState, gt, out_lgt, out_lcf,
+                 k: float = 20.0, lam: float = 0.5, stream=None):
+    """fhgs_ndfd_forward: per-pixel L_gt, L_cf ([H,W] f32 tensors, caller-allocated) of PAPER.md Eq. 5-6."""
+    ctx.check(lib.fhgs_ndfd_forward(ctx.handle, C.byref(g.c), C.byref(cam), C.byref(prm), C.byref(vs.c), _ptr(gt),
+                                    _dtype_code(gt), C.c_float(k), C.c_float(lam), _ptr(out_lgt), _ptr(out_lcf),
+                                    _stream(stream)))
 
 
 def frame_host(ctx: Context, host: dict, g: Gaussians, cam: CCamera, prm: CParams, vs: ViewState, ws: dict,

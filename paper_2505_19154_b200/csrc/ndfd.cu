@@ -1,0 +1,178 @@
+// ndfd.cu -- NDFD forward (fhgs_ndfd_forward): the paper's non-differentiable feature
+// driving losses, evaluated in the same front-to-back traversal as step R without rendering a feature image
+// (Eq. 5-6; Alg. 2):
+//     phi_i = f_i . f_gt(x),  sigma_i = 1 / (1 + exp(k (phi_i - lambda))),  w_i = alpha_i T_i
+//     L_gt(x) = sum_i w_i sigma_i
+//     L_cf(x) = sum_i sigma_i w_i (W_{i-1} - F_{i-1} . f_i),   W, F accumulated in blend order (DESIGN.md reading)
+//
+// First CUDA path of this row (correctness first; not yet the warp-specialised form of render/fuse):
+// one CTA of 256 threads per 16x2 pixel strip of a tile (grid = tiles x 8).  Eight lanes share one pixel and
+// split the D channels; each lane keeps its slice of the pixel's ground-truth vector f_gt and of the running
+// feature F in registers.  The CTA streams the tile's sorted range 256 instances at a time through the
+// traverse.cuh staging (exact ellipse-vs-strip cull); every warp then walks the survivors for its 4 pixels:
+// the normative q / cut-off / alpha / T arithmetic of C1-R, and -- only when one of its pixels has a weight --
+// the two D-length dot products (8-lane shuffle reduction) and the update of F.
+#include <cuda_fp16.h>
+
+#include "traverse.cuh"
+
+namespace {
+
+struct NdfdArgs {
+    TraverseArgs t;
+    const void* feat;   // [n,D]
+    const void* gt;     // [H,W,D]
+    int D;
+    float k_sig, lambda;
+    float* out_lgt;
+    float* out_lcf;
+};
+
+template <typename T>
+__device__ __forceinline__ float4 ld4(const T* p);
+template <>
+__device__ __forceinline__ float4 ld4<float>(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+template <>
+__device__ __forceinline__ float4 ld4<__half>(const __half* p) {
+    const uint2 r = __ldg(reinterpret_cast<const uint2*>(p));
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
+    const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
+    return make_float4(a.x, a.y, b.x, b.y);
+}
+
+constexpr int ND_STRIPS = 8;   // 16x2-pixel strips per tile
+
+// CPL = channels per lane = D / 8
+template <int CPL, typename FT, typename GT>
+__global__ void __launch_bounds__(TR_THREADS) ndfd_strip_kernel(const NdfdArgs a) {
+    __shared__ TileQueue q;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tile = blockIdx.x / ND_STRIPS, strip = blockIdx.x % ND_STRIPS;
+    const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE + 2 * strip;
+    if (ty0 >= a.t.H) return;
+    // pixel of this lane group: warp w covers x = 4 (w & 3) .. +3 of row (w >> 2)
+    const int pxl = lane >> 3, cgl = lane & 7;
+    const int px = tx0 + ((warp & 3) << 2) + pxl, py = ty0 + (warp >> 2);
+    const bool inside = px < a.t.W && py < a.t.H;
+    const float fx = (float)px, fy = (float)py;
+    const float bx0 = (float)tx0, by0 = (float)ty0;
+    const float bx1 = (float)min(tx0 + FHGS_TILE - 1, a.t.W - 1), by1 = (float)min(ty0 + 1, a.t.H - 1);
+    const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
+    const FT* feat = reinterpret_cast<const FT*>(a.feat);
+    const GT* gt = reinterpret_cast<const GT*>(a.gt);
+    const int c_lo = cgl * CPL;
+
+    float g[CPL], F[CPL];
+#pragma unroll
+    for (int j = 0; j < CPL / 4; ++j) {
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (inside) v = ld4<GT>(gt + ((size_t)py * a.t.W + px) * a.D + c_lo + 4 * j);
+        g[4 * j] = v.x; g[4 * j + 1] = v.y; g[4 * j + 2] = v.z; g[4 * j + 3] = v.w;
+    }
+#pragma unroll
+    for (int j = 0; j < CPL; ++j) F[j] = 0.f;
+    float T = 1.f, Wc = 0.f, lgt = 0.f, lcf = 0.f;
+    uint32_t n = 0;
+    bool done = !inside;
+    const float k2 = a.k_sig * 1.44269504088896340736f;   // exp(k z) = exp2(k2 z)
+
+    uint32_t pos = range.x;
+    while (pos < range.y) {
+        const int added = stage_chunk(a.t, q, pos, range.y, 0, bx0, by0, bx1, by1);
+        pos += TR_THREADS;
+        for (int kk = 0; kk < added; ++kk) {
+            const float w = eval_weight(q.xy[kk], q.co[kk], fx, fy, a.t, T, done, n);
+            if (!__any_sync(TR_FULL, w != 0.f)) continue;
+            const FT* f = feat + (size_t)q.id[kk] * a.D + c_lo;
+            float phi = 0.f, Ff = 0.f;
+            float fv[CPL];
+#pragma unroll
+            for (int j = 0; j < CPL / 4; ++j) {
+                const float4 v = ld4<FT>(f + 4 * j);
+                fv[4 * j] = v.x; fv[4 * j + 1] = v.y; fv[4 * j + 2] = v.z; fv[4 * j + 3] = v.w;
+            }
+#pragma unroll
+            for (int j = 0; j < CPL; ++j) {
+                phi = fmaf(fv[j], g[j], phi);
+                Ff = fmaf(fv[j], F[j], Ff);
+            }
+#pragma unroll
+            for (int d = 1; d < 8; d <<= 1) {
+                phi += __shfl_xor_sync(TR_FULL, phi, d);
+                Ff += __shfl_xor_sync(TR_FULL, Ff, d);
+            }
+            const float sigma = 1.0f / (1.0f + exp2f(k2 * (phi - a.lambda)));
+            const float sw = sigma * w;        // w == 0 for pixels the Gaussian does not reach: nothing changes
+            lgt += sw;
+            lcf = fmaf(sw, Wc - Ff, lcf);
+            Wc += w;
+#pragma unroll
+            for (int j = 0; j < CPL; ++j) F[j] = fmaf(w, fv[j], F[j]);
+        }
+        if (__syncthreads_and(done)) break;
+    }
+    if (inside && cgl == 0) {
+        const size_t o = (size_t)py * a.t.W + px;
+        a.out_lgt[o] = lgt;
+        a.out_lcf[o] = lcf;
+    }
+}
+
+template <int CPL, typename FT, typename GT>
+cudaError_t launch(const NdfdArgs& a, int tiles, cudaStream_t st) {
+    ndfd_strip_kernel<CPL, FT, GT><<<tiles * ND_STRIPS, TR_THREADS, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <typename FT, typename GT>
+cudaError_t dispatch(const NdfdArgs& a, int tiles, cudaStream_t st) {
+    switch (a.D / 8) {
+        case 4: return launch<4, FT, GT>(a, tiles, st);
+        case 8: return launch<8, FT, GT>(a, tiles, st);
+        case 16: return launch<16, FT, GT>(a, tiles, st);
+        case 32: return launch<32, FT, GT>(a, tiles, st);
+        case 64: return launch<64, FT, GT>(a, tiles, st);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace
+
+extern "C" fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam,
+                                         const fhgs_params* prm, const fhgs_view_state* vs, const void* gt,
+                                         int32_t gt_dtype, float k_sigmoid, float lambda, float* out_lgt, float* out_lcf,
+                                         void* stream) {
+    if (!ctx) return FHGS_ERR_INVALID;
+    if (!g || !cam || !prm || !vs || !gt || !out_lgt || !out_lcf) FHGS_INVALID(ctx, "fhgs_ndfd_forward: NULL argument");
+    fhgs_status st;
+    if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
+    if ((st = validate_params(ctx, prm)) != FHGS_OK) return st;
+    if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
+    if (!g->feat) FHGS_INVALID(ctx, "fhgs_ndfd_forward: g->feat is NULL");
+    if ((g->feat_dtype != FHGS_F32 && g->feat_dtype != FHGS_F16) || (gt_dtype != FHGS_F32 && gt_dtype != FHGS_F16))
+        FHGS_INVALID(ctx, "fhgs_ndfd_forward: unknown dtype");
+    const int D = g->feat_dim;
+    if (!(D == 32 || D == 64 || D == 128 || D == 256 || D == 512))
+        FHGS_INVALID(ctx, "fhgs_ndfd_forward: feat_dim must be 32, 64, 128, 256 or 512");
+    if (!aligned_to(g->feat, 16) || !aligned_to(gt, 16)) FHGS_INVALID(ctx, "fhgs_ndfd_forward: feat/gt must be 16-byte aligned");
+    if (g->n != vs->n) FHGS_INVALID(ctx, "fhgs_ndfd_forward: g->n != vs->n");
+    if (!finite_f(k_sigmoid) || !finite_f(lambda)) FHGS_INVALID(ctx, "fhgs_ndfd_forward: non-finite k / lambda");
+    NdfdArgs a;
+    a.t.W = cam->width; a.t.H = cam->height; a.t.GW = tiles_x(cam->width);
+    a.t.ranges = vs->ranges; a.t.vals = vs->vals[vs->sorted_buf & 1];
+    a.t.xy = reinterpret_cast<const float2*>(vs->xy);
+    a.t.conic_opacity = reinterpret_cast<const float4*>(vs->conic_opacity);
+    a.t.q_cutoff = prm->q_cutoff; a.t.alpha_max = prm->alpha_max; a.t.t_min = prm->t_min;
+    a.feat = g->feat; a.gt = gt; a.D = D; a.k_sig = k_sigmoid; a.lambda = lambda;
+    a.out_lgt = out_lgt; a.out_lcf = out_lcf;
+    const int tiles = tiles_x(cam->width) * tiles_y(cam->height);
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e;
+    const bool fh = g->feat_dtype == FHGS_F16, gh = gt_dtype == FHGS_F16;
+    if (fh && gh) e = dispatch<__half, __half>(a, tiles, s);
+    else if (fh) e = dispatch<__half, float>(a, tiles, s);
+    else if (gh) e = dispatch<float, __half>(a, tiles, s);
+    else e = dispatch<float, float>(a, tiles, s);
+    FHGS_CUDA(ctx, e);
+    return FHGS_OK;
+}

@@ -1,0 +1,102 @@
+"""GPU parity of fhgs_ndfd_forward against the NDFD oracle: per-pixel L_gt and L_cf within 1e-4
+(2e-3 with fp16 storage) on sampled pixels, all tile/edge cases, plus the closed form that ties it to fhgs_render."""
+import numpy as np
+import pytest
+
+from oracle import fhgs_oracle as fo
+from paper_2505_19154_b200 import inputs
+import parity_util as pu
+
+pytestmark = pytest.mark.gpu
+
+
+def _run(cfg, view, tol, npix=4000, k=20.0, lam=0.5):
+    import torch
+    from paper_2505_19154_b200 import binding as fb
+    scene = inputs.make_scene(cfg)
+    cam = inputs.make_camera(cfg, view)
+    gt = inputs.make_gt_map(cfg, view, cam)
+    pr = pu.oracle_view(scene, cam)
+    m = fo.bins(pr, cfg.width, cfg.height)["M"]
+    gp = pu.GpuPath(scene, cfg.width, cfg.height, m + 64)
+    c, _ = gp.project_sort(cam)
+    dev = gp.g.mean.device
+    H, W = cfg.height, cfg.width
+    lgt = torch.full((H, W), -1.0, dtype=torch.float32, device=dev)
+    lcf = torch.full((H, W), -1.0, dtype=torch.float32, device=dev)
+    gt_d = torch.from_numpy(np.ascontiguousarray(gt)).to(dev)
+    fb.ndfd_forward(gp.ctx, gp.g, c, gp.prm, gp.vs, gt_d, lgt, lcf, k=k, lam=lam)
+    torch.cuda.synchronize()
+    lgt, lcf = lgt.cpu().numpy().ravel(), lcf.cpu().numpy().ravel()
+    rng = np.random.default_rng(17 + view)
+    pix = np.unique(np.concatenate([rng.integers(0, W * H, size=npix), np.arange(W), (H - 1) * W + np.arange(W),
+                                    np.arange(H) * W + W - 1])).astype(np.int32)
+    order = fo.global_order(pr)
+    o_lgt, o_lcf = fo.ndfd(pr, order, scene.feat.astype(np.float32), gt.astype(np.float32), W, H, k=k, lam=lam, pix=pix)
+    frag = fo.render_literal(pr, order, None, W, H, pix=pix)["fragile"].astype(bool)
+    slack = np.where(frag, 3.0 * tol, tol)      # a fragment blended at T ~ t_min adds <= 1e-4 (sigma + W) to either loss
+    e1, e2 = np.abs(lgt[pix] - o_lgt), np.abs(lcf[pix] - o_lcf)
+    assert np.all(e1 <= slack), (e1.max(), int(np.argmax(e1)))
+    assert np.all(e2 <= slack), (e2.max(), int(np.argmax(e2)))
+    assert lgt.min() >= 0.0 and o_lgt.max() > 0.05      # every pixel was written; the case is not trivial
+    return dict(lgt=float(e1.max()), lcf=float(e2.max()), fragile=int(frag.sum()), lcf_max=float(np.abs(o_lcf).max()))
+
+
+def test_ndfd_mid_shape_d128_ragged():
+    """D=128 unit features, 328x200 (ragged right column and bottom row), saturating scene."""
+    cfg = pu.reduced_config("mid", n=60_000, width=328, height=200, log_scale_mu=-3.3)
+    print(_run(cfg, 0, pu.TOL_F32))
+
+
+def test_ndfd_other_dims_and_fp16():
+    """D = 32, 64, 256 (fp32) and D = 512 stored fp16 (Large shape)."""
+    for d in (32, 64, 256):
+        cfg = pu.reduced_config("mid", n=15_000, width=160, height=96, log_scale_mu=-3.0, feat_dim=d)
+        print(d, _run(cfg, 0, pu.TOL_F32, npix=1500))
+    cfg = pu.reduced_config("large", n=20_000, width=200, height=120, log_scale_mu=-3.3)
+    print(512, _run(cfg, 0, pu.TOL_F16, npix=1500))
+
+
+def test_ndfd_multiview_blobs_and_params():
+    """Blob scene (per-blob constant maps: phi close to 1 inside a blob), non-default k and lambda."""
+    cfg = pu.reduced_config("multiview", n=40_000, width=216, height=168, n_views=200, log_scale_mu=-3.0)
+    print(_run(cfg, 67, pu.TOL_F32, npix=2500, k=8.0, lam=0.3))
+
+
+def test_ndfd_constant_polarity_matches_render():
+    """k = 0 -> sigma = 1/2: L_gt = (1 - T_final)/2 and L_cf = ((1 - T_final)^2 - |feat_img|^2)/4 (unit features) with
+    T_final and feat_img from fhgs_render on the same view state: the two kernels share one traversal semantics."""
+    import torch
+    from paper_2505_19154_b200 import binding as fb
+    cfg = pu.reduced_config("mid", n=30_000, width=160, height=96, log_scale_mu=-3.0, feat_dim=64)
+    scene = inputs.make_scene(cfg)
+    cam = inputs.make_camera(cfg, 0)
+    gp = pu.GpuPath(scene, cfg.width, cfg.height, 4_000_000)
+    c, _ = gp.project_sort(cam)
+    r = gp.render(c)
+    dev = gp.g.mean.device
+    lgt = torch.empty((cfg.height, cfg.width), dtype=torch.float32, device=dev)
+    lcf = torch.empty_like(lgt)
+    gt_d = torch.from_numpy(inputs.make_gt_map(cfg, 0, cam)).to(dev)
+    fb.ndfd_forward(gp.ctx, gp.g, c, gp.prm, gp.vs, gt_d, lgt, lcf, k=0.0)
+    torch.cuda.synchronize()
+    Wsum = 1.0 - r["T"].astype(np.float64)
+    assert np.abs(lgt.cpu().numpy() - 0.5 * Wsum).max() <= 1e-5
+    ref = 0.25 * (Wsum ** 2 - (r["feat"].astype(np.float64) ** 2).sum(axis=2))
+    assert np.abs(lcf.cpu().numpy() - ref).max() <= 1e-5
+
+
+def test_ndfd_invalid_arguments():
+    import torch
+    from paper_2505_19154_b200 import binding as fb
+    cfg = inputs.CONFIGS["tiny"]            # D = 8 is not supported by the NDFD kernel
+    scene = inputs.make_scene(cfg)
+    cam = inputs.make_camera(cfg, 0)
+    gp = pu.GpuPath(scene, 64, 64, 8192)
+    c, _ = gp.project_sort(cam)
+    dev = gp.g.mean.device
+    out = torch.empty((64, 64), dtype=torch.float32, device=dev)
+    gt = torch.zeros((64, 64, 8), dtype=torch.float32, device=dev)
+    with pytest.raises(fb.FhgsError) as ei:
+        fb.ndfd_forward(gp.ctx, gp.g, c, gp.prm, gp.vs, gt, out, out.clone())
+    assert ei.value.status == fb.FHGS_ERR_INVALID
