@@ -327,6 +327,25 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     if traffic:
         roofline["traffic_source"] = traffic["source"]
 
+    # ---- optional: the NEXT-1 row (NDFD forward losses) on the same frame, timed for the record
+    ndfd = None
+    if args.ndfd:
+        lgt = torch.empty((H, W), dtype=f32, device=dev)
+        lcf = torch.empty((H, W), dtype=f32, device=dev)
+        for _ in range(2):
+            fb.ndfd_forward(ctx, g, cam, prm, vs, gt, lgt, lcf)
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        ev[0].record(stream)
+        for _ in range(5):
+            fb.ndfd_forward(ctx, g, cam, prm, vs, gt, lgt, lcf)
+        ev[1].record(stream)
+        torch.cuda.synchronize()
+        nms = ev[0].elapsed_time(ev[1]) / 5
+        # lane-ops: 7 n_eval + (3 D + 12) n_contrib (phi, F.f and the F update are D FMAs each)
+        nops = 7 * n_eval_total + (3 * D + 12) * n_contrib_total
+        ndfd = {"ms": nms, "frac_of_nominal_fp32": nops / (nms * 1e-3) / alu_nominal,
+                "mean_lgt": float(lgt.mean().item()), "mean_lcf": float(lcf.mean().item())}
+
     # ---- end to end through fhgs_frame_host: host (pinned) buffers, copies inside the timed region
     e2e = None
     if not args.no_e2e:
@@ -375,7 +394,7 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
                            "parallelism": f"{world} independent frame(s), one per GPU"},
                 "ms": parts, "roofline": roofline, "roofline_steps": steps_roof,
                 "ffma_peak_measured_tflops": 2.0 * ffma_ops / 1e12,
-                "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches_per_frame(W, H) * args.steps,
+                "ndfd_forward": ndfd, "cpu_baseline": cpu_baseline, "e2e": e2e, "gpu_launches": launches_per_frame(W, H) * args.steps,
                 "clocks": clocks}
         print(json.dumps(line), flush=True)
     if world > 1:
@@ -516,6 +535,7 @@ def main():
     ap.add_argument("--small", action="store_true", help="debug-size workload (not a bench line)")
     ap.add_argument("--workload", default="mid", choices=["mid", "tiny", "small", "large", "multiview"],
                     help="mid = the bench line (BASELINE.json metric); the others are timed for the record only")
+    ap.add_argument("--ndfd", action="store_true", help="mid: also time fhgs_ndfd_forward (NEXT-1 row) on the frame")
     ap.add_argument("--views", type=int, default=8, help="multiview: number of evenly spaced orbit cameras per sweep")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

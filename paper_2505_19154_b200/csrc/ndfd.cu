@@ -9,7 +9,8 @@
 // one CTA of 256 threads per 16x2 pixel strip of a tile (grid = tiles x 8).  Eight lanes share one pixel and
 // split the D channels; each lane keeps its slice of the pixel's ground-truth vector f_gt and of the running
 // feature F in registers.  The CTA streams the tile's sorted range 256 instances at a time through the
-// traverse.cuh staging (exact ellipse-vs-strip cull); every warp then walks the survivors for its 4 pixels:
+// traverse.cuh staging (exact ellipse-vs-strip cull), gathers the survivors' feature rows into shared memory with
+// double-buffered cp.async; every warp then walks the survivors for its 4 pixels:
 // the normative q / cut-off / alpha / T arithmetic of C1-R, and -- only when one of its pixels has a weight --
 // the two D-length dot products (8-lane shuffle reduction) and the update of F.
 #include <cuda_fp16.h>
@@ -42,9 +43,31 @@ __device__ __forceinline__ float4 ld4<__half>(const __half* p) {
 
 constexpr int ND_STRIPS = 8;   // 16x2-pixel strips per tile
 
+template <typename T>
+__device__ __forceinline__ float4 lds4(const T* p);
+template <>
+__device__ __forceinline__ float4 lds4<float>(const float* p) { return *reinterpret_cast<const float4*>(p); }
+template <>
+__device__ __forceinline__ float4 lds4<__half>(const __half* p) {
+    const uint2 r = *reinterpret_cast<const uint2*>(p);
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
+    const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
+    return make_float4(a.x, a.y, b.x, b.y);
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// survivors whose feature rows are staged together (one of two 16 KB shared-memory buffers)
+template <int CPL, typename FT>
+struct NdSub {
+    static constexpr int ROW_BYTES = CPL * 8 * (int)sizeof(FT);
+    static constexpr int SB = 16384 / ROW_BYTES > 32 ? 32 : (16384 / ROW_BYTES < 4 ? 4 : 16384 / ROW_BYTES);
+};
+
 // CPL = channels per lane = D / 8
 template <int CPL, typename FT, typename GT>
-__global__ void __launch_bounds__(TR_THREADS) ndfd_strip_kernel(const NdfdArgs a) {
+__global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 1) ndfd_strip_kernel(const NdfdArgs a) {
     __shared__ TileQueue q;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x / ND_STRIPS, strip = blockIdx.x % ND_STRIPS;
@@ -60,13 +83,15 @@ __global__ void __launch_bounds__(TR_THREADS) ndfd_strip_kernel(const NdfdArgs a
     const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
     const FT* feat = reinterpret_cast<const FT*>(a.feat);
     const GT* gt = reinterpret_cast<const GT*>(a.gt);
-    const int c_lo = cgl * CPL;
+    // channel slice of this lane: float4 groups cgl, cgl + 8, cgl + 16, ... (interleaved, so that the 8 lanes of a
+    // pixel read 128 contiguous bytes per load: coalesced from global, conflict-free from shared memory)
+    const int c_lo = cgl * 4;
 
     float g[CPL], F[CPL];
 #pragma unroll
     for (int j = 0; j < CPL / 4; ++j) {
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (inside) v = ld4<GT>(gt + ((size_t)py * a.t.W + px) * a.D + c_lo + 4 * j);
+        if (inside) v = ld4<GT>(gt + ((size_t)py * a.t.W + px) * a.D + c_lo + 32 * j);
         g[4 * j] = v.x; g[4 * j + 1] = v.y; g[4 * j + 2] = v.z; g[4 * j + 3] = v.w;
     }
 #pragma unroll
@@ -76,38 +101,67 @@ __global__ void __launch_bounds__(TR_THREADS) ndfd_strip_kernel(const NdfdArgs a
     bool done = !inside;
     const float k2 = a.k_sig * 1.44269504088896340736f;   // exp(k z) = exp2(k2 z)
 
+    // feature rows of the survivors are gathered into shared memory SB at a time with cp.async, double-buffered,
+    // so that the (L2-latency) gather of the next sub-batch overlaps the walk over the current one
+    constexpr int SB = NdSub<CPL, FT>::SB, ROW_BYTES = NdSub<CPL, FT>::ROW_BYTES;
+    extern __shared__ __align__(16) unsigned char rows_raw[];
+    auto stage_rows = [&](int sb, int added) {
+        unsigned char* dst = rows_raw + (sb & 1) * SB * ROW_BYTES;
+        const int nrows = min(SB, added - sb * SB);
+        for (int c = tid; c < nrows * (ROW_BYTES / 16); c += TR_THREADS) {
+            const int r = c / (ROW_BYTES / 16), o = (c % (ROW_BYTES / 16)) * 16;
+            cp_async16(dst + r * ROW_BYTES + o,
+                       reinterpret_cast<const unsigned char*>(feat + (size_t)q.id[sb * SB + r] * a.D) + o);
+        }
+        cp_async_commit();
+    };
     uint32_t pos = range.x;
     while (pos < range.y) {
         const int added = stage_chunk(a.t, q, pos, range.y, 0, bx0, by0, bx1, by1);
         pos += TR_THREADS;
-        for (int kk = 0; kk < added; ++kk) {
-            const float w = eval_weight(q.xy[kk], q.co[kk], fx, fy, a.t, T, done, n);
-            if (!__any_sync(TR_FULL, w != 0.f)) continue;
-            const FT* f = feat + (size_t)q.id[kk] * a.D + c_lo;
-            float phi = 0.f, Ff = 0.f;
-            float fv[CPL];
-#pragma unroll
-            for (int j = 0; j < CPL / 4; ++j) {
-                const float4 v = ld4<FT>(f + 4 * j);
-                fv[4 * j] = v.x; fv[4 * j + 1] = v.y; fv[4 * j + 2] = v.z; fv[4 * j + 3] = v.w;
+        const int nsb = (added + SB - 1) / SB;
+        if (nsb > 0) stage_rows(0, added);
+        for (int sb = 0; sb < nsb; ++sb) {
+            if (sb + 1 < nsb) {
+                stage_rows(sb + 1, added);
+                cp_async_wait_group<1>();
+            } else {
+                cp_async_wait_group<0>();
             }
+            __syncthreads();
+            const FT* rows = reinterpret_cast<const FT*>(rows_raw + (sb & 1) * SB * ROW_BYTES) + c_lo;
+            const int k_end = min(added, (sb + 1) * SB);
+            for (int kk = sb * SB; kk < k_end; ++kk) {
+                const float w = eval_weight(q.xy[kk], q.co[kk], fx, fy, a.t, T, done, n);
+                if (!__any_sync(TR_FULL, w != 0.f)) continue;
+                const FT* f = rows + (kk - sb * SB) * (CPL * 8);
+                float ph[4] = {0.f, 0.f, 0.f, 0.f}, ff[4] = {0.f, 0.f, 0.f, 0.f};   // 4 independent chains each
+                float fv[CPL];
 #pragma unroll
-            for (int j = 0; j < CPL; ++j) {
-                phi = fmaf(fv[j], g[j], phi);
-                Ff = fmaf(fv[j], F[j], Ff);
+                for (int j = 0; j < CPL / 4; ++j) {
+                    const float4 v = lds4<FT>(f + 32 * j);
+                    fv[4 * j] = v.x; fv[4 * j + 1] = v.y; fv[4 * j + 2] = v.z; fv[4 * j + 3] = v.w;
+                }
+#pragma unroll
+                for (int j = 0; j < CPL; ++j) {
+                    ph[j & 3] = fmaf(fv[j], g[j], ph[j & 3]);
+                    ff[j & 3] = fmaf(fv[j], F[j], ff[j & 3]);
+                }
+                float phi = (ph[0] + ph[1]) + (ph[2] + ph[3]), Ff = (ff[0] + ff[1]) + (ff[2] + ff[3]);
+#pragma unroll
+                for (int d = 1; d < 8; d <<= 1) {
+                    phi += __shfl_xor_sync(TR_FULL, phi, d);
+                    Ff += __shfl_xor_sync(TR_FULL, Ff, d);
+                }
+                const float sigma = 1.0f / (1.0f + exp2f(k2 * (phi - a.lambda)));
+                const float sw = sigma * w;        // w == 0 for pixels the Gaussian does not reach: nothing changes
+                lgt += sw;
+                lcf = fmaf(sw, Wc - Ff, lcf);
+                Wc += w;
+#pragma unroll
+                for (int j = 0; j < CPL; ++j) F[j] = fmaf(w, fv[j], F[j]);
             }
-#pragma unroll
-            for (int d = 1; d < 8; d <<= 1) {
-                phi += __shfl_xor_sync(TR_FULL, phi, d);
-                Ff += __shfl_xor_sync(TR_FULL, Ff, d);
-            }
-            const float sigma = 1.0f / (1.0f + exp2f(k2 * (phi - a.lambda)));
-            const float sw = sigma * w;        // w == 0 for pixels the Gaussian does not reach: nothing changes
-            lgt += sw;
-            lcf = fmaf(sw, Wc - Ff, lcf);
-            Wc += w;
-#pragma unroll
-            for (int j = 0; j < CPL; ++j) F[j] = fmaf(w, fv[j], F[j]);
+            __syncthreads();   // the buffer is refilled two sub-batches later; the ring at the next chunk
         }
         if (__syncthreads_and(done)) break;
     }
@@ -120,7 +174,8 @@ __global__ void __launch_bounds__(TR_THREADS) ndfd_strip_kernel(const NdfdArgs a
 
 template <int CPL, typename FT, typename GT>
 cudaError_t launch(const NdfdArgs& a, int tiles, cudaStream_t st) {
-    ndfd_strip_kernel<CPL, FT, GT><<<tiles * ND_STRIPS, TR_THREADS, 0, st>>>(a);
+    const size_t smem = 2 * (size_t)NdSub<CPL, FT>::SB * NdSub<CPL, FT>::ROW_BYTES;
+    ndfd_strip_kernel<CPL, FT, GT><<<tiles * ND_STRIPS, TR_THREADS, smem, st>>>(a);
     return cudaGetLastError();
 }
 
