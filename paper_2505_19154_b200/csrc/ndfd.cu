@@ -6,13 +6,13 @@
 //     L_cf(x) = sum_i sigma_i w_i (W_{i-1} - F_{i-1} . f_i),   W, F accumulated in blend order (DESIGN.md reading)
 //
 // First CUDA path of this row (correctness first; not yet the warp-specialised form of render/fuse):
-// one CTA of 256 threads per 16x2 pixel strip of a tile (grid = tiles x 8).  Eight lanes share one pixel and
-// split the D channels; each lane keeps its slice of the pixel's ground-truth vector f_gt and of the running
-// feature F in registers.  The CTA streams the tile's sorted range 256 instances at a time through the
-// traverse.cuh staging (exact ellipse-vs-strip cull), gathers the survivors' feature rows into shared memory with
-// double-buffered cp.async; every warp then walks the survivors for its 4 pixels:
-// the normative q / cut-off / alpha / T arithmetic of C1-R, and -- only when one of its pixels has a weight --
-// the two D-length dot products (8-lane shuffle reduction) and the update of F.
+// one CTA of 256 threads per 16 x (16/LPP)-row pixel strip of a tile.  LPP lanes (4 for D <= 128, else 8) share one
+// pixel and split the D channels in interleaved float4 groups; each lane keeps its slice of the pixel's
+// ground-truth vector f_gt and of the running feature F in registers.  The CTA streams the tile's sorted range
+// 256 instances at a time through the traverse.cuh staging (exact ellipse-vs-strip cull) and gathers the
+// survivors' feature rows into shared memory with double-buffered cp.async; every warp then walks the survivors
+// for its 32/LPP pixels: the normative q / cut-off / alpha / T arithmetic of C1-R, and -- only when one of its
+// pixels has a weight -- the two D-length dot products (LPP-lane shuffle reduction) and the update of F.
 #include <cuda_fp16.h>
 
 #include "traverse.cuh"
@@ -41,7 +41,7 @@ __device__ __forceinline__ float4 ld4<__half>(const __half* p) {
     return make_float4(a.x, a.y, b.x, b.y);
 }
 
-constexpr int ND_STRIPS = 8;   // 16x2-pixel strips per tile
+// LPP lanes share one pixel (LPP = 4 or 8): a warp covers 32/LPP pixels, the CTA (8 warps) a 16 x (16/LPP) strip
 
 template <typename T>
 __device__ __forceinline__ float4 lds4(const T* p);
@@ -59,39 +59,40 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // survivors whose feature rows are staged together (one of two 16 KB shared-memory buffers)
-template <int CPL, typename FT>
+template <int D, typename FT>
 struct NdSub {
-    static constexpr int ROW_BYTES = CPL * 8 * (int)sizeof(FT);
+    static constexpr int ROW_BYTES = D * (int)sizeof(FT);
     static constexpr int SB = 16384 / ROW_BYTES > 32 ? 32 : (16384 / ROW_BYTES < 4 ? 4 : 16384 / ROW_BYTES);
 };
 
-// CPL = channels per lane = D / 8
-template <int CPL, typename FT, typename GT>
-__global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 1) ndfd_strip_kernel(const NdfdArgs a) {
+// CPL = channels per lane = D / LPP
+template <int LPP, int CPL, typename FT, typename GT>
+__global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1)) ndfd_strip_kernel(const NdfdArgs a) {
     __shared__ TileQueue q;
+    constexpr int PXW = 32 / LPP, ROWS = 8 * PXW / FHGS_TILE, STRIPS = FHGS_TILE / ROWS;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int tile = blockIdx.x / ND_STRIPS, strip = blockIdx.x % ND_STRIPS;
-    const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE + 2 * strip;
+    const int tile = blockIdx.x / STRIPS, strip = blockIdx.x % STRIPS;
+    const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE + ROWS * strip;
     if (ty0 >= a.t.H) return;
-    // pixel of this lane group: warp w covers x = 4 (w & 3) .. +3 of row (w >> 2)
-    const int pxl = lane >> 3, cgl = lane & 7;
-    const int px = tx0 + ((warp & 3) << 2) + pxl, py = ty0 + (warp >> 2);
+    const int pxl = lane / LPP, cgl = lane % LPP;
+    const int pi = warp * PXW + pxl;   // pixel of this lane group inside the strip, row-major
+    const int px = tx0 + (pi & 15), py = ty0 + (pi >> 4);
     const bool inside = px < a.t.W && py < a.t.H;
     const float fx = (float)px, fy = (float)py;
     const float bx0 = (float)tx0, by0 = (float)ty0;
-    const float bx1 = (float)min(tx0 + FHGS_TILE - 1, a.t.W - 1), by1 = (float)min(ty0 + 1, a.t.H - 1);
+    const float bx1 = (float)min(tx0 + FHGS_TILE - 1, a.t.W - 1), by1 = (float)min(ty0 + ROWS - 1, a.t.H - 1);
     const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
     const FT* feat = reinterpret_cast<const FT*>(a.feat);
     const GT* gt = reinterpret_cast<const GT*>(a.gt);
-    // channel slice of this lane: float4 groups cgl, cgl + 8, cgl + 16, ... (interleaved, so that the 8 lanes of a
-    // pixel read 128 contiguous bytes per load: coalesced from global, conflict-free from shared memory)
+    // channel slice of this lane: float4 groups cgl, cgl + LPP, cgl + 2 LPP, ... (interleaved, so that the lanes of a
+    // pixel read contiguous bytes per load: coalesced from global, conflict-free from shared memory)
     const int c_lo = cgl * 4;
 
     float g[CPL], F[CPL];
 #pragma unroll
     for (int j = 0; j < CPL / 4; ++j) {
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (inside) v = ld4<GT>(gt + ((size_t)py * a.t.W + px) * a.D + c_lo + 32 * j);
+        if (inside) v = ld4<GT>(gt + ((size_t)py * a.t.W + px) * a.D + c_lo + 4 * LPP * j);
         g[4 * j] = v.x; g[4 * j + 1] = v.y; g[4 * j + 2] = v.z; g[4 * j + 3] = v.w;
     }
 #pragma unroll
@@ -103,7 +104,7 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 1) ndfd_strip_kern
 
     // feature rows of the survivors are gathered into shared memory SB at a time with cp.async, double-buffered,
     // so that the (L2-latency) gather of the next sub-batch overlaps the walk over the current one
-    constexpr int SB = NdSub<CPL, FT>::SB, ROW_BYTES = NdSub<CPL, FT>::ROW_BYTES;
+    constexpr int SB = NdSub<LPP * CPL, FT>::SB, ROW_BYTES = NdSub<LPP * CPL, FT>::ROW_BYTES;
     extern __shared__ __align__(16) unsigned char rows_raw[];
     auto stage_rows = [&](int sb, int added) {
         unsigned char* dst = rows_raw + (sb & 1) * SB * ROW_BYTES;
@@ -134,12 +135,12 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 1) ndfd_strip_kern
             for (int kk = sb * SB; kk < k_end; ++kk) {
                 const float w = eval_weight(q.xy[kk], q.co[kk], fx, fy, a.t, T, done, n);
                 if (!__any_sync(TR_FULL, w != 0.f)) continue;
-                const FT* f = rows + (kk - sb * SB) * (CPL * 8);
+                const FT* f = rows + (kk - sb * SB) * (CPL * LPP);
                 float ph[4] = {0.f, 0.f, 0.f, 0.f}, ff[4] = {0.f, 0.f, 0.f, 0.f};   // 4 independent chains each
                 float fv[CPL];
 #pragma unroll
                 for (int j = 0; j < CPL / 4; ++j) {
-                    const float4 v = lds4<FT>(f + 32 * j);
+                    const float4 v = lds4<FT>(f + 4 * LPP * j);
                     fv[4 * j] = v.x; fv[4 * j + 1] = v.y; fv[4 * j + 2] = v.z; fv[4 * j + 3] = v.w;
                 }
 #pragma unroll
@@ -149,7 +150,7 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 1) ndfd_strip_kern
                 }
                 float phi = (ph[0] + ph[1]) + (ph[2] + ph[3]), Ff = (ff[0] + ff[1]) + (ff[2] + ff[3]);
 #pragma unroll
-                for (int d = 1; d < 8; d <<= 1) {
+                for (int d = 1; d < LPP; d <<= 1) {
                     phi += __shfl_xor_sync(TR_FULL, phi, d);
                     Ff += __shfl_xor_sync(TR_FULL, Ff, d);
                 }
@@ -172,21 +173,22 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 1) ndfd_strip_kern
     }
 }
 
-template <int CPL, typename FT, typename GT>
+template <int LPP, int CPL, typename FT, typename GT>
 cudaError_t launch(const NdfdArgs& a, int tiles, cudaStream_t st) {
-    const size_t smem = 2 * (size_t)NdSub<CPL, FT>::SB * NdSub<CPL, FT>::ROW_BYTES;
-    ndfd_strip_kernel<CPL, FT, GT><<<tiles * ND_STRIPS, TR_THREADS, smem, st>>>(a);
+    constexpr int STRIPS = FHGS_TILE / (8 * (32 / LPP) / FHGS_TILE);
+    const size_t smem = 2 * (size_t)NdSub<LPP * CPL, FT>::SB * NdSub<LPP * CPL, FT>::ROW_BYTES;
+    ndfd_strip_kernel<LPP, CPL, FT, GT><<<tiles * STRIPS, TR_THREADS, smem, st>>>(a);
     return cudaGetLastError();
 }
 
 template <typename FT, typename GT>
 cudaError_t dispatch(const NdfdArgs& a, int tiles, cudaStream_t st) {
-    switch (a.D / 8) {
-        case 4: return launch<4, FT, GT>(a, tiles, st);
-        case 8: return launch<8, FT, GT>(a, tiles, st);
-        case 16: return launch<16, FT, GT>(a, tiles, st);
-        case 32: return launch<32, FT, GT>(a, tiles, st);
-        case 64: return launch<64, FT, GT>(a, tiles, st);
+    switch (a.D) {
+        case 32: return launch<4, 8, FT, GT>(a, tiles, st);
+        case 64: return launch<4, 16, FT, GT>(a, tiles, st);
+        case 128: return launch<4, 32, FT, GT>(a, tiles, st);
+        case 256: return launch<8, 32, FT, GT>(a, tiles, st);
+        case 512: return launch<8, 64, FT, GT>(a, tiles, st);
         default: return cudaErrorInvalidValue;
     }
 }
