@@ -15,7 +15,7 @@
 // pixels has a weight -- the two D-length dot products (LPP-lane shuffle reduction) and the update of F.
 #include <cuda_fp16.h>
 
-#include "traverse.cuh"
+#include "ws.cuh"   // packed fma.rn.f32x2 helpers (and traverse.cuh)
 
 namespace {
 
@@ -88,15 +88,16 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1
     // pixel read contiguous bytes per load: coalesced from global, conflict-free from shared memory)
     const int c_lo = cgl * 4;
 
-    float g[CPL], F[CPL];
+    // channel pairs packed for fma.rn.f32x2 (two FMAs per issue slot)
+    unsigned long long g[CPL / 2], F[CPL / 2];
 #pragma unroll
     for (int j = 0; j < CPL / 4; ++j) {
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
         if (inside) v = ld4<GT>(gt + ((size_t)py * a.t.W + px) * a.D + c_lo + 4 * LPP * j);
-        g[4 * j] = v.x; g[4 * j + 1] = v.y; g[4 * j + 2] = v.z; g[4 * j + 3] = v.w;
+        g[2 * j] = pack2(v.x, v.y); g[2 * j + 1] = pack2(v.z, v.w);
     }
 #pragma unroll
-    for (int j = 0; j < CPL; ++j) F[j] = 0.f;
+    for (int j = 0; j < CPL / 2; ++j) F[j] = 0ull;
     float T = 1.f, Wc = 0.f, lgt = 0.f, lcf = 0.f;
     uint32_t n = 0;
     bool done = !inside;
@@ -136,19 +137,20 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1
                 const float w = eval_weight(q.xy[kk], q.co[kk], fx, fy, a.t, T, done, n);
                 if (!__any_sync(TR_FULL, w != 0.f)) continue;
                 const FT* f = rows + (kk - sb * SB) * (CPL * LPP);
-                float ph[4] = {0.f, 0.f, 0.f, 0.f}, ff[4] = {0.f, 0.f, 0.f, 0.f};   // 4 independent chains each
-                float fv[CPL];
+                unsigned long long ph[2] = {0ull, 0ull}, ff[2] = {0ull, 0ull};   // 2 packed chains each
+                unsigned long long fv[CPL / 2];
 #pragma unroll
                 for (int j = 0; j < CPL / 4; ++j) {
                     const float4 v = lds4<FT>(f + 4 * LPP * j);
-                    fv[4 * j] = v.x; fv[4 * j + 1] = v.y; fv[4 * j + 2] = v.z; fv[4 * j + 3] = v.w;
+                    fv[2 * j] = pack2(v.x, v.y); fv[2 * j + 1] = pack2(v.z, v.w);
                 }
 #pragma unroll
-                for (int j = 0; j < CPL; ++j) {
-                    ph[j & 3] = fmaf(fv[j], g[j], ph[j & 3]);
-                    ff[j & 3] = fmaf(fv[j], F[j], ff[j & 3]);
+                for (int j = 0; j < CPL / 2; ++j) {
+                    fma2_acc(ph[j & 1], fv[j], g[j]);
+                    fma2_acc(ff[j & 1], fv[j], F[j]);
                 }
-                float phi = (ph[0] + ph[1]) + (ph[2] + ph[3]), Ff = (ff[0] + ff[1]) + (ff[2] + ff[3]);
+                const float2 p0 = unpack2(ph[0]), p1 = unpack2(ph[1]), q0 = unpack2(ff[0]), q1 = unpack2(ff[1]);
+                float phi = (p0.x + p0.y) + (p1.x + p1.y), Ff = (q0.x + q0.y) + (q1.x + q1.y);
 #pragma unroll
                 for (int d = 1; d < LPP; d <<= 1) {
                     phi += __shfl_xor_sync(TR_FULL, phi, d);
@@ -159,8 +161,9 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1
                 lgt += sw;
                 lcf = fmaf(sw, Wc - Ff, lcf);
                 Wc += w;
+                const unsigned long long w2 = pack2(w, w);
 #pragma unroll
-                for (int j = 0; j < CPL; ++j) F[j] = fmaf(w, fv[j], F[j]);
+                for (int j = 0; j < CPL / 2; ++j) fma2_acc(F[j], w2, fv[j]);
             }
             __syncthreads();   // the buffer is refilled two sub-batches later; the ring at the next chunk
         }
