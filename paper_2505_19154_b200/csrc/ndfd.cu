@@ -58,11 +58,11 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// survivors whose feature rows are staged together (one of two 16 KB shared-memory buffers)
+// survivors whose feature rows are staged together (one of two 32 KB shared-memory buffers)
 template <int D, typename FT>
 struct NdSub {
     static constexpr int ROW_BYTES = D * (int)sizeof(FT);
-    static constexpr int SB = 16384 / ROW_BYTES > 32 ? 32 : (16384 / ROW_BYTES < 4 ? 4 : 16384 / ROW_BYTES);
+    static constexpr int SB = 32768 / ROW_BYTES > 64 ? 64 : (32768 / ROW_BYTES < 4 ? 4 : 32768 / ROW_BYTES);
 };
 
 // CPL = channels per lane = D / LPP
@@ -180,6 +180,8 @@ template <int LPP, int CPL, typename FT, typename GT>
 cudaError_t launch(const NdfdArgs& a, int tiles, cudaStream_t st) {
     constexpr int STRIPS = FHGS_TILE / (8 * (32 / LPP) / FHGS_TILE);
     const size_t smem = 2 * (size_t)NdSub<LPP * CPL, FT>::SB * NdSub<LPP * CPL, FT>::ROW_BYTES;
+    cudaError_t e = cudaFuncSetAttribute(ndfd_strip_kernel<LPP, CPL, FT, GT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
     ndfd_strip_kernel<LPP, CPL, FT, GT><<<tiles * STRIPS, TR_THREADS, smem, st>>>(a);
     return cudaGetLastError();
 }
