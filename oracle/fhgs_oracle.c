@@ -643,3 +643,102 @@ void fo_ndfd_pairwise(int n_order, const uint32_t *order, int D, const float *xy
         free(fr);
     }
 }
+
+/* ------------------------------------------------------------------------------------------
+ * NDFD backward at the w level (PAPER.md:142-146 and appendix A.2,
+ * PAPER.md:361-383).  Total loss over the requested pixels
+ *     L = sum_x ( lam1 L_gt(x) + lam2 L_cf(x) ),   L_gt, L_cf as in fo_ndfd_literal, mode 0
+ * and, per pixel, over its fragment list k = 1..N in blend order:
+ *     dL/dw_k     = lam1 sigma_k
+ *                 + lam2 [ sigma_k (W_{k-1} - F_{k-1}.f_k) + sum_{i>k} sigma_i w_i (1 - f_i.f_k) ]
+ *                                                        (PAPER.md:144 / 365-368)
+ *     dL/dalpha_k = T_k dL/dw_k - (1/(1-alpha_k)) sum_{j>k} dL/dw_j w_j      (
+ *                   w_j = alpha_j T_j, T_j = prod_{i<j}(1-alpha_i))
+ *     dL/dop_g   += dL/dalpha_k G_k   where alpha_k = op_g G_k is not clamped by alpha_max
+ * (alpha = min(alpha_max, op G): a clamped fragment passes no gradient to op).  The fragment list is
+ * the realised one (cut-off, stopping rule); its dependence on the parameters is not
+ * differentiated, exactly as in any alpha-blending rasteriser.  The geometry chain
+ * (dG/d mean, scale, rotation) is out of scope.
+ * Everything in double.  out_grad_op[n] is ACCUMULATED into (caller zeroes it); returns L.
+ * ------------------------------------------------------------------------------------------ */
+double fo_ndfd_backward(int n_order, const uint32_t *order, int D, const float *xy,
+                        const float *conic_opacity, const float *feat, const float *gt, int W, int H,
+                        const float *prm, double k_sig, double lambda, double lam1, double lam2,
+                        int64_t npix, const int32_t *pix, double *out_grad_op) {
+    const float q_cut = prm[P_QCUT], alpha_max = prm[P_AMAX];
+    const double t_min = (double)prm[P_TMIN];
+    double L_total = 0.0;
+    if (!pix) npix = (int64_t)W * H;
+#pragma omp parallel reduction(+ : L_total)
+    {
+        int cap = 0;
+        uint32_t *gid = NULL;
+        double *al = NULL, *Gv = NULL, *Tk = NULL, *wk = NULL, *sg = NULL, *gw = NULL;
+        double *F = (double *)malloc((size_t)D * sizeof(double));
+        double *B = (double *)malloc((size_t)D * sizeof(double));
+#pragma omp for schedule(dynamic, 16)
+        for (int64_t p = 0; p < npix; ++p) {
+            const int id = pix ? pix[p] : (int)p;
+            const int x = id % W, y = id / W;
+            const float *fgt = gt + (size_t)id * D;
+            /* forward: realised fragment list with alpha, G, T, w, sigma */
+            int cnt = 0;
+            double T = 1.0;
+            for (int k = 0; k < n_order; ++k) {
+                if (T < t_min) break;
+                const uint32_t g = order[k];
+                const float q = fo_q(xy[2 * g], xy[2 * g + 1], conic_opacity[4 * g], conic_opacity[4 * g + 1], conic_opacity[4 * g + 2], x, y);
+                if (!(q <= q_cut)) continue;
+                const double G = exp(-0.5 * fmax((double)q, 0.0));
+                const double a_raw = (double)conic_opacity[4 * g + 3] * G;
+                const double a = fmin((double)alpha_max, a_raw);
+                if (cnt == cap) {
+                    cap = cap ? 2 * cap : 256;
+                    gid = (uint32_t *)realloc(gid, (size_t)cap * sizeof(uint32_t));
+                    al = (double *)realloc(al, (size_t)cap * sizeof(double)); Gv = (double *)realloc(Gv, (size_t)cap * sizeof(double));
+                    Tk = (double *)realloc(Tk, (size_t)cap * sizeof(double)); wk = (double *)realloc(wk, (size_t)cap * sizeof(double));
+                    sg = (double *)realloc(sg, (size_t)cap * sizeof(double)); gw = (double *)realloc(gw, (size_t)cap * sizeof(double));
+                }
+                gid[cnt] = g; al[cnt] = a; Gv[cnt] = (a_raw < (double)alpha_max) ? G : 0.0;   /* clamped: no gradient to op */
+                Tk[cnt] = T; wk[cnt] = a * T;
+                sg[cnt] = 1.0 / (1.0 + exp(k_sig * (dotf(feat + (size_t)g * D, fgt, D) - lambda)));
+                T = T * (1.0 - a);
+                ++cnt;
+            }
+            /* loss (mode 0 recurrence) and the prefix part of dL/dw_k */
+            double Wc = 0.0, lgt = 0.0, lcf = 0.0;
+            for (int c = 0; c < D; ++c) F[c] = 0.0;
+            for (int s = 0; s < cnt; ++s) {
+                const float *f = feat + (size_t)gid[s] * D;
+                double Ff = 0.0;
+                for (int c = 0; c < D; ++c) Ff += F[c] * (double)f[c];
+                lgt += wk[s] * sg[s];
+                lcf += sg[s] * wk[s] * (Wc - Ff);
+                gw[s] = lam1 * sg[s] + lam2 * sg[s] * (Wc - Ff);
+                Wc += wk[s];
+                for (int c = 0; c < D; ++c) F[c] += wk[s] * (double)f[c];
+            }
+            L_total += lam1 * lgt + lam2 * lcf;
+            /* suffix part: sum_{i>k} sigma_i w_i (1 - f_i.f_k) = A_k - B_k.f_k, then dL/dalpha */
+            double A = 0.0, Csuf = 0.0;
+            for (int c = 0; c < D; ++c) B[c] = 0.0;
+            for (int s = cnt - 1; s >= 0; --s) {
+                const float *f = feat + (size_t)gid[s] * D;
+                double Bf = 0.0;
+                for (int c = 0; c < D; ++c) Bf += B[c] * (double)f[c];
+                gw[s] += lam2 * (A - Bf);
+                const double dalpha = Tk[s] * gw[s] - Csuf / (1.0 - al[s]);
+                const double contrib = dalpha * Gv[s];
+                if (contrib != 0.0) {
+#pragma omp atomic
+                    out_grad_op[gid[s]] += contrib;
+                }
+                Csuf += gw[s] * wk[s];
+                A += sg[s] * wk[s];
+                for (int c = 0; c < D; ++c) B[c] += sg[s] * wk[s] * (double)f[c];
+            }
+        }
+        free(F); free(B); free(gid); free(al); free(Gv); free(Tk); free(wk); free(sg); free(gw);
+    }
+    return L_total;
+}

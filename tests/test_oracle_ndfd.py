@@ -111,3 +111,90 @@ def test_bounds_and_monotonicity():
     assert np.all(lgt >= 0) and np.all(lgt <= 1.0 - r["T"] + 1e-12) and np.all(lcf >= -1e-9)
     lgt2, _ = fo.ndfd(pr, order, feat, gt, cfg.width, cfg.height, lam=0.7)
     assert np.all(lgt2 >= lgt - 1e-15) and (lgt2 - lgt).max() > 1e-3
+
+
+# ---- NEXT-2: backward at the w level -------------------------------------------------------------
+def _one_pixel_backward(ws, feats, f_gt, lam1, lam2, k=20.0, lam=0.5):
+    ws = np.asarray(ws, np.float64)
+    T, ops = 1.0, []
+    for w in ws:
+        ops.append(w / T)
+        T *= 1.0 - w / T
+    n = len(ws)
+    pr = manual_pr(np.zeros((n, 2)), [1.0, 0.0, 1.0], ops, [0, 0, 0], 3)
+    prm = fo.DEFAULT_PARAMS.copy()
+    prm[4] = 1.0 + 1e-3   # alpha_max above 1: nothing is clamped in the hand examples
+    prm[5] = 0.0
+    gt = np.asarray(f_gt, np.float32).reshape(1, 1, -1)
+    return fo.ndfd_backward(pr, np.arange(n, dtype=np.uint32), np.asarray(feats, np.float32), gt, 1, 1, k=k, lam=lam,
+                            lam1=lam1, lam2=lam2, params=prm), np.asarray(ops)
+
+
+def test_backward_hand_values():
+    """SPEC.md:343 dL_gt/dw = sigma; SPEC.md:354 the two-orthogonal-fragment example: dL_cf/dw_1 = sigma_2 w_2 = 0.5,
+    dL_cf/dw_2 = sigma_2 (W_1 - F_1.f_2) = 0.5; SPEC.md:363 dL/dalpha_near = dL/dw_near - dL/dw_far w_far / (1 - alpha_near).
+    The Gaussians sit on the pixel (G = 1), so dL/dop = dL/dalpha."""
+    # single fragment, L_gt only: dL/dop = T_1 sigma = sigma
+    (L, g), _ = _one_pixel_backward([0.6], [[1.0, 0.0]], [0.5, math.sqrt(0.75)], 1.0, 0.0)
+    assert abs(L - 0.3) < 1e-7 and abs(g[0] - 0.5) < 1e-7
+    # two orthogonal fragments, L_cf only, w = (0.5, 0.25): alpha = (0.5, 0.5), T = (1, 0.5), sigma_2 ~ 1
+    (L, g), ops = _one_pixel_backward([0.5, 0.25], [[1.0, 0.0], [0.0, 1.0]], [0.0, -1.0], 0.0, 1.0)
+    assert abs(L - 0.125) < 1e-7                         # sigma_2 w_2 (W_1 - F_1.f_2) = 0.25 * 0.5
+    gw1, gw2 = 0.25, 0.5                                 # sigma_2 w_2 (1 - 0);  sigma_2 (W_1 - 0)   (SPEC.md:354 pattern)
+    da2 = 0.5 * gw2                                      # far fragment: T_2 dL/dw_2
+    da1 = 1.0 * gw1 - gw2 * 0.25 / (1.0 - 0.5)           # near fragment: SPEC.md:363
+    np.testing.assert_allclose(g, [da1, da2], atol=1e-7)
+    assert abs(g[0]) < 1e-7      # L_cf = a1 (1 - a1) a2: d/da1 vanishes at a1 = 1/2; d/da2 = a1 (1 - a1) = 1/4
+
+
+def test_backward_loss_matches_forward_and_finite_differences():
+    """L equals the forward oracle's sum; dL/d opacity matches central finite differences of the FORWARD oracle
+     on the Tiny scene (t_min = 0 so that the fragment lists do not change)."""
+    cfg, sc, cam, pr = tiny_state(3)
+    order = fo.global_order(pr)
+    rng = np.random.default_rng(21)
+    feat = rng.standard_normal((sc.n, 12)).astype(np.float32)
+    feat /= np.linalg.norm(feat, axis=1, keepdims=True)
+    gt = rng.standard_normal((cfg.height, cfg.width, 12)).astype(np.float32)
+    gt /= np.linalg.norm(gt, axis=2, keepdims=True)
+    prm = fo.DEFAULT_PARAMS.copy()
+    prm[5] = 0.0
+    lam1, lam2 = 0.7, 1.3
+    L, grad = fo.ndfd_backward(pr, order, feat, gt, cfg.width, cfg.height, lam1=lam1, lam2=lam2, params=prm)
+
+    def forward_total(p):
+        lgt, lcf = fo.ndfd(p, order, feat, gt, cfg.width, cfg.height, params=prm)
+        return lam1 * lgt.sum() + lam2 * lcf.sum()
+
+    assert abs(L - forward_total(pr)) <= 1e-9 * abs(L)
+    probe = np.argsort(-np.abs(grad))[[0, 1, 2, 5, 10, 50, 200]]
+    assert np.abs(grad[probe]).min() > 0
+    for g in probe:
+        o0 = pr["conic_opacity"][g, 3]
+        hi, lo = np.float32(o0 * (1 + 2e-3)), np.float32(o0 * (1 - 2e-3))
+        p_hi = dict(pr, conic_opacity=pr["conic_opacity"].copy()); p_hi["conic_opacity"][g, 3] = hi
+        p_lo = dict(pr, conic_opacity=pr["conic_opacity"].copy()); p_lo["conic_opacity"][g, 3] = lo
+        fd = (forward_total(p_hi) - forward_total(p_lo)) / (float(hi) - float(lo))
+        assert abs(fd - grad[g]) <= 2e-4 * max(abs(grad[g]), 1e-3), (g, fd, grad[g])
+
+
+def test_backward_linearity_and_clamp():
+    """dL/dop is linear in (lam1, lam2); a fragment clamped at alpha_max passes no gradient to its opacity."""
+    cfg, sc, cam, pr = tiny_state(0)
+    order = fo.global_order(pr)
+    rng = np.random.default_rng(22)
+    feat = rng.standard_normal((sc.n, 8)).astype(np.float32)
+    feat /= np.linalg.norm(feat, axis=1, keepdims=True)
+    gt = rng.standard_normal((cfg.height, cfg.width, 8)).astype(np.float32)
+    gt /= np.linalg.norm(gt, axis=2, keepdims=True)
+    _, g10 = fo.ndfd_backward(pr, order, feat, gt, cfg.width, cfg.height, lam1=1.0, lam2=0.0)
+    _, g01 = fo.ndfd_backward(pr, order, feat, gt, cfg.width, cfg.height, lam1=0.0, lam2=1.0)
+    _, g23 = fo.ndfd_backward(pr, order, feat, gt, cfg.width, cfg.height, lam1=2.0, lam2=3.0)
+    np.testing.assert_allclose(g23, 2.0 * g10 + 3.0 * g01, rtol=1e-10, atol=1e-12)
+    # one opaque Gaussian on a pixel centre: op * G = 1 > alpha_max -> clamped there; only off-centre pixels pass gradient
+    prm = fo.DEFAULT_PARAMS.copy()
+    p1 = manual_pr([[0.0, 0.0]], [1.0, 0.0, 1.0], [1.0], [0, 0, 0], 3)
+    gt1 = np.zeros((1, 1, 2), np.float32); gt1[..., 0] = 1.0
+    _, gc = fo.ndfd_backward(p1, np.array([0], np.uint32), np.array([[0.0, 1.0]], np.float32), gt1, 1, 1, lam1=1.0, lam2=0.0,
+                             params=prm)
+    assert gc[0] == 0.0
