@@ -215,6 +215,23 @@ FHGS_API fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g, c
                               int32_t gt_dtype, float k_sigmoid, float lambda, float* out_lgt,
                               float* out_lcf, void* stream);
 
+/* NDFD backward at the w level -- PAPER.md:142-146 and appendix A.2.
+ * With L = sum_x ( lam1 out_lgt[x] + lam2 out_lcf[x] ) of fhgs_ndfd_forward, per pixel and fragment k in blend order
+ *     dL/dw_k     = lam1 sigma_k + lam2 [ sigma_k (W_{k-1} - F_{k-1}.f_k) + sum_{i>k} sigma_i w_i (1 - f_i.f_k) ]
+ *     dL/dalpha_k = T_k dL/dw_k - (1/(1 - alpha_k)) sum_{j>k} dL/dw_j w_j
+ * and the result is the opacity gradient  grad_opacity[g] += sum_x dL/dalpha_k(x) G_k(x)  over the fragments k of
+ * Gaussian g that are not clamped at alpha_max (alpha = min(alpha_max, op G)).  The realised fragment lists
+ * (cut-off, stopping rule) are not differentiated; the geometry chain (dG/d mean, scale, rotation) is out of scope.
+ * grad_opacity [n] f32 is ACCUMULATED into (the caller zeroes it; atomic order is free).
+ * work: device scratch of fhgs_ndfd_backward_work_bytes(width, height, D) bytes, 256-byte aligned (per-pixel
+ * totals of the three forward traversals the first path uses).  D in {32,64,128,256}; other arguments as
+ * fhgs_ndfd_forward. */
+FHGS_API size_t fhgs_ndfd_backward_work_bytes(int32_t width, int32_t height, int32_t feat_dim);
+FHGS_API fhgs_status fhgs_ndfd_backward(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam,
+                               const fhgs_params* prm, const fhgs_view_state* vs, const void* gt,
+                               int32_t gt_dtype, float k_sigmoid, float lambda, float lam1, float lam2,
+                               float* grad_opacity, void* work, size_t work_bytes, void* stream);
+
 /* One whole frame (P -> S -> R -> F with ZERO|FINALIZE) from HOST buffers: copies the Gaussian
  * arrays and the GT map host->device into `dev_g` / `dev_gt` (device staging owned by the
  * caller, same shapes), runs the four steps on `stream`, copies out_rgb / out_feat /

@@ -20,7 +20,7 @@ FHGS_SORT_FULL_KEY = 1
 FHGS_FUSE_ZERO, FHGS_FUSE_FINALIZE, FHGS_FUSE_L2NORM, FHGS_FUSE_FINALIZE_ONLY, FHGS_FUSE_ZERO_ONLY = 1, 2, 4, 8, 16
 
 EXPORTS = ["fhgs_create", "fhgs_destroy", "fhgs_last_error", "fhgs_version", "fhgs_default_params",
-           "fhgs_scratch_bytes", "fhgs_scratch_tile_visited", "fhgs_project", "fhgs_bin_sort", "fhgs_render", "fhgs_fuse_features", "fhgs_ndfd_forward",
+           "fhgs_scratch_bytes", "fhgs_scratch_tile_visited", "fhgs_project", "fhgs_bin_sort", "fhgs_render", "fhgs_fuse_features", "fhgs_ndfd_forward", "fhgs_ndfd_backward_work_bytes", "fhgs_ndfd_backward",
            "fhgs_frame_host", "fhgs_ffma_peak"]
 
 
@@ -99,6 +99,10 @@ def _load():
                                     C.POINTER(C.c_uint64), vp]
     lib.fhgs_ndfd_forward.argtypes = [vp, C.POINTER(CGaussians), C.POINTER(CCamera), C.POINTER(CParams), C.POINTER(CViewState),
                                       vp, C.c_int32, C.c_float, C.c_float, vp, vp, vp]
+    lib.fhgs_ndfd_backward_work_bytes.restype = C.c_size_t
+    lib.fhgs_ndfd_backward_work_bytes.argtypes = [C.c_int32, C.c_int32, C.c_int32]
+    lib.fhgs_ndfd_backward.argtypes = [vp, C.POINTER(CGaussians), C.POINTER(CCamera), C.POINTER(CParams), C.POINTER(CViewState),
+                                       vp, C.c_int32, C.c_float, C.c_float, C.c_float, C.c_float, vp, vp, C.c_size_t, vp]
     lib.fhgs_ffma_peak.argtypes = [vp, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
     return lib
 
@@ -312,6 +316,20 @@ def ndfd_forward(ctx: Context, g: Gaussians, cam: CCamera, prm: CParams, vs: Vie
     ctx.check(lib.fhgs_ndfd_forward(ctx.handle, C.byref(g.c), C.byref(cam), C.byref(prm), C.byref(vs.c), _ptr(gt),
                                     _dtype_code(gt), C.c_float(k), C.c_float(lam), _ptr(out_lgt), _ptr(out_lcf),
                                     _stream(stream)))
+
+
+def ndfd_backward(ctx: Context, g: Gaussians, cam: CCamera, prm: CParams, vs: ViewState, gt, grad_opacity,
+                  k: float = 20.0, lam: float = 0.5, lam1: float = 1.0, lam2: float = 1.0, work=None, stream=None):
+    """fhgs_ndfd_backward: accumulates dL/d opacity into grad_opacity [n] f32.  `work`: optional uint8 scratch tensor
+    (allocated here when None); returned for reuse."""
+    nbytes = int(lib.fhgs_ndfd_backward_work_bytes(vs.width, vs.height, g.c.feat_dim))
+    if work is None or work.numel() < nbytes + 256:
+        work = torch.empty((nbytes + 256,), dtype=torch.uint8, device=grad_opacity.device)
+    wp = (work.data_ptr() + 255) // 256 * 256
+    ctx.check(lib.fhgs_ndfd_backward(ctx.handle, C.byref(g.c), C.byref(cam), C.byref(prm), C.byref(vs.c), _ptr(gt),
+                                     _dtype_code(gt), C.c_float(k), C.c_float(lam), C.c_float(lam1), C.c_float(lam2),
+                                     _ptr(grad_opacity), C.c_void_p(wp), C.c_size_t(nbytes), _stream(stream)))
+    return work
 
 
 def frame_host(ctx: Context, host: dict, g: Gaussians, cam: CCamera, prm: CParams, vs: ViewState, ws: dict,

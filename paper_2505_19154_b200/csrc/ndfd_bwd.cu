@@ -1,0 +1,245 @@
+// ndfd_bwd.cu -- NDFD backward at the w level (fhgs_ndfd_backward): dL/d opacity of
+//     L = sum_x ( lam1 L_gt(x) + lam2 L_cf(x) )            (losses of fhgs_ndfd_forward, Eq. 5-6)
+// per pixel, over its fragments k = 1..N in blend order (appendix A.2):
+//     g_k         = dL/dw_k = lam1 sigma_k + lam2 [ sigma_k (W_{k-1} - F_{k-1}.f_k) + A_k - B_k.f_k ]
+//                   with the suffix sums A_k = sum_{i>k} sigma_i w_i,  B_k = sum_{i>k} sigma_i w_i f_i
+//     dL/dalpha_k = T_k g_k - C_k / (1 - alpha_k),   C_k = sum_{j>k} g_j w_j
+//     dL/dop_g   += dL/dalpha_k G_k    (0 where alpha is clamped at alpha_max)
+//
+// First CUDA path of this row: three FORWARD traversals with the strip kernel of ndfd.cu (no reverse walk, no
+// division-recovered transmittance): pass 1 stores the per-pixel totals A_0 (scalar) and B_0 (D-vector), pass 2
+// turns them into running suffixes, evaluates g_k and stores C_0 = sum g_j w_j, pass 3 repeats that with the
+// running suffix of C and adds dL/dalpha_k G_k into grad_opacity: reduced over the pixels of the warp first, then
+// one atomic per (warp, Gaussian).
+#include <cuda_fp16.h>
+
+#include "traverse.cuh"
+
+namespace {
+
+struct BwdArgs {
+    TraverseArgs t;
+    const void* feat;
+    const void* gt;
+    int D;
+    float k_sig, lambda, lam1, lam2;
+    float* A_tot;    // [H*W]
+    float* C_tot;    // [H*W]
+    float* B_tot;    // [H*W, D]
+    float* grad_op;  // [n]
+};
+
+template <typename T>
+__device__ __forceinline__ float4 ldg4(const T* p);
+template <>
+__device__ __forceinline__ float4 ldg4<float>(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
+template <>
+__device__ __forceinline__ float4 ldg4<__half>(const __half* p) {
+    const uint2 r = __ldg(reinterpret_cast<const uint2*>(p));
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
+    const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
+    return make_float4(a.x, a.y, b.x, b.y);
+}
+
+// C1-R steps 1-3 for one (pixel, Gaussian) with everything the chain rule needs.  Returns false when the Gaussian
+// does not contribute.  G_eff = G where alpha = op G is not clamped, else 0.
+__device__ __forceinline__ bool fragment(float2 g, float4 co, float fx, float fy, const TraverseArgs& a, float& T, bool& done,
+                                         float& alpha, float& T_before, float& G_eff) {
+    const float dx = __fsub_rn(g.x, fx), dy = __fsub_rn(g.y, fy);
+    const float q = __fmaf_rn(dx, __fmaf_rn(co.y, dy, __fmul_rn(co.x, dx)), __fmul_rn(__fmul_rn(co.z, dy), dy));
+    if (done || !(q <= a.q_cutoff)) return false;
+    const float G = exp2f(-0.72134752044448170368f * fmaxf(q, 0.f));
+    const float a_raw = co.w * G;
+    alpha = fminf(a.alpha_max, a_raw);
+    G_eff = a_raw < a.alpha_max ? G : 0.f;
+    T_before = T;
+    T = fmaf(-alpha, T, T);
+    if (T < a.t_min) done = true;
+    return true;
+}
+
+// MODE 1: totals A_0, B_0.  MODE 2: C_0.  MODE 3: gradient.
+template <int MODE, int LPP, int CPL, typename FT, typename GT>
+__global__ void __launch_bounds__(TR_THREADS) ndfd_bwd_kernel(const BwdArgs a) {
+    __shared__ TileQueue q;
+    constexpr int PXW = 32 / LPP, ROWS = 8 * PXW / FHGS_TILE, STRIPS = FHGS_TILE / ROWS;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int tile = blockIdx.x / STRIPS, strip = blockIdx.x % STRIPS;
+    const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE + ROWS * strip;
+    if (ty0 >= a.t.H) return;
+    const int pxl = lane / LPP, cgl = lane % LPP;
+    const int pi = warp * PXW + pxl;
+    const int px = tx0 + (pi & 15), py = ty0 + (pi >> 4);
+    const bool inside = px < a.t.W && py < a.t.H;
+    const float fx = (float)px, fy = (float)py;
+    const float bx0 = (float)tx0, by0 = (float)ty0;
+    const float bx1 = (float)min(tx0 + FHGS_TILE - 1, a.t.W - 1), by1 = (float)min(ty0 + ROWS - 1, a.t.H - 1);
+    const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
+    const FT* feat = reinterpret_cast<const FT*>(a.feat);
+    const GT* gt = reinterpret_cast<const GT*>(a.gt);
+    const int c_lo = cgl * 4;   // interleaved float4 groups cgl, cgl + LPP, ...
+    const size_t pix = (size_t)py * a.t.W + px;
+
+    float g[CPL], F[CPL], Bs[CPL];   // f_gt slice; prefix sum w f; MODE 1: running sum sigma w f, else suffix B_k
+#pragma unroll
+    for (int j = 0; j < CPL / 4; ++j) {
+        float4 v = make_float4(0.f, 0.f, 0.f, 0.f), b = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (inside) {
+            v = ldg4<GT>(gt + pix * a.D + c_lo + 4 * LPP * j);
+            if (MODE != 1) b = *reinterpret_cast<const float4*>(a.B_tot + pix * a.D + c_lo + 4 * LPP * j);
+        }
+        g[4 * j] = v.x; g[4 * j + 1] = v.y; g[4 * j + 2] = v.z; g[4 * j + 3] = v.w;
+        Bs[4 * j] = b.x; Bs[4 * j + 1] = b.y; Bs[4 * j + 2] = b.z; Bs[4 * j + 3] = b.w;
+        F[4 * j] = F[4 * j + 1] = F[4 * j + 2] = F[4 * j + 3] = 0.f;
+    }
+    float T = 1.f, Wc = 0.f;
+    float As = (MODE != 1 && inside) ? a.A_tot[pix] : 0.f;      // MODE 1: running sum; else suffix A_k
+    float Cs = (MODE == 3 && inside) ? a.C_tot[pix] : 0.f;      // MODE 2: running sum; MODE 3: suffix C_k
+    bool done = !inside;
+    const float k2 = a.k_sig * 1.44269504088896340736f;
+
+    uint32_t pos = range.x;
+    while (pos < range.y) {
+        const int added = stage_chunk(a.t, q, pos, range.y, 0, bx0, by0, bx1, by1);
+        pos += TR_THREADS;
+        for (int kk = 0; kk < added; ++kk) {
+            float alpha = 0.f, Tb = 0.f, Ge = 0.f;
+            const bool hit = fragment(q.xy[kk], q.co[kk], fx, fy, a.t, T, done, alpha, Tb, Ge);
+            if (!__any_sync(TR_FULL, hit)) continue;
+            const float w = hit ? alpha * Tb : 0.f;
+            const uint32_t id = q.id[kk];
+            const FT* f = feat + (size_t)id * a.D + c_lo;
+            float fv[CPL];
+#pragma unroll
+            for (int j = 0; j < CPL / 4; ++j) {
+                const float4 v = ldg4<FT>(f + 4 * LPP * j);
+                fv[4 * j] = v.x; fv[4 * j + 1] = v.y; fv[4 * j + 2] = v.z; fv[4 * j + 3] = v.w;
+            }
+            float phi = 0.f;
+#pragma unroll
+            for (int j = 0; j < CPL; ++j) phi = fmaf(fv[j], g[j], phi);
+#pragma unroll
+            for (int d = 1; d < LPP; d <<= 1) phi += __shfl_xor_sync(TR_FULL, phi, d);
+            const float sigma = 1.0f / (1.0f + exp2f(k2 * (phi - a.lambda)));
+            const float sw = sigma * w;
+            if (MODE == 1) {
+                As += sw;
+#pragma unroll
+                for (int j = 0; j < CPL; ++j) Bs[j] = fmaf(sw, fv[j], Bs[j]);
+                continue;
+            }
+            // suffixes exclude k
+            As -= sw;
+            float Ff = 0.f, Bf = 0.f;
+#pragma unroll
+            for (int j = 0; j < CPL; ++j) {
+                Bs[j] = fmaf(-sw, fv[j], Bs[j]);
+                Ff = fmaf(fv[j], F[j], Ff);
+                Bf = fmaf(fv[j], Bs[j], Bf);
+            }
+#pragma unroll
+            for (int d = 1; d < LPP; d <<= 1) {
+                Ff += __shfl_xor_sync(TR_FULL, Ff, d);
+                Bf += __shfl_xor_sync(TR_FULL, Bf, d);
+            }
+            const float gk = a.lam1 * sigma + a.lam2 * (sigma * (Wc - Ff) + (As - Bf));
+            Wc += w;
+#pragma unroll
+            for (int j = 0; j < CPL; ++j) F[j] = fmaf(w, fv[j], F[j]);
+            if (MODE == 2) {
+                Cs = fmaf(gk, w, Cs);
+            } else {
+                Cs = fmaf(-gk, w, Cs);   // suffix excludes k
+                float contrib = hit ? (Tb * gk - Cs / (1.0f - alpha)) * Ge : 0.f;
+                if (cgl != 0) contrib = 0.f;   // every lane of the pixel group holds the same value
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) contrib += __shfl_xor_sync(TR_FULL, contrib, d);
+                if (lane == 0 && contrib != 0.f) atomicAdd(a.grad_op + id, contrib);
+            }
+        }
+        if (__syncthreads_and(done)) break;
+    }
+    if (inside) {
+        if (MODE == 1) {
+            if (cgl == 0) a.A_tot[pix] = As;
+#pragma unroll
+            for (int j = 0; j < CPL / 4; ++j)
+                *reinterpret_cast<float4*>(a.B_tot + pix * a.D + c_lo + 4 * LPP * j) =
+                    make_float4(Bs[4 * j], Bs[4 * j + 1], Bs[4 * j + 2], Bs[4 * j + 3]);
+        } else if (MODE == 2) {
+            if (cgl == 0) a.C_tot[pix] = Cs;
+        }
+    }
+}
+
+template <int LPP, int CPL, typename FT, typename GT>
+cudaError_t launch3(const BwdArgs& a, int tiles, cudaStream_t st) {
+    constexpr int STRIPS = FHGS_TILE / (8 * (32 / LPP) / FHGS_TILE);
+    ndfd_bwd_kernel<1, LPP, CPL, FT, GT><<<tiles * STRIPS, TR_THREADS, 0, st>>>(a);
+    ndfd_bwd_kernel<2, LPP, CPL, FT, GT><<<tiles * STRIPS, TR_THREADS, 0, st>>>(a);
+    ndfd_bwd_kernel<3, LPP, CPL, FT, GT><<<tiles * STRIPS, TR_THREADS, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
+template <typename FT, typename GT>
+cudaError_t dispatch(const BwdArgs& a, int tiles, cudaStream_t st) {
+    switch (a.D) {
+        case 32: return launch3<4, 8, FT, GT>(a, tiles, st);
+        case 64: return launch3<4, 16, FT, GT>(a, tiles, st);
+        case 128: return launch3<8, 16, FT, GT>(a, tiles, st);
+        case 256: return launch3<8, 32, FT, GT>(a, tiles, st);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace
+
+extern "C" size_t fhgs_ndfd_backward_work_bytes(int32_t width, int32_t height, int32_t feat_dim) {
+    if (width <= 0 || height <= 0 || feat_dim <= 0) return 0;
+    const size_t px = (size_t)width * height;
+    return (px * 2 + px * (size_t)feat_dim) * sizeof(float) + 512;
+}
+
+extern "C" fhgs_status fhgs_ndfd_backward(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam,
+                                          const fhgs_params* prm, const fhgs_view_state* vs, const void* gt,
+                                          int32_t gt_dtype, float k_sigmoid, float lambda, float lam1, float lam2,
+                                          float* grad_opacity, void* work, size_t work_bytes, void* stream) {
+    if (!ctx) return FHGS_ERR_INVALID;
+    if (!g || !cam || !prm || !vs || !gt || !grad_opacity || !work) FHGS_INVALID(ctx, "fhgs_ndfd_backward: NULL argument");
+    fhgs_status st;
+    if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
+    if ((st = validate_params(ctx, prm)) != FHGS_OK) return st;
+    if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
+    if (!g->feat) FHGS_INVALID(ctx, "fhgs_ndfd_backward: g->feat is NULL");
+    if ((g->feat_dtype != FHGS_F32 && g->feat_dtype != FHGS_F16) || (gt_dtype != FHGS_F32 && gt_dtype != FHGS_F16))
+        FHGS_INVALID(ctx, "fhgs_ndfd_backward: unknown dtype");
+    const int D = g->feat_dim;
+    if (!(D == 32 || D == 64 || D == 128 || D == 256)) FHGS_INVALID(ctx, "fhgs_ndfd_backward: feat_dim must be 32, 64, 128 or 256");
+    if (!aligned_to(g->feat, 16) || !aligned_to(gt, 16) || !aligned_to(work, 256))
+        FHGS_INVALID(ctx, "fhgs_ndfd_backward: feat/gt must be 16-byte, work 256-byte aligned");
+    if (work_bytes < fhgs_ndfd_backward_work_bytes(cam->width, cam->height, D)) FHGS_INVALID(ctx, "fhgs_ndfd_backward: work too small");
+    if (g->n != vs->n) FHGS_INVALID(ctx, "fhgs_ndfd_backward: g->n != vs->n");
+    if (!finite_f(k_sigmoid) || !finite_f(lambda) || !finite_f(lam1) || !finite_f(lam2)) FHGS_INVALID(ctx, "fhgs_ndfd_backward: non-finite scalar");
+    BwdArgs a;
+    a.t.W = cam->width; a.t.H = cam->height; a.t.GW = tiles_x(cam->width);
+    a.t.ranges = vs->ranges; a.t.vals = vs->vals[vs->sorted_buf & 1];
+    a.t.xy = reinterpret_cast<const float2*>(vs->xy);
+    a.t.conic_opacity = reinterpret_cast<const float4*>(vs->conic_opacity);
+    a.t.q_cutoff = prm->q_cutoff; a.t.alpha_max = prm->alpha_max; a.t.t_min = prm->t_min;
+    a.feat = g->feat; a.gt = gt; a.D = D; a.k_sig = k_sigmoid; a.lambda = lambda; a.lam1 = lam1; a.lam2 = lam2;
+    const size_t px = (size_t)cam->width * cam->height;
+    a.A_tot = reinterpret_cast<float*>(work);
+    a.C_tot = a.A_tot + px;
+    a.B_tot = reinterpret_cast<float*>((char*)work + ((px * 2 * sizeof(float) + 255) / 256) * 256);
+    a.grad_op = grad_opacity;
+    const int tiles = tiles_x(cam->width) * tiles_y(cam->height);
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e;
+    const bool fh = g->feat_dtype == FHGS_F16, gh = gt_dtype == FHGS_F16;
+    if (fh && gh) e = dispatch<__half, __half>(a, tiles, s);
+    else if (fh) e = dispatch<__half, float>(a, tiles, s);
+    else if (gh) e = dispatch<float, __half>(a, tiles, s);
+    else e = dispatch<float, float>(a, tiles, s);
+    FHGS_CUDA(ctx, e);
+    return FHGS_OK;
+}

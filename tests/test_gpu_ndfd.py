@@ -100,3 +100,50 @@ def test_ndfd_invalid_arguments():
     with pytest.raises(fb.FhgsError) as ei:
         fb.ndfd_forward(gp.ctx, gp.g, c, gp.prm, gp.vs, gt, out, out.clone())
     assert ei.value.status == fb.FHGS_ERR_INVALID
+
+
+# ---- NEXT-2: backward at the w level --------------------------------------------------------------
+def _run_backward(cfg, view, lam1, lam2, k=20.0, lam=0.5):
+    import torch
+    from paper_2505_19154_b200 import binding as fb
+    scene = inputs.make_scene(cfg)
+    cam = inputs.make_camera(cfg, view)
+    gt = inputs.make_gt_map(cfg, view, cam)
+    pr = pu.oracle_view(scene, cam)
+    m = fo.bins(pr, cfg.width, cfg.height)["M"]
+    gp = pu.GpuPath(scene, cfg.width, cfg.height, m + 64)
+    c, _ = gp.project_sort(cam)
+    dev = gp.g.mean.device
+    grad = torch.zeros((scene.n,), dtype=torch.float32, device=dev)
+    gt_d = torch.from_numpy(np.ascontiguousarray(gt)).to(dev)
+    work = fb.ndfd_backward(gp.ctx, gp.g, c, gp.prm, gp.vs, gt_d, grad, k=k, lam=lam, lam1=lam1, lam2=lam2)
+    fb.ndfd_backward(gp.ctx, gp.g, c, gp.prm, gp.vs, gt_d, grad, k=k, lam=lam, lam1=lam1, lam2=lam2, work=work)   # accumulates
+    torch.cuda.synchronize()
+    g_gpu = 0.5 * grad.cpu().numpy().astype(np.float64)
+    order = fo.global_order(pr)
+    L, g_or = fo.ndfd_backward(pr, order, scene.feat.astype(np.float32), gt.astype(np.float32), cfg.width, cfg.height,
+                               k=k, lam=lam, lam1=lam1, lam2=lam2)
+    # bar: every per-(pixel, fragment) term is O(1) and is summed over the Gaussian's footprint in fp32; the error is
+    # bounded relative to the sum of |terms|, for which max|grad| over the scene is a (loose) stand-in on dense scenes
+    scale = np.abs(g_or).max()
+    err = np.abs(g_gpu - g_or)
+    culled = pr["radius"] == 0
+    assert np.all(g_gpu[culled] == 0.0)
+    assert err.max() <= 2e-4 * scale, (err.max(), scale, int(np.argmax(err)))
+    big = np.abs(g_or) > 0.05 * scale
+    assert big.sum() > 50 and np.all(err[big] <= 2e-3 * np.abs(g_or[big]))
+    return dict(err=float(err.max()), scale=float(scale), L=L, big=int(big.sum()))
+
+
+def test_ndfd_backward_d128_and_d64():
+    cfg = pu.reduced_config("mid", n=40_000, width=200, height=120, log_scale_mu=-3.3)
+    print(_run_backward(cfg, 0, 1.0, 1.0))
+    cfg = pu.reduced_config("mid", n=15_000, width=160, height=96, log_scale_mu=-3.0, feat_dim=64)
+    print(_run_backward(cfg, 0, 0.3, 2.0, k=8.0, lam=0.3))
+
+
+def test_ndfd_backward_blobs_d256_and_fp16_d32():
+    cfg = pu.reduced_config("multiview", n=30_000, width=216, height=168, n_views=200, log_scale_mu=-3.0)
+    print(_run_backward(cfg, 67, 1.0, 0.5))
+    cfg = pu.reduced_config("large", n=15_000, width=160, height=96, log_scale_mu=-3.0, feat_dim=32)
+    print(_run_backward(cfg, 0, 1.0, 1.0))
