@@ -345,6 +345,14 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
         nops = 7 * n_eval_total + (3 * D + 12) * n_contrib_total
         ndfd = {"ms": nms, "frac_of_nominal_fp32": nops / (nms * 1e-3) / alu_nominal,
                 "mean_lgt": float(lgt.mean().item()), "mean_lcf": float(lcf.mean().item())}
+        gop = torch.zeros((n,), dtype=f32, device=dev)
+        work = fb.ndfd_backward(ctx, g, cam, prm, vs, gt, gop)
+        ev[0].record(stream)
+        for _ in range(3):
+            fb.ndfd_backward(ctx, g, cam, prm, vs, gt, gop, work=work)
+        ev[1].record(stream)
+        torch.cuda.synchronize()
+        ndfd["backward_ms"] = ev[0].elapsed_time(ev[1]) / 3
 
     # ---- end to end through fhgs_frame_host: host (pinned) buffers, copies inside the timed region
     e2e = None
