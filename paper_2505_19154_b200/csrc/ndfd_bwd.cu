@@ -6,7 +6,8 @@
 //     dL/dalpha_k = T_k g_k - C_k / (1 - alpha_k),   C_k = sum_{j>k} g_j w_j
 //     dL/dop_g   += dL/dalpha_k G_k    (0 where alpha is clamped at alpha_max)
 //
-// First CUDA path of this row: three FORWARD traversals with the strip kernel of ndfd.cu (no reverse walk, no
+// First CUDA path of this row: three FORWARD traversals with the strip kernel of ndfd.cu (feature rows staged in
+// shared memory with double-buffered cp.async, 4 or 8 lanes per pixel; no reverse walk, no
 // division-recovered transmittance): pass 1 stores the per-pixel totals A_0 (scalar) and B_0 (D-vector), pass 2
 // turns them into running suffixes, evaluates g_k and stores C_0 = sum g_j w_j, pass 3 repeats that with the
 // running suffix of C and adds dL/dalpha_k G_k into grad_opacity: reduced over the pixels of the warp first, then
@@ -41,6 +42,28 @@ __device__ __forceinline__ float4 ldg4<__half>(const __half* p) {
     return make_float4(a.x, a.y, b.x, b.y);
 }
 
+template <typename T>
+__device__ __forceinline__ float4 lds4(const T* p);
+template <>
+__device__ __forceinline__ float4 lds4<float>(const float* p) { return *reinterpret_cast<const float4*>(p); }
+template <>
+__device__ __forceinline__ float4 lds4<__half>(const __half* p) {
+    const uint2 r = *reinterpret_cast<const uint2*>(p);
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
+    const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
+    return make_float4(a.x, a.y, b.x, b.y);
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// survivors whose feature rows are staged together (one of two 32 KB shared-memory buffers), as in ndfd.cu
+template <int D, typename FT>
+struct BwdSub {
+    static constexpr int ROW_BYTES = D * (int)sizeof(FT);
+    static constexpr int SB = 32768 / ROW_BYTES > 64 ? 64 : (32768 / ROW_BYTES < 4 ? 4 : 32768 / ROW_BYTES);
+};
+
 // C1-R steps 1-3 for one (pixel, Gaussian) with everything the chain rule needs.  Returns false when the Gaussian
 // does not contribute.  G_eff = G where alpha = op G is not clamped, else 0.
 __device__ __forceinline__ bool fragment(float2 g, float4 co, float fx, float fy, const TraverseArgs& a, float& T, bool& done,
@@ -60,7 +83,7 @@ __device__ __forceinline__ bool fragment(float2 g, float4 co, float fx, float fy
 
 // MODE 1: totals A_0, B_0.  MODE 2: C_0.  MODE 3: gradient.
 template <int MODE, int LPP, int CPL, typename FT, typename GT>
-__global__ void __launch_bounds__(TR_THREADS) ndfd_bwd_kernel(const BwdArgs a) {
+__global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel(const BwdArgs a) {
     __shared__ TileQueue q;
     constexpr int PXW = 32 / LPP, ROWS = 8 * PXW / FHGS_TILE, STRIPS = FHGS_TILE / ROWS;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -98,64 +121,92 @@ __global__ void __launch_bounds__(TR_THREADS) ndfd_bwd_kernel(const BwdArgs a) {
     bool done = !inside;
     const float k2 = a.k_sig * 1.44269504088896340736f;
 
+    constexpr int SB = BwdSub<LPP * CPL, FT>::SB, ROW_BYTES = BwdSub<LPP * CPL, FT>::ROW_BYTES;
+    extern __shared__ __align__(16) unsigned char rows_raw[];
+    auto stage_rows = [&](int sb, int added) {
+        unsigned char* dst = rows_raw + (sb & 1) * SB * ROW_BYTES;
+        const int nrows = min(SB, added - sb * SB);
+        for (int c = tid; c < nrows * (ROW_BYTES / 16); c += TR_THREADS) {
+            const int r = c / (ROW_BYTES / 16), o = (c % (ROW_BYTES / 16)) * 16;
+            cp_async16(dst + r * ROW_BYTES + o,
+                       reinterpret_cast<const unsigned char*>(feat + (size_t)q.id[sb * SB + r] * a.D) + o);
+        }
+        cp_async_commit();
+    };
     uint32_t pos = range.x;
     while (pos < range.y) {
         const int added = stage_chunk(a.t, q, pos, range.y, 0, bx0, by0, bx1, by1);
         pos += TR_THREADS;
-        for (int kk = 0; kk < added; ++kk) {
-            float alpha = 0.f, Tb = 0.f, Ge = 0.f;
-            const bool hit = fragment(q.xy[kk], q.co[kk], fx, fy, a.t, T, done, alpha, Tb, Ge);
-            if (!__any_sync(TR_FULL, hit)) continue;
-            const float w = hit ? alpha * Tb : 0.f;
-            const uint32_t id = q.id[kk];
-            const FT* f = feat + (size_t)id * a.D + c_lo;
-            float fv[CPL];
-#pragma unroll
-            for (int j = 0; j < CPL / 4; ++j) {
-                const float4 v = ldg4<FT>(f + 4 * LPP * j);
-                fv[4 * j] = v.x; fv[4 * j + 1] = v.y; fv[4 * j + 2] = v.z; fv[4 * j + 3] = v.w;
-            }
-            float phi = 0.f;
-#pragma unroll
-            for (int j = 0; j < CPL; ++j) phi = fmaf(fv[j], g[j], phi);
-#pragma unroll
-            for (int d = 1; d < LPP; d <<= 1) phi += __shfl_xor_sync(TR_FULL, phi, d);
-            const float sigma = 1.0f / (1.0f + exp2f(k2 * (phi - a.lambda)));
-            const float sw = sigma * w;
-            if (MODE == 1) {
-                As += sw;
-#pragma unroll
-                for (int j = 0; j < CPL; ++j) Bs[j] = fmaf(sw, fv[j], Bs[j]);
-                continue;
-            }
-            // suffixes exclude k
-            As -= sw;
-            float Ff = 0.f, Bf = 0.f;
-#pragma unroll
-            for (int j = 0; j < CPL; ++j) {
-                Bs[j] = fmaf(-sw, fv[j], Bs[j]);
-                Ff = fmaf(fv[j], F[j], Ff);
-                Bf = fmaf(fv[j], Bs[j], Bf);
-            }
-#pragma unroll
-            for (int d = 1; d < LPP; d <<= 1) {
-                Ff += __shfl_xor_sync(TR_FULL, Ff, d);
-                Bf += __shfl_xor_sync(TR_FULL, Bf, d);
-            }
-            const float gk = a.lam1 * sigma + a.lam2 * (sigma * (Wc - Ff) + (As - Bf));
-            Wc += w;
-#pragma unroll
-            for (int j = 0; j < CPL; ++j) F[j] = fmaf(w, fv[j], F[j]);
-            if (MODE == 2) {
-                Cs = fmaf(gk, w, Cs);
+        const int nsb = (added + SB - 1) / SB;
+        if (nsb > 0) stage_rows(0, added);
+        for (int sb = 0; sb < nsb; ++sb) {
+            if (sb + 1 < nsb) {
+                stage_rows(sb + 1, added);
+                cp_async_wait_group<1>();
             } else {
-                Cs = fmaf(-gk, w, Cs);   // suffix excludes k
-                float contrib = hit ? (Tb * gk - Cs / (1.0f - alpha)) * Ge : 0.f;
-                if (cgl != 0) contrib = 0.f;   // every lane of the pixel group holds the same value
-#pragma unroll
-                for (int d = 1; d < 32; d <<= 1) contrib += __shfl_xor_sync(TR_FULL, contrib, d);
-                if (lane == 0 && contrib != 0.f) atomicAdd(a.grad_op + id, contrib);
+                cp_async_wait_group<0>();
             }
+            __syncthreads();
+            const FT* rows = reinterpret_cast<const FT*>(rows_raw + (sb & 1) * SB * ROW_BYTES) + c_lo;
+            const int k_end = min(added, (sb + 1) * SB);
+            for (int kk = sb * SB; kk < k_end; ++kk) {
+                float alpha = 0.f, Tb = 0.f, Ge = 0.f;
+                const bool hit = fragment(q.xy[kk], q.co[kk], fx, fy, a.t, T, done, alpha, Tb, Ge);
+                if (!__any_sync(TR_FULL, hit)) continue;
+                const float w = hit ? alpha * Tb : 0.f;
+                const uint32_t id = q.id[kk];
+                const FT* f = rows + (kk - sb * SB) * (CPL * LPP);
+                float fv[CPL];
+#pragma unroll
+                for (int j = 0; j < CPL / 4; ++j) {
+                    const float4 v = lds4<FT>(f + 4 * LPP * j);
+                    fv[4 * j] = v.x; fv[4 * j + 1] = v.y; fv[4 * j + 2] = v.z; fv[4 * j + 3] = v.w;
+                }
+                float ph[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                for (int j = 0; j < CPL; ++j) ph[j & 3] = fmaf(fv[j], g[j], ph[j & 3]);
+                float phi = (ph[0] + ph[1]) + (ph[2] + ph[3]);
+#pragma unroll
+                for (int d = 1; d < LPP; d <<= 1) phi += __shfl_xor_sync(TR_FULL, phi, d);
+                const float sigma = 1.0f / (1.0f + exp2f(k2 * (phi - a.lambda)));
+                const float sw = sigma * w;
+                if (MODE == 1) {
+                    As += sw;
+#pragma unroll
+                    for (int j = 0; j < CPL; ++j) Bs[j] = fmaf(sw, fv[j], Bs[j]);
+                    continue;
+                }
+                // suffixes exclude k
+                As -= sw;
+                float fa[4] = {0.f, 0.f, 0.f, 0.f}, ba[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+                for (int j = 0; j < CPL; ++j) {
+                    Bs[j] = fmaf(-sw, fv[j], Bs[j]);
+                    fa[j & 3] = fmaf(fv[j], F[j], fa[j & 3]);
+                    ba[j & 3] = fmaf(fv[j], Bs[j], ba[j & 3]);
+                }
+                float Ff = (fa[0] + fa[1]) + (fa[2] + fa[3]), Bf = (ba[0] + ba[1]) + (ba[2] + ba[3]);
+#pragma unroll
+                for (int d = 1; d < LPP; d <<= 1) {
+                    Ff += __shfl_xor_sync(TR_FULL, Ff, d);
+                    Bf += __shfl_xor_sync(TR_FULL, Bf, d);
+                }
+                const float gk = a.lam1 * sigma + a.lam2 * (sigma * (Wc - Ff) + (As - Bf));
+                Wc += w;
+#pragma unroll
+                for (int j = 0; j < CPL; ++j) F[j] = fmaf(w, fv[j], F[j]);
+                if (MODE == 2) {
+                    Cs = fmaf(gk, w, Cs);
+                } else {
+                    Cs = fmaf(-gk, w, Cs);   // suffix excludes k
+                    float contrib = hit ? (Tb * gk - Cs / (1.0f - alpha)) * Ge : 0.f;
+                    if (cgl != 0) contrib = 0.f;   // every lane of the pixel group holds the same value
+#pragma unroll
+                    for (int d = 1; d < 32; d <<= 1) contrib += __shfl_xor_sync(TR_FULL, contrib, d);
+                    if (lane == 0 && contrib != 0.f) atomicAdd(a.grad_op + id, contrib);
+                }
+            }
+            __syncthreads();
         }
         if (__syncthreads_and(done)) break;
     }
@@ -172,13 +223,22 @@ __global__ void __launch_bounds__(TR_THREADS) ndfd_bwd_kernel(const BwdArgs a) {
     }
 }
 
+template <int MODE, int LPP, int CPL, typename FT, typename GT>
+cudaError_t launch1(const BwdArgs& a, int tiles, cudaStream_t st) {
+    constexpr int STRIPS = FHGS_TILE / (8 * (32 / LPP) / FHGS_TILE);
+    const size_t smem = 2 * (size_t)BwdSub<LPP * CPL, FT>::SB * BwdSub<LPP * CPL, FT>::ROW_BYTES;
+    cudaError_t e = cudaFuncSetAttribute(ndfd_bwd_kernel<MODE, LPP, CPL, FT, GT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    ndfd_bwd_kernel<MODE, LPP, CPL, FT, GT><<<tiles * STRIPS, TR_THREADS, smem, st>>>(a);
+    return cudaGetLastError();
+}
+
 template <int LPP, int CPL, typename FT, typename GT>
 cudaError_t launch3(const BwdArgs& a, int tiles, cudaStream_t st) {
-    constexpr int STRIPS = FHGS_TILE / (8 * (32 / LPP) / FHGS_TILE);
-    ndfd_bwd_kernel<1, LPP, CPL, FT, GT><<<tiles * STRIPS, TR_THREADS, 0, st>>>(a);
-    ndfd_bwd_kernel<2, LPP, CPL, FT, GT><<<tiles * STRIPS, TR_THREADS, 0, st>>>(a);
-    ndfd_bwd_kernel<3, LPP, CPL, FT, GT><<<tiles * STRIPS, TR_THREADS, 0, st>>>(a);
-    return cudaGetLastError();
+    cudaError_t e;
+    if ((e = launch1<1, LPP, CPL, FT, GT>(a, tiles, st)) != cudaSuccess) return e;
+    if ((e = launch1<2, LPP, CPL, FT, GT>(a, tiles, st)) != cudaSuccess) return e;
+    return launch1<3, LPP, CPL, FT, GT>(a, tiles, st);
 }
 
 template <typename FT, typename GT>
@@ -186,7 +246,7 @@ cudaError_t dispatch(const BwdArgs& a, int tiles, cudaStream_t st) {
     switch (a.D) {
         case 32: return launch3<4, 8, FT, GT>(a, tiles, st);
         case 64: return launch3<4, 16, FT, GT>(a, tiles, st);
-        case 128: return launch3<8, 16, FT, GT>(a, tiles, st);
+        case 128: return launch3<4, 32, FT, GT>(a, tiles, st);
         case 256: return launch3<8, 32, FT, GT>(a, tiles, st);
         default: return cudaErrorInvalidValue;
     }
