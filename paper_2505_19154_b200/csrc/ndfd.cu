@@ -99,7 +99,6 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1
 #pragma unroll
     for (int j = 0; j < CPL / 2; ++j) F[j] = 0ull;
     float T = 1.f, Wc = 0.f, lgt = 0.f, lcf = 0.f;
-    uint32_t n = 0;
     bool done = !inside;
     const float k2 = a.k_sig * 1.44269504088896340736f;   // exp(k z) = exp2(k2 z)
 
@@ -133,8 +132,29 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1
             __syncthreads();
             const FT* rows = reinterpret_cast<const FT*>(rows_raw + (sb & 1) * SB * ROW_BYTES) + c_lo;
             const int k_end = min(added, (sb + 1) * SB);
-            for (int kk = sb * SB; kk < k_end; ++kk) {
-                const float w = eval_weight(q.xy[kk], q.co[kk], fx, fy, a.t, T, done, n);
+            // The T-independent part of the weight (normative q, cut-off, alpha = min(alpha_max, op G)) is evaluated for
+            // LPP consecutive survivors at once, one per lane of the pixel group, and handed round by shuffles; only
+            // w = alpha T, the T update and the stop test run per fragment.
+            for (int k0 = sb * SB; k0 < k_end; k0 += LPP) {
+              float a_c = 0.f;
+              if (k0 + cgl < k_end) {
+                  const float2 gxy = q.xy[k0 + cgl];
+                  const float4 co = q.co[k0 + cgl];
+                  const float dx = __fsub_rn(gxy.x, fx), dy = __fsub_rn(gxy.y, fy);
+                  const float qv = __fmaf_rn(dx, __fmaf_rn(co.y, dy, __fmul_rn(co.x, dx)), __fmul_rn(__fmul_rn(co.z, dy), dy));
+                  if (qv <= a.t.q_cutoff) a_c = fminf(a.t.alpha_max, co.w * exp2f(-0.72134752044448170368f * fmaxf(qv, 0.f)));
+              }
+#pragma unroll
+              for (int jj = 0; jj < LPP; ++jj) {
+                const int kk = k0 + jj;
+                if (kk >= k_end) break;
+                const float aj = __shfl_sync(TR_FULL, a_c, (lane & ~(LPP - 1)) + jj);
+                float w = 0.f;
+                if (!done && aj > 0.f) {
+                    w = aj * T;
+                    T = fmaf(-aj, T, T);
+                    if (T < a.t.t_min) done = true;
+                }
                 if (!__any_sync(TR_FULL, w != 0.f)) continue;
                 const FT* f = rows + (kk - sb * SB) * (CPL * LPP);
                 unsigned long long ph[2] = {0ull, 0ull}, ff[2] = {0ull, 0ull};   // 2 packed chains each
@@ -164,6 +184,7 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1
                 const unsigned long long w2 = pack2(w, w);
 #pragma unroll
                 for (int j = 0; j < CPL / 2; ++j) fma2_acc(F[j], w2, fv[j]);
+              }
             }
             __syncthreads();   // the buffer is refilled two sub-batches later; the ring at the next chunk
         }
