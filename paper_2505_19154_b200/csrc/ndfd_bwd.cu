@@ -64,23 +64,6 @@ struct BwdSub {
     static constexpr int SB = 32768 / ROW_BYTES > 64 ? 64 : (32768 / ROW_BYTES < 4 ? 4 : 32768 / ROW_BYTES);
 };
 
-// C1-R steps 1-3 for one (pixel, Gaussian) with everything the chain rule needs.  Returns false when the Gaussian
-// does not contribute.  G_eff = G where alpha = op G is not clamped, else 0.
-__device__ __forceinline__ bool fragment(float2 g, float4 co, float fx, float fy, const TraverseArgs& a, float& T, bool& done,
-                                         float& alpha, float& T_before, float& G_eff) {
-    const float dx = __fsub_rn(g.x, fx), dy = __fsub_rn(g.y, fy);
-    const float q = __fmaf_rn(dx, __fmaf_rn(co.y, dy, __fmul_rn(co.x, dx)), __fmul_rn(__fmul_rn(co.z, dy), dy));
-    if (done || !(q <= a.q_cutoff)) return false;
-    const float G = exp2f(-0.72134752044448170368f * fmaxf(q, 0.f));
-    const float a_raw = co.w * G;
-    alpha = fminf(a.alpha_max, a_raw);
-    G_eff = a_raw < a.alpha_max ? G : 0.f;
-    T_before = T;
-    T = fmaf(-alpha, T, T);
-    if (T < a.t_min) done = true;
-    return true;
-}
-
 // MODE 1: totals A_0, B_0.  MODE 2: C_0.  MODE 3: gradient.
 template <int MODE, int LPP, int CPL, typename FT, typename GT>
 __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel(const BwdArgs a) {
@@ -149,9 +132,34 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
             __syncthreads();
             const FT* rows = reinterpret_cast<const FT*>(rows_raw + (sb & 1) * SB * ROW_BYTES) + c_lo;
             const int k_end = min(added, (sb + 1) * SB);
-            for (int kk = sb * SB; kk < k_end; ++kk) {
-                float alpha = 0.f, Tb = 0.f, Ge = 0.f;
-                const bool hit = fragment(q.xy[kk], q.co[kk], fx, fy, a.t, T, done, alpha, Tb, Ge);
+            // alpha and G_eff (T-independent) are evaluated for LPP consecutive survivors at once, one per lane of the
+            // pixel group, and handed round by shuffles (as in ndfd.cu)
+            for (int k0 = sb * SB; k0 < k_end; k0 += LPP) {
+              float a_c = 0.f, g_c = 0.f;
+              if (k0 + cgl < k_end) {
+                  const float2 gxy = q.xy[k0 + cgl];
+                  const float4 co = q.co[k0 + cgl];
+                  const float dx = __fsub_rn(gxy.x, fx), dy = __fsub_rn(gxy.y, fy);
+                  const float qv = __fmaf_rn(dx, __fmaf_rn(co.y, dy, __fmul_rn(co.x, dx)), __fmul_rn(__fmul_rn(co.z, dy), dy));
+                  if (qv <= a.t.q_cutoff) {
+                      const float G = exp2f(-0.72134752044448170368f * fmaxf(qv, 0.f));
+                      const float a_raw = co.w * G;
+                      a_c = fminf(a.t.alpha_max, a_raw);
+                      g_c = a_raw < a.t.alpha_max ? G : 0.f;
+                  }
+              }
+#pragma unroll
+              for (int jj = 0; jj < LPP; ++jj) {
+                const int kk = k0 + jj;
+                if (kk >= k_end) break;
+                const float alpha = __shfl_sync(TR_FULL, a_c, (lane & ~(LPP - 1)) + jj);
+                const float Ge = __shfl_sync(TR_FULL, g_c, (lane & ~(LPP - 1)) + jj);
+                const bool hit = !done && alpha > 0.f;
+                const float Tb = T;
+                if (hit) {
+                    T = fmaf(-alpha, T, T);
+                    if (T < a.t.t_min) done = true;
+                }
                 if (!__any_sync(TR_FULL, hit)) continue;
                 const float w = hit ? alpha * Tb : 0.f;
                 const uint32_t id = q.id[kk];
@@ -205,6 +213,7 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
                     for (int d = 1; d < 32; d <<= 1) contrib += __shfl_xor_sync(TR_FULL, contrib, d);
                     if (lane == 0 && contrib != 0.f) atomicAdd(a.grad_op + id, contrib);
                 }
+              }
             }
             __syncthreads();
         }
