@@ -206,12 +206,13 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT>& sm, con
                     fv[2 * j] = f.x;
                     fv[2 * j + 1] = f.y;
                 }
+                unsigned long long w2[8];
 #pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    const unsigned long long w2 = pack2(wv[i], wv[i]);
+                for (int i = 0; i < 8; ++i) w2[i] = pack2(wv[i], wv[i]);
 #pragma unroll
-                    for (int j = 0; j < NJ * 2; ++j) fma2_acc(acc[i][j], w2, fv[j]);
-                }
+                for (int j = 0; j < NJ * 2; ++j)
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) fma2_acc(acc[i][j], w2[i], fv[j]);
             }
             mbar_arrive(&sm.ct.empty[stage]);
             if (++stage == R_STAGES) { stage = 0; phase ^= 1u; }
