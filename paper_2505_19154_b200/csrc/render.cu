@@ -66,6 +66,11 @@ template <> struct FeatIO<__half> {
 // TILED variant (DC in {64,128}): warp-specialised persistent pipeline (ws.cuh)
 // ---------------------------------------------------------------------------------------------
 constexpr int R_STAGES = 3;
+// Which warps are the consumers.  The SMSP arbiter favours high warp ids: with fp32 rows the consumers are the
+// critical path and get the high ids (-6 % on Mid); with fp16 rows (conversion work in the consumer loop, four
+// channel passes per tile) the producers are the ones that must not starve (measured on Large).
+template <typename FT>
+constexpr bool kConsHigh = sizeof(FT) == 4;
 
 template <int DC, typename FT>
 struct RenderWsSmem {
@@ -77,7 +82,7 @@ struct RenderWsSmem {
 
 template <int DC, typename FT>
 __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, const RenderArgs& a, const WsWork& wk) {
-    const int p = threadIdx.x, lane = p & 31, pw = p >> 5;   // p = pixel slot, pw = warp-block (producers: warps 0-7)
+    const int p = threadIdx.x - (kConsHigh<FT> ? 0 : WS_CONS), lane = p & 31, pw = p >> 5;   // p = pixel slot, pw = warp-block
     const FT* feat = reinterpret_cast<const FT*>(a.feat);
     const float q_cutoff = a.t.q_cutoff, alpha_max = a.t.alpha_max, t_min = a.t.t_min;
     int stage = 0;
@@ -109,7 +114,6 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
         ws_chunk_issue(a.t, a.rgb_g, ch);
         ws_chunk_prefetch_id(a.t, pos + WS_PROD, range.y, p, ch);
         bool last = false;
-        uint32_t last_used = 0u;
         do {
             while (qt - qh < WS_KB && pos < range.y) {
                 qt += ws_chunk_append(sm.ct, ch, pos, qt, bx0, by0, bx1, by1, q_cutoff, p,
@@ -149,12 +153,17 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
             last = all_done || (pos >= range.y && qt == qh);
             if (p == 0) sm.ct.meta[stage] = WsMeta{nb, tile, c0, last ? WS_FLAG_LAST : 0};
             mbar_arrive(&sm.ct.full[stage]);
-            if (p == 32 && c0 == 0) {   // diagnostics, off the critical path: list position of the last blended instance
-                uint32_t any = 0u;
+            if (last && c0 == 0 && p == 32) {
+                // diagnostics, once per tile and off the critical path: if the tile stopped early, the last blended
+                // instance lies in this final batch (the pixel that completed the tile blended it)
+                uint32_t visited = range.y - range.x;
+                if (all_done) {
+                    uint32_t any = 0u;
 #pragma unroll
-                for (int w8 = 0; w8 < 8; ++w8) any |= sm.ct.mask[stage][w8];
-                if (any) last_used = __float_as_uint(sm.ct.rec1[(qh - nb + 31 - __clz(any)) & (WS_QCAP - 1)].w) + 1u - range.x;
-                if (last) a.tile_visited[tile] = all_done ? last_used : range.y - range.x;
+                    for (int w8 = 0; w8 < 8; ++w8) any |= sm.ct.mask[stage][w8];
+                    visited = any ? __float_as_uint(sm.ct.rec1[(qh - nb + 31 - __clz(any)) & (WS_QCAP - 1)].w) + 1u - range.x : 0u;
+                }
+                a.tile_visited[tile] = visited;
             }
             if (++stage == R_STAGES) { stage = 0; phase ^= 1u; }
         } while (!last);
@@ -174,7 +183,7 @@ template <int DC, typename FT>
 __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT>& sm, const RenderArgs& a) {
     constexpr int NJ = DC / 32;   // float4 channel groups per thread
     // consumers are the HIGH warps (8-15): the SMSP arbiter favours high warp ids, and the consumers are the critical path
-    const int tid = threadIdx.x - WS_PROD, lane = tid & 31, warp = tid >> 5;
+    const int tid = threadIdx.x - (kConsHigh<FT> ? WS_PROD : 0), lane = tid & 31, warp = tid >> 5;
     const int pgl = lane >> 3, cg = lane & 7;
     const int pg = warp * 4 + pgl;   // 8-pixel row run: slots pg*8 .. pg*8+7
     FT* out_feat = reinterpret_cast<FT*>(a.out_feat);
@@ -251,13 +260,14 @@ __global__ void __launch_bounds__(WS_THREADS, 1) render_ws_kernel(const RenderAr
         asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     }
     __syncthreads();
-    if (threadIdx.x < WS_PROD) {
+    const bool is_producer = kConsHigh<FT> ? threadIdx.x < WS_PROD : threadIdx.x >= WS_CONS;
+    if (is_producer) {
         setmaxnreg_dec<72>();
         render_ws_producer<DC, FT>(sm, a, wk);
     } else {
         setmaxnreg_inc<184>();
         render_ws_consumer<DC, FT>(sm, a);
-        if (threadIdx.x == WS_PROD) ws_queue_release(wk);
+        if (threadIdx.x == (kConsHigh<FT> ? WS_PROD : 0)) ws_queue_release(wk);
     }
 }
 
