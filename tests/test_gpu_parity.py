@@ -142,6 +142,23 @@ def test_multiview_full_size_two_views():
     print(w)
 
 
+def test_randomized_shapes_sweep():
+    """16 seeded random cases: scene family, N, odd image sizes (ragged tiles in both directions, images narrower than
+    a tile row), D over every kernel variant (4..512, fp32/fp16), splat size, camera; full P/S/R/F parity each."""
+    rng = np.random.default_rng(20251104)
+    for it in range(16):
+        base = str(rng.choice(["tiny", "mid", "multiview", "large"]))
+        d = int(rng.choice([4, 8, 16, 24, 64, 128, 192, 256] if base != "large" else [64, 128, 256, 512]))
+        kw = dict(n=int(rng.integers(200, 25000)), width=int(rng.integers(17, 400)), height=int(rng.integers(17, 300)),
+                  feat_dim=d, log_scale_mu=float(rng.uniform(-4.0, -2.0)), seed=int(rng.integers(1, 10 ** 6)))
+        if base == "multiview":
+            kw["n_views"] = 200
+        cfg = pu.reduced_config(base, **kw)
+        view = int(rng.integers(0, cfg.n_views))
+        w = run_case(cfg, [view], pu.TOL_F16 if base == "large" else pu.TOL_F32, sort_flags=(0, 1) if it % 4 == 0 else (0,))
+        print(it, base, kw, view, w)
+
+
 def test_large_tile_grid_fallback_sort():
     """2064x1616 px -> (GW+1)*(GH+1) = 130*102 > 12288: fhgs_bin_sort leaves the shared-memory tile-count
     path and derives histograms / ranges from the instance list; both schedules, integers bit-exact."""
