@@ -318,7 +318,7 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     dominant = max(("render", "fuse_accumulate", "bin_sort", "project", "fuse_finalize"), key=lambda k: parts[k])
     roofline = dict(steps_roof[dominant])
     roofline["kernel"] = {"render": "render_ws_kernel<128,float>", "fuse_accumulate": "fuse_ws_kernel<float>",
-                          "bin_sort": "fhgs_bin_sort (14 launches)", "project": "project_kernel<3>",
+                          "bin_sort": "fhgs_bin_sort (13 launches)", "project": "project_kernel<3>",
                           "fuse_finalize": "finalize_kernel<float>"}[dominant]
     roofline["peak_source"] = ("148 SMs x 128 FP32 lanes x sm_max_mhz (MEASURED_PEAKS.json), FMA = 2 flop"
                                if roofline["bound"] == "alu" else f"hbm_gbs of MEASURED_PEAKS.json ({peaks['source']})")
