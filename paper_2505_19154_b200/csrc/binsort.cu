@@ -506,6 +506,7 @@ __global__ void __launch_bounds__(TS_THREADS) tile_scan_kernel(const int* diff, 
 // ------------------------------------------------------------------------------------------------
 constexpr int OS_THREADS = 256;
 constexpr int OS_WARPS = OS_THREADS / 32;
+constexpr int OS_LOOKBACK = 8;    // predecessors fetched per look-back round trip
 constexpr uint32_t OS_AGG = 1u << 30, OS_INC = 2u << 30, OS_VAL = (1u << 30) - 1;
 
 template <typename KeyT>
@@ -609,15 +610,30 @@ __global__ void __launch_bounds__(OS_THREADS, ITEMS >= 16 ? 3 : 5) onesweep_kern
         s_keys[rank[i]] = key[i];
     }
     // look back over the earlier CTAs (digit `tid`)
+    // (OS_LOOKBACK predecessors are fetched per round trip: the walk back to the nearest inclusive prefix is a chain of
+    // dependent L2 loads, and with ~450 CTAs in flight it is tens of entries long)
     uint32_t excl = 0;
     if (ticket != 0) {
         const uint32_t* p = my - 256;
+        int remaining = (int)ticket;   // predecessors not consumed yet; p points at the nearest of them
         while (true) {
-            const uint32_t v = ld_volatile_u32(p);
-            if ((v >> 30) == 0) continue;
-            excl += v & OS_VAL;
-            if ((v >> 30) == 2) break;
-            p -= 256;
+            uint32_t v[OS_LOOKBACK];
+#pragma unroll
+            for (int j = 0; j < OS_LOOKBACK; ++j) v[j] = j < remaining ? ld_volatile_u32(p - 256 * j) : OS_INC;
+            int used = 0;
+            bool fin = false;
+#pragma unroll
+            for (int j = 0; j < OS_LOOKBACK; ++j) {
+                const uint32_t f = v[j] >> 30;
+                if (!fin && used == j && f != 0) {   // consume in order; stop at the first entry that is not published yet
+                    excl += v[j] & OS_VAL;
+                    used = j + 1;
+                    fin = f == 2;
+                }
+            }
+            if (fin) break;
+            p -= 256 * used;
+            remaining -= used;
         }
         st_volatile_u32(my, OS_INC | (excl + cnt));
     }
