@@ -131,13 +131,24 @@ __global__ void __launch_bounds__(SCAN_THREADS) scan_dup_kernel(const ScanDupArg
             st_volatile_u64(a.status, ST_INC | (uint64_t)total);
         } else {
             st_volatile_u64(a.status + ticket, ST_AGG | (uint64_t)total);
-            int p = (int)ticket - 1;
+            int p = (int)ticket - 1;   // nearest predecessor not consumed yet; 8 are fetched per round trip
             while (true) {
-                const uint64_t v = ld_volatile_u64(a.status + p);
-                if ((v >> 62) == 0) continue;
-                excl += v & ST_VAL;
-                if ((v >> 62) == 2) break;
-                --p;
+                uint64_t v[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) v[j] = p - j >= 0 ? ld_volatile_u64(a.status + p - j) : ST_INC;
+                int used = 0;
+                bool fin = false;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    const uint64_t f = v[j] >> 62;
+                    if (!fin && used == j && f != 0) {
+                        excl += v[j] & ST_VAL;
+                        used = j + 1;
+                        fin = f == 2;
+                    }
+                }
+                if (fin) break;
+                p -= used;
             }
             st_volatile_u64(a.status + ticket, ST_INC | (excl + total));
         }
