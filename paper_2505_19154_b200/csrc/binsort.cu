@@ -288,20 +288,71 @@ __global__ void __launch_bounds__(EMIT_THREADS) emit_kernel(const EmitArgs a) {
     if (M == 0 || M > a.capacity) return;
     for (int j = tid; j < a.npass * 256; j += EMIT_THREADS) (&s_hist[0][0])[j] = 0;
     const uint32_t units = (uint32_t)((M + EMIT_TILE - 1) / EMIT_TILE);
-    for (uint32_t b = blockIdx.x; b < units; b += gridDim.x) {
+    // The staging of a unit is a chain of three dependent global loads (starts -> perm/incl -> depth/rect).  It is
+    // software-pipelined over this CTA's units: while unit u is expanded, the second level of unit u+1 and the first
+    // level of unit u+2 are in flight, so only the last gather of a unit is waited for.
+    constexpr int EPT = (EMIT_TILE + 1 + EMIT_THREADS - 1) / EMIT_THREADS;   // staged entries per thread (5)
+    const uint32_t stride = gridDim.x;
+    uint32_t b = blockIdx.x;
+    // level 1 of units b and b + stride
+    uint32_t lo_c = 0, hi_c = 0, lo_n = 0, hi_n = 0;
+    if (b < units) { lo_c = __ldg(a.starts + b); hi_c = __ldg(a.starts + b + 1); }
+    if (b + stride < units) { lo_n = __ldg(a.starts + b + stride); hi_n = __ldg(a.starts + b + stride + 1); }
+    // level 2 of unit b
+    uint32_t r_incl[EPT], r_gid[EPT], r_before = 0;
+    if (b < units) {
+        const int span0 = (int)(hi_c - lo_c) + 1;
+#pragma unroll
+        for (int k = 0; k < EPT; ++k) {
+            const int i = tid + k * EMIT_THREADS;
+            r_incl[k] = i < span0 ? __ldg(a.incl + lo_c + i) : 0u;
+            r_gid[k] = i < span0 ? __ldg(a.perm + lo_c + i) : 0u;
+        }
+        r_before = lo_c ? __ldg(a.incl + lo_c - 1) : 0u;
+    }
+    for (; b < units; b += stride) {
         const uint32_t j0 = b * EMIT_TILE;
         const uint32_t cnt = (uint32_t)min((uint64_t)EMIT_TILE, M - j0);
-        const uint32_t g_lo = __ldg(a.starts + b), g_hi = __ldg(a.starts + b + 1);
-        const int span = (int)(g_hi - g_lo) + 1;   // <= EMIT_TILE + 1
-        __syncthreads();   // previous unit done with the staging arrays (and s_hist zeroed)
-        for (int i = tid; i < span; i += EMIT_THREADS) {
-            const uint32_t g = __ldg(a.perm + g_lo + i);
-            s_incl[i] = __ldg(a.incl + g_lo + i);
-            s_gid[i] = g;
-            s_depth[i] = __float_as_uint(__ldg(a.depth + g));
-            s_rect[i] = __ldg(reinterpret_cast<const uint2*>(a.rect) + g);
+        const int span = (int)(hi_c - lo_c) + 1;   // <= EMIT_TILE + 1
+        const uint32_t before = r_before;
+        // level 3 of this unit
+        uint32_t r_depth[EPT];
+        uint2 r_rect[EPT];
+#pragma unroll
+        for (int k = 0; k < EPT; ++k) {
+            const int i = tid + k * EMIT_THREADS;
+            r_depth[k] = 0u;
+            r_rect[k] = make_uint2(0u, 0u);
+            if (i < span) {
+                r_depth[k] = __float_as_uint(__ldg(a.depth + r_gid[k]));
+                r_rect[k] = __ldg(reinterpret_cast<const uint2*>(a.rect) + r_gid[k]);
+            }
         }
-        const uint32_t before = g_lo ? __ldg(a.incl + g_lo - 1) : 0u;
+        __syncthreads();   // previous unit done with the staging arrays (and s_hist zeroed)
+#pragma unroll
+        for (int k = 0; k < EPT; ++k) {
+            const int i = tid + k * EMIT_THREADS;
+            if (i < span) { s_incl[i] = r_incl[k]; s_gid[i] = r_gid[k]; }
+        }
+        // level 2 of the next unit, level 1 of the one after (their registers are free now)
+        const uint32_t lo_nn = b + 2 * stride < units ? __ldg(a.starts + b + 2 * stride) : 0u;
+        const uint32_t hi_nn = b + 2 * stride < units ? __ldg(a.starts + b + 2 * stride + 1) : 0u;
+        if (b + stride < units) {
+            const int span1 = (int)(hi_n - lo_n) + 1;
+#pragma unroll
+            for (int k = 0; k < EPT; ++k) {
+                const int i = tid + k * EMIT_THREADS;
+                r_incl[k] = i < span1 ? __ldg(a.incl + lo_n + i) : 0u;
+                r_gid[k] = i < span1 ? __ldg(a.perm + lo_n + i) : 0u;
+            }
+            r_before = lo_n ? __ldg(a.incl + lo_n - 1) : 0u;
+        }
+#pragma unroll
+        for (int k = 0; k < EPT; ++k) {
+            const int i = tid + k * EMIT_THREADS;
+            if (i < span) { s_depth[i] = r_depth[k]; s_rect[i] = r_rect[k]; }
+        }
+        lo_c = lo_n; hi_c = hi_n; lo_n = lo_nn; hi_n = hi_nn;
         __syncthreads();
         const uint32_t jl = tid * EMIT_ITEMS;
         if (jl < cnt) {
