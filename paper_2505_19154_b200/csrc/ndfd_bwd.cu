@@ -6,12 +6,13 @@
 //     dL/dalpha_k = T_k g_k - C_k / (1 - alpha_k),   C_k = sum_{j>k} g_j w_j
 //     dL/dop_g   += dL/dalpha_k G_k    (0 where alpha is clamped at alpha_max)
 //
-// First CUDA path of this row: three FORWARD traversals with the strip kernel of ndfd.cu (feature rows staged in
-// shared memory with double-buffered cp.async, 4 or 8 lanes per pixel; no reverse walk, no
-// division-recovered transmittance): pass 1 stores the per-pixel totals A_0 (scalar) and B_0 (D-vector), pass 2
-// turns them into running suffixes, evaluates g_k and stores C_0 = sum g_j w_j, pass 3 repeats that with the
-// running suffix of C and adds dL/dalpha_k G_k into grad_opacity: reduced over the pixels of the warp first, then
-// one atomic per (warp, Gaussian).
+// First CUDA path of this row: two FORWARD traversals with the strip kernel of ndfd.cu (feature rows staged in
+// shared memory with double-buffered cp.async, 4 or 8 lanes per pixel; no reverse walk, no division-recovered
+// transmittance).  Pass 1 stores the per-pixel totals A_0 (scalar), B_0 (D-vector) and C_0, where
+//     C_0 = sum_j g_j w_j = lam1 L_gt + 2 lam2 L_cf
+// because sum_j w_j (A_j - B_j.f_j) = sum_i sigma_i w_i (W_{i-1} - F_{i-1}.f_i) = L_cf (swap the double sum), so the
+// forward recurrence suffices.  Pass 2 (MODE 3) turns the totals into running suffixes, evaluates g_k and adds
+// dL/dalpha_k G_k into grad_opacity: reduced over the pixels of the warp first, then one atomic per (warp, Gaussian).
 #include <cuda_fp16.h>
 
 #include "traverse.cuh"
@@ -64,7 +65,7 @@ struct BwdSub {
     static constexpr int SB = 32768 / ROW_BYTES > 64 ? 64 : (32768 / ROW_BYTES < 4 ? 4 : 32768 / ROW_BYTES);
 };
 
-// MODE 1: totals A_0, B_0.  MODE 2: C_0.  MODE 3: gradient.
+// MODE 1: totals A_0, B_0, C_0.  MODE 3: gradient.
 template <int MODE, int LPP, int CPL, typename FT, typename GT>
 __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel(const BwdArgs a) {
     __shared__ TileQueue q;
@@ -100,7 +101,7 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
     }
     float T = 1.f, Wc = 0.f;
     float As = (MODE != 1 && inside) ? a.A_tot[pix] : 0.f;      // MODE 1: running sum; else suffix A_k
-    float Cs = (MODE == 3 && inside) ? a.C_tot[pix] : 0.f;      // MODE 2: running sum; MODE 3: suffix C_k
+    float Cs = (MODE == 3 && inside) ? a.C_tot[pix] : 0.f;      // MODE 1: running sum of C_0; MODE 3: suffix C_k
     bool done = !inside;
     const float k2 = a.k_sig * 1.44269504088896340736f;
 
@@ -179,9 +180,21 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
                 const float sigma = 1.0f / (1.0f + exp2f(k2 * (phi - a.lambda)));
                 const float sw = sigma * w;
                 if (MODE == 1) {
-                    As += sw;
+                    // totals A_0, B_0 and the forward losses (prefix recurrence), from which C_0 follows (see the header)
+                    float fa1[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-                    for (int j = 0; j < CPL; ++j) Bs[j] = fmaf(sw, fv[j], Bs[j]);
+                    for (int j = 0; j < CPL; ++j) fa1[j & 3] = fmaf(fv[j], F[j], fa1[j & 3]);
+                    float Ff1 = (fa1[0] + fa1[1]) + (fa1[2] + fa1[3]);
+#pragma unroll
+                    for (int d = 1; d < LPP; d <<= 1) Ff1 += __shfl_xor_sync(TR_FULL, Ff1, d);
+                    As += sw;
+                    Cs += a.lam1 * sw + 2.0f * a.lam2 * sw * (Wc - Ff1);
+                    Wc += w;
+#pragma unroll
+                    for (int j = 0; j < CPL; ++j) {
+                        Bs[j] = fmaf(sw, fv[j], Bs[j]);
+                        F[j] = fmaf(w, fv[j], F[j]);
+                    }
                     continue;
                 }
                 // suffixes exclude k
@@ -203,9 +216,7 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
                 Wc += w;
 #pragma unroll
                 for (int j = 0; j < CPL; ++j) F[j] = fmaf(w, fv[j], F[j]);
-                if (MODE == 2) {
-                    Cs = fmaf(gk, w, Cs);
-                } else {
+                {
                     Cs = fmaf(-gk, w, Cs);   // suffix excludes k
                     float contrib = hit ? (Tb * gk - Cs / (1.0f - alpha)) * Ge : 0.f;
                     if (cgl != 0) contrib = 0.f;   // every lane of the pixel group holds the same value
@@ -221,13 +232,11 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
     }
     if (inside) {
         if (MODE == 1) {
-            if (cgl == 0) a.A_tot[pix] = As;
+            if (cgl == 0) { a.A_tot[pix] = As; a.C_tot[pix] = Cs; }
 #pragma unroll
             for (int j = 0; j < CPL / 4; ++j)
                 *reinterpret_cast<float4*>(a.B_tot + pix * a.D + c_lo + 4 * LPP * j) =
                     make_float4(Bs[4 * j], Bs[4 * j + 1], Bs[4 * j + 2], Bs[4 * j + 3]);
-        } else if (MODE == 2) {
-            if (cgl == 0) a.C_tot[pix] = Cs;
         }
     }
 }
@@ -246,7 +255,6 @@ template <int LPP, int CPL, typename FT, typename GT>
 cudaError_t launch3(const BwdArgs& a, int tiles, cudaStream_t st) {
     cudaError_t e;
     if ((e = launch1<1, LPP, CPL, FT, GT>(a, tiles, st)) != cudaSuccess) return e;
-    if ((e = launch1<2, LPP, CPL, FT, GT>(a, tiles, st)) != cudaSuccess) return e;
     return launch1<3, LPP, CPL, FT, GT>(a, tiles, st);
 }
 
