@@ -280,8 +280,11 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     tile_bits = max(1, (tiles - 1).bit_length())
     p_full = (32 + tile_bits + 7) // 8
     # n_eval of SURVEY 8(d): instances of a tile's list walked before the whole tile stopped (fhgs_render's
-    # tile_visited diagnostics of the last timed frame) x the tile's valid pixels
+    # tile_visited diagnostics) x the tile's valid pixels
     gw, gh = (W + 15) // 16, (H + 15) // 16
+    ctx.set_diagnostics(True)     # one extra, un-timed render with the diagnostics variant of the kernel
+    fb.render(ctx, g, cam, prm, vs, out_rgb, out_feat, out_T, out_n)
+    ctx.set_diagnostics(False)
     tv = vs.tile_visited().to(torch.int64).view(gh, gw)
     px_x = torch.clamp(W - 16 * torch.arange(gw, device=dev), max=16)
     px_y = torch.clamp(H - 16 * torch.arange(gh, device=dev), max=16)

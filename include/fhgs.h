@@ -124,12 +124,14 @@ typedef struct {
 } fhgs_view_state;
 
 FHGS_API size_t fhgs_scratch_bytes(int32_t n, int32_t width, int32_t height, uint64_t capacity);
-/* Diagnostics for the work accounting of SURVEY 8(d) (n_eval): byte offset inside `scratch` of a
- * uint32_t[GW*GH] array that fhgs_render fills with, per tile, the length of the prefix of the
+/* Diagnostics for the work accounting of SURVEY 8(d) (n_eval), off by default: after
+ * fhgs_set_diagnostics(ctx, 1), fhgs_render also fills a uint32_t[GW*GH] array inside `scratch` (byte offset
+ * returned by fhgs_scratch_tile_visited) with, per tile, the length of the prefix of the
  * tile's sorted list that was walked before every pixel of the tile had stopped (the whole list if
  * it never stopped; exact -- one past the last instance any pixel blended -- for D % 64 == 0,
  * rounded up to 256-instance chunks otherwise).  Same arguments as fhgs_scratch_bytes.  Not an output of the method. */
 FHGS_API size_t fhgs_scratch_tile_visited(int32_t n, int32_t width, int32_t height, uint64_t capacity);
+FHGS_API void fhgs_set_diagnostics(fhgs_ctx* ctx, int enable);
 
 /* Step P -- PAPER.md:302 (CullGaussian), PAPER.md:309-310 (2DScreenGaussians); EWA reading
  * per Gaussian, camera-space position, cull (z < z_near, det <= 0, non-finite,

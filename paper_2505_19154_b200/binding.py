@@ -20,7 +20,7 @@ FHGS_SORT_FULL_KEY = 1
 FHGS_FUSE_ZERO, FHGS_FUSE_FINALIZE, FHGS_FUSE_L2NORM, FHGS_FUSE_FINALIZE_ONLY, FHGS_FUSE_ZERO_ONLY = 1, 2, 4, 8, 16
 
 EXPORTS = ["fhgs_create", "fhgs_destroy", "fhgs_last_error", "fhgs_version", "fhgs_default_params",
-           "fhgs_scratch_bytes", "fhgs_scratch_tile_visited", "fhgs_project", "fhgs_bin_sort", "fhgs_render", "fhgs_fuse_features", "fhgs_ndfd_forward", "fhgs_ndfd_backward_work_bytes", "fhgs_ndfd_backward",
+           "fhgs_scratch_bytes", "fhgs_scratch_tile_visited", "fhgs_set_diagnostics", "fhgs_project", "fhgs_bin_sort", "fhgs_render", "fhgs_fuse_features", "fhgs_ndfd_forward", "fhgs_ndfd_backward_work_bytes", "fhgs_ndfd_backward",
            "fhgs_frame_host", "fhgs_ffma_peak"]
 
 
@@ -86,6 +86,8 @@ def _load():
     lib.fhgs_scratch_bytes.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_uint64]
     lib.fhgs_scratch_tile_visited.restype = C.c_size_t
     lib.fhgs_scratch_tile_visited.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.c_uint64]
+    lib.fhgs_set_diagnostics.restype = None
+    lib.fhgs_set_diagnostics.argtypes = [vp, C.c_int]
     lib.fhgs_project.argtypes = [vp, C.POINTER(CGaussians), C.POINTER(CCamera), C.POINTER(CParams),
                                  C.POINTER(CViewState), vp]
     lib.fhgs_bin_sort.argtypes = [vp, C.POINTER(CCamera), C.POINTER(CViewState), C.POINTER(C.c_uint64),
@@ -180,6 +182,10 @@ class Context:
             self.close()
         except Exception:
             pass
+
+    def set_diagnostics(self, enable: bool):
+        """fhgs_set_diagnostics: make fhgs_render fill ViewState.tile_visited() (work accounting only)."""
+        lib.fhgs_set_diagnostics(self.handle, 1 if enable else 0)
 
     def check(self, st: int):
         if st != FHGS_OK:

@@ -17,6 +17,7 @@ extern "C" fhgs_status fhgs_create(fhgs_ctx** out, int device) {
     if (!c) return FHGS_ERR_INTERNAL;
     c->device = device;
     c->err[0] = 0;
+    c->diagnostics = 0;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { delete c; return FHGS_ERR_INTERNAL; }
     c->num_sms = prop.multiProcessorCount;
@@ -41,6 +42,10 @@ extern "C" void fhgs_destroy(fhgs_ctx* ctx) {
     cudaStreamDestroy(ctx->copy_out);
     for (cudaEvent_t e : {ctx->ev_start, ctx->ev_feat, ctx->ev_gt, ctx->ev_render, ctx->ev_out}) cudaEventDestroy(e);
     delete ctx;
+}
+
+extern "C" void fhgs_set_diagnostics(fhgs_ctx* ctx, int enable) {
+    if (ctx) ctx->diagnostics = enable ? 1 : 0;
 }
 
 extern "C" const char* fhgs_last_error(const fhgs_ctx* ctx) { return ctx ? ctx->err : "NULL context"; }

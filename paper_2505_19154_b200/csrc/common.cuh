@@ -14,6 +14,7 @@ struct fhgs_ctx {
     int device;
     int num_sms;
     int max_smem_optin;
+    int diagnostics;   // fhgs_set_diagnostics: fhgs_render also fills the tile_visited array
     // fhgs_frame_host only: copy streams / events that overlap host<->device copies with the steps
     cudaStream_t copy_in, copy_out;
     cudaEvent_t ev_start, ev_feat, ev_gt, ev_render, ev_out;

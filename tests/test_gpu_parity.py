@@ -280,7 +280,12 @@ def test_tile_visited_diagnostics():
         cam = inputs.make_camera(cfg, 0)
         gp = pu.GpuPath(scene, cfg.width, cfg.height, 4_000_000)
         c, m = gp.project_sort(cam)
-        gp.render(c)
+        gp.ctx.set_diagnostics(True)
+        g_diag = gp.render(c)
+        gp.ctx.set_diagnostics(False)
+        g_plain = gp.render(c)
+        for k in ("rgb", "feat", "T", "n"):
+            assert np.array_equal(g_diag[k], g_plain[k])   # the diagnostics variant computes the same image
         tv = gp.vs.tile_visited().cpu().numpy().astype(np.int64)
         rg = gp.vs.ranges.cpu().numpy().view(np.uint32).astype(np.int64)
         ln = rg[:, 1] - rg[:, 0]
