@@ -390,11 +390,11 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT>& sm, const FuseA
         ulonglong2 wb = *reinterpret_cast<const ulonglong2*>(Ws + FW_WQ);
         float4 g = ld_g4(Gs);
 #pragma unroll 1
-        for (int s0 = 0; s0 < (kg * 8 < m.nb ? 128 : 0); s0 += 16) {
+        for (int s0 = 0; s0 < (kg * 8 < m.nb ? 128 : 0); s0 += 32) {
             const float* Wb = Ws + s0 * 4;
             const GT* Gb = Gs + s0 * FW_DC;
 #pragma unroll
-            for (int u = 0; u < 16; ++u) {
+            for (int u = 0; u < 32; ++u) {
                 const int un = u + 1;   // the prefetch past the last pixel lands in the row pad / G_pad (never used)
                 const ulonglong2 wa_n = *reinterpret_cast<const ulonglong2*>(Wb + un * 4);
                 const ulonglong2 wb_n = *reinterpret_cast<const ulonglong2*>(Wb + FW_WQ + un * 4);
