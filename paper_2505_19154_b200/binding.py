@@ -12,7 +12,7 @@ import numpy as np
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libfhgs.so")
+LIB_PATH = os.environ.get("FHGS_LIB") or os.path.join(_HERE, "libfhgs.so")   # FHGS_LIB: load another build of the same ABI
 
 FHGS_OK, FHGS_ERR_INTERNAL, FHGS_ERR_INVALID, FHGS_ERR_CAPACITY = 0, 1, 2, 3
 FHGS_F32, FHGS_F16 = 0, 1

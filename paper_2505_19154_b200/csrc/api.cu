@@ -27,20 +27,24 @@ extern "C" fhgs_status fhgs_create(fhgs_ctx** out, int device) {
         return FHGS_ERR_INTERNAL;
     }
     if (cudaSetDevice(device) != cudaSuccess) { delete c; return FHGS_ERR_INTERNAL; }
+    c->copy_in = c->copy_out = nullptr;
+    c->ev_start = c->ev_feat = c->ev_gt = c->ev_render = c->ev_out = nullptr;
     bool ok = cudaStreamCreateWithFlags(&c->copy_in, cudaStreamNonBlocking) == cudaSuccess &&
               cudaStreamCreateWithFlags(&c->copy_out, cudaStreamNonBlocking) == cudaSuccess;
     for (cudaEvent_t* e : {&c->ev_start, &c->ev_feat, &c->ev_gt, &c->ev_render, &c->ev_out})
         ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
-    if (!ok) { delete c; return FHGS_ERR_INTERNAL; }
+    if (!ok) { fhgs_destroy(c); return FHGS_ERR_INTERNAL; }   // releases whatever was created
     *out = c;
     return FHGS_OK;
 }
 
 extern "C" void fhgs_destroy(fhgs_ctx* ctx) {
     if (!ctx) return;
-    cudaStreamDestroy(ctx->copy_in);
-    cudaStreamDestroy(ctx->copy_out);
-    for (cudaEvent_t e : {ctx->ev_start, ctx->ev_feat, ctx->ev_gt, ctx->ev_render, ctx->ev_out}) cudaEventDestroy(e);
+    DeviceGuard dg(ctx);
+    if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
+    if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
+    for (cudaEvent_t e : {ctx->ev_start, ctx->ev_feat, ctx->ev_gt, ctx->ev_render, ctx->ev_out})
+        if (e) cudaEventDestroy(e);
     delete ctx;
 }
 
@@ -76,6 +80,8 @@ fhgs_status validate_camera(fhgs_ctx* ctx, const fhgs_camera* cam) {
     if (cam->width <= 0 || cam->height <= 0) FHGS_INVALID(ctx, "camera: width/height must be > 0");
     const long long tiles = (long long)tiles_x(cam->width) * tiles_y(cam->height);
     if (tiles >= (1LL << 31)) FHGS_INVALID(ctx, "camera: too many tiles for the 32-bit tile id");
+    if (tiles_x(cam->width) > 65535 || tiles_y(cam->height) > 65535)
+        FHGS_INVALID(ctx, "camera: more than 65535 tiles along one axis (rect is uint16)");
     for (int i = 0; i < 16; ++i)
         if (!finite_f(cam->view[i]) || !finite_f(cam->proj[i])) FHGS_INVALID(ctx, "camera: non-finite matrix entry");
     for (int i = 0; i < 3; ++i)
@@ -90,13 +96,13 @@ fhgs_status validate_params(fhgs_ctx* ctx, const fhgs_params* p) {
     for (int i = 0; i < 10; ++i)
         if (!finite_f(v[i])) FHGS_INVALID(ctx, "params: non-finite value");
     if (!(p->z_near > 0.0f)) FHGS_INVALID(ctx, "params: z_near must be > 0 (depth bits must order like depth)");
-    if (!(p->q_cutoff >= 0.0f) || !(p->alpha_max > 0.0f && p->alpha_max <= 1.0f) || !(p->t_min >= 0.0f))
-        FHGS_INVALID(ctx, "params: q_cutoff >= 0, 0 < alpha_max <= 1, t_min >= 0 required");
+    if (!(p->q_cutoff >= 0.0f) || !(p->alpha_max > 0.0f && p->alpha_max < 1.0f) || !(p->t_min >= 0.0f))
+        FHGS_INVALID(ctx, "params: q_cutoff >= 0, 0 < alpha_max < 1, t_min >= 0 required");   // 1/(1-alpha) in the backward
     return FHGS_OK;
 }
 
 fhgs_status validate_view_state(fhgs_ctx* ctx, const fhgs_view_state* vs, const fhgs_camera* cam) {
-    if (vs->n < 0) FHGS_INVALID(ctx, "view_state: n < 0");
+    if (vs->n < 0 || vs->n >= (1 << 30)) FHGS_INVALID(ctx, "view_state: n must be in [0, 2^30)");   // 30-bit packed counts
     if (cam && (vs->width != cam->width || vs->height != cam->height))
         FHGS_INVALID(ctx, "view_state: width/height differ from the camera's");
     if (vs->capacity >= (1ull << 30)) FHGS_INVALID(ctx, "view_state: capacity must be < 2^30");
@@ -129,46 +135,69 @@ extern "C" fhgs_status fhgs_frame_host(fhgs_ctx* ctx, const fhgs_host_frame* hos
         FHGS_INVALID(ctx, "fhgs_frame_host: NULL host input");
     if (!ws->out_rgb || !ws->out_feat || !ws->gt || !ws->num || !ws->den || !ws->fused_feat)
         FHGS_INVALID(ctx, "fhgs_frame_host: NULL workspace buffer");
+    // Everything that can be rejected is rejected HERE, before the first event record or copy (fhgs.h: "Nothing is
+    // enqueued when FHGS_ERR_INVALID is returned"): the same checks the four steps repeat on entry.
     fhgs_status st;
     if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
+    if ((st = validate_params(ctx, prm)) != FHGS_OK) return st;
+    if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
+    if (g->n != vs->n) FHGS_INVALID(ctx, "fhgs_frame_host: g->n != vs->n");
+    if (!g->mean || !g->scale || !g->quat || !g->opacity || !g->sh) FHGS_INVALID(ctx, "fhgs_frame_host: NULL device Gaussian array");
+    if (g->feat_dtype != FHGS_F32 && g->feat_dtype != FHGS_F16) FHGS_INVALID(ctx, "fhgs_frame_host: unknown feat_dtype");
+    if (g->feat_dim % (g->feat_dtype == FHGS_F16 ? 8 : 4)) FHGS_INVALID(ctx, "fhgs_frame_host: feat_dim must be a multiple of 4 (f32) / 8 (f16)");
+    if (!aligned_to(g->feat, 16) || !aligned_to(ws->out_feat, 16) || !aligned_to(ws->gt, 16) || !aligned_to(ws->num, 16) ||
+        !aligned_to(ws->den, 4) || !aligned_to(ws->fused_feat, 16))
+        FHGS_INVALID(ctx, "fhgs_frame_host: feat / workspace buffers must be 16-byte aligned");
+    DeviceGuard dg(ctx);
     cudaStream_t s = (cudaStream_t)stream;
     const size_t n = (size_t)g->n, K = (size_t)(g->sh_degree + 1) * (g->sh_degree + 1);
     const size_t e = g->feat_dtype == FHGS_F16 ? 2 : 4, D = (size_t)g->feat_dim;
     const size_t px = (size_t)cam->width * cam->height;
+    uint64_t m = 0;
     // Schedule (three streams, so that PCIe runs in both directions while the steps execute):
     //   s        : H2D geometry -> P -> S -> [wait feat] R -> [wait gt] F -> D2H fused -> [wait image copies]
     //   copy_in  : H2D feat -> H2D gt                      (behind everything already enqueued on s)
     //   copy_out : [wait R] D2H rgb, feature image         (overlaps H2D gt and F)
-    FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_start, s));
-    FHGS_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_in, ctx->ev_start, 0));
-    FHGS_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_out, ctx->ev_start, 0));
-    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->mean, host->mean, n * 12, cudaMemcpyHostToDevice, s));
-    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->scale, host->scale, n * 12, cudaMemcpyHostToDevice, s));
-    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->quat, host->quat, n * 16, cudaMemcpyHostToDevice, s));
-    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->opacity, host->opacity, n * 4, cudaMemcpyHostToDevice, s));
-    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->sh, host->sh, n * K * 12, cudaMemcpyHostToDevice, s));
-    FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->feat, host->feat, n * D * e, cudaMemcpyHostToDevice, ctx->copy_in));
-    FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_feat, ctx->copy_in));
-    FHGS_CUDA(ctx, cudaMemcpyAsync(ws->gt, host->gt, px * D * e, cudaMemcpyHostToDevice, ctx->copy_in));
-    FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_gt, ctx->copy_in));
-    if ((st = fhgs_project(ctx, g, cam, prm, vs, stream)) != FHGS_OK) return st;
-    if ((st = fhgs_bin_sort(ctx, cam, vs, nullptr, 0, stream)) != FHGS_OK) return st;
-    FHGS_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_feat, 0));
-    if ((st = fhgs_render(ctx, g, cam, prm, vs, ws->out_rgb, ws->out_feat, nullptr, nullptr, stream)) != FHGS_OK) return st;
-    FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_render, s));
-    FHGS_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_out, ctx->ev_render, 0));
-    if (host->out_rgb) FHGS_CUDA(ctx, cudaMemcpyAsync(host->out_rgb, ws->out_rgb, px * 12, cudaMemcpyDeviceToHost, ctx->copy_out));
-    if (host->out_feat) FHGS_CUDA(ctx, cudaMemcpyAsync(host->out_feat, ws->out_feat, px * D * e, cudaMemcpyDeviceToHost, ctx->copy_out));
-    FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_out, ctx->copy_out));
-    FHGS_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_gt, 0));
-    if ((st = fhgs_fuse_features(ctx, cam, prm, vs, ws->gt, g->feat_dim, g->feat_dtype, ws->num, ws->den,
-                                 ws->fused_feat, g->feat_dtype, FHGS_FUSE_ZERO | FHGS_FUSE_FINALIZE, stream)) != FHGS_OK)
-        return st;
-    if (host->fused_feat) FHGS_CUDA(ctx, cudaMemcpyAsync(host->fused_feat, ws->fused_feat, n * D * e, cudaMemcpyDeviceToHost, s));
-    FHGS_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_out, 0));
-    uint64_t m = 0;
-    FHGS_CUDA(ctx, cudaMemcpyAsync(&m, vs->num_instances, 8, cudaMemcpyDeviceToHost, s));
-    FHGS_CUDA(ctx, cudaStreamSynchronize(s));
+    // Once anything is enqueued, every exit -- also an error exit -- first drains s, copy_in and copy_out, so that no
+    // DMA is still running against the caller's host buffers or device staging when the call returns.
+    st = [&]() -> fhgs_status {
+        FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_start, s));
+        FHGS_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_in, ctx->ev_start, 0));
+        FHGS_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_out, ctx->ev_start, 0));
+        FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->mean, host->mean, n * 12, cudaMemcpyHostToDevice, s));
+        FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->scale, host->scale, n * 12, cudaMemcpyHostToDevice, s));
+        FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->quat, host->quat, n * 16, cudaMemcpyHostToDevice, s));
+        FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->opacity, host->opacity, n * 4, cudaMemcpyHostToDevice, s));
+        FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->sh, host->sh, n * K * 12, cudaMemcpyHostToDevice, s));
+        FHGS_CUDA(ctx, cudaMemcpyAsync((void*)g->feat, host->feat, n * D * e, cudaMemcpyHostToDevice, ctx->copy_in));
+        FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_feat, ctx->copy_in));
+        FHGS_CUDA(ctx, cudaMemcpyAsync(ws->gt, host->gt, px * D * e, cudaMemcpyHostToDevice, ctx->copy_in));
+        FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_gt, ctx->copy_in));
+        fhgs_status r;
+        if ((r = fhgs_project(ctx, g, cam, prm, vs, stream)) != FHGS_OK) return r;
+        if ((r = fhgs_bin_sort(ctx, cam, vs, nullptr, 0, stream)) != FHGS_OK) return r;
+        FHGS_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_feat, 0));
+        if ((r = fhgs_render(ctx, g, cam, prm, vs, ws->out_rgb, ws->out_feat, nullptr, nullptr, stream)) != FHGS_OK) return r;
+        FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_render, s));
+        FHGS_CUDA(ctx, cudaStreamWaitEvent(ctx->copy_out, ctx->ev_render, 0));
+        if (host->out_rgb) FHGS_CUDA(ctx, cudaMemcpyAsync(host->out_rgb, ws->out_rgb, px * 12, cudaMemcpyDeviceToHost, ctx->copy_out));
+        if (host->out_feat) FHGS_CUDA(ctx, cudaMemcpyAsync(host->out_feat, ws->out_feat, px * D * e, cudaMemcpyDeviceToHost, ctx->copy_out));
+        FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_out, ctx->copy_out));
+        FHGS_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_gt, 0));
+        if ((r = fhgs_fuse_features(ctx, cam, prm, vs, ws->gt, g->feat_dim, g->feat_dtype, ws->num, ws->den,
+                                    ws->fused_feat, g->feat_dtype, FHGS_FUSE_ZERO | FHGS_FUSE_FINALIZE, stream)) != FHGS_OK)
+            return r;
+        if (host->fused_feat) FHGS_CUDA(ctx, cudaMemcpyAsync(host->fused_feat, ws->fused_feat, n * D * e, cudaMemcpyDeviceToHost, s));
+        FHGS_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_out, 0));
+        FHGS_CUDA(ctx, cudaMemcpyAsync(&m, vs->num_instances, 8, cudaMemcpyDeviceToHost, s));
+        return FHGS_OK;
+    }();
+    // drain all three streams (copy_in / copy_out first: on an error path `s` may not be waiting for them)
+    const cudaError_t d0 = cudaStreamSynchronize(ctx->copy_in), d1 = cudaStreamSynchronize(ctx->copy_out), d2 = cudaStreamSynchronize(s);
+    if (st != FHGS_OK) return st;
+    FHGS_CUDA(ctx, d0);
+    FHGS_CUDA(ctx, d1);
+    FHGS_CUDA(ctx, d2);
     if (num_instances_host) *num_instances_host = m;
     if (m > vs->capacity) return set_err(ctx, FHGS_ERR_CAPACITY, "fhgs_frame_host: %s%lld instances exceed capacity", "", (long long)m);
     return FHGS_OK;
@@ -211,6 +240,7 @@ __global__ void __launch_bounds__(256) ffma_peak_kernel(float* out, int iters, f
 extern "C" fhgs_status fhgs_ffma_peak(fhgs_ctx* ctx, int32_t iters, double* lane_ops_per_s, double* ms, void* stream) {
     if (!ctx) return FHGS_ERR_INVALID;
     if (iters <= 0 || !lane_ops_per_s) FHGS_INVALID(ctx, "fhgs_ffma_peak: iters <= 0 or NULL output");
+    DeviceGuard dg(ctx);
     cudaStream_t s = (cudaStream_t)stream;
     float* d = nullptr;
     FHGS_CUDA(ctx, cudaMalloc(&d, 4));

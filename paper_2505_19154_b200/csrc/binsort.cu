@@ -762,6 +762,7 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
     if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
     if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
     if (flags & ~(uint32_t)FHGS_SORT_FULL_KEY) FHGS_INVALID(ctx, "fhgs_bin_sort: unknown flag");
+    DeviceGuard dg(ctx);
     cudaStream_t s = (cudaStream_t)stream;
     const int GW = tiles_x(cam->width), GH = tiles_y(cam->height);
     const size_t ntiles = (size_t)GW * GH;

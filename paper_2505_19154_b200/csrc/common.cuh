@@ -21,6 +21,21 @@ struct fhgs_ctx {
     char err[512];
 };
 
+// Every entry point that enqueues work makes the context's device current for the duration of the call and
+// restores the caller's device afterwards (a process driving several GPUs may call with any device current).
+struct DeviceGuard {
+    int prev = -1;
+    bool switched = false;
+    explicit DeviceGuard(const fhgs_ctx* ctx) {
+        if (cudaGetDevice(&prev) == cudaSuccess && prev != ctx->device) switched = cudaSetDevice(ctx->device) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (switched) cudaSetDevice(prev);
+    }
+    DeviceGuard(const DeviceGuard&) = delete;
+    DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
+
 // Pinhole intrinsics derived from proj[] (fhgs.h "Conventions"): double, rounded once.
 struct Intrinsics {
     float fx, fy, cx, cy, tanx, tany;

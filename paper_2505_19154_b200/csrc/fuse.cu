@@ -285,8 +285,10 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseA
     const int sx = p & 15, sy = p >> 4;   // row-major pixel slot (matches the GT tile rows)
     int stage = 0, islot = 0;
     uint32_t phase = 0, iphase = 0;
+    WS_TDECL;
     while (true) {
         mbar_wait(&sm.item_full[islot], iphase);
+        WS_TACC(0);
         const int item = sm.items[islot];
         mbar_arrive(&sm.item_empty[islot]);
         if (++islot == 2) { islot = 0; iphase ^= 1u; }
@@ -296,6 +298,7 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseA
             mbar_arrive(&sm.ct.full[stage]);
             break;
         }
+        WS_TCNT(6);
         const int tile = ws_item_tile(wk, item), c0 = (item % wk.n_chunks) * FW_DC;
         const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
         const int px = tx0 + sx, py = ty0 + sy;
@@ -320,7 +323,10 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseA
                 ws_chunk_prefetch_id(a.t, pos + WS_PROD, range.y, p, ch);
             }
             const int nb = min(WS_KB, qt - qh);
+            WS_TACC(1);
             mbar_wait_backoff(&sm.ct.empty[stage], phase ^ 1u);
+            WS_TACC(2);
+            WS_TCNT(5);
             if (p < WS_KB) sm.ids[stage][p] = p < nb ? __float_as_uint(sm.ct.rec1[(qh + p) & (WS_QCAP - 1)].z) : 0u;
             float* Wd = sm.W[stage] + p * 4;
             const bool warp_done = __all_sync(TR_FULL, P.done);
@@ -342,39 +348,58 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseA
                 *reinterpret_cast<float4*>(Wd + kq * FW_WQ) = make_float4(w4[0], w4[1], w4[2], w4[3]);
             }
             qh += nb;
+            WS_TACC(3);
             const bool all_done = named_bar_and(WS_BAR_PROD_RED, WS_PROD, P.done);
             last = all_done || (pos >= range.y && qt == qh);
             if (p == 0) sm.ct.meta[stage] = WsMeta{nb, tile, c0, (last ? WS_FLAG_LAST : 0) | (first ? FW_FLAG_FIRST : 0)};
             first = false;
             mbar_arrive(&sm.ct.full[stage]);
+            WS_TACC(4);
             if (++stage == FW_STAGES) { stage = 0; phase ^= 1u; }
         } while (!last);
     }
+    WS_TFLUSH(16, p == 0);
     (void)lane;
 }
 
+// Consumer warp w: pixel half w>>2 (pixels [128 half, +128)), channel quarter w&3 (32 channels).  Lane = (lane group
+// lg = lane>>3, channel group cg = lane&7): thread tile = 8 instances x 4 channels, so that per pixel the warp reads
+// ONE 128-byte wavefront of G (8 channel groups x 16 B) and two of W (4 instance groups x 16 B each) for 16 FFMA2 per
+// thread -- half the shared-memory traffic of a warp-per-instance-group layout, which was the co-limiter (ncu: 69 % of
+// the LSU wavefront slots next to 64 % of the FMA pipe).  A full batch maps lane group -> instance group (8 lg .. 8 lg + 7)
+// over the 128 pixels of the half.  A SHORT batch (nb <= 16, the last one of a tile) gives every instance group to
+// several lane groups, each over a slice of the pixels, and adds the slices up with shuffles: no lane multiplies padding.
 template <typename GT>
 __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT>& sm, const FuseArgs& a) {
     // consumers are warps 8-15: the SMSP arbiter favours high warp ids and the consumers are the critical path
     const int tid = threadIdx.x - WS_PROD, lane = tid & 31, warp = tid >> 5;
-    const int half = warp >> 2, cw = warp & 3;
-    const int kg = warp & 3;                  // the warp's 8 instances of the batch (a short batch idles whole warps)
-    const int ch = lane * 4;                  // this thread's 4 channels inside the chunk
-    const GT* Gs = sm.G + half * 128 * FW_DC + ch;
+    const int half = warp >> 2, cq = warp & 3;
+    const int lg = lane >> 3, cg = lane & 7;
+    const int ch = cq * 32 + cg * 4;          // this thread's 4 channels inside the chunk
     int stage = 0;
     uint32_t phase = 0, gphase = 0, batch = 0;
+    WS_TDECL;
     while (true) {
         mbar_wait(&sm.ct.full[stage], phase);
+        WS_TACC(0);
         const WsMeta m = sm.ct.meta[stage];
         if (m.flags & WS_FLAG_EXIT) break;
         if (m.flags & FW_FLAG_FIRST) {
             mbar_wait(&sm.g_full, gphase);
             gphase ^= 1u;
+            WS_TACC(1);
         }
+        WS_TCNT(5);
+        if (m.nb <= 16) WS_TCNT(6);
+        // lane group -> (instance group, pixel slice) for this batch
+        const int ngrp = m.nb > 16 ? 4 : (m.nb > 8 ? 2 : 1);     // instance groups the lane groups are spread over
+        const int ig = lg & (ngrp - 1);
+        const int npx = 32 * ngrp;                               // pixels per slice (4/ngrp slices per half)
+        const int px0 = half * 128 + (lg / ngrp) * npx;
         uint32_t id[8];
         {
-            const uint4 i0 = *reinterpret_cast<const uint4*>(&sm.ids[stage][kg * 8]);
-            const uint4 i1 = *reinterpret_cast<const uint4*>(&sm.ids[stage][kg * 8 + 4]);
+            const uint4 i0 = *reinterpret_cast<const uint4*>(&sm.ids[stage][ig * 8]);
+            const uint4 i1 = *reinterpret_cast<const uint4*>(&sm.ids[stage][ig * 8 + 4]);
             id[0] = i0.x; id[1] = i0.y; id[2] = i0.z; id[3] = i0.w;
             id[4] = i1.x; id[5] = i1.y; id[6] = i1.z; id[7] = i1.w;
         }
@@ -383,36 +408,54 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT>& sm, const FuseA
         for (int i = 0; i < 4; ++i)
 #pragma unroll
             for (int c = 0; c < 4; ++c) acc[i][c] = 0ull;
-        // W for pixel s, instances 8 kg .. 8 kg + 7: two float4 at fixed offsets from one base -> no address arithmetic
-        const float* Ws = sm.W[stage] + (2 * kg) * FW_WQ + half * 128 * 4;
+        // W for pixel s, instances 8 ig .. 8 ig + 7: two float4 at fixed offsets from one base -> no address arithmetic
+        const float* Ws = sm.W[stage] + (2 * ig) * FW_WQ + px0 * 4;
+        const GT* Gs = sm.G + px0 * FW_DC + ch;
         // software-pipelined over pixels: the operands of pixel s+1 are in flight while pixel s is multiplied
         ulonglong2 wa = *reinterpret_cast<const ulonglong2*>(Ws);
         ulonglong2 wb = *reinterpret_cast<const ulonglong2*>(Ws + FW_WQ);
         float4 g = ld_g4(Gs);
 #pragma unroll 1
-        for (int s0 = 0; s0 < (kg * 8 < m.nb ? 128 : 0); s0 += 32) {
+        for (int s0 = 0; s0 < npx; s0 += 32) {
             const float* Wb = Ws + s0 * 4;
             const GT* Gb = Gs + s0 * FW_DC;
 #pragma unroll
             for (int u = 0; u < 32; ++u) {
-                const int un = u + 1;   // the prefetch past the last pixel lands in the row pad / G_pad (never used)
+                const int un = u + 1;   // the prefetch past the last pixel lands in the next slice / the row pad / G_pad (never used)
                 const ulonglong2 wa_n = *reinterpret_cast<const ulonglong2*>(Wb + un * 4);
                 const ulonglong2 wb_n = *reinterpret_cast<const ulonglong2*>(Wb + FW_WQ + un * 4);
                 const float4 g_n = ld_g4(Gb + un * FW_DC);
                 const unsigned long long g2[4] = {pack2(g.x, g.x), pack2(g.y, g.y), pack2(g.z, g.z), pack2(g.w, g.w)};
+                // pair operand outermost: consecutive FFMA2 keep the 64-bit weight pair in the operand reuse cache and
+                // stream the broadcast scalar
+                const unsigned long long wp[4] = {wa.x, wa.y, wb.x, wb.y};
 #pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    fma2_acc(acc[0][c], wa.x, g2[c]);
-                    fma2_acc(acc[1][c], wa.y, g2[c]);
-                    fma2_acc(acc[2][c], wb.x, g2[c]);
-                    fma2_acc(acc[3][c], wb.y, g2[c]);
-                }
+                for (int i = 0; i < 4; ++i)
+#pragma unroll
+                    for (int c = 0; c < 4; ++c) fma2_acc(acc[i][c], wp[i], g2[c]);
                 wa = wa_n; wb = wb_n; g = g_n;
             }
         }
-        // den partial: warp (half, cw) sums pixels [128 half + 32 cw, +32) for instance kk = lane
+        WS_TACC(2);
+        if (ngrp < 4) {   // add the pixel slices up (lane groups that share an instance group)
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    float2 v = unpack2(acc[i][c]);
+                    v.x += __shfl_xor_sync(TR_FULL, v.x, 16);
+                    v.y += __shfl_xor_sync(TR_FULL, v.y, 16);
+                    if (ngrp == 1) {
+                        v.x += __shfl_xor_sync(TR_FULL, v.x, 8);
+                        v.y += __shfl_xor_sync(TR_FULL, v.y, 8);
+                    }
+                    acc[i][c] = pack2(v.x, v.y);
+                }
+        }
+        const bool owner = lg < ngrp;   // one lane group per instance group carries the result
+        // den partial: warp (half, cq) sums pixels [128 half + 32 cq, +32) for instance kk = lane
         {
-            const float* Wp = sm.W[stage] + (lane >> 2) * FW_WQ + (half * 128 + cw * 32) * 4 + (lane & 3);
+            const float* Wp = sm.W[stage] + (lane >> 2) * FW_WQ + (half * 128 + cq * 32) * 4 + (lane & 3);
             float d0 = 0.f, d1 = 0.f;
 #pragma unroll
             for (int j = 0; j < 32; j += 2) { d0 += Wp[j * 4]; d1 += Wp[j * 4 + 4]; }
@@ -421,41 +464,46 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT>& sm, const FuseA
         mbar_arrive(&sm.ct.empty[stage]);
         if (m.flags & WS_FLAG_LAST) mbar_arrive(&sm.g_free);
         if (++stage == FW_STAGES) { stage = 0; phase ^= 1u; }
+        WS_TACC(3);
         const bool writer = ((batch & 1u) != 0u) == (half != 0);
-        if (writer) {
+        if (writer && owner) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 const float2 v0 = unpack2(acc[i][0]), v1 = unpack2(acc[i][1]), v2 = unpack2(acc[i][2]), v3 = unpack2(acc[i][3]);
-                *reinterpret_cast<float4*>(&sm.P[(kg * 8 + 2 * i) * FW_DC + ch]) = make_float4(v0.x, v1.x, v2.x, v3.x);
-                *reinterpret_cast<float4*>(&sm.P[(kg * 8 + 2 * i + 1) * FW_DC + ch]) = make_float4(v0.y, v1.y, v2.y, v3.y);
+                *reinterpret_cast<float4*>(&sm.P[(ig * 8 + 2 * i) * FW_DC + ch]) = make_float4(v0.x, v1.x, v2.x, v3.x);
+                *reinterpret_cast<float4*>(&sm.P[(ig * 8 + 2 * i + 1) * FW_DC + ch]) = make_float4(v0.y, v1.y, v2.y, v3.y);
             }
         }
         named_bar_sync(FW_BAR_CONS, WS_CONS);
         if (!writer) {
-            const float4 d0 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][kg * 8]);
-            const float4 d1 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][kg * 8 + 4]);
-            const float dv[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+            if (owner) {
+                const float4 d0 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][ig * 8]);
+                const float4 d1 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][ig * 8 + 4]);
+                const float dv[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const float2 v0 = unpack2(acc[i][0]), v1 = unpack2(acc[i][1]), v2 = unpack2(acc[i][2]), v3 = unpack2(acc[i][3]);
+                for (int i = 0; i < 4; ++i) {
+                    const float2 v0 = unpack2(acc[i][0]), v1 = unpack2(acc[i][1]), v2 = unpack2(acc[i][2]), v3 = unpack2(acc[i][3]);
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    const int k8 = 2 * i + e, kk = kg * 8 + k8;
-                    if (kk < m.nb && dv[k8] != 0.f) {
-                        const float4 pp = *reinterpret_cast<const float4*>(&sm.P[kk * FW_DC + ch]);
-                        const float4 mine = e ? make_float4(v0.y, v1.y, v2.y, v3.y) : make_float4(v0.x, v1.x, v2.x, v3.x);
-                        red_add_v4(a.num + (size_t)id[k8] * a.D + m.c0 + ch,
-                                   make_float4(mine.x + pp.x, mine.y + pp.y, mine.z + pp.z, mine.w + pp.w));
-                        if (m.c0 == 0 && ch == 0) red_add(a.den + id[k8], dv[k8]);
+                    for (int e = 0; e < 2; ++e) {
+                        const int k8 = 2 * i + e, kk = ig * 8 + k8;
+                        if (kk < m.nb && dv[k8] != 0.f) {
+                            const float4 pp = *reinterpret_cast<const float4*>(&sm.P[kk * FW_DC + ch]);
+                            const float4 mine = e ? make_float4(v0.y, v1.y, v2.y, v3.y) : make_float4(v0.x, v1.x, v2.x, v3.x);
+                            red_add_v4(a.num + (size_t)id[k8] * a.D + m.c0 + ch,
+                                       make_float4(mine.x + pp.x, mine.y + pp.y, mine.z + pp.z, mine.w + pp.w));
+                            if (m.c0 == 0 && ch == 0) red_add(a.den + id[k8], dv[k8]);
+                        }
                     }
                 }
             }
             // all four channel warps of this half must have read den_s before it is cleared
             asm volatile("bar.sync %0, %1;" ::"r"(4 + half), "r"(128) : "memory");
-            if (cw == 0) sm.den_s[batch & 1][lane] = 0.f;
+            if (cq == 0) sm.den_s[batch & 1][lane] = 0.f;
         }
+        WS_TACC(4);
         ++batch;
     }
+    WS_TFLUSH(0, tid == 0);
 }
 
 template <typename GT>
@@ -615,16 +663,16 @@ cudaError_t launch(K kernel, size_t smem, int grid, cudaStream_t st, const FuseA
 }
 
 template <typename GT>
-cudaError_t launch_fuse_ws(const FuseArgs& a, int tiles, int num_sms, uint32_t* queue, const uint32_t* order, cudaStream_t st) {
+cudaError_t launch_fuse_ws(const FuseArgs& a, int tiles, int num_sms, uint32_t* ctrl, const uint32_t* order, cudaStream_t st) {
     const size_t smem = sizeof(FuseWsSmem<GT>);
     cudaError_t e = cudaFuncSetAttribute(fuse_ws_kernel<GT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     WsWork wk;
-    wk.queue = queue;
+    wk.queue = ctrl + CTRL_FUSE_QUEUE;
     wk.n_chunks = a.D / FW_DC;
     wk.n_items = tiles * wk.n_chunks;
     wk.order = order;
-    wk.order_valid = queue - CTRL_TILE_QUEUE + CTRL_ORDER_VALID;
+    wk.order_valid = ctrl + CTRL_ORDER_VALID;
     const int grid = wk.n_items < num_sms ? wk.n_items : num_sms;
     fuse_ws_kernel<GT><<<grid, FW_THREADS, smem, st>>>(a, wk);
     return cudaGetLastError();
@@ -633,7 +681,6 @@ cudaError_t launch_fuse_ws(const FuseArgs& a, int tiles, int num_sms, uint32_t* 
 template <typename GT>
 cudaError_t dispatch(const FuseArgs& a, int grid, int num_sms, uint32_t* queue, const uint32_t* order, cudaStream_t st) {
     if (a.D % FW_DC == 0) return launch_fuse_ws<GT>(a, grid, num_sms, queue, order, st);
-    if (a.D % 128 == 0) return launch(fuse_tiled_kernel<128, GT>, sizeof(FuseTiledSmem<128>), grid, st, a);
     if (a.D % 64 == 0) return launch(fuse_tiled_kernel<64, GT>, sizeof(FuseTiledSmem<64>), grid, st, a);
     if (a.D % 16 == 0) return launch(fuse_pixel_kernel<16, GT>, 0, grid, st, a);
     if (a.D % 8 == 0) return launch(fuse_pixel_kernel<8, GT>, 0, grid, st, a);
@@ -641,6 +688,17 @@ cudaError_t dispatch(const FuseArgs& a, int grid, int num_sms, uint32_t* queue, 
 }
 
 }  // namespace
+
+#ifdef FHGS_WS_TIMING
+extern "C" __attribute__((visibility("default"))) int fhgs_debug_fuse_timing(unsigned long long* out32, int reset) {
+    if (out32 && cudaMemcpyFromSymbol(out32, g_ws_timing, sizeof(g_ws_timing)) != cudaSuccess) return 1;
+    if (reset) {
+        unsigned long long z[32] = {0};
+        if (cudaMemcpyToSymbol(g_ws_timing, z, sizeof(z)) != cudaSuccess) return 1;
+    }
+    return 0;
+}
+#endif
 
 extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam, const fhgs_params* prm,
                                           const fhgs_view_state* vs, const void* gt, int32_t feat_dim,
@@ -672,6 +730,7 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
         if (!out_feat) FHGS_INVALID(ctx, "fhgs_fuse_features: FINALIZE needs out_feat");
         if (!aligned_to(out_feat, 16)) FHGS_INVALID(ctx, "fhgs_fuse_features: out_feat must be 16-byte aligned");
     }
+    DeviceGuard dg(ctx);
     cudaStream_t s = (cudaStream_t)stream;
     const size_t n = (size_t)vs->n;
     if (flags & (FHGS_FUSE_ZERO | FHGS_FUSE_ZERO_ONLY)) {
@@ -688,7 +747,7 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
         a.gt = gt; a.D = feat_dim; a.num = num; a.den = den;
         const int grid = tiles_x(cam->width) * tiles_y(cam->height);
         const ScratchLayout L = make_scratch_layout(vs->n, vs->capacity, cam->width, cam->height);
-        uint32_t* queue = reinterpret_cast<uint32_t*>((char*)vs->scratch + L.ctrl) + CTRL_TILE_QUEUE;
+        uint32_t* queue = reinterpret_cast<uint32_t*>((char*)vs->scratch + L.ctrl);
         const uint32_t* order = reinterpret_cast<const uint32_t*>((char*)vs->scratch + L.tile_order);
         cudaError_t e = gt_dtype == FHGS_F16 ? dispatch<__half>(a, grid, ctx->num_sms, queue, order, s)
                                              : dispatch<float>(a, grid, ctx->num_sms, queue, order, s);

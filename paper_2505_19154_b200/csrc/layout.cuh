@@ -16,7 +16,9 @@ enum {
     CTRL_SCAN2_TICKET = 13,   // same, for the index-order offsets scan of the depth-pre-sorted mode
     CTRL_SORT_TICKET = 1,     // [1..8]  dynamic CTA ids, one per instance-sort pass
     CTRL_PRESORT_TICKET = 9,  // [9..12] dynamic CTA ids of the depth pre-sort passes
-    CTRL_TILE_QUEUE = 16,     // render / fuse tile queue heads
+    CTRL_RENDER_QUEUE = 16,   // [16,17] work queue of fhgs_render (next item, finished CTAs; self-resetting)
+    CTRL_FUSE_QUEUE = 18,     // [18,19] work queue of fhgs_fuse_features -- its own, so a render and a fuse on one view
+                              //         state may overlap on two streams
     CTRL_ORDER_VALID = 20,    // 1 when tile_order holds the longest-first tile permutation of this view
     CTRL_WORDS = 64
 };

@@ -249,6 +249,7 @@ extern "C" fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g,
     a.feat = g->feat; a.gt = gt; a.D = D; a.k_sig = k_sigmoid; a.lambda = lambda;
     a.out_lgt = out_lgt; a.out_lcf = out_lcf;
     const int tiles = tiles_x(cam->width) * tiles_y(cam->height);
+    DeviceGuard dg(ctx);
     cudaStream_t s = (cudaStream_t)stream;
     cudaError_t e;
     const bool fh = g->feat_dtype == FHGS_F16, gh = gt_dtype == FHGS_F16;

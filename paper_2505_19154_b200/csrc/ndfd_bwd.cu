@@ -310,6 +310,7 @@ extern "C" fhgs_status fhgs_ndfd_backward(fhgs_ctx* ctx, const fhgs_gaussians* g
     a.B_tot = reinterpret_cast<float*>((char*)work + ((px * 2 * sizeof(float) + 255) / 256) * 256);
     a.grad_op = grad_opacity;
     const int tiles = tiles_x(cam->width) * tiles_y(cam->height);
+    DeviceGuard dg(ctx);
     cudaStream_t s = (cudaStream_t)stream;
     cudaError_t e;
     const bool fh = g->feat_dtype == FHGS_F16, gh = gt_dtype == FHGS_F16;

@@ -271,6 +271,7 @@ extern "C" fhgs_status fhgs_project(fhgs_ctx* ctx, const fhgs_gaussians* g, cons
     a.xy = vs->xy; a.depth = vs->depth; a.conic_opacity = vs->conic_opacity; a.rgb = vs->rgb;
     a.radius = vs->radius; a.rect = vs->rect; a.tiles_touched = vs->tiles_touched;
 
+    DeviceGuard dg(ctx);
     cudaStream_t s = (cudaStream_t)stream;
     cudaError_t e;
     switch (g->sh_degree) {

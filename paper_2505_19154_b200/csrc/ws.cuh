@@ -21,6 +21,21 @@
 #pragma once
 #include "traverse.cuh"
 
+// Development aid (never defined in the product build): -DFHGS_WS_TIMING makes one consumer and one producer thread
+// per CTA accumulate clock64() intervals of their pipeline phases into a device array the TU exports.
+#ifdef FHGS_WS_TIMING
+static __device__ unsigned long long g_ws_timing[32];
+#define WS_TDECL long long ws_t_[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}; long long ws_c_ = clock64()
+#define WS_TACC(slot) do { const long long t__ = clock64(); ws_t_[slot] += t__ - ws_c_; ws_c_ = t__; } while (0)
+#define WS_TCNT(slot) (ws_t_[slot] += 1)
+#define WS_TFLUSH(base, pred) do { if (pred) { for (int i__ = 0; i__ < 16; ++i__) atomicAdd(&g_ws_timing[(base) + i__], (unsigned long long)ws_t_[i__]); } } while (0)
+#else
+#define WS_TDECL do { } while (0)
+#define WS_TACC(slot) do { } while (0)
+#define WS_TCNT(slot) do { } while (0)
+#define WS_TFLUSH(base, pred) do { } while (0)
+#endif
+
 constexpr int WS_CONS = 256;
 constexpr int WS_PROD = 256;
 constexpr int WS_THREADS = WS_CONS + WS_PROD;

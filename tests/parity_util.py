@@ -119,40 +119,124 @@ def check_render(o, g, feat_absmax, tol, pix=None, with_feat=True):
     return worst
 
 
-def gaussians_touching(pr, pix, W):
-    """Per Gaussian, the number of the given pixels that lie inside its radius box."""
-    touched = np.zeros(pr["radius"].shape[0], np.int64)
-    r = pr["radius"].astype(np.float32)
-    vis = r > 0
-    for p in np.asarray(pix):
-        x, y = float(p % W), float(p // W)
-        touched += vis & (np.abs(pr["xy"][:, 0] - x) <= r) & (np.abs(pr["xy"][:, 1] - y) <= r)
-    return touched
+class Borderline:
+    """Borderline fragments of a set of views: fragments whose incoming transmittance T lies within `window`
+    (relative) of t_min, so that the stop test `T < t_min` may legitimately come out differently on the two sides
+    (exp differs by a few ulp between them).  Fragments in front of them are blended by both sides, fragments behind
+    them by neither.  For each: Gaussian index, weight w = alpha*T, whether the ORACLE blended it, and the GT row of
+    its pixel.  Where several results are correct the tests accept each of them -- and nothing else."""
+
+    def __init__(self, n, D):
+        self.n, self.D = n, D
+        self.g, self.w, self.blended, self.G = [], [], [], []
+
+    def add_view(self, pr, pix, W, bins, gt, q_cutoff=9.0, alpha_max=0.9999, t_min=1e-4, window=2e-4):
+        """pix: the view's fragile pixels (oracle flag).  The pixel's fragment sequence is rebuilt from the oracle's
+        projection and its sorted tile list `bins` (fo.bins): binary32 q as C1-R states it, then double."""
+        f32, f64 = np.float32, np.float64
+        gx, gy = pr["xy"][:, 0], pr["xy"][:, 1]
+        co = pr["conic_opacity"]
+        GW = (W + 15) // 16
+        gt2 = gt.reshape(-1, gt.shape[-1])
+        for p in np.asarray(pix):
+            x, y = int(p % W), int(p // W)
+            r0, r1 = bins["ranges"][(y // 16) * GW + x // 16]
+            cand = bins["vals"][int(r0):int(r1)].astype(np.int64)          # front to back
+            if cand.size == 0:
+                continue
+            dx, dy = (gx[cand] - f32(x)).astype(f32), (gy[cand] - f32(y)).astype(f32)
+            A, B2, Cc = co[cand, 0], (f32(2.0) * co[cand, 1]).astype(f32), co[cand, 2]
+            adx = (A * dx).astype(f32)
+            inner = (B2.astype(f64) * dy.astype(f64) + adx.astype(f64)).astype(f32)          # fmaf(2B, dy, A dx)
+            cdy2 = ((Cc * dy).astype(f32) * dy).astype(f32)
+            q = (dx.astype(f64) * inner.astype(f64) + cdy2.astype(f64)).astype(f32)          # fmaf(dx, inner, (C dy) dy)
+            c = q <= f32(q_cutoff)
+            alpha = np.where(c, np.minimum(f64(f32(alpha_max)), co[cand, 3].astype(f64) * np.exp(-0.5 * np.maximum(q.astype(f64), 0.0))), 0.0)
+            T_before = np.concatenate([[1.0], np.cumprod(1.0 - alpha)[:-1]])
+            for j in np.nonzero(c & (np.abs(T_before / t_min - 1.0) <= window))[0]:
+                self.g.append(int(cand[j])); self.w.append(float(alpha[j] * T_before[j]))
+                self.blended.append(bool(T_before[j] >= t_min)); self.G.append(gt2[p].astype(f64))
+
+    def weight_mass(self):
+        """Per Gaussian, the total weight of its borderline fragments."""
+        m = np.zeros(self.n)
+        if self.g:
+            np.add.at(m, np.asarray(self.g), np.asarray(self.w))
+        return m
+
+    def by_gaussian(self):
+        out = {}
+        for j, g in enumerate(self.g):
+            out.setdefault(g, []).append(j)
+        return out
 
 
-def check_fuse(num_o, den_o, num_g, den_g, gt_absmax, tol, fragile_touch=None):
-    """num/den: |d den| <= tol*max(den,1), |d num| <= tol*max(den,1)*|G|max; Gaussians touching a fragile
-    pixel get the extra 1e-4 per fragile pixel that one borderline contributor may add or drop."""
+def check_fuse(num_o, den_o, num_g, den_g, gt_absmax, tol, border=None):
+    """Accumulators, RELATIVE to the row's own weight mass (no absolute floor):
+        |d den_i| <= tol den_i + b_i,   |d num_i|max <= (tol den_i + b_i) |G|max
+    with b_i = 1.01 x the weight mass of Gaussian i's borderline fragments (0 for almost every row).  A row the oracle
+    never blends (den_i = 0) must therefore be exactly zero on the GPU unless it has a borderline fragment."""
     num_g = num_g.cpu().numpy().astype(np.float64)
     den_g = den_g.cpu().numpy().astype(np.float64)
-    scale = np.maximum(den_o, 1.0)
-    extra = np.zeros_like(den_o) if fragile_touch is None else fragile_touch.astype(np.float64) * 1.1e-4
+    b = np.zeros_like(den_o) if border is None else 1.01 * border.weight_mass()
+    bound = tol * den_o + b
     d_den = np.abs(den_g - den_o)
-    assert np.all(d_den <= tol * scale + extra), f"den max err {d_den.max():.3e}"
+    bad = d_den > bound
+    assert not bad.any(), f"den: {int(bad.sum())} rows off, worst {d_den[bad].max():.3e} at den {den_o[bad][np.argmax(d_den[bad])]:.3e}"
     d_num = np.abs(num_g - num_o).max(axis=1)
-    assert np.all(d_num <= (tol * scale + extra) * max(gt_absmax, 1.0)), f"num max err {d_num.max():.3e}"
-    return dict(den=float(d_den.max(initial=0)), num=float(d_num.max(initial=0)))
+    bad = d_num > bound * max(gt_absmax, 1.0)
+    assert not bad.any(), f"num: {int(bad.sum())} rows off, worst {d_num[bad].max():.3e}"
+    live = den_o > 0
+    rel = float((d_den[live] / den_o[live]).max(initial=0.0))
+    return dict(den=float(d_den.max(initial=0)), num=float(d_num.max(initial=0)), den_rel=rel)
 
 
-def check_finalized(f_o, f_g, den_o, tol, den_floor=1e-3, fragile_mask=None):
-    """Finalised vectors within tol for every Gaussian with den >= den_floor that touches no fragile pixel
-    (below the floor one borderline weight of 1e-4 legitimately moves the mean)."""
-    sel = den_o >= den_floor
-    if fragile_mask is not None:
-        sel &= ~(fragile_mask.astype(bool))
-    d = np.abs(f_g.astype(np.float64)[sel] - f_o[sel])
-    assert d.size == 0 or d.max() <= tol, f"fused feature max abs err {d.max():.3e} (tol {tol})"
-    return float(d.max(initial=0)), int(sel.sum())
+def check_finalized(f_o, f_g, prev, num_o, den_o, den_g, tol, den_eps=1e-8, border=None, max_alt=10):
+    """Finalised vectors of EVERY row, no floor on den.  f_o: the oracle's finalised table (prev where not finalised).
+    Rows without borderline fragments: finalised on both sides (den > den_eps; a den within a factor 2 of den_eps may
+    be finalised on one side only and is skipped) and |f_g - f_o|max <= tol, or untouched on both sides.
+    Rows WITH borderline fragments have several correct results: each subset of these fragments blended / not
+    blended gives one (num', den') and f' = num'/den' (or the previous row when den' <= den_eps); f_g must be
+    within tol of one of them.  Returns (worst error over all rows, rows finalised, rows resolved through an
+    alternative, rows with more than `max_alt` borderline fragments = unchecked; the last must be 0)."""
+    f_g = f_g.astype(np.float64)
+    prev = np.asarray(prev, np.float64)
+    den_g = np.asarray(den_g, np.float64)
+    d = np.abs(f_g - f_o).max(axis=1)
+    frag_rows = border.by_gaussian() if border is not None else {}
+    has_frag = np.zeros(den_o.shape[0], bool)
+    if frag_rows:
+        has_frag[np.fromiter(frag_rows.keys(), np.int64)] = True
+    fin_o, fin_g = den_o > den_eps, den_g > den_eps
+    ambiguous = (den_o > 0.5 * den_eps) & (den_o < 2.0 * den_eps)
+    plain = ~has_frag & ~ambiguous
+    assert np.array_equal(fin_o[plain], fin_g[plain]), "a row is finalised on one side only"
+    bad = plain & (d > tol)
+    assert not bad.any(), (f"fused feature: {int(bad.sum())} rows off, worst {d[bad].max():.3e} (tol {tol}) at den "
+                           f"{den_o[bad][np.argmax(d[bad])]:.3e}")
+    worst = float(d[plain].max(initial=0))
+    n_alt = n_unchecked = 0
+    for g, idx in frag_rows.items():
+        if d[g] <= tol and fin_o[g] == fin_g[g]:
+            continue
+        if len(idx) > max_alt:
+            n_unchecked += 1
+            continue
+        n_alt += 1
+        best = np.inf
+        for mask in range(1 << len(idx)):
+            num_a, den_a = num_o[g].copy(), den_o[g]
+            for b, j in enumerate(idx):
+                if mask >> b & 1:       # flip fragment j: remove it if the oracle blended it, else add it
+                    sgn = -1.0 if border.blended[j] else 1.0
+                    num_a += sgn * border.w[j] * border.G[j]
+                    den_a += sgn * border.w[j]
+            f_a = num_a / den_a if den_a > den_eps else prev[g]
+            best = min(best, float(np.abs(f_g[g] - f_a).max()))
+        assert best <= tol, f"fused feature of Gaussian {g}: no valid alternative within tol (best {best:.3e}, den {den_o[g]:.3e})"
+        worst = max(worst, best)
+    assert n_unchecked == 0, f"{n_unchecked} rows with more than {max_alt} borderline fragments"
+    return worst, int(fin_o.sum()), n_alt, n_unchecked
 
 
 def reduced_config(name, **kw):
