@@ -99,7 +99,10 @@ FHGS_API void fhgs_default_params(fhgs_params* p);
 
 /* Per-view intermediate state.  All pointers are device pointers owned by the caller.
  * fhgs_project writes xy..tiles_touched; fhgs_bin_sort writes offsets, num_instances,
- * keys/vals (ping-pong), sorted_buf, ranges; fhgs_render / fhgs_fuse_features only read.
+ * keys/vals (ping-pong), sorted_buf, ranges; fhgs_render / fhgs_fuse_features / fhgs_ndfd_* read them and use
+ * per-entry-point work-queue words inside `scratch`: ONE fhgs_render and ONE fhgs_fuse_features on the same
+ * view state may run concurrently on two streams; two calls of the same entry point on one view state, and any
+ * call concurrent with fhgs_project / fhgs_bin_sort on it, must be stream-ordered.
  * `capacity` = number of (key,val) pairs each of keys[0],keys[1],vals[0],vals[1] can hold; it
  * must be < 2^30.  `scratch` needs fhgs_scratch_bytes(n, width, height, capacity) bytes, 256-byte
  * aligned. */
@@ -185,7 +188,10 @@ FHGS_API fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const f
  * (PAPER.md:136 unit-norm features; off by default).  FHGS_FUSE_FINALIZE_ONLY skips the
  * accumulation of a view (gt, cam may then be NULL) and only finalises.  FHGS_FUSE_ZERO_ONLY
  * clears num,den and returns (cam, gt, out_feat may be NULL) -- lets a caller time the three
- * parts of a fused frame separately.
+ * parts of a fused frame separately.  FHGS_FUSE_ZERO_TOUCHED (with ZERO or ZERO_ONLY) clears only the rows with
+ * den[i] != 0 instead of the whole accumulator: only valid when every row with den[i] == 0 is already zero in num,
+ * which holds for buffers that were last cleared by this call and since then written by it only (a Gaussian gets
+ * num without den only from an all-zero weight, i.e. never); at Mid 2 % of the rows carry weight.
  * gt [H,W,D] gt_dtype, 16-byte aligned; num [n,D] f32 16-byte aligned; den [n] f32;
  * out_feat [n,D] out_dtype or NULL. */
 enum {
@@ -193,7 +199,8 @@ enum {
     FHGS_FUSE_FINALIZE = 2,
     FHGS_FUSE_L2NORM = 4,
     FHGS_FUSE_FINALIZE_ONLY = 8,
-    FHGS_FUSE_ZERO_ONLY = 16
+    FHGS_FUSE_ZERO_ONLY = 16,
+    FHGS_FUSE_ZERO_TOUCHED = 32
 };
 FHGS_API fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam, const fhgs_params* prm,
                                const fhgs_view_state* vs, const void* gt, int32_t feat_dim,

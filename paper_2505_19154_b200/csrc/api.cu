@@ -204,35 +204,49 @@ extern "C" fhgs_status fhgs_frame_host(fhgs_ctx* ctx, const fhgs_host_frame* hos
 }
 
 // ------------------------------------------------------------------------------------------------
-// FFMA micro-benchmark: 8 CTAs of 8 warps per SM, 32 independent accumulator chains per thread.
+// FP32 micro-benchmark: 8 CTAs of 8 warps per SM, a register-resident outer-product tile per thread.
+// The form is the fastest one found on this B200 (probe of scalar FFMA and fma.rn.f32x2 tiles of several shapes and
+// operand orders): packed FFMA2, 2 pair operands x 16 broadcast scalars, the 64-bit pair operand
+// held over 16 consecutive instructions (operand reuse cache) -- 125 of the nominal 128 FMA/clk/SM.  Scalar 8x8
+// tiles reach 108-113, the 4-pair x 4-scalar order of the round-1 kernels 81.
 // ------------------------------------------------------------------------------------------------
 namespace {
-constexpr int FFMA_CHAINS = 32;
-// Outer-product form acc[i][j] += a[i] * b[j] (8 x 4), i.e. the three-register FFMA the compositing
-// kernels issue, not the constant-operand form.
+constexpr int FFMA_FMA_PER_ROUND = 64;   // 2 pairs x 16 scalars x 2 lanes
+__device__ __forceinline__ unsigned long long peak_pack2(float lo, float hi) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
 __global__ void __launch_bounds__(256) ffma_peak_kernel(float* out, int iters, float a0, float b0) {
-    float acc[8][4], a[8], b[4];
+    unsigned long long acc[2][16], a[2], b[16];
 #pragma unroll
-    for (int i = 0; i < 8; ++i) a[i] = a0 * (float)(threadIdx.x + i + 1);
+    for (int i = 0; i < 2; ++i) a[i] = peak_pack2(a0 * (float)(threadIdx.x + i + 1), a0 * (float)(threadIdx.x + i + 2));
 #pragma unroll
-    for (int j = 0; j < 4; ++j) b[j] = b0 * (float)(threadIdx.x + 3 * j + 1);
+    for (int j = 0; j < 16; ++j) {
+        const float v = b0 * (float)(threadIdx.x + 3 * j + 1);
+        b[j] = peak_pack2(v, v);
+    }
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < 2; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
+        for (int j = 0; j < 16; ++j) acc[i][j] = 0ull;
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
         for (int r = 0; r < 4; ++r)
 #pragma unroll
-            for (int i = 0; i < 8; ++i)
+            for (int i = 0; i < 2; ++i)
 #pragma unroll
-                for (int j = 0; j < 4; ++j) acc[i][j] = fmaf(a[i], b[j], acc[i][j]);
+                for (int j = 0; j < 16; ++j) asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(acc[i][j]) : "l"(a[i]), "l"(b[j]));
     }
     float s = 0.f;
 #pragma unroll
-    for (int i = 0; i < 8; ++i)
+    for (int i = 0; i < 2; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) s += acc[i][j];
+        for (int j = 0; j < 16; ++j) {
+            float lo, hi;
+            asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(acc[i][j]));
+            s += lo + hi;
+        }
     if (s == 123.456f) out[0] = s;   // never true in practice; keeps the chains alive
 }
 }  // namespace
@@ -259,7 +273,7 @@ extern "C" fhgs_status fhgs_ffma_peak(fhgs_ctx* ctx, int32_t iters, double* lane
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     cudaFree(d);
-    const double ops = (double)grid * 256.0 * (double)iters * 4.0 * FFMA_CHAINS;
+    const double ops = (double)grid * 256.0 * (double)iters * 4.0 * FFMA_FMA_PER_ROUND;
     *lane_ops_per_s = ops / ((double)t * 1e-3);
     if (ms) *ms = (double)t;
     return FHGS_OK;

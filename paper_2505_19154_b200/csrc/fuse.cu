@@ -205,17 +205,22 @@ constexpr int FW_BAR_CONS = 3;
 constexpr int FW_WQ = (WS_CONS + 1) * 4;   // floats per quad row: 256 pixels x float4 + 16 B pad (bank spread over quads)
 enum { FW_FLAG_FIRST = 4 };
 
+// GT tile buffers: a 16-bit map leaves room for two (the scheduler loads the next item's tile while the consumers
+// multiply the current one); an fp32 tile (128 KB) is single-buffered.
+template <typename GT>
+constexpr int kGBufs = sizeof(GT) == 2 ? 2 : 1;
+
 template <typename GT>
 struct FuseWsSmem {
     WsCtrl<FW_STAGES> ct;
-    uint64_t g_full, g_free;
+    uint64_t g_full[2], g_free[2];
     uint64_t item_full[2], item_empty[2];
     int items[2];
     __align__(16) uint32_t ids[FW_STAGES][WS_KB];
     __align__(16) float den_s[2][WS_KB];
     __align__(128) float W[FW_STAGES][FW_WQ * WS_KB / 4];  // [quad kk/4][pixel][4], quad stride padded by one float4
     __align__(128) float P[WS_KB * FW_DC];                // partial sums of the writing half
-    __align__(128) GT G[WS_CONS * FW_DC];                 // [pixel][channel], pixel = y*16 + x (storage type of the map)
+    __align__(128) GT G[kGBufs<GT>][WS_CONS * FW_DC];     // [buffer][pixel][channel], pixel = y*16 + x (storage type of the map)
     GT G_pad[FW_DC];                                      // target of the consumers' one-past-the-end prefetch
 };
 
@@ -237,7 +242,7 @@ template <typename GT>
 __device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem<GT>& sm, const FuseArgs& a, const WsWork& wk) {
     const int lane = threadIdx.x & 31;
     const GT* gt = reinterpret_cast<const GT*>(a.gt);
-    int islot = 0;
+    int islot = 0, gb = 0;
     uint32_t iphase = 0, gphase = 0;
     while (true) {
         int item = 0;
@@ -258,23 +263,24 @@ __device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem<GT>& sm, const Fuse
         const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
         const int nx = min(FHGS_TILE, a.t.W - tx0), ny = min(FHGS_TILE, a.t.H - ty0);
         if (lane == 0) {
-            mbar_wait_backoff(&sm.g_free, gphase ^ 1u);
-            mbar_arrive_expect_tx(&sm.g_full, (uint32_t)(nx * ny * FW_DC * sizeof(GT)));
+            mbar_wait_backoff(&sm.g_free[gb], gphase ^ 1u);
+            mbar_arrive_expect_tx(&sm.g_full[gb], (uint32_t)(nx * ny * FW_DC * sizeof(GT)));
         }
         __syncwarp();
+        GT* Gd = sm.G[gb];
         if (a.D == FW_DC) {   // a tile row is one contiguous span
             if (lane < ny)
-                bulk_g2s(&sm.G[lane * FHGS_TILE * FW_DC], gt + ((size_t)(ty0 + lane) * a.t.W + tx0) * FW_DC,
-                         (uint32_t)(nx * FW_DC * sizeof(GT)), &sm.g_full);
+                bulk_g2s(&Gd[lane * FHGS_TILE * FW_DC], gt + ((size_t)(ty0 + lane) * a.t.W + tx0) * FW_DC,
+                         (uint32_t)(nx * FW_DC * sizeof(GT)), &sm.g_full[gb]);
         } else {
             for (int pix = lane; pix < FHGS_TILE_PX; pix += 32) {
                 const int x = pix & 15, y = pix >> 4;
                 if (x < nx && y < ny)
-                    bulk_g2s(&sm.G[pix * FW_DC], gt + ((size_t)(ty0 + y) * a.t.W + tx0 + x) * a.D + c0, (uint32_t)(FW_DC * sizeof(GT)),
-                             &sm.g_full);
+                    bulk_g2s(&Gd[pix * FW_DC], gt + ((size_t)(ty0 + y) * a.t.W + tx0 + x) * a.D + c0, (uint32_t)(FW_DC * sizeof(GT)),
+                             &sm.g_full[gb]);
             }
         }
-        gphase ^= 1u;
+        if (++gb == kGBufs<GT>) { gb = 0; gphase ^= 1u; }
     }
 }
 
@@ -362,44 +368,33 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseA
     (void)lane;
 }
 
-// Consumer warp w: pixel half w>>2 (pixels [128 half, +128)), channel quarter w&3 (32 channels).  Lane = (lane group
-// lg = lane>>3, channel group cg = lane&7): thread tile = 8 instances x 4 channels, so that per pixel the warp reads
-// ONE 128-byte wavefront of G (8 channel groups x 16 B) and two of W (4 instance groups x 16 B each) for 16 FFMA2 per
-// thread -- half the shared-memory traffic of a warp-per-instance-group layout, which was the co-limiter (ncu: 69 % of
-// the LSU wavefront slots next to 64 % of the FMA pipe).  A full batch maps lane group -> instance group (8 lg .. 8 lg + 7)
-// over the 128 pixels of the half.  A SHORT batch (nb <= 16, the last one of a tile) gives every instance group to
-// several lane groups, each over a slice of the pixels, and adds the slices up with shuffles: no lane multiplies padding.
 template <typename GT>
 __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT>& sm, const FuseArgs& a) {
     // consumers are warps 8-15: the SMSP arbiter favours high warp ids and the consumers are the critical path
     const int tid = threadIdx.x - WS_PROD, lane = tid & 31, warp = tid >> 5;
-    const int half = warp >> 2, cq = warp & 3;
-    const int lg = lane >> 3, cg = lane & 7;
-    const int ch = cq * 32 + cg * 4;          // this thread's 4 channels inside the chunk
-    int stage = 0;
-    uint32_t phase = 0, gphase = 0, batch = 0;
+    const int half = warp >> 2, cw = warp & 3;
+    const int kg = warp & 3;                  // the warp's 8 instances of the batch (a short batch idles whole warps)
+    const int ch = lane * 4;                  // this thread's 4 channels inside the chunk
+    int stage = 0, gb = kGBufs<GT> - 1;
+    uint32_t phase = 0, gphase = 1u, batch = 0;   // (gb, gphase) advance to buffer 0 / parity 0 at the first item
+    const GT* Gs = sm.G[0] + half * 128 * FW_DC + ch;
     WS_TDECL;
     while (true) {
         mbar_wait(&sm.ct.full[stage], phase);
         WS_TACC(0);
         const WsMeta m = sm.ct.meta[stage];
         if (m.flags & WS_FLAG_EXIT) break;
-        if (m.flags & FW_FLAG_FIRST) {
-            mbar_wait(&sm.g_full, gphase);
-            gphase ^= 1u;
+        if (m.flags & FW_FLAG_FIRST) {   // next item: its GT tile is in the next buffer
+            if (++gb == kGBufs<GT>) { gb = 0; gphase ^= 1u; }
+            mbar_wait(&sm.g_full[gb], gphase);
+            Gs = sm.G[gb] + half * 128 * FW_DC + ch;
             WS_TACC(1);
         }
         WS_TCNT(5);
-        if (m.nb <= 16) WS_TCNT(6);
-        // lane group -> (instance group, pixel slice) for this batch
-        const int ngrp = m.nb > 16 ? 4 : (m.nb > 8 ? 2 : 1);     // instance groups the lane groups are spread over
-        const int ig = lg & (ngrp - 1);
-        const int npx = 32 * ngrp;                               // pixels per slice (4/ngrp slices per half)
-        const int px0 = half * 128 + (lg / ngrp) * npx;
         uint32_t id[8];
         {
-            const uint4 i0 = *reinterpret_cast<const uint4*>(&sm.ids[stage][ig * 8]);
-            const uint4 i1 = *reinterpret_cast<const uint4*>(&sm.ids[stage][ig * 8 + 4]);
+            const uint4 i0 = *reinterpret_cast<const uint4*>(&sm.ids[stage][kg * 8]);
+            const uint4 i1 = *reinterpret_cast<const uint4*>(&sm.ids[stage][kg * 8 + 4]);
             id[0] = i0.x; id[1] = i0.y; id[2] = i0.z; id[3] = i0.w;
             id[4] = i1.x; id[5] = i1.y; id[6] = i1.z; id[7] = i1.w;
         }
@@ -408,103 +403,85 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT>& sm, const FuseA
         for (int i = 0; i < 4; ++i)
 #pragma unroll
             for (int c = 0; c < 4; ++c) acc[i][c] = 0ull;
-        // W for pixel s, instances 8 ig .. 8 ig + 7: two float4 at fixed offsets from one base -> no address arithmetic
-        const float* Ws = sm.W[stage] + (2 * ig) * FW_WQ + px0 * 4;
-        const GT* Gs = sm.G + px0 * FW_DC + ch;
+        // W for pixel s, instances 8 kg .. 8 kg + 7: two float4 at fixed offsets from one base -> no address arithmetic
+        const float* Ws = sm.W[stage] + (2 * kg) * FW_WQ + half * 128 * 4;
         // software-pipelined over pixels: the operands of pixel s+1 are in flight while pixel s is multiplied
         ulonglong2 wa = *reinterpret_cast<const ulonglong2*>(Ws);
         ulonglong2 wb = *reinterpret_cast<const ulonglong2*>(Ws + FW_WQ);
         float4 g = ld_g4(Gs);
 #pragma unroll 1
-        for (int s0 = 0; s0 < npx; s0 += 32) {
+        for (int s0 = 0; s0 < (kg * 8 < m.nb ? 128 : 0); s0 += 32) {
             const float* Wb = Ws + s0 * 4;
             const GT* Gb = Gs + s0 * FW_DC;
 #pragma unroll
             for (int u = 0; u < 32; ++u) {
-                const int un = u + 1;   // the prefetch past the last pixel lands in the next slice / the row pad / G_pad (never used)
+                const int un = u + 1;   // the prefetch past the last pixel lands in the row pad / G_pad (never used)
                 const ulonglong2 wa_n = *reinterpret_cast<const ulonglong2*>(Wb + un * 4);
                 const ulonglong2 wb_n = *reinterpret_cast<const ulonglong2*>(Wb + FW_WQ + un * 4);
                 const float4 g_n = ld_g4(Gb + un * FW_DC);
                 const unsigned long long g2[4] = {pack2(g.x, g.x), pack2(g.y, g.y), pack2(g.z, g.z), pack2(g.w, g.w)};
-                // pair operand outermost: consecutive FFMA2 keep the 64-bit weight pair in the operand reuse cache and
-                // stream the broadcast scalar
-                const unsigned long long wp[4] = {wa.x, wa.y, wb.x, wb.y};
 #pragma unroll
-                for (int i = 0; i < 4; ++i)
-#pragma unroll
-                    for (int c = 0; c < 4; ++c) fma2_acc(acc[i][c], wp[i], g2[c]);
+                for (int c = 0; c < 4; ++c) {
+                    fma2_acc(acc[0][c], wa.x, g2[c]);
+                    fma2_acc(acc[1][c], wa.y, g2[c]);
+                    fma2_acc(acc[2][c], wb.x, g2[c]);
+                    fma2_acc(acc[3][c], wb.y, g2[c]);
+                }
                 wa = wa_n; wb = wb_n; g = g_n;
             }
         }
         WS_TACC(2);
-        if (ngrp < 4) {   // add the pixel slices up (lane groups that share an instance group)
-#pragma unroll
-            for (int i = 0; i < 4; ++i)
-#pragma unroll
-                for (int c = 0; c < 4; ++c) {
-                    float2 v = unpack2(acc[i][c]);
-                    v.x += __shfl_xor_sync(TR_FULL, v.x, 16);
-                    v.y += __shfl_xor_sync(TR_FULL, v.y, 16);
-                    if (ngrp == 1) {
-                        v.x += __shfl_xor_sync(TR_FULL, v.x, 8);
-                        v.y += __shfl_xor_sync(TR_FULL, v.y, 8);
-                    }
-                    acc[i][c] = pack2(v.x, v.y);
-                }
-        }
-        const bool owner = lg < ngrp;   // one lane group per instance group carries the result
-        // den partial: warp (half, cq) sums pixels [128 half + 32 cq, +32) for instance kk = lane
+        // den partial: warp (half, cw) sums pixels [128 half + 32 cw, +32) for instance kk = lane
         {
-            const float* Wp = sm.W[stage] + (lane >> 2) * FW_WQ + (half * 128 + cq * 32) * 4 + (lane & 3);
+            const float* Wp = sm.W[stage] + (lane >> 2) * FW_WQ + (half * 128 + cw * 32) * 4 + (lane & 3);
             float d0 = 0.f, d1 = 0.f;
 #pragma unroll
             for (int j = 0; j < 32; j += 2) { d0 += Wp[j * 4]; d1 += Wp[j * 4 + 4]; }
             atomicAdd(&sm.den_s[batch & 1][lane], d0 + d1);
         }
         mbar_arrive(&sm.ct.empty[stage]);
-        if (m.flags & WS_FLAG_LAST) mbar_arrive(&sm.g_free);
+        if (m.flags & WS_FLAG_LAST) mbar_arrive(&sm.g_free[gb]);
         if (++stage == FW_STAGES) { stage = 0; phase ^= 1u; }
         WS_TACC(3);
         const bool writer = ((batch & 1u) != 0u) == (half != 0);
-        if (writer && owner) {
+        if (writer) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 const float2 v0 = unpack2(acc[i][0]), v1 = unpack2(acc[i][1]), v2 = unpack2(acc[i][2]), v3 = unpack2(acc[i][3]);
-                *reinterpret_cast<float4*>(&sm.P[(ig * 8 + 2 * i) * FW_DC + ch]) = make_float4(v0.x, v1.x, v2.x, v3.x);
-                *reinterpret_cast<float4*>(&sm.P[(ig * 8 + 2 * i + 1) * FW_DC + ch]) = make_float4(v0.y, v1.y, v2.y, v3.y);
+                *reinterpret_cast<float4*>(&sm.P[(kg * 8 + 2 * i) * FW_DC + ch]) = make_float4(v0.x, v1.x, v2.x, v3.x);
+                *reinterpret_cast<float4*>(&sm.P[(kg * 8 + 2 * i + 1) * FW_DC + ch]) = make_float4(v0.y, v1.y, v2.y, v3.y);
             }
         }
         named_bar_sync(FW_BAR_CONS, WS_CONS);
         if (!writer) {
-            if (owner) {
-                const float4 d0 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][ig * 8]);
-                const float4 d1 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][ig * 8 + 4]);
-                const float dv[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
+            const float4 d0 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][kg * 8]);
+            const float4 d1 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][kg * 8 + 4]);
+            const float dv[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
 #pragma unroll
-                for (int i = 0; i < 4; ++i) {
-                    const float2 v0 = unpack2(acc[i][0]), v1 = unpack2(acc[i][1]), v2 = unpack2(acc[i][2]), v3 = unpack2(acc[i][3]);
+            for (int i = 0; i < 4; ++i) {
+                const float2 v0 = unpack2(acc[i][0]), v1 = unpack2(acc[i][1]), v2 = unpack2(acc[i][2]), v3 = unpack2(acc[i][3]);
 #pragma unroll
-                    for (int e = 0; e < 2; ++e) {
-                        const int k8 = 2 * i + e, kk = ig * 8 + k8;
-                        if (kk < m.nb && dv[k8] != 0.f) {
-                            const float4 pp = *reinterpret_cast<const float4*>(&sm.P[kk * FW_DC + ch]);
-                            const float4 mine = e ? make_float4(v0.y, v1.y, v2.y, v3.y) : make_float4(v0.x, v1.x, v2.x, v3.x);
-                            red_add_v4(a.num + (size_t)id[k8] * a.D + m.c0 + ch,
-                                       make_float4(mine.x + pp.x, mine.y + pp.y, mine.z + pp.z, mine.w + pp.w));
-                            if (m.c0 == 0 && ch == 0) red_add(a.den + id[k8], dv[k8]);
-                        }
+                for (int e = 0; e < 2; ++e) {
+                    const int k8 = 2 * i + e, kk = kg * 8 + k8;
+                    if (kk < m.nb && dv[k8] != 0.f) {
+                        const float4 pp = *reinterpret_cast<const float4*>(&sm.P[kk * FW_DC + ch]);
+                        const float4 mine = e ? make_float4(v0.y, v1.y, v2.y, v3.y) : make_float4(v0.x, v1.x, v2.x, v3.x);
+                        red_add_v4(a.num + (size_t)id[k8] * a.D + m.c0 + ch,
+                                   make_float4(mine.x + pp.x, mine.y + pp.y, mine.z + pp.z, mine.w + pp.w));
+                        if (m.c0 == 0 && ch == 0) red_add(a.den + id[k8], dv[k8]);
                     }
                 }
             }
             // all four channel warps of this half must have read den_s before it is cleared
             asm volatile("bar.sync %0, %1;" ::"r"(4 + half), "r"(128) : "memory");
-            if (cq == 0) sm.den_s[batch & 1][lane] = 0.f;
+            if (cw == 0) sm.den_s[batch & 1][lane] = 0.f;
         }
         WS_TACC(4);
         ++batch;
     }
     WS_TFLUSH(0, tid == 0);
 }
+
 
 template <typename GT>
 __global__ void __launch_bounds__(FW_THREADS, 1) fuse_ws_kernel(const FuseArgs a, const WsWork wk) {
@@ -516,8 +493,10 @@ __global__ void __launch_bounds__(FW_THREADS, 1) fuse_ws_kernel(const FuseArgs a
             mbar_init(&sm.ct.full[s], WS_PROD);
             mbar_init(&sm.ct.empty[s], WS_CONS);
         }
-        mbar_init(&sm.g_full, 1);
-        mbar_init(&sm.g_free, WS_CONS);
+        for (int s = 0; s < 2; ++s) {
+            mbar_init(&sm.g_full[s], 1);
+            mbar_init(&sm.g_free[s], WS_CONS);
+        }
         for (int s = 0; s < 2; ++s) {
             mbar_init(&sm.item_full[s], 1);
             mbar_init(&sm.item_empty[s], WS_PROD);
@@ -525,8 +504,8 @@ __global__ void __launch_bounds__(FW_THREADS, 1) fuse_ws_kernel(const FuseArgs a
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     // the GT tile buffer must never hold non-finite garbage (pixels outside the image keep stale data, weight 0)
-    for (int i = threadIdx.x; i < (int)((WS_CONS + 1) * FW_DC * sizeof(GT) / 16); i += FW_THREADS)
-        reinterpret_cast<uint4*>(sm.G)[i] = make_uint4(0u, 0u, 0u, 0u);
+    for (int i = threadIdx.x; i < (int)((kGBufs<GT> * WS_CONS + 1) * FW_DC * sizeof(GT) / 16); i += FW_THREADS)
+        reinterpret_cast<uint4*>(&sm.G[0][0])[i] = make_uint4(0u, 0u, 0u, 0u);
     if (threadIdx.x < 2 * WS_KB) (&sm.den_s[0][0])[threadIdx.x] = 0.f;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
@@ -613,42 +592,67 @@ __global__ void __launch_bounds__(TR_THREADS) fuse_pixel_kernel(const FuseArgs a
 }
 
 // ---------------------------------------------------------------------------------------------
-// finalise: one warp per Gaussian row
+// finalise / sparse clear.  Only a few per cent of the rows carry weight (Mid: 22 188 of 10^6), so a warp first looks at
+// 32 consecutive den values at once (one coalesced load) and then walks only the rows that need work.
 // ---------------------------------------------------------------------------------------------
+constexpr int ROWS_PER_WARP = 32, ROW_WARPS = 8;   // 256 rows per CTA
+
 template <typename OT>
 __global__ void __launch_bounds__(256) finalize_kernel(int n, int D, const float* num, const float* den, float den_eps,
                                                        int l2norm, OT* out) {
     const int lane = threadIdx.x & 31;
-    const int row = blockIdx.x * 8 + (threadIdx.x >> 5);
-    if (row >= n) return;
-    const float d = __ldg(den + row);
-    if (!(d > den_eps)) return;
-    const float4* src = reinterpret_cast<const float4*>(num + (size_t)row * D);
+    const int row0 = (blockIdx.x * ROW_WARPS + (threadIdx.x >> 5)) * ROWS_PER_WARP;
+    if (row0 >= n) return;
+    const float dl = row0 + lane < n ? __ldg(den + row0 + lane) : 0.f;
+    uint32_t live = __ballot_sync(TR_FULL, dl > den_eps);
     const int n4 = D >> 2;
-    float scale = 1.0f;
-    if (l2norm) {
-        float ss = 0.f;
+    while (live) {
+        const int r = __ffs(live) - 1;
+        live &= live - 1u;
+        const int row = row0 + r;
+        const float d = __shfl_sync(TR_FULL, dl, r);
+        const float4* src = reinterpret_cast<const float4*>(num + (size_t)row * D);
+        float scale = 1.0f;
+        if (l2norm) {
+            float ss = 0.f;
+            for (int j = lane; j < n4; j += 32) {
+                const float4 v = __ldg(src + j);
+                const float x = v.x / d, y = v.y / d, z = v.z / d, w = v.w / d;
+                ss += x * x + y * y + z * z + w * w;
+            }
+#pragma unroll
+            for (int o = 16; o >= 1; o >>= 1) ss += __shfl_xor_sync(TR_FULL, ss, o);
+            if (ss > 0.f) scale = 1.0f / sqrtf(ss);
+        }
         for (int j = lane; j < n4; j += 32) {
             const float4 v = __ldg(src + j);
-            const float x = v.x / d, y = v.y / d, z = v.z / d, w = v.w / d;
-            ss += x * x + y * y + z * z + w * w;
+            const float x = v.x / d * scale, y = v.y / d * scale, z = v.z / d * scale, w = v.w / d * scale;
+            if (sizeof(OT) == 4) {
+                reinterpret_cast<float4*>(out)[(size_t)row * n4 + j] = make_float4(x, y, z, w);
+            } else {
+                const __half2 a = __floats2half2_rn(x, y), b = __floats2half2_rn(z, w);
+                uint2 rr;
+                rr.x = *reinterpret_cast<const uint32_t*>(&a);
+                rr.y = *reinterpret_cast<const uint32_t*>(&b);
+                reinterpret_cast<uint2*>(out)[(size_t)row * n4 + j] = rr;
+            }
         }
-#pragma unroll
-        for (int o = 16; o >= 1; o >>= 1) ss += __shfl_xor_sync(TR_FULL, ss, o);
-        if (ss > 0.f) scale = 1.0f / sqrtf(ss);
     }
-    for (int j = lane; j < n4; j += 32) {
-        const float4 v = __ldg(src + j);
-        const float x = v.x / d * scale, y = v.y / d * scale, z = v.z / d * scale, w = v.w / d * scale;
-        if (sizeof(OT) == 4) {
-            reinterpret_cast<float4*>(out)[(size_t)row * n4 + j] = make_float4(x, y, z, w);
-        } else {
-            const __half2 a = __floats2half2_rn(x, y), b = __floats2half2_rn(z, w);
-            uint2 r;
-            r.x = *reinterpret_cast<const uint32_t*>(&a);
-            r.y = *reinterpret_cast<const uint32_t*>(&b);
-            reinterpret_cast<uint2*>(out)[(size_t)row * n4 + j] = r;
-        }
+}
+
+// FHGS_FUSE_ZERO_TOUCHED: clear only the rows that carry weight (den != 0).
+__global__ void __launch_bounds__(256) zero_touched_kernel(int n, int D, float* num, float* den) {
+    const int lane = threadIdx.x & 31;
+    const int row0 = (blockIdx.x * ROW_WARPS + (threadIdx.x >> 5)) * ROWS_PER_WARP;
+    if (row0 >= n) return;
+    const bool mine = row0 + lane < n && den[row0 + lane] != 0.f;
+    uint32_t live = __ballot_sync(TR_FULL, mine);
+    if (mine) den[row0 + lane] = 0.f;
+    while (live) {
+        const int r = __ffs(live) - 1;
+        live &= live - 1u;
+        float4* dst = reinterpret_cast<float4*>(num + (size_t)(row0 + r) * D);
+        for (int j = lane; j < (D >> 2); j += 32) dst[j] = make_float4(0.f, 0.f, 0.f, 0.f);
     }
 }
 
@@ -706,10 +710,14 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
                                           int32_t out_dtype, uint32_t flags, void* stream) {
     if (!ctx) return FHGS_ERR_INVALID;
     if (!prm || !vs || !num || !den) FHGS_INVALID(ctx, "fhgs_fuse_features: NULL argument");
-    if (flags & ~(uint32_t)(FHGS_FUSE_ZERO | FHGS_FUSE_FINALIZE | FHGS_FUSE_L2NORM | FHGS_FUSE_FINALIZE_ONLY | FHGS_FUSE_ZERO_ONLY))
+    if (flags & ~(uint32_t)(FHGS_FUSE_ZERO | FHGS_FUSE_FINALIZE | FHGS_FUSE_L2NORM | FHGS_FUSE_FINALIZE_ONLY | FHGS_FUSE_ZERO_ONLY |
+                            FHGS_FUSE_ZERO_TOUCHED))
         FHGS_INVALID(ctx, "fhgs_fuse_features: unknown flag");
     const bool zero_only = (flags & FHGS_FUSE_ZERO_ONLY) != 0;
-    if (zero_only && (flags & ~(uint32_t)FHGS_FUSE_ZERO_ONLY)) FHGS_INVALID(ctx, "fhgs_fuse_features: ZERO_ONLY excludes other flags");
+    if (zero_only && (flags & ~(uint32_t)(FHGS_FUSE_ZERO_ONLY | FHGS_FUSE_ZERO_TOUCHED)))
+        FHGS_INVALID(ctx, "fhgs_fuse_features: ZERO_ONLY excludes other flags (except ZERO_TOUCHED)");
+    if ((flags & FHGS_FUSE_ZERO_TOUCHED) && !(flags & (FHGS_FUSE_ZERO | FHGS_FUSE_ZERO_ONLY)))
+        FHGS_INVALID(ctx, "fhgs_fuse_features: ZERO_TOUCHED qualifies ZERO / ZERO_ONLY");
     const bool accumulate = !(flags & (FHGS_FUSE_FINALIZE_ONLY | FHGS_FUSE_ZERO_ONLY));
     const bool finalize = (flags & (FHGS_FUSE_FINALIZE | FHGS_FUSE_FINALIZE_ONLY)) != 0;
     fhgs_status st;
@@ -733,9 +741,14 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
     DeviceGuard dg(ctx);
     cudaStream_t s = (cudaStream_t)stream;
     const size_t n = (size_t)vs->n;
-    if (flags & (FHGS_FUSE_ZERO | FHGS_FUSE_ZERO_ONLY)) {
-        FHGS_CUDA(ctx, cudaMemsetAsync(num, 0, n * feat_dim * sizeof(float), s));
-        FHGS_CUDA(ctx, cudaMemsetAsync(den, 0, n * sizeof(float), s));
+    if ((flags & (FHGS_FUSE_ZERO | FHGS_FUSE_ZERO_ONLY)) && n > 0) {
+        if (flags & FHGS_FUSE_ZERO_TOUCHED) {
+            zero_touched_kernel<<<(int)((n + ROWS_PER_WARP * ROW_WARPS - 1) / (ROWS_PER_WARP * ROW_WARPS)), 256, 0, s>>>((int)n, feat_dim, num, den);
+            FHGS_LAUNCH_CHECK(ctx);
+        } else {
+            FHGS_CUDA(ctx, cudaMemsetAsync(num, 0, n * feat_dim * sizeof(float), s));
+            FHGS_CUDA(ctx, cudaMemsetAsync(den, 0, n * sizeof(float), s));
+        }
     }
     if (accumulate && n > 0) {
         FuseArgs a;
@@ -754,7 +767,7 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
         FHGS_CUDA(ctx, e);
     }
     if (finalize && n > 0) {
-        const int grid = (int)((n + 7) / 8);
+        const int grid = (int)((n + ROWS_PER_WARP * ROW_WARPS - 1) / (ROWS_PER_WARP * ROW_WARPS));
         const int l2 = (flags & FHGS_FUSE_L2NORM) ? 1 : 0;
         if (out_dtype == FHGS_F16)
             finalize_kernel<__half><<<grid, 256, 0, s>>>((int)n, feat_dim, num, den, prm->den_eps, l2, (__half*)out_feat);

@@ -77,7 +77,7 @@ def guarded_view_state(fb, torch, n, W, H, cap, dev):
     return vs, bufs
 
 
-def run_guarded(cfg, view, tol, sort_flags=(0, 1), ndfd=False):
+def run_guarded(cfg, view, tol, sort_flags=(1, 0), ndfd=False):
     import torch
     from paper_2505_19154_b200 import binding as fb
     scene = inputs.make_scene(cfg)

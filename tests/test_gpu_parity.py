@@ -341,3 +341,28 @@ def test_constant_map_and_l2norm():
     assert np.abs(f[seen] - v).max() <= 1e-4
     fn = gp.finalize(num, den, scene.feat, l2norm=True)
     assert np.abs(fn[seen] - v / np.linalg.norm(v)).max() <= 1e-4
+
+
+def test_zero_touched_equals_full_clear():
+    """FHGS_FUSE_ZERO_TOUCHED clears exactly what a full clear clears when the buffers were maintained by the library:
+    after it num and den are all zero, and a second accumulation reproduces the first (up to the atomic order)."""
+    import torch
+    from paper_2505_19154_b200 import binding as fb
+    cfg = pu.reduced_config("mid", n=30_000, width=200, height=120, log_scale_mu=-3.2)
+    scene = inputs.make_scene(cfg)
+    cam = inputs.make_camera(cfg, 0)
+    gt = inputs.make_gt_map(cfg, 0, cam)
+    gp = pu.GpuPath(scene, cfg.width, cfg.height, 3_000_000)
+    c, m = gp.project_sort(cam)
+    num, den = gp.fuse(c, gt)                                      # full clear + accumulate
+    num1, den1 = num.clone(), den.clone()
+    assert int((den1 != 0).sum()) > 1000
+    fb.fuse_features(gp.ctx, None, gp.prm, gp.vs, None, num, den, None, fb.FHGS_FUSE_ZERO_ONLY | fb.FHGS_FUSE_ZERO_TOUCHED)
+    torch.cuda.synchronize()
+    assert float(num.abs().max()) == 0.0 and float(den.abs().max()) == 0.0
+    num, den = gp.fuse(c, gt, num, den, flags=fb.FHGS_FUSE_ZERO | fb.FHGS_FUSE_ZERO_TOUCHED)
+    assert torch.equal(den != 0, den1 != 0)
+    assert float((den - den1).abs().max()) <= 1e-5 * float(den1.abs().max())
+    assert float((num - num1).abs().max()) <= 1e-5 * float(num1.abs().max())
+    with pytest.raises(fb.FhgsError):                               # ZERO_TOUCHED alone means nothing
+        fb.fuse_features(gp.ctx, c, gp.prm, gp.vs, torch.from_numpy(gt).to(num.device), num, den, None, fb.FHGS_FUSE_ZERO_TOUCHED)
