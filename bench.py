@@ -223,7 +223,7 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
     ctx = fb.Context(local_rank)
     g = fb.Gaussians(scene.mean, scene.scale, scene.quat, scene.opacity, scene.sh, scene.feat, scene.sh_degree, device=dev)
     vs = fb.ViewState(n, W, H, capacity, device=dev)
-    prm = fb.default_params()
+    prm = fb.default_params(rect_mode=1 if args.rect == 'tight' else 0)
     cam = fb.make_camera(cam_np.view, cam_np.proj, cam_np.cam_pos, W, H)
     f32 = torch.float32
     gt = torch.from_numpy(gt_np).to(dev)
@@ -370,6 +370,15 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
         nops = 7 * n_eval_total + (3 * D + 12) * n_contrib_total
         ndfd = {"ms": nms, "frac_of_nominal_fp32": nops / (nms * 1e-3) / alu_nominal,
                 "mean_lgt": float(lgt.mean().item()), "mean_lcf": float(lcf.mean().item())}
+        for _ in range(2):
+            fb.ndfd_forward(ctx, g, cam, prm, vs, gt, lgt, lcf, mode=fb.FHGS_NDFD_FAR_TO_NEAR)
+        ev[0].record(stream)
+        for _ in range(5):
+            fb.ndfd_forward(ctx, g, cam, prm, vs, gt, lgt, lcf, mode=fb.FHGS_NDFD_FAR_TO_NEAR)
+        ev[1].record(stream)
+        torch.cuda.synchronize()
+        ndfd["far_to_near_ms"] = ev[0].elapsed_time(ev[1]) / 5   # one more D-vector per pixel: (4 D + 12) n_contrib lane-ops
+        ndfd["far_to_near_mean_lcf"] = float(lcf.mean().item())
         gop = torch.zeros((n,), dtype=f32, device=dev)
         work = fb.ndfd_backward(ctx, g, cam, prm, vs, gt, gop)
         ev[0].record(stream)
@@ -419,6 +428,7 @@ def run_cuda(args, rank: int, world: int, local_rank: int):
                 "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": f"mid: N={n} SH{scene.sh_degree} D={D} f32, 1 view {W}x{H} + one {W}x{H}x{D} GT map"
+                                       + (" [--rect tight: NEXT-4 (i) variant, not the bench line]" if args.rect == "tight" else "")
                                        + (" [--small debug size, not a bench line]" if args.small else ""),
                            "instances_M": M, "visible": n_vis, "contributors_per_px": n_contrib_total / (W * H),
                            "evaluated_per_px": n_eval_total / (W * H),
@@ -460,7 +470,7 @@ def run_cuda_workload(args, local_rank: int):
     cams = [fb.make_camera(c.view, c.proj, c.cam_pos, W, H) for c in cams_np]
     ctx = fb.Context(local_rank)
     g = fb.Gaussians(scene.mean, scene.scale, scene.quat, scene.opacity, scene.sh, scene.feat, scene.sh_degree, device=dev)
-    prm = fb.default_params()
+    prm = fb.default_params(rect_mode=1 if args.rect == 'tight' else 0)
     fdt = g.feat.dtype
     # instance counts (capacity) from a capacity-0 pass per view
     vs0 = fb.ViewState(n, W, H, 0, device=dev)
@@ -568,6 +578,8 @@ def main():
     ap.add_argument("--small", action="store_true", help="debug-size workload (not a bench line)")
     ap.add_argument("--workload", default="mid", choices=["mid", "tiny", "small", "large", "multiview"],
                     help="mid = the bench line (BASELINE.json metric); the others are timed for the record only")
+    ap.add_argument("--rect", default="radius", choices=["radius", "tight"],
+                    help="tile rectangle rule: north_star's scalar 3-sigma radius (default, the bench line) or the tight per-axis extents (NEXT-4 i)")
     ap.add_argument("--ndfd", action="store_true", help="mid: also time fhgs_ndfd_forward (NEXT-1 row) on the frame")
     ap.add_argument("--views", type=int, default=8, help="multiview: number of evenly spaced orbit cameras per sweep")
     args = ap.parse_args()

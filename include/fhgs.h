@@ -94,7 +94,16 @@ typedef struct {
     float t_min;        /* 1e-4    stop a pixel once T < t_min   */
     float den_eps;      /* 1e-8    a Gaussian is fused only if den > den_eps               */
     float bg[3];        /* 0,0,0   background colour, rgb += T_final * bg   */
+    int32_t rect_mode;  /* FHGS_RECT_RADIUS (default): tile rectangle from the scalar radius ceil(3 sqrt(lambda_max)), as
+                           north_star states it; FHGS_RECT_TIGHT: from the per-axis 3-sigma extents ceil(3 sqrt(Sigma_xx)),
+                           ceil(3 sqrt(Sigma_yy)) -- the exact bounding box of the q <= 9 ellipse, so the images and fused
+                           vectors are the same while step S handles ~40 % fewer instances (SURVEY 8(f) NEXT-4 i)        */
+    int32_t primitive;  /* FHGS_PRIM_EWA (default): 3-axis Gaussian, EWA projection (north_star).  FHGS_PRIM_SURFEL:
+                           the paper's own 2-D surfel with exact ray-splat intersection (Eq. 1-3;
+                           SURVEY 8(f) NEXT-3): scale[:,0:2] = (s_u, s_v), scale[:,2] is ignored                        */
 } fhgs_params;
+enum { FHGS_RECT_RADIUS = 0, FHGS_RECT_TIGHT = 1 };
+enum { FHGS_PRIM_EWA = 0, FHGS_PRIM_SURFEL = 1 };
 FHGS_API void fhgs_default_params(fhgs_params* p);
 
 /* Per-view intermediate state.  All pointers are device pointers owned by the caller.
@@ -213,15 +222,20 @@ FHGS_API fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam, c
  *     phi_i = f_i . f_gt (features unit-norm),  sigma_i = 1 / (1 + exp(k (phi_i - lambda)))
  *     out_lgt[x] = sum_i w_i sigma_i                                   (Eq. 5)
  *     out_lcf[x] = sum_i sigma_i w_i (W_{i-1} - F_{i-1} . f_i)          (Eq. 6)
- * where W_n = sum_{i<=n} w_i, F_n = sum_{i<=n} w_i f_i are accumulated in blend order, front to back
- * (the far-to-near wording of PAPER.md:136 is the other reading).  No feature image
+ * where W_n = sum_{i<=n} w_i, F_n = sum_{i<=n} w_i f_i are accumulated
+ *   mode = FHGS_NDFD_BLEND_ORDER:  in blend order, front to back ("updated one time in each step during the
+ *          front-to-back blend");
+ *   mode = FHGS_NDFD_FAR_TO_NEAR:  "along the ray from far to near": the partners
+ *          of fragment i are the fragments behind it.  Same single traversal (the sum is split around the ray totals).
+ * The two readings give different L_cf; out_lgt is the same.  No feature image
  * is rendered.  Paper defaults: k = 20, lambda = 0.5.
  * g->feat [n,D] f32/f16 and gt [H,W,D] f32/f16, both 16-byte aligned; D in {32,64,128,256,512};
  * out_lgt, out_lcf [H,W] f32 (every pixel is written; pixels no Gaussian reaches get 0).
  * Uses vs->{xy,conic_opacity,ranges,vals[sorted_buf]} as fhgs_render does. */
+enum { FHGS_NDFD_BLEND_ORDER = 0, FHGS_NDFD_FAR_TO_NEAR = 1 };
 FHGS_API fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam,
                               const fhgs_params* prm, const fhgs_view_state* vs, const void* gt,
-                              int32_t gt_dtype, float k_sigmoid, float lambda, float* out_lgt,
+                              int32_t gt_dtype, float k_sigmoid, float lambda, int32_t mode, float* out_lgt,
                               float* out_lcf, void* stream);
 
 /* NDFD backward at the w level -- PAPER.md:142-146 and appendix A.2.

@@ -36,9 +36,11 @@
 
 #define TILE 16
 
-/* params layout (10 floats): z_near, cov_dilation, jac_clamp, q_cutoff, alpha_max, t_min,
- * den_eps, bg[3].  cam layout (35 floats): view[16], proj[16], cam_pos[3]. */
-enum { P_ZNEAR = 0, P_DIL, P_JCLAMP, P_QCUT, P_AMAX, P_TMIN, P_DENEPS, P_BG0, P_BG1, P_BG2 };
+/* params layout (12 floats): z_near, cov_dilation, jac_clamp, q_cutoff, alpha_max, t_min,
+ * den_eps, bg[3], rect_mode (0 = scalar radius, 1 = tight per-axis extents; SURVEY 8(f) NEXT-4 i),
+ * primitive (0 = 3-axis EWA Gaussian, 1 = 2-D surfel).
+ * cam layout (35 floats): view[16], proj[16], cam_pos[3]. */
+enum { P_ZNEAR = 0, P_DIL, P_JCLAMP, P_QCUT, P_AMAX, P_TMIN, P_DENEPS, P_BG0, P_BG1, P_BG2, P_RECT, P_PRIM };
 
 int fo_num_threads(void) {
 #ifdef _OPENMP
@@ -129,6 +131,7 @@ void fo_project(int n, int sh_degree, const float *mean, const float *scale, con
     const int K = (sh_degree + 1) * (sh_degree + 1);
     const float z_near = prm[P_ZNEAR], dil = prm[P_DIL];
     const float Lx = prm[P_JCLAMP] * tanx, Ly = prm[P_JCLAMP] * tany;
+    const int tight = prm[P_RECT] != 0.0f;
 #pragma omp parallel for schedule(static)
     for (int i = 0; i < n; ++i) {
         xy[2 * i] = xy[2 * i + 1] = 0.0f; depth[i] = 0.0f;
@@ -188,10 +191,13 @@ void fo_project(int n, int sh_degree, const float *mean, const float *scale, con
         const float r = ceilf(3.0f * sqrtf(lam));
         /* 9. tile rectangle */
         if (!(isfinite(px) && isfinite(py) && isfinite(r))) continue;
-        const float x0 = clampf(floorf((px - r) / 16.0f), 0.0f, (float)GW);
-        const float x1 = clampf(floorf((px + r) / 16.0f) + 1.0f, 0.0f, (float)GW);
-        const float y0 = clampf(floorf((py - r) / 16.0f), 0.0f, (float)GH);
-        const float y1 = clampf(floorf((py + r) / 16.0f) + 1.0f, 0.0f, (float)GH);
+        /* rect_mode 1 (NEXT-4 i): q <= 9 means |dx| <= 3 sqrt(Sigma_xx), |dy| <= 3 sqrt(Sigma_yy) (the exact bounding
+         * box of the ellipse d^T Sigma^-1 d <= 9), so the per-axis extents replace the scalar radius */
+        const float rx = tight ? ceilf(3.0f * sqrtf(ca)) : r, ry = tight ? ceilf(3.0f * sqrtf(cc)) : r;
+        const float x0 = clampf(floorf((px - rx) / 16.0f), 0.0f, (float)GW);
+        const float x1 = clampf(floorf((px + rx) / 16.0f) + 1.0f, 0.0f, (float)GW);
+        const float y0 = clampf(floorf((py - ry) / 16.0f), 0.0f, (float)GH);
+        const float y1 = clampf(floorf((py + ry) / 16.0f) + 1.0f, 0.0f, (float)GH);
         const int ix0 = (int)x0, ix1 = (int)x1, iy0 = (int)y0, iy1 = (int)y1;
         const int cnt = (ix1 - ix0) * (iy1 - iy0);
         if (cnt <= 0 || ix1 <= ix0 || iy1 <= iy0) continue;

@@ -15,8 +15,26 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "fhgs_oracle.c")
 _LIB = os.path.join(_HERE, "libfhgs_oracle.so")
 
-DEFAULT_PARAMS = np.array([0.2, 0.3, 1.3, 9.0, 0.9999, 1e-4, 1e-8, 0.0, 0.0, 0.0], dtype=np.float32)
-# order: z_near, cov_dilation, jac_clamp, q_cutoff, alpha_max, t_min, den_eps, bg[3]
+DEFAULT_PARAMS = np.array([0.2, 0.3, 1.3, 9.0, 0.9999, 1e-4, 1e-8, 0.0, 0.0, 0.0, 0.0, 0.0], dtype=np.float32)
+# order: z_near, cov_dilation, jac_clamp, q_cutoff, alpha_max, t_min, den_eps, bg[3],
+#        rect_mode (0 scalar radius | 1 tight per-axis extents), primitive (0 EWA Gaussian | 1 surfel)
+P_RECT, P_PRIM = 10, 11
+
+
+def params(**kw) -> np.ndarray:
+    """DEFAULT_PARAMS with overrides by name (rect_mode=1, primitive=1, bg=(r,g,b), ...)."""
+    names = ["z_near", "cov_dilation", "jac_clamp", "q_cutoff", "alpha_max", "t_min", "den_eps"]
+    p = DEFAULT_PARAMS.copy()
+    for k, v in kw.items():
+        if k == "bg":
+            p[7:10] = v
+        elif k == "rect_mode":
+            p[P_RECT] = v
+        elif k == "primitive":
+            p[P_PRIM] = v
+        else:
+            p[names.index(k)] = v
+    return p
 
 
 def build(force: bool = False) -> str:

@@ -19,6 +19,9 @@ FHGS_F32, FHGS_F16 = 0, 1
 FHGS_SORT_FULL_KEY = 1
 FHGS_FUSE_ZERO, FHGS_FUSE_FINALIZE, FHGS_FUSE_L2NORM, FHGS_FUSE_FINALIZE_ONLY, FHGS_FUSE_ZERO_ONLY = 1, 2, 4, 8, 16
 FHGS_FUSE_ZERO_TOUCHED = 32
+FHGS_RECT_RADIUS, FHGS_RECT_TIGHT = 0, 1
+FHGS_PRIM_EWA, FHGS_PRIM_SURFEL = 0, 1
+FHGS_NDFD_BLEND_ORDER, FHGS_NDFD_FAR_TO_NEAR = 0, 1
 
 EXPORTS = ["fhgs_create", "fhgs_destroy", "fhgs_last_error", "fhgs_version", "fhgs_default_params",
            "fhgs_scratch_bytes", "fhgs_scratch_tile_visited", "fhgs_set_diagnostics", "fhgs_project", "fhgs_bin_sort", "fhgs_render", "fhgs_fuse_features", "fhgs_ndfd_forward", "fhgs_ndfd_backward_work_bytes", "fhgs_ndfd_backward",
@@ -45,7 +48,7 @@ class CCamera(C.Structure):
 class CParams(C.Structure):
     _fields_ = [("z_near", C.c_float), ("cov_dilation", C.c_float), ("jac_clamp", C.c_float),
                 ("q_cutoff", C.c_float), ("alpha_max", C.c_float), ("t_min", C.c_float),
-                ("den_eps", C.c_float), ("bg", C.c_float * 3)]
+                ("den_eps", C.c_float), ("bg", C.c_float * 3), ("rect_mode", C.c_int32), ("primitive", C.c_int32)]
 
 
 class CViewState(C.Structure):
@@ -101,7 +104,7 @@ def _load():
                                     C.POINTER(CParams), C.POINTER(CViewState), C.POINTER(CFrameWorkspace),
                                     C.POINTER(C.c_uint64), vp]
     lib.fhgs_ndfd_forward.argtypes = [vp, C.POINTER(CGaussians), C.POINTER(CCamera), C.POINTER(CParams), C.POINTER(CViewState),
-                                      vp, C.c_int32, C.c_float, C.c_float, vp, vp, vp]
+                                      vp, C.c_int32, C.c_float, C.c_float, C.c_int32, vp, vp, vp]
     lib.fhgs_ndfd_backward_work_bytes.restype = C.c_size_t
     lib.fhgs_ndfd_backward_work_bytes.argtypes = [C.c_int32, C.c_int32, C.c_int32]
     lib.fhgs_ndfd_backward.argtypes = [vp, C.POINTER(CGaussians), C.POINTER(CCamera), C.POINTER(CParams), C.POINTER(CViewState),
@@ -123,6 +126,8 @@ def default_params(**overrides) -> CParams:
     for k, v in overrides.items():
         if k == "bg":
             p.bg[0], p.bg[1], p.bg[2] = [float(x) for x in v]
+        elif k in ("rect_mode", "primitive"):
+            setattr(p, k, int(v))
         else:
             setattr(p, k, float(v))
     return p
@@ -318,11 +323,12 @@ def fuse_features(ctx: Context, cam, prm: CParams, vs: ViewState, gt, num, den, 
 
 
 def ndfd_forward(ctx: Context, g: Gaussians, cam: CCamera, prm: CParams, vs: ViewState, gt, out_lgt, out_lcf,
-                 k: float = 20.0, lam: float = 0.5, stream=None):
-    """fhgs_ndfd_forward: per-pixel L_gt, L_cf ([H,W] f32 tensors, caller-allocated) of PAPER.md Eq. 5-6."""
+                 k: float = 20.0, lam: float = 0.5, mode: int = 0, stream=None):
+    """fhgs_ndfd_forward: per-pixel L_gt, L_cf ([H,W] f32 tensors, caller-allocated) of PAPER.md Eq. 5-6.
+    mode: FHGS_NDFD_BLEND_ORDER (0) or FHGS_NDFD_FAR_TO_NEAR (1)."""
     ctx.check(lib.fhgs_ndfd_forward(ctx.handle, C.byref(g.c), C.byref(cam), C.byref(prm), C.byref(vs.c), _ptr(gt),
-                                    _dtype_code(gt), C.c_float(k), C.c_float(lam), _ptr(out_lgt), _ptr(out_lcf),
-                                    _stream(stream)))
+                                    _dtype_code(gt), C.c_float(k), C.c_float(lam), C.c_int32(mode), _ptr(out_lgt),
+                                    _ptr(out_lcf), _stream(stream)))
 
 
 def ndfd_backward(ctx: Context, g: Gaussians, cam: CCamera, prm: CParams, vs: ViewState, gt, grad_opacity,

@@ -64,6 +64,8 @@ extern "C" void fhgs_default_params(fhgs_params* p) {
     p->t_min = 1e-4f;
     p->den_eps = 1e-8f;
     p->bg[0] = p->bg[1] = p->bg[2] = 0.0f;
+    p->rect_mode = FHGS_RECT_RADIUS;
+    p->primitive = FHGS_PRIM_EWA;
 }
 
 extern "C" size_t fhgs_scratch_bytes(int32_t n, int32_t width, int32_t height, uint64_t capacity) {
@@ -98,6 +100,8 @@ fhgs_status validate_params(fhgs_ctx* ctx, const fhgs_params* p) {
     if (!(p->z_near > 0.0f)) FHGS_INVALID(ctx, "params: z_near must be > 0 (depth bits must order like depth)");
     if (!(p->q_cutoff >= 0.0f) || !(p->alpha_max > 0.0f && p->alpha_max < 1.0f) || !(p->t_min >= 0.0f))
         FHGS_INVALID(ctx, "params: q_cutoff >= 0, 0 < alpha_max < 1, t_min >= 0 required");   // 1/(1-alpha) in the backward
+    if (p->rect_mode != FHGS_RECT_RADIUS && p->rect_mode != FHGS_RECT_TIGHT) FHGS_INVALID(ctx, "params: unknown rect_mode");
+    if (p->primitive != FHGS_PRIM_EWA && p->primitive != FHGS_PRIM_SURFEL) FHGS_INVALID(ctx, "params: unknown primitive");
     return FHGS_OK;
 }
 

@@ -4,6 +4,14 @@
 //     phi_i = f_i . f_gt(x),  sigma_i = 1 / (1 + exp(k (phi_i - lambda))),  w_i = alpha_i T_i
 //     L_gt(x) = sum_i w_i sigma_i
 //     L_cf(x) = sum_i sigma_i w_i (W_{i-1} - F_{i-1} . f_i),   W, F accumulated in blend order (DESIGN.md reading)
+// MODE 1 (FHGS_NDFD_FAR_TO_NEAR, "along the ray from far to near"): the partners of fragment i are the
+// fragments BEHIND it, W_behind = W_tot - W_<=i, F_behind = F_tot - F_<=i.  The totals are only known at the end of the
+// front-to-back walk, but the sum splits:
+//     L_cf = sum_i sigma_i w_i (W_tot - F_tot . f_i) - sum_i sigma_i w_i (W_<=i - F_<=i . f_i)
+//          = W_tot L_gt - F_tot . S - B,      S = sum_i sigma_i w_i f_i  (one more D-vector per pixel),
+//                                             B = the blend-order recurrence with INCLUSIVE prefixes
+// so the same single traversal serves (no fragment list, no second pass); the oracle's mode 1 walks the collected
+// fragment list backwards instead.
 //
 // First CUDA path of this row (correctness first; not yet the warp-specialised form of render/fuse):
 // one CTA of 256 threads per 16 x (16/LPP)-row pixel strip of a tile.  LPP lanes (4 for D <= 128, else 8) share one
@@ -66,8 +74,9 @@ struct NdSub {
 };
 
 // CPL = channels per lane = D / LPP
-template <int LPP, int CPL, typename FT, typename GT>
-__global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1)) ndfd_strip_kernel(const NdfdArgs a) {
+template <int LPP, int CPL, typename FT, typename GT, int MODE>
+__global__ void __launch_bounds__(TR_THREADS, MODE ? (CPL <= 16 ? 2 : 1) : (CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1)))
+    ndfd_strip_kernel(const NdfdArgs a) {
     __shared__ TileQueue q;
     constexpr int PXW = 32 / LPP, ROWS = 8 * PXW / FHGS_TILE, STRIPS = FHGS_TILE / ROWS;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -89,7 +98,9 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1
     const int c_lo = cgl * 4;
 
     // channel pairs packed for fma.rn.f32x2 (two FMAs per issue slot)
-    unsigned long long g[CPL / 2], F[CPL / 2];
+    unsigned long long g[CPL / 2], F[CPL / 2], S[MODE ? CPL / 2 : 1];
+#pragma unroll
+    for (int j = 0; j < (MODE ? CPL / 2 : 1); ++j) S[j] = 0ull;
 #pragma unroll
     for (int j = 0; j < CPL / 4; ++j) {
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -164,6 +175,12 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1
                     const float4 v = lds4<FT>(f + 4 * LPP * j);
                     fv[2 * j] = pack2(v.x, v.y); fv[2 * j + 1] = pack2(v.z, v.w);
                 }
+                if (MODE) {   // inclusive prefixes: F_<=i, W_<=i
+                    const unsigned long long w2 = pack2(w, w);
+#pragma unroll
+                    for (int j = 0; j < CPL / 2; ++j) fma2_acc(F[j], w2, fv[j]);
+                    Wc += w;
+                }
 #pragma unroll
                 for (int j = 0; j < CPL / 2; ++j) {
                     fma2_acc(ph[j & 1], fv[j], g[j]);
@@ -180,15 +197,31 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1
                 const float sw = sigma * w;        // w == 0 for pixels the Gaussian does not reach: nothing changes
                 lgt += sw;
                 lcf = fmaf(sw, Wc - Ff, lcf);
-                Wc += w;
-                const unsigned long long w2 = pack2(w, w);
+                if (MODE) {
+                    const unsigned long long sw2 = pack2(sw, sw);
 #pragma unroll
-                for (int j = 0; j < CPL / 2; ++j) fma2_acc(F[j], w2, fv[j]);
+                    for (int j = 0; j < CPL / 2; ++j) fma2_acc(S[j], sw2, fv[j]);
+                } else {
+                    Wc += w;
+                    const unsigned long long w2 = pack2(w, w);
+#pragma unroll
+                    for (int j = 0; j < CPL / 2; ++j) fma2_acc(F[j], w2, fv[j]);
+                }
               }
             }
             __syncthreads();   // the buffer is refilled two sub-batches later; the ring at the next chunk
         }
         if (__syncthreads_and(done)) break;
+    }
+    if (MODE) {   // L_cf = W_tot L_gt - F_tot . S - B  (B = lcf so far)
+        unsigned long long fs[2] = {0ull, 0ull};
+#pragma unroll
+        for (int j = 0; j < CPL / 2; ++j) fma2_acc(fs[j & 1], F[j], S[j]);
+        const float2 s0 = unpack2(fs[0]), s1 = unpack2(fs[1]);
+        float FS = (s0.x + s0.y) + (s1.x + s1.y);
+#pragma unroll
+        for (int d = 1; d < LPP; d <<= 1) FS += __shfl_xor_sync(TR_FULL, FS, d);
+        lcf = fmaf(Wc, lgt, -FS) - lcf;
     }
     if (inside && cgl == 0) {
         const size_t o = (size_t)py * a.t.W + px;
@@ -197,34 +230,38 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1
     }
 }
 
-template <int LPP, int CPL, typename FT, typename GT>
+template <int LPP, int CPL, typename FT, typename GT, int MODE>
 cudaError_t launch(const NdfdArgs& a, int tiles, cudaStream_t st) {
     constexpr int STRIPS = FHGS_TILE / (8 * (32 / LPP) / FHGS_TILE);
     const size_t smem = 2 * (size_t)NdSub<LPP * CPL, FT>::SB * NdSub<LPP * CPL, FT>::ROW_BYTES;
-    cudaError_t e = cudaFuncSetAttribute(ndfd_strip_kernel<LPP, CPL, FT, GT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(ndfd_strip_kernel<LPP, CPL, FT, GT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    ndfd_strip_kernel<LPP, CPL, FT, GT><<<tiles * STRIPS, TR_THREADS, smem, st>>>(a);
+    ndfd_strip_kernel<LPP, CPL, FT, GT, MODE><<<tiles * STRIPS, TR_THREADS, smem, st>>>(a);
     return cudaGetLastError();
 }
 
-template <typename FT, typename GT>
-cudaError_t dispatch(const NdfdArgs& a, int tiles, cudaStream_t st) {
+template <typename FT, typename GT, int MODE>
+cudaError_t dispatch_d(const NdfdArgs& a, int tiles, cudaStream_t st) {
     switch (a.D) {
-        case 32: return launch<4, 8, FT, GT>(a, tiles, st);
-        case 64: return launch<4, 16, FT, GT>(a, tiles, st);
-        case 128: return launch<4, 32, FT, GT>(a, tiles, st);
-        case 256: return launch<8, 32, FT, GT>(a, tiles, st);
-        case 512: return launch<8, 64, FT, GT>(a, tiles, st);
+        case 32: return launch<4, 8, FT, GT, MODE>(a, tiles, st);
+        case 64: return launch<4, 16, FT, GT, MODE>(a, tiles, st);
+        case 128: return launch<4, 32, FT, GT, MODE>(a, tiles, st);
+        case 256: return launch<8, 32, FT, GT, MODE>(a, tiles, st);
+        case 512: return launch<8, 64, FT, GT, MODE>(a, tiles, st);
         default: return cudaErrorInvalidValue;
     }
+}
+template <typename FT, typename GT>
+cudaError_t dispatch(const NdfdArgs& a, int tiles, int mode, cudaStream_t st) {
+    return mode ? dispatch_d<FT, GT, 1>(a, tiles, st) : dispatch_d<FT, GT, 0>(a, tiles, st);
 }
 
 }  // namespace
 
 extern "C" fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam,
                                          const fhgs_params* prm, const fhgs_view_state* vs, const void* gt,
-                                         int32_t gt_dtype, float k_sigmoid, float lambda, float* out_lgt, float* out_lcf,
-                                         void* stream) {
+                                         int32_t gt_dtype, float k_sigmoid, float lambda, int32_t mode, float* out_lgt,
+                                         float* out_lcf, void* stream) {
     if (!ctx) return FHGS_ERR_INVALID;
     if (!g || !cam || !prm || !vs || !gt || !out_lgt || !out_lcf) FHGS_INVALID(ctx, "fhgs_ndfd_forward: NULL argument");
     fhgs_status st;
@@ -240,6 +277,7 @@ extern "C" fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g,
     if (!aligned_to(g->feat, 16) || !aligned_to(gt, 16)) FHGS_INVALID(ctx, "fhgs_ndfd_forward: feat/gt must be 16-byte aligned");
     if (g->n != vs->n) FHGS_INVALID(ctx, "fhgs_ndfd_forward: g->n != vs->n");
     if (!finite_f(k_sigmoid) || !finite_f(lambda)) FHGS_INVALID(ctx, "fhgs_ndfd_forward: non-finite k / lambda");
+    if (mode != FHGS_NDFD_BLEND_ORDER && mode != FHGS_NDFD_FAR_TO_NEAR) FHGS_INVALID(ctx, "fhgs_ndfd_forward: unknown mode");
     NdfdArgs a;
     a.t.W = cam->width; a.t.H = cam->height; a.t.GW = tiles_x(cam->width);
     a.t.ranges = vs->ranges; a.t.vals = vs->vals[vs->sorted_buf & 1];
@@ -253,10 +291,10 @@ extern "C" fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g,
     cudaStream_t s = (cudaStream_t)stream;
     cudaError_t e;
     const bool fh = g->feat_dtype == FHGS_F16, gh = gt_dtype == FHGS_F16;
-    if (fh && gh) e = dispatch<__half, __half>(a, tiles, s);
-    else if (fh) e = dispatch<__half, float>(a, tiles, s);
-    else if (gh) e = dispatch<float, __half>(a, tiles, s);
-    else e = dispatch<float, float>(a, tiles, s);
+    if (fh && gh) e = dispatch<__half, __half>(a, tiles, mode, s);
+    else if (fh) e = dispatch<__half, float>(a, tiles, mode, s);
+    else if (gh) e = dispatch<float, __half>(a, tiles, mode, s);
+    else e = dispatch<float, float>(a, tiles, mode, s);
     FHGS_CUDA(ctx, e);
     return FHGS_OK;
 }

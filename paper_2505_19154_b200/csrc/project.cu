@@ -29,6 +29,7 @@ struct ProjectArgs {
     float cam_pos[3];
     float fx, fy, cx, cy, Lx, Ly;
     float z_near, dil;
+    int tight;   // FHGS_RECT_TIGHT: per-axis 3-sigma extents instead of the scalar radius
     float *xy, *depth, *conic_opacity, *rgb;
     int32_t* radius;
     uint16_t* rect;
@@ -188,10 +189,12 @@ __global__ void __launch_bounds__(PROJ_THREADS) project_kernel(const ProjectArgs
         const float r = ceilf(mul(3.0f, sq(lam)));
         // 9. tile rectangle
         if (!(finite_dev(px) && finite_dev(py) && finite_dev(r))) break;
-        const float x0 = clampf(floorf(dvd(sub(px, r), 16.0f)), 0.0f, (float)a.GW);
-        const float x1 = clampf(add(floorf(dvd(add(px, r), 16.0f)), 1.0f), 0.0f, (float)a.GW);
-        const float y0 = clampf(floorf(dvd(sub(py, r), 16.0f)), 0.0f, (float)a.GH);
-        const float y1 = clampf(add(floorf(dvd(add(py, r), 16.0f)), 1.0f), 0.0f, (float)a.GH);
+        // tight mode: the q <= 9 ellipse spans exactly +-3 sqrt(Sigma_xx) in x and +-3 sqrt(Sigma_yy) in y
+        const float rx = a.tight ? ceilf(mul(3.0f, sq(ca))) : r, ry = a.tight ? ceilf(mul(3.0f, sq(cc))) : r;
+        const float x0 = clampf(floorf(dvd(sub(px, rx), 16.0f)), 0.0f, (float)a.GW);
+        const float x1 = clampf(add(floorf(dvd(add(px, rx), 16.0f)), 1.0f), 0.0f, (float)a.GW);
+        const float y0 = clampf(floorf(dvd(sub(py, ry), 16.0f)), 0.0f, (float)a.GH);
+        const float y1 = clampf(add(floorf(dvd(add(py, ry), 16.0f)), 1.0f), 0.0f, (float)a.GH);
         const int ix0 = (int)x0, ix1 = (int)x1, iy0 = (int)y0, iy1 = (int)y1;
         if (ix1 <= ix0 || iy1 <= iy0) break;
         // 10. SH colour
@@ -268,6 +271,7 @@ extern "C" fhgs_status fhgs_project(fhgs_ctx* ctx, const fhgs_gaussians* g, cons
     a.Lx = prm->jac_clamp * k.tanx;   // single binary32 multiply, as C1-P step 3
     a.Ly = prm->jac_clamp * k.tany;
     a.z_near = prm->z_near; a.dil = prm->cov_dilation;
+    a.tight = prm->rect_mode == FHGS_RECT_TIGHT;
     a.xy = vs->xy; a.depth = vs->depth; a.conic_opacity = vs->conic_opacity; a.rgb = vs->rgb;
     a.radius = vs->radius; a.rect = vs->rect; a.tiles_touched = vs->tiles_touched;
 

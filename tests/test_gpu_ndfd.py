@@ -10,7 +10,9 @@ import parity_util as pu
 pytestmark = pytest.mark.gpu
 
 
-def _run(cfg, view, tol, npix=4000, k=20.0, lam=0.5):
+def _run(cfg, view, tol, npix=4000, k=20.0, lam=0.5, modes=(0, 1)):
+    """Both accumulation orders of W, F (DESIGN.md reading): mode 0 = blend order, mode 1 = far to near
+    (PAPER.md:136); the oracle's mode 1 walks the collected fragment list backwards, the kernel uses the split sum."""
     import torch
     from paper_2505_19154_b200 import binding as fb
     scene = inputs.make_scene(cfg)
@@ -25,21 +27,31 @@ def _run(cfg, view, tol, npix=4000, k=20.0, lam=0.5):
     lgt = torch.full((H, W), -1.0, dtype=torch.float32, device=dev)
     lcf = torch.full((H, W), -1.0, dtype=torch.float32, device=dev)
     gt_d = torch.from_numpy(np.ascontiguousarray(gt)).to(dev)
-    fb.ndfd_forward(gp.ctx, gp.g, c, gp.prm, gp.vs, gt_d, lgt, lcf, k=k, lam=lam)
-    torch.cuda.synchronize()
-    lgt, lcf = lgt.cpu().numpy().ravel(), lcf.cpu().numpy().ravel()
     rng = np.random.default_rng(17 + view)
     pix = np.unique(np.concatenate([rng.integers(0, W * H, size=npix), np.arange(W), (H - 1) * W + np.arange(W),
                                     np.arange(H) * W + W - 1])).astype(np.int32)
     order = fo.global_order(pr)
-    o_lgt, o_lcf = fo.ndfd(pr, order, scene.feat.astype(np.float32), gt.astype(np.float32), W, H, k=k, lam=lam, pix=pix)
     frag = fo.render_literal(pr, order, None, W, H, pix=pix)["fragile"].astype(bool)
     slack = np.where(frag, 3.0 * tol, tol)      # a fragment blended at T ~ t_min adds <= 1e-4 (sigma + W) to either loss
-    e1, e2 = np.abs(lgt[pix] - o_lgt), np.abs(lcf[pix] - o_lcf)
-    assert np.all(e1 <= slack), (e1.max(), int(np.argmax(e1)))
-    assert np.all(e2 <= slack), (e2.max(), int(np.argmax(e2)))
-    assert lgt.min() >= 0.0 and o_lgt.max() > 0.05      # every pixel was written; the case is not trivial
-    return dict(lgt=float(e1.max()), lcf=float(e2.max()), fragile=int(frag.sum()), lcf_max=float(np.abs(o_lcf).max()))
+    out = {}
+    lcf_by_mode = []
+    for mode in modes:
+        lgt.fill_(-1.0); lcf.fill_(-1.0)
+        fb.ndfd_forward(gp.ctx, gp.g, c, gp.prm, gp.vs, gt_d, lgt, lcf, k=k, lam=lam, mode=mode)
+        torch.cuda.synchronize()
+        g_lgt, g_lcf = lgt.cpu().numpy().ravel(), lcf.cpu().numpy().ravel()
+        o_lgt, o_lcf = fo.ndfd(pr, order, scene.feat.astype(np.float32), gt.astype(np.float32), W, H, k=k, lam=lam, mode=mode, pix=pix)
+        e1, e2 = np.abs(g_lgt[pix] - o_lgt), np.abs(g_lcf[pix] - o_lcf)
+        assert np.all(e1 <= slack), (mode, e1.max(), int(np.argmax(e1)))
+        assert np.all(e2 <= slack), (mode, e2.max(), int(np.argmax(e2)))
+        assert g_lgt.min() >= 0.0 and o_lgt.max() > 0.05      # every pixel was written; the case is not trivial
+        lcf_by_mode.append(o_lcf)
+        out[f"mode{mode}"] = dict(lgt=float(e1.max()), lcf=float(e2.max()), lcf_max=float(np.abs(o_lcf).max()))
+    if len(lcf_by_mode) == 2:   # the two readings really differ on this case (else the mode-1 check proves nothing)
+        out["modes_differ_by"] = float(np.abs(lcf_by_mode[0] - lcf_by_mode[1]).max())
+        assert out["modes_differ_by"] > 10 * tol
+    out["fragile"] = int(frag.sum())
+    return out
 
 
 def test_ndfd_mid_shape_d128_ragged():

@@ -13,7 +13,7 @@ pytestmark = pytest.mark.gpu
 
 
 def run_case(cfg, views, tol, literal_pixels=None, sort_flags=(0, 1), capacity_slack=1.25, check_finalize=True,
-             fixed_capacity=None, full_frame=True):
+             fixed_capacity=None, full_frame=True, rect_mode=0):
     """Full P -> S -> R -> F parity of one config over `views`; returns worst errors.
     full_frame: compare the whole rendered frame with fo_render_scatter; literal_pixels: additionally (or instead)
     compare that many random pixels with the tile-free, box-free fo_render_literal.  Fusion is always compared on
@@ -21,15 +21,17 @@ def run_case(cfg, views, tol, literal_pixels=None, sort_flags=(0, 1), capacity_s
     import time
     scene = inputs.make_scene(cfg)
     cams = [inputs.make_camera(cfg, v) for v in views]
-    prs = [pu.oracle_view(scene, cam) for cam in cams]
+    prm_o = fo.params(rect_mode=rect_mode)
+    prs = [pu.oracle_view(scene, cam, prm_o) for cam in cams]
     Ms = [int(pr["tiles_touched"].astype(np.int64).sum()) for pr in prs]
     cap = int(max(Ms) * capacity_slack) + 16
     if fixed_capacity is not None:
         cap = fixed_capacity
     gp = pu.GpuPath(scene, cfg.width, cfg.height, cap)
+    gp.prm.rect_mode = rect_mode
     feat32 = scene.feat.astype(np.float32)
     fabs = float(np.abs(feat32).max())
-    worst = {}
+    worst = {"M": max(Ms)}
     num_o = np.zeros((scene.n, cfg.feat_dim)); den_o = np.zeros(scene.n)
     num_g = den_g = None
     border = pu.Borderline(scene.n, cfg.feat_dim)
@@ -147,6 +149,19 @@ def test_mid_full_size_bench_configuration():
     cfg = inputs.CONFIGS["mid"]
     w = run_case(cfg, [0], pu.TOL_F32, sort_flags=(0,), capacity_slack=1.0, fixed_capacity=int(40e6))
     print(w)
+
+
+def test_tight_rect_mode():
+    """SURVEY 8(f) NEXT-4 (i), fhgs_params.rect_mode = FHGS_RECT_TIGHT: per-axis 3-sigma tile rectangles.  Same parity
+    bars (rect, tiles_touched, M, all sorted pairs, ranges bit-exact against the oracle run with the same rule; images
+    and fused vectors within 1e-4 of the oracle, whose renderer does not depend on the rule) on the Tiny config, a
+    ragged D=128 case and the Mid config at FULL size, where it must shed at least a third of the instances."""
+    print(run_case(inputs.CONFIGS["tiny"], range(4), pu.TOL_F32, rect_mode=1))
+    cfg = pu.reduced_config("mid", n=60_000, width=328, height=200, log_scale_mu=-3.3)
+    print(run_case(cfg, [0], pu.TOL_F32, rect_mode=1))
+    w = run_case(inputs.CONFIGS["mid"], [0], pu.TOL_F32, sort_flags=(0,), capacity_slack=1.0, fixed_capacity=int(40e6), rect_mode=1)
+    print(w)
+    assert w["M"] < 0.67 * 31_666_264
 
 
 def test_large_full_size():

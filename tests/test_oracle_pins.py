@@ -571,3 +571,77 @@ def test_culling_and_clamp():
     c = (fx * s / z) ** 2 + 0.3
     np.testing.assert_allclose(pr["conic_opacity"][0, :3], [1 / a, 0.0, 1 / c], rtol=1e-5, atol=1e-7)
     np.testing.assert_allclose(pr["xy"][0, 0], fx * 3.0 + 31.5, rtol=1e-6)   # the centre is NOT clamped
+
+
+# ---- NEXT-4 (i): tight per-axis tile rectangles (fhgs_params.rect_mode = 1) ------------------------
+def test_pin22_tight_rect_closed_form_and_conservative():
+    """rect_mode 1 takes the exact bounding box of the q <= 9 ellipse: half extents 3 sqrt(Sigma_xx), 3 sqrt(Sigma_yy).
+    (a) closed form on a hand-made anisotropic splat; (b) exhaustive scan: every pixel with q <= 9 lies in a tile of
+    the tight rectangle, which is never larger than the radius rectangle; (c) a strongly anisotropic scene really
+    shrinks; (d) everything but rect / tiles_touched is bit-identical between the two modes."""
+    tight = fo.params(rect_mode=1)
+    # (a) axis-aligned splat at depth 4 on the optical axis, scales (0.4, 0.05, 0.05): Sigma_xx = (fx*0.4/4)^2 + 0.3
+    cam = front_camera(256, 256)
+    pr = project_simple((0.0, 0.0, 4.0), (0.4, 0.05, 0.05), (1, 0, 0, 0), 0.5, (0.2, 0.4, 0.6), cam, tight)
+    fx = (256 / 2) / math.tan(math.radians(30.0))
+    sxx, syy = (fx * 0.4 / 4) ** 2 + 0.3, (fx * 0.05 / 4) ** 2 + 0.3
+    rx, ry = math.ceil(3 * math.sqrt(sxx)), math.ceil(3 * math.sqrt(syy))
+    cx = cy = 127.5
+    want = [int((cx - rx) // 16), int((cy - ry) // 16), int((cx + rx) // 16) + 1, int((cy + ry) // 16) + 1]
+    assert pr["rect"][0].astype(int).tolist() == want
+    assert int(pr["radius"][0]) == rx                                    # the scalar radius is still ceil(3 sqrt(lambda_max))
+    pr_r = project_simple((0.0, 0.0, 4.0), (0.4, 0.05, 0.05), (1, 0, 0, 0), 0.5, (0.2, 0.4, 0.6), cam)
+    assert int(pr_r["tiles_touched"][0]) > int(pr["tiles_touched"][0]) > 0
+    # (b), (d) random anisotropic scene
+    cfg = inputs.scaled(inputs.CONFIGS["tiny"], n=300, log_scale_sigma=1.2)
+    sc = inputs.make_scene(cfg)
+    cam = inputs.make_camera(cfg, 1)
+    args = (sc.mean, sc.scale, sc.quat, sc.opacity, sc.sh, sc.sh_degree, cam35(cam), 64, 64)
+    p0, p1 = fo.project(*args), fo.project(*args, tight)
+    for k in ("xy", "depth", "conic_opacity", "rgb", "radius"):
+        vis = p1["radius"] > 0
+        assert np.array_equal(p0[k][vis], p1[k][vis]), k
+    assert np.all(p1["tiles_touched"] <= p0["tiles_touched"])
+    assert p1["tiles_touched"].sum() < p0["tiles_touched"].sum()         # (c)
+    ys, xs = np.mgrid[0:64, 0:64]
+    seen = 0
+    for i in np.nonzero(p1["radius"] > 0)[0]:
+        A, B, Cc, _ = p1["conic_opacity"][i].astype(np.float64)
+        dx = p1["xy"][i, 0].astype(np.float64) - xs
+        dy = p1["xy"][i, 1].astype(np.float64) - ys
+        inside = (A * dx * dx + 2 * B * dx * dy + Cc * dy * dy) <= 9.0 + 1e-3
+        if not inside.any():
+            continue
+        seen += 1
+        x0, y0, x1, y1 = p1["rect"][i].astype(int)
+        tx, ty = xs[inside] // 16, ys[inside] // 16
+        assert np.all((tx >= x0) & (tx < x1) & (ty >= y0) & (ty < y1))
+    assert seen > 100
+
+
+def test_pin23_tight_rect_renders_the_same_image():
+    """The tile lists only serve to find the Gaussians that can reach a pixel: with either rectangle rule a tiled
+    traversal (per-tile sorted ranges of fo_bins) blends exactly the fragments the tile-free literal oracle blends."""
+    cfg = inputs.scaled(inputs.CONFIGS["tiny"], n=400)
+    sc = inputs.make_scene(cfg)
+    cam = inputs.make_camera(cfg, 2)
+    for prm in (fo.DEFAULT_PARAMS, fo.params(rect_mode=1)):
+        pr = fo.project(sc.mean, sc.scale, sc.quat, sc.opacity, sc.sh, sc.sh_degree, cam35(cam), 64, 64, prm)
+        order = fo.global_order(pr)
+        lit = fo.render_literal(pr, order, sc.feat, 64, 64)
+        b = fo.bins(pr, 64, 64)
+        rng = np.random.default_rng(5)
+        for p in rng.integers(0, 64 * 64, size=150):
+            x, y = int(p % 64), int(p // 64)
+            r0, r1 = b["ranges"][(y // 16) * 4 + x // 16]
+            T, n = 1.0, 0
+            for g in b["vals"][int(r0):int(r1)]:
+                if T < 1e-4:
+                    break
+                q = fo.q_value(pr["xy"][g, 0], pr["xy"][g, 1], *pr["conic_opacity"][g, :3], x, y)
+                if not q <= 9.0:
+                    continue
+                al = min(float(np.float32(0.9999)), float(pr["conic_opacity"][g, 3]) * math.exp(-0.5 * max(float(q), 0.0)))
+                T *= 1.0 - al
+                n += 1
+            assert n == int(lit["n"][p]) and abs(T - lit["T"][p]) < 1e-12
