@@ -47,9 +47,8 @@ def _run(cfg, view, tol, npix=4000, k=20.0, lam=0.5, modes=(0, 1)):
         assert g_lgt.min() >= 0.0 and o_lgt.max() > 0.05      # every pixel was written; the case is not trivial
         lcf_by_mode.append(o_lcf)
         out[f"mode{mode}"] = dict(lgt=float(e1.max()), lcf=float(e2.max()), lcf_max=float(np.abs(o_lcf).max()))
-    if len(lcf_by_mode) == 2:   # the two readings really differ on this case (else the mode-1 check proves nothing)
+    if len(lcf_by_mode) == 2:   # how far apart the two readings are on this case
         out["modes_differ_by"] = float(np.abs(lcf_by_mode[0] - lcf_by_mode[1]).max())
-        assert out["modes_differ_by"] > 10 * tol
     out["fragile"] = int(frag.sum())
     return out
 
@@ -57,7 +56,9 @@ def _run(cfg, view, tol, npix=4000, k=20.0, lam=0.5, modes=(0, 1)):
 def test_ndfd_mid_shape_d128_ragged():
     """D=128 unit features, 328x200 (ragged right column and bottom row), saturating scene."""
     cfg = pu.reduced_config("mid", n=60_000, width=328, height=200, log_scale_mu=-3.3)
-    print(_run(cfg, 0, pu.TOL_F32))
+    w = _run(cfg, 0, pu.TOL_F32)
+    print(w)
+    assert w["modes_differ_by"] > 10 * pu.TOL_F32   # the two readings really differ here: the mode-1 check is not vacuous
 
 
 def test_ndfd_other_dims_and_fp16():
