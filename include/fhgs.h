@@ -133,6 +133,10 @@ typedef struct {
     uint32_t* ranges;        /* [GW*GH,2] [first,last+1) into the sorted list; (0,0) = empty */
     void* scratch;
     size_t scratch_bytes;
+    float* ray_transform;    /* [n,12] FHGS_PRIM_SURFEL only (else may be NULL): per splat the 3x3 matrix adj(T) of
+                                PAPER.md Eq. 3, rows padded to float4 -- (u,v,1) ~ adj(T) (x,y,1)^T; 16-B aligned.
+                                In surfel mode xy holds the centre of the footprint's bounding box and
+                                conic_opacity = (half_x, half_y, 0, opacity) of that box */
 } fhgs_view_state;
 
 FHGS_API size_t fhgs_scratch_bytes(int32_t n, int32_t width, int32_t height, uint64_t capacity);
@@ -153,7 +157,14 @@ FHGS_API void fhgs_set_diagnostics(fhgs_ctx* ctx, int enable);
  * integer outputs are reproducible bit for bit.  A culled Gaussian gets radius = 0,
  * tiles_touched = 0, rect = 0 and zeros in the float outputs.
  * Reads g->{mean,scale,quat,opacity,sh}; writes vs->{xy,depth,conic_opacity,rgb,radius,rect,
- * tiles_touched}; sets vs->n/width/height must equal g->n / cam->width / cam->height. */
+ * tiles_touched}; sets vs->n/width/height must equal g->n / cam->width / cam->height.
+ * prm->primitive == FHGS_PRIM_SURFEL: the paper's 2-D surfel: centre p, tangents
+ * t_u, t_v = columns 0, 1 of R(quat), scales (s_u, s_v) = scale[:,0:2]; P(u,v) = p + s_u t_u u + s_v t_v v (Eq. 2) and
+ * the pixel's (u,v) from the exact ray-splat intersection (Eq. 3) through the homography T = K [R_v s_u t_u, R_v s_v t_v,
+ * c]; G = exp(-(u^2+v^2)/2).  Writes vs->ray_transform = adj(T) (scaled by a power of two), the footprint's bounding
+ * box (dual conic) into xy / conic_opacity / radius / rect, depth = z of the centre.  Culled: centre or any point of the
+ * 3-sigma disc in front of z_near, degenerate transform.  No low-pass filter (the paper states none).  Steps S, R, F
+ * run unchanged on the result (R, F evaluate u^2+v^2 from ray_transform when prm->primitive says so). */
 FHGS_API fhgs_status fhgs_project(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam,
                          const fhgs_params* prm, fhgs_view_state* vs, void* stream);
 

@@ -223,6 +223,137 @@ void fo_project(int n, int sh_degree, const float *mean, const float *scale, con
 }
 
 /* ------------------------------------------------------------------------------------------
+ * Step P for the paper's own primitive (prm[P_PRIM] = 1): the 2-D surfel of
+ * PAPER.md:77-90.  Centre p, tangents t_u, t_v = columns 0, 1 of R(quat), planar scales
+ * (s_u, s_v) = scale[0..1] (scale[2] is ignored).  Eq. 2: P(u,v) = p + s_u t_u u + s_v t_v v.
+ * Eq. 3: the pixel x = (x, y) sees the point (u,v) with  (x z, y z, z)^T = K W P(u,v), i.e. in
+ * homogeneous pixel coordinates  (X, Y, Wc)^T = T (u, v, 1)^T  with the 3x3 matrix
+ *     T = [ fx a_x + cx a_z   fx b_x + cx b_z   fx c_x + cx c_z ]     a = R_v (s_u t_u)
+ *         [ fy a_y + cy a_z   fy b_y + cy b_z   fy c_y + cy c_z ]     b = R_v (s_v t_v)
+ *         [       a_z               b_z               c_z       ]     c = camera-space centre
+ * so (u, v, 1) is proportional to T^-1 (x, y, 1)^T = adj(T) (x, y, 1)^T / det T.  The 9 entries of
+ * adj(T) (rows: the cross products T_y x T_w, T_w x T_x, T_x x T_y taken as COLUMNS), scaled by an
+ * exact power of two, are the per-splat "ray transform" ray_transform[i][0..8] (3 rows padded to
+ * float4: [i][4 r + c]); fo_q_surfel evaluates u^2 + v^2 from it.  G = exp(-(u^2+v^2)/2)
+ * (PAPER.md:85).  Readings: depth of the key = z of the centre; a splat is culled when
+ * its centre or any point of its 3-sigma disc lies in front of z_near (z_min = c_z -
+ * 3 sqrt(a_z^2 + b_z^2)); no low-pass filter (the paper states none).
+ * Screen bounds (conservative AABB of the pixels with u^2+v^2 <= q_cut): the
+ * 3-sigma disc maps to the conic x~^T T^-T diag(1,1,-q) T^-1 x~ <= 0, whose bounding box follows
+ * from the dual conic T diag(q,q,-1) T^T:  centre_x = (q T_x0 T_w0 + q T_x1 T_w1 - T_x2 T_w2)/d,
+ * half_x^2 = centre_x^2 - (q T_x0^2 + q T_x1^2 - T_x2^2)/d,  d = q T_w0^2 + q T_w1^2 - T_w2^2 < 0;
+ * one pixel of margin absorbs the binary32 rounding.  Outputs: xy = box centre, conic_opacity =
+ * (half_x, half_y, 0, opacity), radius = max of the two integer half extents, rect from the box.
+ * Same arithmetic rule as fo_project: single binary32 operations in the written order.
+ * ------------------------------------------------------------------------------------------ */
+static void cross3(const float *a, const float *b, float *o) {
+    o[0] = a[1] * b[2] - a[2] * b[1];
+    o[1] = a[2] * b[0] - a[0] * b[2];
+    o[2] = a[0] * b[1] - a[1] * b[0];
+}
+
+void fo_project_surfel(int n, int sh_degree, const float *mean, const float *scale, const float *quat,
+                       const float *opacity, const float *sh, const float *cam, int W, int H,
+                       const float *prm, float *xy, float *depth, float *conic_opacity, float *rgb,
+                       int32_t *radius, uint16_t *rect, uint32_t *tiles_touched, float *ray_transform) {
+    float fx, fy, cx, cy, tanx, tany;
+    intrinsics(cam, W, H, &fx, &fy, &cx, &cy, &tanx, &tany);
+    const float *V = cam;
+    const float *cp = cam + 32;
+    const int GW = (W + TILE - 1) / TILE, GH = (H + TILE - 1) / TILE;
+    const int K = (sh_degree + 1) * (sh_degree + 1);
+    const float z_near = prm[P_ZNEAR], qc = prm[P_QCUT];
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < n; ++i) {
+        xy[2 * i] = xy[2 * i + 1] = 0.0f; depth[i] = 0.0f;
+        for (int k = 0; k < 4; ++k) conic_opacity[4 * i + k] = 0.0f;
+        for (int k = 0; k < 3; ++k) rgb[3 * i + k] = 0.0f;
+        radius[i] = 0; tiles_touched[i] = 0;
+        for (int k = 0; k < 4; ++k) rect[4 * i + k] = 0;
+        for (int k = 0; k < 12; ++k) ray_transform[12 * i + k] = 0.0f;
+
+        const float p0 = mean[3 * i], p1 = mean[3 * i + 1], p2 = mean[3 * i + 2];
+        /* 1. camera-space centre */
+        float c[3];
+        for (int k = 0; k < 3; ++k)
+            c[k] = ((V[4 * k] * p0 + V[4 * k + 1] * p1) + V[4 * k + 2] * p2) + V[4 * k + 3];
+        if (!(c[2] >= z_near)) continue;
+        /* 2. scaled tangents in camera space: a = R_v (s_u t_u), b = R_v (s_v t_v) */
+        float R[9];
+        fo_quat_to_rot(quat + 4 * i, R);
+        const float su = scale[3 * i], sv = scale[3 * i + 1];
+        const float aw[3] = {R[0] * su, R[3] * su, R[6] * su}, bw[3] = {R[1] * sv, R[4] * sv, R[7] * sv};
+        float a[3], b[3];
+        for (int k = 0; k < 3; ++k) {
+            a[k] = (V[4 * k] * aw[0] + V[4 * k + 1] * aw[1]) + V[4 * k + 2] * aw[2];
+            b[k] = (V[4 * k] * bw[0] + V[4 * k + 1] * bw[1]) + V[4 * k + 2] * bw[2];
+        }
+        /* 3. the whole 3-sigma disc must lie behind the near plane */
+        const float zmin = c[2] - 3.0f * sqrtf(a[2] * a[2] + b[2] * b[2]);
+        if (!(zmin >= z_near)) continue;
+        /* 4. T (rows x, y, w) */
+        const float Tx[3] = {fx * a[0] + cx * a[2], fx * b[0] + cx * b[2], fx * c[0] + cx * c[2]};
+        const float Ty[3] = {fy * a[1] + cy * a[2], fy * b[1] + cy * b[2], fy * c[1] + cy * c[2]};
+        const float Tw[3] = {a[2], b[2], c[2]};
+        /* 5. adj(T): columns A0 = Ty x Tw, A1 = Tw x Tx, A2 = Tx x Ty; scaled by 2^-e, e = exponent of max |entry| */
+        float A0[3], A1[3], A2[3];
+        cross3(Ty, Tw, A0); cross3(Tw, Tx, A1); cross3(Tx, Ty, A2);
+        float mx = 0.0f;
+        for (int k = 0; k < 3; ++k) mx = fmaxf(mx, fmaxf(fabsf(A0[k]), fmaxf(fabsf(A1[k]), fabsf(A2[k]))));
+        if (!(mx > 0.0f) || !isfinite(mx)) continue;
+        int e; (void)frexpf(mx, &e);
+        const float sc = ldexpf(1.0f, -e);
+        /* 6. bounding box of the q <= q_cut footprint from the dual conic */
+        const float d = (qc * (Tw[0] * Tw[0]) + qc * (Tw[1] * Tw[1])) - Tw[2] * Tw[2];
+        if (!(d < 0.0f)) continue;
+        const float ccx = ((qc * (Tx[0] * Tw[0]) + qc * (Tx[1] * Tw[1])) - Tx[2] * Tw[2]) / d;
+        const float ccy = ((qc * (Ty[0] * Tw[0]) + qc * (Ty[1] * Tw[1])) - Ty[2] * Tw[2]) / d;
+        const float ex = ccx * ccx - ((qc * (Tx[0] * Tx[0]) + qc * (Tx[1] * Tx[1])) - Tx[2] * Tx[2]) / d;
+        const float ey = ccy * ccy - ((qc * (Ty[0] * Ty[0]) + qc * (Ty[1] * Ty[1])) - Ty[2] * Ty[2]) / d;
+        const float hx = sqrtf(fmaxf(ex, 1e-4f)) + 1.0f, hy = sqrtf(fmaxf(ey, 1e-4f)) + 1.0f;
+        if (!(isfinite(ccx) && isfinite(ccy) && isfinite(hx) && isfinite(hy))) continue;
+        const float rx = ceilf(hx), ry = ceilf(hy);
+        const float x0 = clampf(floorf((ccx - rx) / 16.0f), 0.0f, (float)GW);
+        const float x1 = clampf(floorf((ccx + rx) / 16.0f) + 1.0f, 0.0f, (float)GW);
+        const float y0 = clampf(floorf((ccy - ry) / 16.0f), 0.0f, (float)GH);
+        const float y1 = clampf(floorf((ccy + ry) / 16.0f) + 1.0f, 0.0f, (float)GH);
+        const int ix0 = (int)x0, ix1 = (int)x1, iy0 = (int)y0, iy1 = (int)y1;
+        if (ix1 <= ix0 || iy1 <= iy0) continue;
+        /* 7. SH colour (C1-P step 10) */
+        float dx = p0 - cp[0], dy = p1 - cp[1], dz = p2 - cp[2];
+        const float dn = sqrtf((dx * dx + dy * dy) + dz * dz);
+        dx = dx / dn; dy = dy / dn; dz = dz / dn;
+        float Yb[16];
+        fo_sh_basis(sh_degree, dx, dy, dz, Yb);
+        for (int k = 0; k < 3; ++k) {
+            float col = 0.5f;
+            for (int l = 0; l < K; ++l) col = col + Yb[l] * sh[((size_t)i * K + l) * 3 + k];
+            rgb[3 * i + k] = fmaxf(col, 0.0f);
+        }
+        xy[2 * i] = ccx; xy[2 * i + 1] = ccy; depth[i] = c[2];
+        conic_opacity[4 * i] = hx; conic_opacity[4 * i + 1] = hy; conic_opacity[4 * i + 3] = opacity[i];
+        radius[i] = (int32_t)fmaxf(rx, ry);
+        rect[4 * i] = (uint16_t)ix0; rect[4 * i + 1] = (uint16_t)iy0;
+        rect[4 * i + 2] = (uint16_t)ix1; rect[4 * i + 3] = (uint16_t)iy1;
+        tiles_touched[i] = (uint32_t)((ix1 - ix0) * (iy1 - iy0));
+        float *rt = ray_transform + 12 * i;
+        for (int r = 0; r < 3; ++r) { rt[4 * r] = A0[r] * sc; rt[4 * r + 1] = A1[r] * sc; rt[4 * r + 2] = A2[r] * sc; }
+    }
+}
+
+/* The per-(pixel, surfel) decision quantities in binary32 (both sides evaluate exactly this):
+ *   p = adj(T) (x, y, 1)^T,  num = p_x^2 + p_y^2,  den = p_z^2;  (u, v) = (p_x, p_y)/p_z.
+ * The surfel contributes iff den > 0 and num <= q_cut * den  (u^2 + v^2 <= q_cut without a division). */
+void fo_surfel_terms(const float *rt, int x, int y, float *p /*[3]*/, float *num, float *den) {
+    const float fxp = (float)x, fyp = (float)y;
+    p[0] = fmaf(fxp, rt[0], fmaf(fyp, rt[1], rt[2]));
+    p[1] = fmaf(fxp, rt[4], fmaf(fyp, rt[5], rt[6]));
+    p[2] = fmaf(fxp, rt[8], fmaf(fyp, rt[9], rt[10]));
+    *num = fmaf(p[0], p[0], p[1] * p[1]);
+    *den = p[2] * p[2];
+}
+
+/* ------------------------------------------------------------------------------------------
  * Step S (C1-S): PAPER.md:302 DuplicateWithKeys / SortByKeys / IdentifyTileRanges.
  * key = (tile_id << 32) | float_bits(z_cam); stable sort (ties keep ascending Gaussian index,
  * SPEC.md:186); ranges[t] = [first, last+1), (0,0) for an empty tile.
@@ -305,8 +436,21 @@ float fo_q(float pxg, float pyg, float A, float B, float C, int x, int y) {
     return fmaf(dx, fmaf(2.0f * B, dy, A * dx), (C * dy) * dy);
 }
 
+/* Surfel mode (NEXT-3): g_rt != NULL selects the ray-transform evaluation for every driver below.  It is set by
+ * fo_set_surfel() around a call (the drivers' argument lists stay those of the EWA path). */
+static const float *g_rt = NULL;
+void fo_set_surfel(const float *ray_transform /* [n,12] or NULL */) { g_rt = ray_transform; }
+
 static inline int eval_alpha(const float *xy, const float *co, uint32_t g, int x, int y,
                              float q_cut, float alpha_max, double *alpha) {
+    if (g_rt) {
+        float p[3], num, den;
+        fo_surfel_terms(g_rt + 12 * (size_t)g, x, y, p, &num, &den);
+        if (!(den > 0.0f) || !(num <= q_cut * den)) return 0;
+        const double G = exp(-0.5 * ((double)num / (double)den));
+        *alpha = fmin((double)alpha_max, (double)co[4 * g + 3] * G);
+        return 1;
+    }
     const float q = fo_q(xy[2 * g], xy[2 * g + 1], co[4 * g], co[4 * g + 1], co[4 * g + 2], x, y);
     if (!(q <= q_cut)) return 0;
     const double G = exp(-0.5 * fmax((double)q, 0.0));

@@ -101,11 +101,41 @@ def project(mean, scale, quat, opacity, sh, sh_degree, cam, W, H, params=DEFAULT
                conic_opacity=np.zeros((n, 4), np.float32), rgb=np.zeros((n, 3), np.float32),
                radius=np.zeros(n, np.int32), rect=np.zeros((n, 4), np.uint16),
                tiles_touched=np.zeros(n, np.uint32))
-    lib().fo_project(C.c_int(n), C.c_int(sh_degree), _p(mean), _p(scale), _p(quat), _p(opacity),
-                     _p(sh), _p(_f32(cam)), C.c_int(W), C.c_int(H), _p(_f32(params)),
-                     _p(out["xy"]), _p(out["depth"]), _p(out["conic_opacity"]), _p(out["rgb"]),
-                     _p(out["radius"]), _p(out["rect"]), _p(out["tiles_touched"]))
+    common = (C.c_int(n), C.c_int(sh_degree), _p(mean), _p(scale), _p(quat), _p(opacity),
+              _p(sh), _p(_f32(cam)), C.c_int(W), C.c_int(H), _p(_f32(params)),
+              _p(out["xy"]), _p(out["depth"]), _p(out["conic_opacity"]), _p(out["rgb"]),
+              _p(out["radius"]), _p(out["rect"]), _p(out["tiles_touched"]))
+    if float(params[P_PRIM]) != 0.0:      # NEXT-3: 2-D surfels; the projected state carries the per-splat ray transform
+        out["ray_transform"] = np.zeros((n, 12), np.float32)
+        lib().fo_project_surfel(*common, _p(out["ray_transform"]))
+    else:
+        lib().fo_project(*common)
     return out
+
+
+class _surfel:
+    """Selects the surfel evaluation (fo_set_surfel) for the duration of one oracle call when the projected state
+    `pr` came from the surfel projection."""
+
+    def __init__(self, pr):
+        self.rt = pr.get("ray_transform")
+
+    def __enter__(self):
+        if self.rt is not None:
+            lib().fo_set_surfel(_p(np.ascontiguousarray(self.rt)))
+
+    def __exit__(self, *a):
+        if self.rt is not None:
+            lib().fo_set_surfel(None)
+
+
+def surfel_terms(rt_row, x, y):
+    """(p[3], num, den) of fo_surfel_terms for one surfel and pixel: (u, v) = p[:2] / p[2], q = num / den."""
+    rt_row = _f32(rt_row)
+    p3 = np.zeros(3, np.float32)
+    num, den = C.c_float(0), C.c_float(0)
+    lib().fo_surfel_terms(_p(rt_row), C.c_int(int(x)), C.c_int(int(y)), _p(p3), C.byref(num), C.byref(den))
+    return p3, float(num.value), float(den.value)
 
 
 def bins(pr, W, H, want_unsorted=False):
@@ -152,7 +182,8 @@ def render_literal(pr, order, feat, W, H, params=DEFAULT_PARAMS, pix=None):
         pix = np.ascontiguousarray(pix, dtype=np.int32)
     npix = W * H if pix is None else pix.shape[0]
     o = _render_out(npix, D, feat32 is not None)
-    lib().fo_render_literal(C.c_int(order.shape[0]), _p(order), C.c_int(D), _p(pr["xy"]),
+    with _surfel(pr):
+      lib().fo_render_literal(C.c_int(order.shape[0]), _p(order), C.c_int(D), _p(pr["xy"]),
                             _p(pr["conic_opacity"]), _p(pr["rgb"]), _p(feat32), C.c_int(W),
                             C.c_int(H), _p(_f32(params)), C.c_int64(npix), _p(pix), _p(o["rgb"]),
                             _p(o["feat"]), _p(o["T"]), _p(o["n"]), _p(o["fragile"]))
@@ -163,7 +194,8 @@ def render_scatter(pr, order, feat, W, H, params=DEFAULT_PARAMS):
     feat32 = None if feat is None else _f32(feat)
     D = 0 if feat32 is None else feat32.shape[1]
     o = _render_out(W * H, D, feat32 is not None)
-    lib().fo_render_scatter(C.c_int(order.shape[0]), _p(order), C.c_int(D), _p(pr["xy"]),
+    with _surfel(pr):
+      lib().fo_render_scatter(C.c_int(order.shape[0]), _p(order), C.c_int(D), _p(pr["xy"]),
                             _p(pr["conic_opacity"]), _p(pr["rgb"]), _p(feat32), _p(pr["radius"]),
                             C.c_int(W), C.c_int(H), _p(_f32(params)), _p(o["rgb"]), _p(o["feat"]),
                             _p(o["T"]), _p(o["n"]), _p(o["fragile"]))
@@ -179,10 +211,12 @@ def fuse(pr, order, gt, W, H, params=DEFAULT_PARAMS, num=None, den=None, literal
         num = np.zeros((n, D), np.float64)
         den = np.zeros(n, np.float64)
     if literal:
+      with _surfel(pr):
         lib().fo_fuse_literal(C.c_int(n), C.c_int(order.shape[0]), _p(order), C.c_int(D),
                               _p(pr["xy"]), _p(pr["conic_opacity"]), _p(gt32), C.c_int(W),
                               C.c_int(H), _p(_f32(params)), _p(num), _p(den))
     else:
+      with _surfel(pr):
         lib().fo_fuse_scatter(C.c_int(n), C.c_int(order.shape[0]), _p(order), C.c_int(D),
                               _p(pr["xy"]), _p(pr["conic_opacity"]), _p(pr["radius"]), _p(gt32),
                               C.c_int(W), C.c_int(H), _p(_f32(params)), _p(num), _p(den))
@@ -209,17 +243,20 @@ def ndfd(pr, order, feat, gt, W, H, k=20.0, lam=0.5, mode=0, params=DEFAULT_PARA
     lgt, lcf = np.zeros(npix, np.float64), np.zeros(npix, np.float64)
     args = (C.c_int(order.shape[0]), _p(order), C.c_int(D), _p(pr["xy"]), _p(pr["conic_opacity"]), _p(feat32), _p(gt32),
             C.c_int(W), C.c_int(H), _p(_f32(params)), C.c_double(k), C.c_double(lam), C.c_int(mode), C.c_int64(npix), _p(pix))
-    lib().fo_ndfd_literal(*args, _p(lgt), _p(lcf))
+    with _surfel(pr):
+        lib().fo_ndfd_literal(*args, _p(lgt), _p(lcf))
     if not pairwise:
         return lgt, lcf
     pw = np.zeros(npix, np.float64)
-    lib().fo_ndfd_pairwise(*args, _p(pw))
+    with _surfel(pr):
+        lib().fo_ndfd_pairwise(*args, _p(pw))
     return lgt, lcf, pw
 
 
 def ndfd_backward(pr, order, feat, gt, W, H, k=20.0, lam=0.5, lam1=1.0, lam2=1.0, params=DEFAULT_PARAMS, pix=None):
     """NDFD backward at the w level: returns (L, grad_opacity[n]) with
     L = sum over `pix` of lam1 L_gt + lam2 L_cf (blend-order accumulation) and grad_opacity = dL/d opacity."""
+    assert "ray_transform" not in pr, "the w-level backward is built for the EWA primitive only"
     feat32, gt32 = _f32(feat), _f32(gt)
     D = feat32.shape[1]
     n = pr["radius"].shape[0]

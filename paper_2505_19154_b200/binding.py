@@ -58,7 +58,7 @@ class CViewState(C.Structure):
                 ("radius", C.c_void_p), ("rect", C.c_void_p), ("tiles_touched", C.c_void_p),
                 ("offsets", C.c_void_p), ("num_instances", C.c_void_p),
                 ("keys", C.c_void_p * 2), ("vals", C.c_void_p * 2), ("ranges", C.c_void_p),
-                ("scratch", C.c_void_p), ("scratch_bytes", C.c_size_t)]
+                ("scratch", C.c_void_p), ("scratch_bytes", C.c_size_t), ("ray_transform", C.c_void_p)]
 
 
 class CHostFrame(C.Structure):
@@ -237,7 +237,7 @@ class Gaussians:
 class ViewState:
     """Caller-owned per-view buffers (fhgs_view_state)."""
 
-    def __init__(self, n: int, width: int, height: int, capacity: int, device="cuda"):
+    def __init__(self, n: int, width: int, height: int, capacity: int, device="cuda", surfel: bool = False):
         self.n, self.width, self.height, self.capacity = int(n), int(width), int(height), int(capacity)
         gw, gh = (width + 15) // 16, (height + 15) // 16
         z = lambda shape, dt: torch.zeros(shape, dtype=dt, device=device)
@@ -267,6 +267,8 @@ class ViewState:
         sp = self.scratch.data_ptr()
         c.scratch = (sp + 255) // 256 * 256
         c.scratch_bytes = sb
+        self.ray_transform = z((m, 12), torch.float32) if surfel else None     # FHGS_PRIM_SURFEL only
+        c.ray_transform = self.ray_transform.data_ptr() if surfel else None
 
     def tile_visited(self) -> torch.Tensor:
         """Diagnostics written by fhgs_render (see fhgs_scratch_tile_visited): int32 tensor [GW*GH] (device)."""
@@ -287,7 +289,8 @@ class ViewState:
         return dict(xy=self.xy[:n].cpu().numpy(), depth=self.depth[:n].cpu().numpy(),
                     conic_opacity=self.conic_opacity[:n].cpu().numpy(), rgb=self.rgb[:n].cpu().numpy(),
                     radius=self.radius[:n].cpu().numpy(), rect=self.rect[:n].cpu().numpy().view(np.uint16),
-                    tiles_touched=self.tiles_touched[:n].cpu().numpy().view(np.uint32))
+                    tiles_touched=self.tiles_touched[:n].cpu().numpy().view(np.uint32),
+                    **({} if self.ray_transform is None else {"ray_transform": self.ray_transform[:n].cpu().numpy()}))
 
 
 def project(ctx: Context, g: Gaussians, cam: CCamera, prm: CParams, vs: ViewState, stream=None):

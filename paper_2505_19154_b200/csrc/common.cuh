@@ -82,3 +82,9 @@ static inline int tiles_y(int h) { return (h + FHGS_TILE - 1) / FHGS_TILE; }
 fhgs_status validate_camera(fhgs_ctx* ctx, const fhgs_camera* cam);
 fhgs_status validate_params(fhgs_ctx* ctx, const fhgs_params* prm);
 fhgs_status validate_view_state(fhgs_ctx* ctx, const fhgs_view_state* vs, const fhgs_camera* cam);
+// FHGS_PRIM_SURFEL needs the per-splat ray transform in the view state
+static inline fhgs_status validate_primitive(fhgs_ctx* ctx, const fhgs_params* prm, const fhgs_view_state* vs) {
+    if (prm->primitive == FHGS_PRIM_SURFEL && (!vs->ray_transform || !aligned_to(vs->ray_transform, 16)))
+        FHGS_INVALID(ctx, "surfel mode needs vs->ray_transform ([n,12] f32, 16-byte aligned)");
+    return FHGS_OK;
+}

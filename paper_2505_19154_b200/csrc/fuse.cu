@@ -49,9 +49,9 @@ __device__ __forceinline__ float4 load_gt4<__half>(const __half* p) {
     return make_float4(a.x, a.y, b.x, b.y);
 }
 
-template <int DC>
+template <int DC, int PRIM>
 struct FuseTiledSmem {
-    TileQueue q;
+    TileQueueT<PRIM> q;
     __align__(16) float W[F_KB * TR_THREADS];   // W[kk][slot]
     __align__(16) float G[TR_THREADS * DC];     // G[slot][channel]
     float den[F_KB];
@@ -103,10 +103,10 @@ __device__ __forceinline__ void fuse_gemm(const float* __restrict__ W, const flo
     }
 }
 
-template <int DC, typename GT>
+template <int DC, typename GT, int PRIM>
 __global__ void __launch_bounds__(TR_THREADS, 1) fuse_tiled_kernel(const FuseArgs a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    FuseTiledSmem<DC>& sm = *reinterpret_cast<FuseTiledSmem<DC>*>(smem_raw);
+    FuseTiledSmem<DC, PRIM>& sm = *reinterpret_cast<FuseTiledSmem<DC, PRIM>*>(smem_raw);
 
     const int tid = threadIdx.x;
     const int tile = blockIdx.x;
@@ -151,7 +151,7 @@ __global__ void __launch_bounds__(TR_THREADS, 1) fuse_tiled_kernel(const FuseArg
             // phase B
             for (int kk = 0; kk < nb; ++kk) {
                 const int s = (q_head + kk) & (TR_QCAP - 1);
-                sm.W[kk * TR_THREADS + tid] = eval_weight(sm.q.xy[s], sm.q.co[s], fx, fy, a.t, T, done, n);
+                sm.W[kk * TR_THREADS + tid] = eval_weight_q<PRIM>(sm.q, s, fx, fy, a.t, T, done, n);
             }
             __syncthreads();
             // row sums (den): thread t sums quarter t%4 of row t/4
@@ -522,13 +522,14 @@ __global__ void __launch_bounds__(FW_THREADS, 1) fuse_ws_kernel(const FuseArgs a
 // ---------------------------------------------------------------------------------------------
 // PIXEL variant: CH channels per pass held by the pixel's thread; warp-segment reduction
 // ---------------------------------------------------------------------------------------------
+template <int PRIM>
 struct FusePixelSmem {
-    TileQueue q;
+    TileQueueT<PRIM> q;
 };
 
-template <int CH, typename GT>
+template <int CH, typename GT, int PRIM>
 __global__ void __launch_bounds__(TR_THREADS) fuse_pixel_kernel(const FuseArgs a) {
-    __shared__ FusePixelSmem sm;
+    __shared__ FusePixelSmem<PRIM> sm;
     const int tid = threadIdx.x, lane = tid & 31;
     const int tile = blockIdx.x;
     const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
@@ -566,7 +567,7 @@ __global__ void __launch_bounds__(TR_THREADS) fuse_pixel_kernel(const FuseArgs a
             if (nb == 0) break;
             for (int kk = 0; kk < nb; ++kk) {
                 const int s = (q_head + kk) & (TR_QCAP - 1);
-                const float w = eval_weight(sm.q.xy[s], sm.q.co[s], fx, fy, a.t, T, done, n);
+                const float w = eval_weight_q<PRIM>(sm.q, s, fx, fy, a.t, T, done, n);
                 if (!__any_sync(TR_FULL, w != 0.f)) continue;
                 const uint32_t id = sm.q.id[s];
                 float v[CH + 1];
@@ -684,11 +685,17 @@ cudaError_t launch_fuse_ws(const FuseArgs& a, int tiles, int num_sms, uint32_t* 
 
 template <typename GT>
 cudaError_t dispatch(const FuseArgs& a, int grid, int num_sms, uint32_t* queue, const uint32_t* order, cudaStream_t st) {
+    if (a.t.ray_transform) {   // surfel mode (NEXT-3): the tile-per-CTA kernels for every D
+        if (a.D % 64 == 0) return launch(fuse_tiled_kernel<64, GT, 1>, sizeof(FuseTiledSmem<64, 1>), grid, st, a);
+        if (a.D % 16 == 0) return launch(fuse_pixel_kernel<16, GT, 1>, 0, grid, st, a);
+        if (a.D % 8 == 0) return launch(fuse_pixel_kernel<8, GT, 1>, 0, grid, st, a);
+        return launch(fuse_pixel_kernel<4, GT, 1>, 0, grid, st, a);
+    }
     if (a.D % FW_DC == 0) return launch_fuse_ws<GT>(a, grid, num_sms, queue, order, st);
-    if (a.D % 64 == 0) return launch(fuse_tiled_kernel<64, GT>, sizeof(FuseTiledSmem<64>), grid, st, a);
-    if (a.D % 16 == 0) return launch(fuse_pixel_kernel<16, GT>, 0, grid, st, a);
-    if (a.D % 8 == 0) return launch(fuse_pixel_kernel<8, GT>, 0, grid, st, a);
-    return launch(fuse_pixel_kernel<4, GT>, 0, grid, st, a);
+    if (a.D % 64 == 0) return launch(fuse_tiled_kernel<64, GT, 0>, sizeof(FuseTiledSmem<64, 0>), grid, st, a);
+    if (a.D % 16 == 0) return launch(fuse_pixel_kernel<16, GT, 0>, 0, grid, st, a);
+    if (a.D % 8 == 0) return launch(fuse_pixel_kernel<8, GT, 0>, 0, grid, st, a);
+    return launch(fuse_pixel_kernel<4, GT, 0>, 0, grid, st, a);
 }
 
 }  // namespace
@@ -733,6 +740,7 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
         if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
         if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
         if (!aligned_to(gt, 16)) FHGS_INVALID(ctx, "fhgs_fuse_features: gt must be 16-byte aligned");
+        if ((st = validate_primitive(ctx, prm, vs)) != FHGS_OK) return st;
     }
     if (finalize) {
         if (!out_feat) FHGS_INVALID(ctx, "fhgs_fuse_features: FINALIZE needs out_feat");
@@ -757,6 +765,7 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
         a.t.xy = reinterpret_cast<const float2*>(vs->xy);
         a.t.conic_opacity = reinterpret_cast<const float4*>(vs->conic_opacity);
         a.t.q_cutoff = prm->q_cutoff; a.t.alpha_max = prm->alpha_max; a.t.t_min = prm->t_min;
+        a.t.ray_transform = prm->primitive == FHGS_PRIM_SURFEL ? reinterpret_cast<const float4*>(vs->ray_transform) : nullptr;
         a.gt = gt; a.D = feat_dim; a.num = num; a.den = den;
         const int grid = tiles_x(cam->width) * tiles_y(cam->height);
         const ScratchLayout L = make_scratch_layout(vs->n, vs->capacity, cam->width, cam->height);

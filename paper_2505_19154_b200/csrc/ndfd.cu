@@ -268,6 +268,7 @@ extern "C" fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g,
     if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
     if ((st = validate_params(ctx, prm)) != FHGS_OK) return st;
     if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
+    if (prm->primitive != FHGS_PRIM_EWA) FHGS_INVALID(ctx, "the NDFD calls are built for FHGS_PRIM_EWA only");
     if (!g->feat) FHGS_INVALID(ctx, "fhgs_ndfd_forward: g->feat is NULL");
     if ((g->feat_dtype != FHGS_F32 && g->feat_dtype != FHGS_F16) || (gt_dtype != FHGS_F32 && gt_dtype != FHGS_F16))
         FHGS_INVALID(ctx, "fhgs_ndfd_forward: unknown dtype");
@@ -284,6 +285,7 @@ extern "C" fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g,
     a.t.xy = reinterpret_cast<const float2*>(vs->xy);
     a.t.conic_opacity = reinterpret_cast<const float4*>(vs->conic_opacity);
     a.t.q_cutoff = prm->q_cutoff; a.t.alpha_max = prm->alpha_max; a.t.t_min = prm->t_min;
+    a.t.ray_transform = nullptr;
     a.feat = g->feat; a.gt = gt; a.D = D; a.k_sig = k_sigmoid; a.lambda = lambda;
     a.out_lgt = out_lgt; a.out_lcf = out_lcf;
     const int tiles = tiles_x(cam->width) * tiles_y(cam->height);

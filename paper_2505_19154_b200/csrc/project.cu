@@ -34,6 +34,8 @@ struct ProjectArgs {
     int32_t* radius;
     uint16_t* rect;
     uint32_t* tiles_touched;
+    float q_cutoff;          // surfel mode: the footprint u^2 + v^2 <= q_cutoff
+    float* ray_transform;    // surfel mode: [n,12]
 };
 
 constexpr int PROJ_THREADS = 256;
@@ -64,18 +66,12 @@ __device__ __forceinline__ void sh_basis(int degree, float x, float y, float z, 
     Y[15] = mul(mul(-0.5900435899266435f, x), sub(xx, mul(3.0f, yy)));
 }
 
+// Stage the CTA's SH rows: contiguous span [base*ROW, (base+cnt)*ROW), coalesced; row r lands at s_sh[r * PAD].
 template <int DEG>
-__global__ void __launch_bounds__(PROJ_THREADS) project_kernel(const ProjectArgs a) {
+__device__ __forceinline__ void stage_sh_rows(const ProjectArgs& a, float* s_sh, int base, int cnt) {
     constexpr int K = (DEG + 1) * (DEG + 1);
-    constexpr int ROW = 3 * K;                 // floats per Gaussian
-    constexpr int PAD = (ROW % 2 == 0) ? ROW + 1 : ROW;  // odd stride -> conflict-free rows
-    extern __shared__ float s_sh[];            // [PROJ_THREADS][PAD]
-
-    const int base = blockIdx.x * PROJ_THREADS;
-    const int i = base + threadIdx.x;
-    const int cnt = min(PROJ_THREADS, a.n - base);
-
-    // Stage this CTA's SH rows: contiguous span [base*ROW, (base+cnt)*ROW), coalesced.
+    constexpr int ROW = 3 * K;
+    constexpr int PAD = (ROW % 2 == 0) ? ROW + 1 : ROW;
     {
         const float* src = a.sh + (size_t)base * ROW;
         const int total = cnt * ROW;
@@ -97,6 +93,37 @@ __global__ void __launch_bounds__(PROJ_THREADS) project_kernel(const ProjectArgs
                 s_sh[(e / ROW) * PAD + e % ROW] = __ldg(src + e);
         }
     }
+}
+
+// C1-P step 10: SH colour of Gaussian at world position (p0,p1,p2) from its staged SH row.
+template <int DEG>
+__device__ __forceinline__ void sh_colour(const ProjectArgs& a, const float* row, float p0, float p1, float p2, float* o_rgb) {
+    constexpr int K = (DEG + 1) * (DEG + 1);
+    float dx = sub(p0, a.cam_pos[0]), dy = sub(p1, a.cam_pos[1]), dz = sub(p2, a.cam_pos[2]);
+    const float dn = sq(add(add(mul(dx, dx), mul(dy, dy)), mul(dz, dz)));
+    dx = dvd(dx, dn); dy = dvd(dy, dn); dz = dvd(dz, dn);
+    float Yb[K];
+    sh_basis(DEG, dx, dy, dz, Yb);
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        float c = 0.5f;
+#pragma unroll
+        for (int l = 0; l < K; ++l) c = add(c, mul(Yb[l], row[3 * l + k]));
+        o_rgb[k] = fmaxf(c, 0.0f);
+    }
+}
+
+template <int DEG>
+__global__ void __launch_bounds__(PROJ_THREADS) project_kernel(const ProjectArgs a) {
+    constexpr int K = (DEG + 1) * (DEG + 1);
+    constexpr int ROW = 3 * K;                 // floats per Gaussian
+    constexpr int PAD = (ROW % 2 == 0) ? ROW + 1 : ROW;  // odd stride -> conflict-free rows
+    extern __shared__ float s_sh[];            // [PROJ_THREADS][PAD]
+
+    const int base = blockIdx.x * PROJ_THREADS;
+    const int i = base + threadIdx.x;
+    const int cnt = min(PROJ_THREADS, a.n - base);
+    stage_sh_rows<DEG>(a, s_sh, base, cnt);
     __syncthreads();
     if (i >= a.n) return;
 
@@ -198,19 +225,7 @@ __global__ void __launch_bounds__(PROJ_THREADS) project_kernel(const ProjectArgs
         const int ix0 = (int)x0, ix1 = (int)x1, iy0 = (int)y0, iy1 = (int)y1;
         if (ix1 <= ix0 || iy1 <= iy0) break;
         // 10. SH colour
-        float dx = sub(p0, a.cam_pos[0]), dy = sub(p1, a.cam_pos[1]), dz = sub(p2, a.cam_pos[2]);
-        const float dn = sq(add(add(mul(dx, dx), mul(dy, dy)), mul(dz, dz)));
-        dx = dvd(dx, dn); dy = dvd(dy, dn); dz = dvd(dz, dn);
-        float Yb[K];
-        sh_basis(DEG, dx, dy, dz, Yb);
-        const float* row = s_sh + threadIdx.x * PAD;
-#pragma unroll
-        for (int k = 0; k < 3; ++k) {
-            float c = 0.5f;
-#pragma unroll
-            for (int l = 0; l < K; ++l) c = add(c, mul(Yb[l], row[3 * l + k]));
-            o_rgb[k] = fmaxf(c, 0.0f);
-        }
+        sh_colour<DEG>(a, s_sh + threadIdx.x * PAD, p0, p1, p2, o_rgb);
         o_xy0 = px; o_xy1 = py; o_depth = z;
         o_co = make_float4(conA, conB, conC, __ldg(a.opacity + i));
         o_radius = (int)r;
@@ -229,6 +244,127 @@ __global__ void __launch_bounds__(PROJ_THREADS) project_kernel(const ProjectArgs
     a.tiles_touched[i] = o_tt;
 }
 
+// ---------------------------------------------------------------------------------------------
+// Surfel mode (FHGS_PRIM_SURFEL, Eq. 1-3): homography T = K [a b c] of the splat's
+// tangent plane, its adjugate as the per-splat ray transform, the footprint's bounding box from the dual conic.
+// Same arithmetic rule: single binary32 operations in the written order (bit-identical to the oracle's statement).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void cross3(const float* x, const float* y, float* o) {
+    o[0] = sub(mul(x[1], y[2]), mul(x[2], y[1]));
+    o[1] = sub(mul(x[2], y[0]), mul(x[0], y[2]));
+    o[2] = sub(mul(x[0], y[1]), mul(x[1], y[0]));
+}
+
+template <int DEG>
+__global__ void __launch_bounds__(PROJ_THREADS) project_surfel_kernel(const ProjectArgs a) {
+    constexpr int K = (DEG + 1) * (DEG + 1);
+    constexpr int ROW = 3 * K;
+    constexpr int PAD = (ROW % 2 == 0) ? ROW + 1 : ROW;
+    extern __shared__ float s_sh[];
+    const int base = blockIdx.x * PROJ_THREADS;
+    const int i = base + threadIdx.x;
+    const int cnt = min(PROJ_THREADS, a.n - base);
+    stage_sh_rows<DEG>(a, s_sh, base, cnt);
+    __syncthreads();
+    if (i >= a.n) return;
+
+    float o_xy0 = 0.f, o_xy1 = 0.f, o_depth = 0.f;
+    float4 o_co = make_float4(0.f, 0.f, 0.f, 0.f);
+    float o_rgb[3] = {0.f, 0.f, 0.f};
+    int o_radius = 0;
+    uint32_t o_tt = 0;
+    ushort4 o_rect = make_ushort4(0, 0, 0, 0);
+    float4 o_rt[3] = {make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f), make_float4(0.f, 0.f, 0.f, 0.f)};
+
+    do {
+        const float p0 = __ldg(a.mean + 3 * (size_t)i), p1 = __ldg(a.mean + 3 * (size_t)i + 1),
+                    p2 = __ldg(a.mean + 3 * (size_t)i + 2);
+        const float* V = a.V;
+        // 1. camera-space centre
+        float c[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k)
+            c[k] = add(add(add(mul(V[4 * k], p0), mul(V[4 * k + 1], p1)), mul(V[4 * k + 2], p2)), V[4 * k + 3]);
+        if (!(c[2] >= a.z_near)) break;
+        // 2. scaled tangents in camera space
+        const float4 qv = __ldg(reinterpret_cast<const float4*>(a.quat) + i);
+        float qw = qv.x, qx = qv.y, qy = qv.z, qz = qv.w;
+        const float qn = sq(add(add(add(mul(qw, qw), mul(qx, qx)), mul(qy, qy)), mul(qz, qz)));
+        qw = dvd(qw, qn); qx = dvd(qx, qn); qy = dvd(qy, qn); qz = dvd(qz, qn);
+        float R[9];
+        R[0] = sub(1.0f, mul(2.0f, add(mul(qy, qy), mul(qz, qz))));
+        R[1] = mul(2.0f, sub(mul(qx, qy), mul(qw, qz)));
+        R[3] = mul(2.0f, add(mul(qx, qy), mul(qw, qz)));
+        R[4] = sub(1.0f, mul(2.0f, add(mul(qx, qx), mul(qz, qz))));
+        R[6] = mul(2.0f, sub(mul(qx, qz), mul(qw, qy)));
+        R[7] = mul(2.0f, add(mul(qy, qz), mul(qw, qx)));
+        const float su = __ldg(a.scale + 3 * (size_t)i), sv = __ldg(a.scale + 3 * (size_t)i + 1);
+        const float aw[3] = {mul(R[0], su), mul(R[3], su), mul(R[6], su)};
+        const float bw[3] = {mul(R[1], sv), mul(R[4], sv), mul(R[7], sv)};
+        float ta[3], tb[3];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            ta[k] = add(add(mul(V[4 * k], aw[0]), mul(V[4 * k + 1], aw[1])), mul(V[4 * k + 2], aw[2]));
+            tb[k] = add(add(mul(V[4 * k], bw[0]), mul(V[4 * k + 1], bw[1])), mul(V[4 * k + 2], bw[2]));
+        }
+        // 3. the whole 3-sigma disc behind the near plane
+        const float zmin = sub(c[2], mul(3.0f, sq(add(mul(ta[2], ta[2]), mul(tb[2], tb[2])))));
+        if (!(zmin >= a.z_near)) break;
+        // 4. T rows
+        const float Tx[3] = {add(mul(a.fx, ta[0]), mul(a.cx, ta[2])), add(mul(a.fx, tb[0]), mul(a.cx, tb[2])), add(mul(a.fx, c[0]), mul(a.cx, c[2]))};
+        const float Ty[3] = {add(mul(a.fy, ta[1]), mul(a.cy, ta[2])), add(mul(a.fy, tb[1]), mul(a.cy, tb[2])), add(mul(a.fy, c[1]), mul(a.cy, c[2]))};
+        const float Tw[3] = {ta[2], tb[2], c[2]};
+        // 5. adjugate, scaled by an exact power of two
+        float A0[3], A1[3], A2[3];
+        cross3(Ty, Tw, A0); cross3(Tw, Tx, A1); cross3(Tx, Ty, A2);
+        float mx = 0.0f;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) mx = fmaxf(mx, fmaxf(fabsf(A0[k]), fmaxf(fabsf(A1[k]), fabsf(A2[k]))));
+        if (!(mx > 0.0f) || !finite_dev(mx)) break;
+        int e;
+        (void)frexpf(mx, &e);
+        const float sc = ldexpf(1.0f, -e);
+        // 6. bounding box of the footprint (dual conic)
+        const float qc = a.q_cutoff;
+        const float d = sub(add(mul(qc, mul(Tw[0], Tw[0])), mul(qc, mul(Tw[1], Tw[1]))), mul(Tw[2], Tw[2]));
+        if (!(d < 0.0f)) break;
+        const float ccx = dvd(sub(add(mul(qc, mul(Tx[0], Tw[0])), mul(qc, mul(Tx[1], Tw[1]))), mul(Tx[2], Tw[2])), d);
+        const float ccy = dvd(sub(add(mul(qc, mul(Ty[0], Tw[0])), mul(qc, mul(Ty[1], Tw[1]))), mul(Ty[2], Tw[2])), d);
+        const float ex = sub(mul(ccx, ccx), dvd(sub(add(mul(qc, mul(Tx[0], Tx[0])), mul(qc, mul(Tx[1], Tx[1]))), mul(Tx[2], Tx[2])), d));
+        const float ey = sub(mul(ccy, ccy), dvd(sub(add(mul(qc, mul(Ty[0], Ty[0])), mul(qc, mul(Ty[1], Ty[1]))), mul(Ty[2], Ty[2])), d));
+        const float hx = add(sq(fmaxf(ex, 1e-4f)), 1.0f), hy = add(sq(fmaxf(ey, 1e-4f)), 1.0f);
+        if (!(finite_dev(ccx) && finite_dev(ccy) && finite_dev(hx) && finite_dev(hy))) break;
+        const float rx = ceilf(hx), ry = ceilf(hy);
+        const float x0 = clampf(floorf(dvd(sub(ccx, rx), 16.0f)), 0.0f, (float)a.GW);
+        const float x1 = clampf(add(floorf(dvd(add(ccx, rx), 16.0f)), 1.0f), 0.0f, (float)a.GW);
+        const float y0 = clampf(floorf(dvd(sub(ccy, ry), 16.0f)), 0.0f, (float)a.GH);
+        const float y1 = clampf(add(floorf(dvd(add(ccy, ry), 16.0f)), 1.0f), 0.0f, (float)a.GH);
+        const int ix0 = (int)x0, ix1 = (int)x1, iy0 = (int)y0, iy1 = (int)y1;
+        if (ix1 <= ix0 || iy1 <= iy0) break;
+        // 7. SH colour
+        sh_colour<DEG>(a, s_sh + threadIdx.x * PAD, p0, p1, p2, o_rgb);
+        o_xy0 = ccx; o_xy1 = ccy; o_depth = c[2];
+        o_co = make_float4(hx, hy, 0.0f, __ldg(a.opacity + i));
+        o_radius = (int)fmaxf(rx, ry);
+        o_rect = make_ushort4((unsigned short)ix0, (unsigned short)iy0, (unsigned short)ix1, (unsigned short)iy1);
+        o_tt = (uint32_t)((ix1 - ix0) * (iy1 - iy0));
+#pragma unroll
+        for (int r = 0; r < 3; ++r) o_rt[r] = make_float4(mul(A0[r], sc), mul(A1[r], sc), mul(A2[r], sc), 0.0f);
+    } while (0);
+
+    reinterpret_cast<float2*>(a.xy)[i] = make_float2(o_xy0, o_xy1);
+    a.depth[i] = o_depth;
+    reinterpret_cast<float4*>(a.conic_opacity)[i] = o_co;
+    a.rgb[3 * (size_t)i] = o_rgb[0];
+    a.rgb[3 * (size_t)i + 1] = o_rgb[1];
+    a.rgb[3 * (size_t)i + 2] = o_rgb[2];
+    a.radius[i] = o_radius;
+    reinterpret_cast<ushort4*>(a.rect)[i] = o_rect;
+    a.tiles_touched[i] = o_tt;
+#pragma unroll
+    for (int r = 0; r < 3; ++r) reinterpret_cast<float4*>(a.ray_transform)[3 * (size_t)i + r] = o_rt[r];
+}
+
 template <int DEG>
 cudaError_t launch_project(const ProjectArgs& a, cudaStream_t st) {
     constexpr int K = (DEG + 1) * (DEG + 1);
@@ -238,7 +374,13 @@ cudaError_t launch_project(const ProjectArgs& a, cudaStream_t st) {
     cudaError_t e = cudaFuncSetAttribute(project_kernel<DEG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const int grid = (a.n + PROJ_THREADS - 1) / PROJ_THREADS;
-    project_kernel<DEG><<<grid, PROJ_THREADS, smem, st>>>(a);
+    if (a.ray_transform) {
+        e = cudaFuncSetAttribute(project_surfel_kernel<DEG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        project_surfel_kernel<DEG><<<grid, PROJ_THREADS, smem, st>>>(a);
+    } else {
+        project_kernel<DEG><<<grid, PROJ_THREADS, smem, st>>>(a);
+    }
     return cudaGetLastError();
 }
 
@@ -254,6 +396,7 @@ extern "C" fhgs_status fhgs_project(fhgs_ctx* ctx, const fhgs_gaussians* g, cons
     if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
     if (g->n < 0 || g->n != vs->n) FHGS_INVALID(ctx, "fhgs_project: g->n < 0 or != vs->n");
     if (g->sh_degree < 0 || g->sh_degree > 3) FHGS_INVALID(ctx, "fhgs_project: sh_degree not in [0,3]");
+    if ((st = validate_primitive(ctx, prm, vs)) != FHGS_OK) return st;
     if (g->n == 0) return FHGS_OK;
     if (!g->mean || !g->scale || !g->quat || !g->opacity || !g->sh)
         FHGS_INVALID(ctx, "fhgs_project: NULL Gaussian array");
@@ -272,6 +415,8 @@ extern "C" fhgs_status fhgs_project(fhgs_ctx* ctx, const fhgs_gaussians* g, cons
     a.Ly = prm->jac_clamp * k.tany;
     a.z_near = prm->z_near; a.dil = prm->cov_dilation;
     a.tight = prm->rect_mode == FHGS_RECT_TIGHT;
+    a.q_cutoff = prm->q_cutoff;
+    a.ray_transform = prm->primitive == FHGS_PRIM_SURFEL ? vs->ray_transform : nullptr;
     a.xy = vs->xy; a.depth = vs->depth; a.conic_opacity = vs->conic_opacity; a.rgb = vs->rgb;
     a.radius = vs->radius; a.rect = vs->rect; a.tiles_touched = vs->tiles_touched;
 

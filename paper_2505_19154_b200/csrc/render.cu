@@ -274,17 +274,17 @@ __global__ void __launch_bounds__(WS_THREADS, 1) render_ws_kernel(const RenderAr
 // ---------------------------------------------------------------------------------------------
 // PIXEL variant: CH in {0,4,8,16} feature channels per pass, accumulated by the pixel's own thread
 // ---------------------------------------------------------------------------------------------
-template <int CH>
+template <int CH, int PRIM>
 struct PixelSmem {
-    TileQueue q;
+    TileQueueT<PRIM> q;
     float4 rgb[TR_QCAP];
     __align__(16) float F[TR_QCAP * (CH > 0 ? CH : 1)];
 };
 
-template <int CH, typename FT>
+template <int CH, typename FT, int PRIM>
 __global__ void __launch_bounds__(TR_THREADS) render_pixel_kernel(const RenderArgs a) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    PixelSmem<CH>& sm = *reinterpret_cast<PixelSmem<CH>*>(smem_raw);
+    PixelSmem<CH, PRIM>& sm = *reinterpret_cast<PixelSmem<CH, PRIM>*>(smem_raw);
 
     const int tid = threadIdx.x;
     const int tile = blockIdx.x;
@@ -336,7 +336,7 @@ __global__ void __launch_bounds__(TR_THREADS) render_pixel_kernel(const RenderAr
             __syncthreads();
             for (int kk = 0; kk < nb; ++kk) {
                 const int s = (q_head + kk) & (TR_QCAP - 1);
-                const float w = eval_weight(sm.q.xy[s], sm.q.co[s], fx, fy, a.t, T, done, n);
+                const float w = eval_weight_q<PRIM>(sm.q, s, fx, fy, a.t, T, done, n);
                 if (w != 0.f) {
                     const float4 c = sm.rgb[s];
                     C0 = fmaf(w, c.x, C0); C1 = fmaf(w, c.y, C1); C2 = fmaf(w, c.z, C2);
@@ -409,12 +409,18 @@ cudaError_t launch_ws(const RenderArgs& a, int tiles, int num_sms, uint32_t* ctr
 
 template <typename FT>
 cudaError_t dispatch(const RenderArgs& a, int grid, int num_sms, uint32_t* queue, const uint32_t* order, cudaStream_t st, bool has_feat) {
-    if (!has_feat) return launch(render_pixel_kernel<0, FT>, sizeof(PixelSmem<0>), grid, st, a);
+    if (a.t.ray_transform) {   // surfel mode (NEXT-3): the per-pixel kernels, CH channels per pass, for every D
+        if (!has_feat) return launch(render_pixel_kernel<0, FT, 1>, sizeof(PixelSmem<0, 1>), grid, st, a);
+        if (a.D % 16 == 0) return launch(render_pixel_kernel<16, FT, 1>, sizeof(PixelSmem<16, 1>), grid, st, a);
+        if (a.D % 8 == 0) return launch(render_pixel_kernel<8, FT, 1>, sizeof(PixelSmem<8, 1>), grid, st, a);
+        return launch(render_pixel_kernel<4, FT, 1>, sizeof(PixelSmem<4, 1>), grid, st, a);
+    }
+    if (!has_feat) return launch(render_pixel_kernel<0, FT, 0>, sizeof(PixelSmem<0, 0>), grid, st, a);
     if (a.D % 128 == 0) return launch_ws<128, FT>(a, grid, num_sms, queue, order, st);
     if (a.D % 64 == 0) return launch_ws<64, FT>(a, grid, num_sms, queue, order, st);
-    if (a.D % 16 == 0) return launch(render_pixel_kernel<16, FT>, sizeof(PixelSmem<16>), grid, st, a);
-    if (a.D % 8 == 0) return launch(render_pixel_kernel<8, FT>, sizeof(PixelSmem<8>), grid, st, a);
-    return launch(render_pixel_kernel<4, FT>, sizeof(PixelSmem<4>), grid, st, a);
+    if (a.D % 16 == 0) return launch(render_pixel_kernel<16, FT, 0>, sizeof(PixelSmem<16, 0>), grid, st, a);
+    if (a.D % 8 == 0) return launch(render_pixel_kernel<8, FT, 0>, sizeof(PixelSmem<8, 0>), grid, st, a);
+    return launch(render_pixel_kernel<4, FT, 0>, sizeof(PixelSmem<4, 0>), grid, st, a);
 }
 
 }  // namespace
@@ -428,6 +434,7 @@ extern "C" fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const
     if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
     if ((st = validate_params(ctx, prm)) != FHGS_OK) return st;
     if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
+    if ((st = validate_primitive(ctx, prm, vs)) != FHGS_OK) return st;
     if (!out_rgb) FHGS_INVALID(ctx, "fhgs_render: out_rgb is required");
     const bool has_feat = out_feat != nullptr;
     if (has_feat) {
@@ -444,6 +451,7 @@ extern "C" fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const
     a.t.xy = reinterpret_cast<const float2*>(vs->xy);
     a.t.conic_opacity = reinterpret_cast<const float4*>(vs->conic_opacity);
     a.t.q_cutoff = prm->q_cutoff; a.t.alpha_max = prm->alpha_max; a.t.t_min = prm->t_min;
+    a.t.ray_transform = prm->primitive == FHGS_PRIM_SURFEL ? reinterpret_cast<const float4*>(vs->ray_transform) : nullptr;
     a.rgb_g = vs->rgb; a.feat = g->feat; a.D = has_feat ? g->feat_dim : 0;
     a.bg[0] = prm->bg[0]; a.bg[1] = prm->bg[1]; a.bg[2] = prm->bg[2];
     a.out_rgb = out_rgb; a.out_feat = out_feat; a.out_T = out_T; a.out_n = out_ncontrib;

@@ -31,14 +31,20 @@ struct TraverseArgs {
     const float2* xy;
     const float4* conic_opacity;
     float q_cutoff, alpha_max, t_min;
+    const float4* ray_transform;   // [n,3] float4 rows of adj(T): surfel mode (PRIM = 1) only
 };
 
-struct TileQueue {            // shared-memory ring of staged survivors
+// PRIM = 0: 3-axis Gaussian, EWA conic (north_star).  PRIM = 1: the paper's 2-D surfel, u^2 + v^2 from
+// the per-splat ray transform; the staged record then also carries its three rows (m[2].w = opacity).
+template <int PRIM>
+struct TileQueueT {           // shared-memory ring of staged survivors
     float2 xy[TR_QCAP];
-    float4 co[TR_QCAP];       // A, 2B, C, opacity
+    float4 co[TR_QCAP];       // A, 2B, C, opacity   (surfel: half_x, half_y, 0, opacity)
     uint32_t id[TR_QCAP];
     uint32_t wcount[TR_THREADS / 32];
+    float4 m[PRIM ? 3 : 1][PRIM ? TR_QCAP : 1];
 };
+using TileQueue = TileQueueT<0>;
 
 __device__ __forceinline__ void slot_to_xy(int slot, int& x, int& y) {
     const int warp = slot >> 5, lane = slot & 31;
@@ -78,7 +84,8 @@ __device__ __forceinline__ bool tile_may_contribute(float2 g, float4 co, float b
 
 // Examine instances [pos, min(pos+256, end)) and append the survivors to the ring at q_tail.
 // Returns the number appended (same value in every thread).  Contains two __syncthreads().
-__device__ __forceinline__ int stage_chunk(const TraverseArgs& a, TileQueue& q, uint32_t pos, uint32_t end, int q_tail,
+template <int PRIM>
+__device__ __forceinline__ int stage_chunk(const TraverseArgs& a, TileQueueT<PRIM>& q, uint32_t pos, uint32_t end, int q_tail,
                                            float bx0, float by0, float bx1, float by1) {
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t idx = pos + tid;
@@ -90,8 +97,12 @@ __device__ __forceinline__ int stage_chunk(const TraverseArgs& a, TileQueue& q, 
         id = __ldg(a.vals + idx);
         g = __ldg(a.xy + id);
         co = __ldg(a.conic_opacity + id);
-        co.y = 2.0f * co.y;   // exact
-        keep = tile_may_contribute(g, co, bx0, by0, bx1, by1, a.q_cutoff);
+        if (PRIM) {   // footprint bounding box (centre g, half extents co.x, co.y; one pixel of margin is inside) vs the pixel box
+            keep = !(g.x + co.x < bx0 || g.x - co.x > bx1 || g.y + co.y < by0 || g.y - co.y > by1);
+        } else {
+            co.y = 2.0f * co.y;   // exact
+            keep = tile_may_contribute(g, co, bx0, by0, bx1, by1, a.q_cutoff);
+        }
     }
     const uint32_t ballot = __ballot_sync(TR_FULL, keep);
     if (lane == 0) q.wcount[warp] = __popc(ballot);
@@ -108,6 +119,10 @@ __device__ __forceinline__ int stage_chunk(const TraverseArgs& a, TileQueue& q, 
         q.xy[s] = g;
         q.co[s] = co;
         q.id[s] = id;
+        if (PRIM) {
+#pragma unroll
+            for (int r = 0; r < 3; ++r) q.m[PRIM ? r : 0][PRIM ? s : 0] = __ldg(a.ray_transform + 3 * (size_t)id + r);
+        }
     }
     __syncthreads();
     return total;
@@ -127,6 +142,33 @@ __device__ __forceinline__ float eval_weight(float2 g, float4 co, float fx, floa
     ++n;
     if (T < a.t_min) done = true;
     return w;
+}
+
+// Surfel form: p = adj(T) (x, y, 1)^T in binary32 fmaf form, num = p_x^2 + p_y^2, den = p_z^2; the
+// splat contributes iff den > 0 and num <= q_cutoff * den (the decision needs no division; both sides evaluate exactly
+// this expression); G = exp(-(num/den)/2).
+__device__ __forceinline__ float eval_weight_surfel(float4 m0, float4 m1, float4 m2, float op, float fx, float fy,
+                                                    const TraverseArgs& a, float& T, bool& done, uint32_t& n) {
+    const float p0 = __fmaf_rn(fx, m0.x, __fmaf_rn(fy, m0.y, m0.z));
+    const float p1 = __fmaf_rn(fx, m1.x, __fmaf_rn(fy, m1.y, m1.z));
+    const float p2 = __fmaf_rn(fx, m2.x, __fmaf_rn(fy, m2.y, m2.z));
+    const float num = __fmaf_rn(p0, p0, __fmul_rn(p1, p1)), den = __fmul_rn(p2, p2);
+    if (done || !(den > 0.f) || !(num <= __fmul_rn(a.q_cutoff, den))) return 0.f;
+    const float G = exp2f(-0.72134752044448170368f * __fdividef(num, den));
+    const float alpha = fminf(a.alpha_max, op * G);
+    const float w = alpha * T;
+    T = fmaf(-alpha, T, T);
+    ++n;
+    if (T < a.t_min) done = true;
+    return w;
+}
+
+// weight of staged survivor s of the ring for the pixel (fx, fy)
+template <int PRIM>
+__device__ __forceinline__ float eval_weight_q(const TileQueueT<PRIM>& q, int s, float fx, float fy, const TraverseArgs& a, float& T,
+                                               bool& done, uint32_t& n) {
+    if (PRIM) return eval_weight_surfel(q.m[0][PRIM ? s : 0], q.m[PRIM ? 1 : 0][PRIM ? s : 0], q.m[PRIM ? 2 : 0][PRIM ? s : 0], q.co[s].w, fx, fy, a, T, done, n);
+    return eval_weight(q.xy[s], q.co[s], fx, fy, a, T, done, n);
 }
 
 __device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {

@@ -25,14 +25,14 @@ def oracle_view(scene, cam, params=fo.DEFAULT_PARAMS):
 class GpuPath:
     """One scene on the device + a reusable view state."""
 
-    def __init__(self, scene, width, height, capacity, device=0):
+    def __init__(self, scene, width, height, capacity, device=0, surfel=False):
         import torch
         from paper_2505_19154_b200 import binding as fb
         self.torch, self.fb = torch, fb
         self.ctx = fb.Context(device)
         self.g = fb.Gaussians(scene.mean, scene.scale, scene.quat, scene.opacity, scene.sh, scene.feat, scene.sh_degree)
-        self.vs = fb.ViewState(scene.n, width, height, capacity)
-        self.prm = fb.default_params()
+        self.vs = fb.ViewState(scene.n, width, height, capacity, surfel=surfel)
+        self.prm = fb.default_params(primitive=fb.FHGS_PRIM_SURFEL if surfel else fb.FHGS_PRIM_EWA)
         self.W, self.H = width, height
         self.D = scene.feat_dim
 
@@ -82,7 +82,7 @@ def check_projection(pr_o, pr_g):
     """Integer outputs bit-exact; float outputs bit-exact by construction (C1-P), rgb within 1e-4."""
     for k in ("radius", "rect", "tiles_touched"):
         assert np.array_equal(pr_o[k], pr_g[k]), f"projection integer output {k} differs"
-    for k in ("xy", "depth", "conic_opacity"):
+    for k in ("xy", "depth", "conic_opacity") + (("ray_transform",) if "ray_transform" in pr_o else ()):
         assert np.array_equal(pr_o[k].view(np.uint32), pr_g[k].view(np.uint32)), f"projection float output {k} not bit-equal"
     assert np.max(np.abs(pr_o["rgb"] - pr_g["rgb"]), initial=0.0) <= TOL_F32
 
@@ -144,13 +144,20 @@ class Borderline:
             cand = bins["vals"][int(r0):int(r1)].astype(np.int64)          # front to back
             if cand.size == 0:
                 continue
-            dx, dy = (gx[cand] - f32(x)).astype(f32), (gy[cand] - f32(y)).astype(f32)
-            A, B2, Cc = co[cand, 0], (f32(2.0) * co[cand, 1]).astype(f32), co[cand, 2]
-            adx = (A * dx).astype(f32)
-            inner = (B2.astype(f64) * dy.astype(f64) + adx.astype(f64)).astype(f32)          # fmaf(2B, dy, A dx)
-            cdy2 = ((Cc * dy).astype(f32) * dy).astype(f32)
-            q = (dx.astype(f64) * inner.astype(f64) + cdy2.astype(f64)).astype(f32)          # fmaf(dx, inner, (C dy) dy)
-            c = q <= f32(q_cutoff)
+            if "ray_transform" in pr:   # surfel mode: u^2 + v^2 from the ray transform (the cut-off edge itself is not at stake here)
+                rt = pr["ray_transform"][cand].astype(f64)
+                p0, p1, p2 = (x * rt[:, 4 * r] + y * rt[:, 4 * r + 1] + rt[:, 4 * r + 2] for r in range(3))
+                num, den = p0 * p0 + p1 * p1, p2 * p2
+                c = (den > 0) & (num <= q_cutoff * den)
+                q = np.where(c, num / np.where(den > 0, den, 1.0), 0.0)
+            else:
+                dx, dy = (gx[cand] - f32(x)).astype(f32), (gy[cand] - f32(y)).astype(f32)
+                A, B2, Cc = co[cand, 0], (f32(2.0) * co[cand, 1]).astype(f32), co[cand, 2]
+                adx = (A * dx).astype(f32)
+                inner = (B2.astype(f64) * dy.astype(f64) + adx.astype(f64)).astype(f32)          # fmaf(2B, dy, A dx)
+                cdy2 = ((Cc * dy).astype(f32) * dy).astype(f32)
+                q = (dx.astype(f64) * inner.astype(f64) + cdy2.astype(f64)).astype(f32)          # fmaf(dx, inner, (C dy) dy)
+                c = q <= f32(q_cutoff)
             alpha = np.where(c, np.minimum(f64(f32(alpha_max)), co[cand, 3].astype(f64) * np.exp(-0.5 * np.maximum(q.astype(f64), 0.0))), 0.0)
             T_before = np.concatenate([[1.0], np.cumprod(1.0 - alpha)[:-1]])
             for j in np.nonzero(c & (np.abs(T_before / t_min - 1.0) <= window))[0]:

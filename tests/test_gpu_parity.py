@@ -13,7 +13,7 @@ pytestmark = pytest.mark.gpu
 
 
 def run_case(cfg, views, tol, literal_pixels=None, sort_flags=(0, 1), capacity_slack=1.25, check_finalize=True,
-             fixed_capacity=None, full_frame=True, rect_mode=0):
+             fixed_capacity=None, full_frame=True, rect_mode=0, primitive=0):
     """Full P -> S -> R -> F parity of one config over `views`; returns worst errors.
     full_frame: compare the whole rendered frame with fo_render_scatter; literal_pixels: additionally (or instead)
     compare that many random pixels with the tile-free, box-free fo_render_literal.  Fusion is always compared on
@@ -21,13 +21,13 @@ def run_case(cfg, views, tol, literal_pixels=None, sort_flags=(0, 1), capacity_s
     import time
     scene = inputs.make_scene(cfg)
     cams = [inputs.make_camera(cfg, v) for v in views]
-    prm_o = fo.params(rect_mode=rect_mode)
+    prm_o = fo.params(rect_mode=rect_mode, primitive=primitive)
     prs = [pu.oracle_view(scene, cam, prm_o) for cam in cams]
     Ms = [int(pr["tiles_touched"].astype(np.int64).sum()) for pr in prs]
     cap = int(max(Ms) * capacity_slack) + 16
     if fixed_capacity is not None:
         cap = fixed_capacity
-    gp = pu.GpuPath(scene, cfg.width, cfg.height, cap)
+    gp = pu.GpuPath(scene, cfg.width, cfg.height, cap, surfel=bool(primitive))
     gp.prm.rect_mode = rect_mode
     feat32 = scene.feat.astype(np.float32)
     fabs = float(np.abs(feat32).max())
@@ -162,6 +162,19 @@ def test_tight_rect_mode():
     w = run_case(inputs.CONFIGS["mid"], [0], pu.TOL_F32, sort_flags=(0,), capacity_slack=1.0, fixed_capacity=int(40e6), rect_mode=1)
     print(w)
     assert w["M"] < 0.67 * 31_666_264
+
+
+def test_surfel_primitive():
+    """SURVEY 8(f) NEXT-3, fhgs_params.primitive = FHGS_PRIM_SURFEL: the paper's 2-D surfel with exact ray-splat
+    intersection.  Same bars as the EWA path: ray transform, bounding box, rect, tiles_touched, M, all
+    sorted pairs and ranges bit-exact; n_contrib exact off fragile pixels; images, accumulators and fused vectors within
+    1e-4 (2e-3 for fp16 storage).  Tiny-shape (4 views, per-pixel kernels), Small-shape (2 views accumulated), a ragged
+    D=128 case (16-channel render passes, tile-GEMM fusion), D=64 and fp16 storage."""
+    print(run_case(pu.reduced_config("tiny", n=3000, log_scale_mu=-2.3), range(4), pu.TOL_F32, primitive=1, literal_pixels=150))
+    print(run_case(pu.reduced_config("small", n=20_000, log_scale_mu=-2.6), [0, 3], pu.TOL_F32, primitive=1, sort_flags=(0,)))
+    print(run_case(pu.reduced_config("mid", n=40_000, width=328, height=200, log_scale_mu=-2.8), [0], pu.TOL_F32, primitive=1, sort_flags=(0,)))
+    print(run_case(pu.reduced_config("mid", n=10_000, width=160, height=96, log_scale_mu=-2.6, feat_dim=64), [0], pu.TOL_F32, primitive=1, sort_flags=(0,)))
+    print(run_case(pu.reduced_config("large", n=15_000, width=200, height=120, log_scale_mu=-2.8), [0], pu.TOL_F16, primitive=1, sort_flags=(0,)))
 
 
 def test_large_full_size():
