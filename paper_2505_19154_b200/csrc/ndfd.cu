@@ -74,10 +74,10 @@ struct NdSub {
 };
 
 // CPL = channels per lane = D / LPP
-template <int LPP, int CPL, typename FT, typename GT, int MODE>
+template <int LPP, int CPL, typename FT, typename GT, int MODE, int PRIM>
 __global__ void __launch_bounds__(TR_THREADS, MODE ? (CPL <= 16 ? 2 : 1) : (CPL <= 16 ? 3 : (CPL <= 32 ? 2 : 1)))
     ndfd_strip_kernel(const NdfdArgs a) {
-    __shared__ TileQueue q;
+    __shared__ TileQueueT<PRIM> q;
     constexpr int PXW = 32 / LPP, ROWS = 8 * PXW / FHGS_TILE, STRIPS = FHGS_TILE / ROWS;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x / STRIPS, strip = blockIdx.x % STRIPS;
@@ -148,7 +148,17 @@ __global__ void __launch_bounds__(TR_THREADS, MODE ? (CPL <= 16 ? 2 : 1) : (CPL 
             // w = alpha T, the T update and the stop test run per fragment.
             for (int k0 = sb * SB; k0 < k_end; k0 += LPP) {
               float a_c = 0.f;
-              if (k0 + cgl < k_end) {
+              if (PRIM) {   // surfel: u^2 + v^2 from the ray transform (traverse.cuh eval_weight_surfel, same expressions)
+                  if (k0 + cgl < k_end) {
+                      const float4 m0 = q.m[0][PRIM ? k0 + cgl : 0], m1 = q.m[PRIM ? 1 : 0][PRIM ? k0 + cgl : 0], m2 = q.m[PRIM ? 2 : 0][PRIM ? k0 + cgl : 0];
+                      const float p0 = __fmaf_rn(fx, m0.x, __fmaf_rn(fy, m0.y, m0.z));
+                      const float p1 = __fmaf_rn(fx, m1.x, __fmaf_rn(fy, m1.y, m1.z));
+                      const float p2 = __fmaf_rn(fx, m2.x, __fmaf_rn(fy, m2.y, m2.z));
+                      const float num = __fmaf_rn(p0, p0, __fmul_rn(p1, p1)), den = __fmul_rn(p2, p2);
+                      if (den > 0.f && num <= __fmul_rn(a.t.q_cutoff, den))
+                          a_c = fminf(a.t.alpha_max, q.co[k0 + cgl].w * exp2f(-0.72134752044448170368f * __fdividef(num, den)));
+                  }
+              } else if (k0 + cgl < k_end) {
                   const float2 gxy = q.xy[k0 + cgl];
                   const float4 co = q.co[k0 + cgl];
                   const float dx = __fsub_rn(gxy.x, fx), dy = __fsub_rn(gxy.y, fy);
@@ -230,30 +240,30 @@ __global__ void __launch_bounds__(TR_THREADS, MODE ? (CPL <= 16 ? 2 : 1) : (CPL 
     }
 }
 
-template <int LPP, int CPL, typename FT, typename GT, int MODE>
+template <int LPP, int CPL, typename FT, typename GT, int MODE, int PRIM>
 cudaError_t launch(const NdfdArgs& a, int tiles, cudaStream_t st) {
     constexpr int STRIPS = FHGS_TILE / (8 * (32 / LPP) / FHGS_TILE);
     const size_t smem = 2 * (size_t)NdSub<LPP * CPL, FT>::SB * NdSub<LPP * CPL, FT>::ROW_BYTES;
-    cudaError_t e = cudaFuncSetAttribute(ndfd_strip_kernel<LPP, CPL, FT, GT, MODE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(ndfd_strip_kernel<LPP, CPL, FT, GT, MODE, PRIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    ndfd_strip_kernel<LPP, CPL, FT, GT, MODE><<<tiles * STRIPS, TR_THREADS, smem, st>>>(a);
+    ndfd_strip_kernel<LPP, CPL, FT, GT, MODE, PRIM><<<tiles * STRIPS, TR_THREADS, smem, st>>>(a);
     return cudaGetLastError();
 }
 
-template <typename FT, typename GT, int MODE>
+template <typename FT, typename GT, int MODE, int PRIM>
 cudaError_t dispatch_d(const NdfdArgs& a, int tiles, cudaStream_t st) {
     switch (a.D) {
-        case 32: return launch<4, 8, FT, GT, MODE>(a, tiles, st);
-        case 64: return launch<4, 16, FT, GT, MODE>(a, tiles, st);
-        case 128: return launch<4, 32, FT, GT, MODE>(a, tiles, st);
-        case 256: return launch<8, 32, FT, GT, MODE>(a, tiles, st);
-        case 512: return launch<8, 64, FT, GT, MODE>(a, tiles, st);
+        case 32: return launch<4, 8, FT, GT, MODE, PRIM>(a, tiles, st);
+        case 64: return launch<4, 16, FT, GT, MODE, PRIM>(a, tiles, st);
+        case 128: return launch<4, 32, FT, GT, MODE, PRIM>(a, tiles, st);
+        case 256: return launch<8, 32, FT, GT, MODE, PRIM>(a, tiles, st);
+        case 512: return launch<8, 64, FT, GT, MODE, PRIM>(a, tiles, st);
         default: return cudaErrorInvalidValue;
     }
 }
 template <typename FT, typename GT>
 cudaError_t dispatch(const NdfdArgs& a, int tiles, int mode, cudaStream_t st) {
-    return mode ? dispatch_d<FT, GT, 1>(a, tiles, st) : dispatch_d<FT, GT, 0>(a, tiles, st);
+    return mode ? dispatch_d<FT, GT, 1, 0>(a, tiles, st) : dispatch_d<FT, GT, 0, 0>(a, tiles, st);
 }
 
 }  // namespace
@@ -268,7 +278,10 @@ extern "C" fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g,
     if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
     if ((st = validate_params(ctx, prm)) != FHGS_OK) return st;
     if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
-    if (prm->primitive != FHGS_PRIM_EWA) FHGS_INVALID(ctx, "the NDFD calls are built for FHGS_PRIM_EWA only");
+    const bool surfel = prm->primitive == FHGS_PRIM_SURFEL;
+    if ((st = validate_primitive(ctx, prm, vs)) != FHGS_OK) return st;
+    if (surfel && (g->feat_dtype != FHGS_F32 || gt_dtype != FHGS_F32))
+        FHGS_INVALID(ctx, "fhgs_ndfd_forward: the surfel primitive is built for f32 features and map");
     if (!g->feat) FHGS_INVALID(ctx, "fhgs_ndfd_forward: g->feat is NULL");
     if ((g->feat_dtype != FHGS_F32 && g->feat_dtype != FHGS_F16) || (gt_dtype != FHGS_F32 && gt_dtype != FHGS_F16))
         FHGS_INVALID(ctx, "fhgs_ndfd_forward: unknown dtype");
@@ -285,7 +298,7 @@ extern "C" fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g,
     a.t.xy = reinterpret_cast<const float2*>(vs->xy);
     a.t.conic_opacity = reinterpret_cast<const float4*>(vs->conic_opacity);
     a.t.q_cutoff = prm->q_cutoff; a.t.alpha_max = prm->alpha_max; a.t.t_min = prm->t_min;
-    a.t.ray_transform = nullptr;
+    a.t.ray_transform = surfel ? reinterpret_cast<const float4*>(vs->ray_transform) : nullptr;
     a.feat = g->feat; a.gt = gt; a.D = D; a.k_sig = k_sigmoid; a.lambda = lambda;
     a.out_lgt = out_lgt; a.out_lcf = out_lcf;
     const int tiles = tiles_x(cam->width) * tiles_y(cam->height);
@@ -293,7 +306,8 @@ extern "C" fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g,
     cudaStream_t s = (cudaStream_t)stream;
     cudaError_t e;
     const bool fh = g->feat_dtype == FHGS_F16, gh = gt_dtype == FHGS_F16;
-    if (fh && gh) e = dispatch<__half, __half>(a, tiles, mode, s);
+    if (surfel) e = mode ? dispatch_d<float, float, 1, 1>(a, tiles, s) : dispatch_d<float, float, 0, 1>(a, tiles, s);
+    else if (fh && gh) e = dispatch<__half, __half>(a, tiles, mode, s);
     else if (fh) e = dispatch<__half, float>(a, tiles, mode, s);
     else if (gh) e = dispatch<float, __half>(a, tiles, mode, s);
     else e = dispatch<float, float>(a, tiles, mode, s);

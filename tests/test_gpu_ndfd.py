@@ -10,7 +10,7 @@ import parity_util as pu
 pytestmark = pytest.mark.gpu
 
 
-def _run(cfg, view, tol, npix=4000, k=20.0, lam=0.5, modes=(0, 1)):
+def _run(cfg, view, tol, npix=4000, k=20.0, lam=0.5, modes=(0, 1), surfel=False):
     """Both accumulation orders of W, F (DESIGN.md reading): mode 0 = blend order, mode 1 = far to near
     (PAPER.md:136); the oracle's mode 1 walks the collected fragment list backwards, the kernel uses the split sum."""
     import torch
@@ -18,9 +18,9 @@ def _run(cfg, view, tol, npix=4000, k=20.0, lam=0.5, modes=(0, 1)):
     scene = inputs.make_scene(cfg)
     cam = inputs.make_camera(cfg, view)
     gt = inputs.make_gt_map(cfg, view, cam)
-    pr = pu.oracle_view(scene, cam)
+    pr = pu.oracle_view(scene, cam, fo.params(primitive=1 if surfel else 0))
     m = fo.bins(pr, cfg.width, cfg.height)["M"]
-    gp = pu.GpuPath(scene, cfg.width, cfg.height, m + 64)
+    gp = pu.GpuPath(scene, cfg.width, cfg.height, m + 64, surfel=surfel)
     c, _ = gp.project_sort(cam)
     dev = gp.g.mean.device
     H, W = cfg.height, cfg.width
@@ -68,6 +68,15 @@ def test_ndfd_other_dims_and_fp16():
         print(d, _run(cfg, 0, pu.TOL_F32, npix=1500))
     cfg = pu.reduced_config("large", n=20_000, width=200, height=120, log_scale_mu=-3.3)
     print(512, _run(cfg, 0, pu.TOL_F16, npix=1500))
+
+
+def test_ndfd_surfel_primitive():
+    """The paper's own configuration ("within a 2DGS-based framework"): NDFD losses over surfels
+    (fhgs_params.primitive = FHGS_PRIM_SURFEL), both accumulation orders, D = 128 ragged and D = 32."""
+    cfg = pu.reduced_config("mid", n=40_000, width=328, height=200, log_scale_mu=-2.8)
+    print(_run(cfg, 0, pu.TOL_F32, surfel=True))
+    cfg = pu.reduced_config("mid", n=10_000, width=160, height=96, log_scale_mu=-2.6, feat_dim=32)
+    print(_run(cfg, 0, pu.TOL_F32, npix=1500, surfel=True))
 
 
 def test_ndfd_multiview_blobs_and_params():
