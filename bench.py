@@ -566,6 +566,133 @@ def run_cuda_workload(args, local_rank: int):
             "e2e": None, "gpu_launches": None, "clocks": clocks}
     print(json.dumps(line), flush=True)
 
+# --------------------------------------------------------------------------------------------------
+# BASELINE.json configs[4] as stated: the 200-view fusion sweep, on 1 GPU or view-sharded over N ranks
+# --------------------------------------------------------------------------------------------------
+def run_multiview_sweep(args, rank: int, world: int, local_rank: int):
+    """`--workload multiview --views V` (V = 200 is the config): every view's GT map is generated on the device
+    (inputs.make_gt_map_blobs_torch, seeded per view) OUTSIDE the timed spans, then P + S + F of that view are timed
+    with CUDA events; the accumulators persist across the views, one finalise at the end.  With N ranks (torchrun) the
+    views are sharded round-robin through parallel.fuse_views_sharded: private accumulators per rank, ONE NCCL
+    all-reduce(sum) of num [N,D] and den [N], finalise on every rank.  Reported: end-to-end device time of the sweep
+    (sum of the timed spans + all-reduce + finalise, max over ranks), views/s over all ranks, per-view mean; and two
+    invariants of the result: conservation sum_i den_i = sum_views sum_x (1 - T_final(x))
+    against RGB-only renders of the same views, and the cosine between every well-covered Gaussian's fused vector and
+    its blob's vector."""
+    import torch
+    import torch.distributed as dist
+    from paper_2505_19154_b200 import binding as fb
+    from paper_2505_19154_b200 import inputs, parallel
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the FHGS path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    cfg = inputs.CONFIGS["multiview"]
+    if args.small:
+        cfg = inputs.scaled(cfg, n=100_000, width=432, height=320, log_scale_mu=-3.2)
+    scene = inputs.make_scene(cfg)
+    W, H, D, n = cfg.width, cfg.height, cfg.feat_dim, scene.n
+    views = [int(round(k * cfg.n_views / args.views)) % cfg.n_views for k in range(args.views)]
+    ctx = fb.Context(local_rank)
+    g = fb.Gaussians(scene.mean, scene.scale, scene.quat, scene.opacity, scene.sh, scene.feat, scene.sh_degree, device=dev)
+    prm = fb.default_params(rect_mode=1 if args.rect == "tight" else 0)
+    capacity = int(48e6) if not args.small else int(8e6)     # > the largest view of the orbit (2.2e7 instances; checked below)
+    vs = fb.ViewState(n, W, H, capacity, device=dev)
+    f32 = torch.float32
+    gt = torch.empty((H, W, D), dtype=f32, device=dev)
+    num = torch.empty((n, D), dtype=f32, device=dev)
+    den = torch.empty((n,), dtype=f32, device=dev)
+    fused = g.feat.clone()
+    out_rgb = torch.empty((H, W, 3), dtype=f32, device=dev)
+    out_T = torch.empty((H, W), dtype=f32, device=dev)
+    stream = torch.cuda.current_stream()
+    spans, Ms, one_minus_T = [], [], [0.0]
+
+    def fuse_one_view(v, first):
+        cam_np = inputs.make_camera(cfg, v)
+        cam = fb.make_camera(cam_np.view, cam_np.proj, cam_np.cam_pos, W, H)
+        inputs.make_gt_map_blobs_torch(cfg, v, cam_np, dev, out=gt)          # not timed
+        e = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+        e[0].record(stream)
+        fb.project(ctx, g, cam, prm, vs)
+        e[1].record(stream)
+        fb.bin_sort(ctx, cam, vs, sync=False)
+        e[2].record(stream)
+        fb.fuse_features(ctx, cam, prm, vs, gt, num, den, None, fb.FHGS_FUSE_ZERO if first else 0)
+        e[3].record(stream)
+        spans.append(e)
+        # the invariants' reference, outside the timed spans: RGB-only render of the same view state
+        fb.render(ctx, g, cam, prm, vs, out_rgb, None, out_T, None)
+        one_minus_T[0] += float((1.0 - out_T.double()).sum().item())
+        m = int(vs.num_instances.item())
+        if m > capacity:
+            raise RuntimeError(f"view {v}: {m} instances exceed the capacity {capacity}")
+        Ms.append(m)
+
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+
+    def finalize():
+        ev[1].record(stream)
+        fb.fuse_features(ctx, None, prm, vs, None, num, den, fused, fb.FHGS_FUSE_FINALIZE_ONLY)
+        ev[2].record(stream)
+
+    # warm-up: three views into scratch accumulators (module load, clocks), then the sweep
+    for v in views[:3]:
+        fuse_one_view(v, True)
+    torch.cuda.synchronize()
+    spans.clear(); Ms.clear(); one_minus_T[0] = 0.0
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    t_wall = time.perf_counter()
+    # parallel.fuse_views_sharded: this rank's views, then the all-reduce (between ev[0] and ev[1]), then finalise
+    mine = parallel.fuse_views_sharded(views, fuse_one_view, num, den, finalize, before_reduce=lambda: ev[0].record(stream))
+    torch.cuda.synchronize()
+    wall_s = time.perf_counter() - t_wall
+    clocks = sampler.stop()
+    parts = {"project": 0.0, "bin_sort": 0.0, "fuse": 0.0}
+    for e in spans:
+        for i, k in enumerate(parts):
+            parts[k] += e[i].elapsed_time(e[i + 1])
+    parts["all_reduce"] = ev[0].elapsed_time(ev[1]) if world > 1 else 0.0
+    parts["finalize"] = ev[1].elapsed_time(ev[2])
+    sweep_ms = parallel.max_over_ranks(sum(parts.values()), dev)
+    # invariants on the reduced result (every rank holds all of num/den after the all-reduce)
+    omt = torch.tensor([one_minus_T[0]], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(omt)
+    den_sum = float(den.double().sum().item())
+    conservation_rel = abs(den_sum - float(omt.item())) / max(float(omt.item()), 1e-30)
+    vec = torch.from_numpy(inputs.blob_vectors(cfg).astype(np.float32)).to(dev)
+    centres = torch.from_numpy(inputs.blob_centres(cfg).astype(np.float32)).to(dev)
+    owner = torch.arange(n, device=dev) % 64
+    dist_c = (g.mean - centres[owner]).norm(dim=1)
+    well = (den > 1.0) & (dist_c < 0.6)             # well covered, inside its blob's 2-sigma ball (the map's labelling radius)
+    cos = torch.nn.functional.cosine_similarity(fused[well].float(), vec[owner[well]], dim=1)
+    cos_stats = {"gaussians": int(well.sum().item()), "median": float(cos.median().item()),
+                 "p10": float(cos.quantile(0.10).item()), "frac_above_0.9": float((cos > 0.9).float().mean().item())}
+    if rank == 0:
+        nv = len(views)
+        line = {"metric": "[multiview] fused views/s (BASELINE.json configs[4]: P+S+F per view, one finalise)",
+                "value": nv / (sweep_ms * 1e-3), "unit": "views/s", "n_gpus": world, "steps": 1, "warmup": 3,
+                "ms_per_step": sweep_ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+                "data": "synthetic",
+                "config": {"workload": f"multiview: N={n} SH{scene.sh_degree} D={D} f32, {nv} views {W}x{H} of the {cfg.n_views}-camera orbit"
+                                       + (" [--small debug size]" if args.small else ""),
+                           "parallelism": f"views sharded round-robin over {world} rank(s), one all-reduce(sum) of num/den",
+                           "gt": "inputs.make_gt_map_blobs_torch per view on the device, outside the timed spans",
+                           "views_this_rank": len(mine), "instances_M_min_mean_max": [min(Ms), sum(Ms) / len(Ms), max(Ms)]},
+                "ms": parts, "ms_per_view": sweep_ms / nv * world, "end_to_end_s": sweep_ms * 1e-3,
+                "wall_s_incl_map_generation_and_checks": wall_s,
+                "invariants": {"conservation_rel_err": conservation_rel, "den_sum": den_sum, "one_minus_T_sum": float(omt.item()),
+                               "cosine_to_blob_vector": cos_stats},
+                "cpu_baseline": None, "e2e": None, "gpu_launches": None, "clocks": clocks}
+        print(json.dumps(line), flush=True)
+    assert conservation_rel < 2e-4, f"conservation violated: {conservation_rel}"
+    if world > 1:
+        dist.destroy_process_group()
+
 
 def main():
     ap = argparse.ArgumentParser()
@@ -588,6 +715,9 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.workload == "multiview" and (args.views > 8 or world > 1):
+        run_multiview_sweep(args, rank, world, local_rank)      # the config as BASELINE.json states it (and its sharded form)
         return
     if args.workload != "mid":
         if rank == 0:

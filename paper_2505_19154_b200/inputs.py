@@ -242,6 +242,24 @@ def make_gt_map(cfg: Config, view_idx: int, cam: Camera | None = None) -> np.nda
     return np.ascontiguousarray(g)
 
 
+def make_gt_map_blobs_torch(cfg: Config, view_idx: int, cam: Camera, device, out=None):
+    """The Multi-view config's per-view map built ON THE DEVICE (1.28 GB each, 257 GB for the 200 views:
+    generated per view, seeded `cfg.seed * 1000 + view_idx`, never all resident): the same recipe as make_gt_map's
+    "blobs" branch -- label map from the pinhole rays (host, 64 blobs), blob vector + N(0, 0.05^2) noise drawn by torch's
+    generator.  The values differ from make_gt_map's numpy draws (another generator); the parity tests use make_gt_map
+    on both sides, the 200-view sweep uses this one and is checked through invariants."""
+    import torch
+    assert cfg.gt_kind == "blobs"
+    label = torch.from_numpy(blob_label_map(cfg, cam)).to(device)
+    vecs = torch.from_numpy(blob_vectors(cfg).astype(np.float32)).to(device)
+    gen = torch.Generator(device=device).manual_seed(cfg.seed * 1000 + view_idx)
+    if out is None:
+        out = torch.empty((cfg.height, cfg.width, cfg.feat_dim), dtype=torch.float32, device=device)
+    out.normal_(0.0, 0.05, generator=gen)
+    out += vecs[label]
+    return out
+
+
 def blob_label_map(cfg: Config, cam: Camera) -> np.ndarray:
     """[H,W] int: index of the nearest blob along the pixel ray whose centre lies within 0.6 of
     the ray, else 64 (background).  Pure input geometry (pinhole rays), not the splatting method."""

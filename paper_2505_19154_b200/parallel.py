@@ -62,12 +62,14 @@ def allreduce_accumulators(num: torch.Tensor, den: torch.Tensor, group=None) -> 
 
 
 def fuse_views_sharded(views: Sequence[int], fuse_one_view: Callable[[int, bool], None], num: torch.Tensor,
-                       den: torch.Tensor, finalize: Callable[[], None]) -> List[int]:
+                       den: torch.Tensor, finalize: Callable[[], None],
+                       before_reduce: Callable[[], None] | None = None) -> List[int]:
     """Driver of the view-sharded fusion.  `views` = all view indices; this rank handles shard_views of
     them.  `fuse_one_view(v, first)` must project + bin_sort view v and call fhgs_fuse_features to
     accumulate into (num, den), with FHGS_FUSE_ZERO when `first`; a rank with no view zeroes its
     accumulators itself.  Then one all-reduce, then `finalize()` (FHGS_FUSE_FINALIZE_ONLY) on every
-    rank.  Returns the views this rank fused."""
+    rank.  `before_reduce()` (optional) runs right before the all-reduce is enqueued (bench.py records a CUDA event
+    there).  Returns the views this rank fused."""
     rank, world = world_info()
     mine = [views[i] for i in shard_views(len(views), rank, world)]
     if not mine:
@@ -75,6 +77,8 @@ def fuse_views_sharded(views: Sequence[int], fuse_one_view: Callable[[int, bool]
         den.zero_()
     for k, v in enumerate(mine):
         fuse_one_view(v, k == 0)
+    if before_reduce is not None:
+        before_reduce()
     allreduce_accumulators(num, den)
     finalize()
     return mine

@@ -394,3 +394,19 @@ def test_zero_touched_equals_full_clear():
     assert float((num - num1).abs().max()) <= 1e-5 * float(num1.abs().max())
     with pytest.raises(fb.FhgsError):                               # ZERO_TOUCHED alone means nothing
         fb.fuse_features(gp.ctx, c, gp.prm, gp.vs, torch.from_numpy(gt).to(num.device), num, den, None, fb.FHGS_FUSE_ZERO_TOUCHED)
+
+
+def test_multiview_sweep_driver_small():
+    """bench.py's 200-view sweep driver (BASELINE.json configs[4]; parallel.fuse_views_sharded with the CUDA calls, maps
+    generated on the device) at debug size, 12 views, one rank: runs, conserves weight, and the fused vectors of
+    well-covered Gaussians point at their blob's vector."""
+    import json, os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--workload", "multiview", "--views", "12", "--small"],
+                       capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    inv = line["invariants"]
+    print(line["ms"], inv)
+    assert inv["conservation_rel_err"] < 2e-4
+    assert inv["cosine_to_blob_vector"]["gaussians"] > 1000 and inv["cosine_to_blob_vector"]["median"] > 0.9

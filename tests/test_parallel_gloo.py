@@ -55,7 +55,12 @@ def _worker(rank, world, port, n_views, out_dir):
         def finalize():
             state["feat"] = fo.finalize(num.numpy(), den.numpy(), scene.feat.astype(np.float32))
 
-        mine = parallel.fuse_views_sharded(list(range(n_views)), fuse_one_view, num, den, finalize)
+        def before_reduce():    # bench.py records its CUDA event here: must run once, after the last view, before finalize
+            assert "feat" not in state
+            state["hook"] = state.get("hook", 0) + 1
+
+        mine = parallel.fuse_views_sharded(list(range(n_views)), fuse_one_view, num, den, finalize, before_reduce=before_reduce)
+        assert state["hook"] == 1
         t = parallel.max_over_ranks(10.0 + rank)
         np.savez(os.path.join(out_dir, f"rank{rank}.npz"), num=num.numpy(), den=den.numpy(), feat=state["feat"],
                  mine=np.array(mine, dtype=np.int64), t=np.array([t]))
