@@ -66,6 +66,10 @@ template <> struct FeatIO<__half> {
 // TILED variant (DC in {64,128}): warp-specialised persistent pipeline (ws.cuh)
 // ---------------------------------------------------------------------------------------------
 constexpr int R_STAGES = 3;
+#ifndef R_PROD_REGS
+#define R_PROD_REGS 72
+#define R_CONS_REGS 184
+#endif
 // Which warps are the consumers.  The SMSP arbiter favours high warp ids: with fp32 rows the consumers are the
 // critical path and get the high ids (-6 % on Mid); with fp16 rows (conversion work in the consumer loop, four
 // channel passes per tile) the producers are the ones that must not starve (measured on Large).
@@ -190,11 +194,12 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT>& sm, con
     int stage = 0;
     uint32_t phase = 0;
     while (true) {   // one iteration per work item: accumulators live exactly one item
-        unsigned long long acc[8][NJ * 2];   // packed channel pairs (fma.rn.f32x2)
+        unsigned long long acc[NJ * 2][8];   // [channel pair][pixel], packed (fma.rn.f32x2); this index order leaves ptxas the fewest
+                                           // accumulator copies in the loop below (8 instead of 21 per 64 FFMA2)
 #pragma unroll
         for (int i = 0; i < 8; ++i)
 #pragma unroll
-            for (int j = 0; j < NJ * 2; ++j) acc[i][j] = 0ull;
+            for (int j = 0; j < NJ * 2; ++j) acc[j][i] = 0ull;
         WsMeta m;
         while (true) {   // batches of the item
             mbar_wait(&sm.ct.full[stage], phase);
@@ -222,7 +227,7 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT>& sm, con
 #pragma unroll
                 for (int j = 0; j < NJ * 2; ++j)
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) fma2_acc(acc[i][j], w2[i], fv[j]);
+                    for (int i = 0; i < 8; ++i) fma2_acc(acc[j][i], w2[i], fv[j]);
             }
             mbar_arrive(&sm.ct.empty[stage]);
             if (++stage == R_STAGES) { stage = 0; phase ^= 1u; }
@@ -238,7 +243,7 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT>& sm, con
                 FT* dst = out_feat + ((size_t)oy * a.t.W + ox) * a.D + m.c0 + cg * 4;
 #pragma unroll
                 for (int j = 0; j < NJ; ++j) {
-                    const float2 lo = unpack2(acc[i][2 * j]), hi = unpack2(acc[i][2 * j + 1]);
+                    const float2 lo = unpack2(acc[2 * j][i]), hi = unpack2(acc[2 * j + 1][i]);
                     FeatIO<FT>::store4(dst + j * 32, make_float4(lo.x, lo.y, hi.x, hi.y));
                 }
             }
@@ -262,10 +267,10 @@ __global__ void __launch_bounds__(WS_THREADS, 1) render_ws_kernel(const RenderAr
     __syncthreads();
     const bool is_producer = kConsHigh<FT> ? threadIdx.x < WS_PROD : threadIdx.x >= WS_CONS;
     if (is_producer) {
-        setmaxnreg_dec<72>();
+        setmaxnreg_dec<R_PROD_REGS>();
         render_ws_producer<DC, FT, DIAG>(sm, a, wk);
     } else {
-        setmaxnreg_inc<184>();
+        setmaxnreg_inc<R_CONS_REGS>();
         render_ws_consumer<DC, FT>(sm, a);
         if (threadIdx.x == (kConsHigh<FT> ? WS_PROD : 0)) ws_queue_release(wk);
     }
