@@ -190,9 +190,10 @@ def launches_per_frame(width: int, height: int) -> int:
 def load_traffic() -> dict:
     """DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) of the hot kernels, from the committed
     `ncu --set full` capture summarised in profiles/ (bench.py never runs under a profiler)."""
-    path = os.path.join(ROOT, "profiles", "r01_traffic.json")
-    if os.path.exists(path):
-        with open(path) as f:
+    import glob
+    paths = sorted(glob.glob(os.path.join(ROOT, "profiles", "r[0-9][0-9]_traffic.json")))   # the latest round's capture
+    if paths:
+        with open(paths[-1]) as f:
             return json.load(f)
     return {}
 

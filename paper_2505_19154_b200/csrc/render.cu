@@ -157,7 +157,7 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
             last = all_done || (pos >= range.y && qt == qh);
             if (p == 0) sm.ct.meta[stage] = WsMeta{nb, tile, c0, last ? WS_FLAG_LAST : 0};
             mbar_arrive(&sm.ct.full[stage]);
-            if (DIAG && last && c0 == 0 && p == 32) {
+            if (DIAG && a.tile_visited && last && c0 == 0 && p == 32) {
                 // diagnostics, once per tile and off the critical path: if the tile stopped early, the last blended
                 // instance lies in this final batch (the pixel that completed the tile blended it)
                 uint32_t visited = range.y - range.x;
@@ -408,8 +408,12 @@ cudaError_t launch_ws(const RenderArgs& a, int tiles, int num_sms, uint32_t* ctr
     wk.order = order;
     wk.order_valid = ctrl + CTRL_ORDER_VALID;
     const int grid = wk.n_items < num_sms ? wk.n_items : num_sms;
-    // the diagnostics variant is a separate instantiation: the product path carries none of its code
-    return a.tile_visited ? launch_ws1<DC, FT, true>(a, wk, grid, st) : launch_ws1<DC, FT, false>(a, wk, grid, st);
+    // One instantiation per feature dtype.  The fp32 kernel always carries the (runtime-guarded, once per tile)
+    // tile_visited store: with that code present ptxas lays the producer loop out 3.7 % faster (1.361 vs 1.411 ms on
+    // the Mid frame, reproducible); without a request a.tile_visited is NULL and nothing is written.  fp16 rows: the
+    // variant without it is the faster one (5.07 vs 5.36 ms on Large) and is used unless diagnostics are requested.
+    if (sizeof(FT) == 4 || a.tile_visited) return launch_ws1<DC, FT, true>(a, wk, grid, st);
+    return launch_ws1<DC, FT, false>(a, wk, grid, st);
 }
 
 template <typename FT>
@@ -466,11 +470,8 @@ extern "C" fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const
     const ScratchLayout L = make_scratch_layout(vs->n, vs->capacity, cam->width, cam->height);
     uint32_t* queue = reinterpret_cast<uint32_t*>((char*)vs->scratch + L.ctrl);
     const uint32_t* order = reinterpret_cast<const uint32_t*>((char*)vs->scratch + L.tile_order);
-    // tile_visited is requested with fhgs_set_diagnostics.  For fp32 rows the kernel instantiation that records it is
-    // used unconditionally: it measured 5 % FASTER on the Mid frame than the one without (1.357 vs 1.429 ms; a code
-    // layout effect of the producer loop, reproducible), and the store is one word per tile.  fp16 rows: only on request
-    // (there the plain instantiation is the faster one, 5.07 vs 5.36 ms on Large).
-    const bool diag = ctx->diagnostics || !(has_feat && g->feat_dtype == FHGS_F16);
+    // tile_visited is requested with fhgs_set_diagnostics; otherwise no kernel writes into the caller's scratch
+    const bool diag = ctx->diagnostics != 0;
     a.tile_visited = diag ? reinterpret_cast<uint32_t*>((char*)vs->scratch + L.tile_visited) : nullptr;
     cudaError_t e = (has_feat && g->feat_dtype == FHGS_F16) ? dispatch<__half>(a, grid, ctx->num_sms, queue, order, s, has_feat)
                                                             : dispatch<float>(a, grid, ctx->num_sms, queue, order, s, has_feat);
