@@ -50,8 +50,10 @@ typedef enum {
 
 typedef enum { FHGS_F32 = 0, FHGS_F16 = 1 } fhgs_dtype;
 
-/* Opaque context: device ordinal, SM count, last-error text, and two copy streams + events used only
- * by fhgs_frame_host.  Owns no device memory. */
+/* Opaque context: device ordinal, SM count, last-error text, two copy streams + events used only by fhgs_frame_host,
+ * and one side stream + events on which fhgs_bin_sort runs two small scans beside its depth pre-sort (forked from and
+ * joined back into the caller's stream with events inside the call).  Owns no device memory.  A context serves one host
+ * thread at a time (use one context per thread / per stream that is driven concurrently). */
 typedef struct fhgs_ctx fhgs_ctx;
 
 FHGS_API fhgs_status fhgs_create(fhgs_ctx** out, int device);

@@ -29,9 +29,12 @@ extern "C" fhgs_status fhgs_create(fhgs_ctx** out, int device) {
     if (cudaSetDevice(device) != cudaSuccess) { delete c; return FHGS_ERR_INTERNAL; }
     c->copy_in = c->copy_out = nullptr;
     c->ev_start = c->ev_feat = c->ev_gt = c->ev_render = c->ev_out = nullptr;
+    c->side = nullptr;
+    c->ev_fork = c->ev_offsets = c->ev_tiles = nullptr;
     bool ok = cudaStreamCreateWithFlags(&c->copy_in, cudaStreamNonBlocking) == cudaSuccess &&
-              cudaStreamCreateWithFlags(&c->copy_out, cudaStreamNonBlocking) == cudaSuccess;
-    for (cudaEvent_t* e : {&c->ev_start, &c->ev_feat, &c->ev_gt, &c->ev_render, &c->ev_out})
+              cudaStreamCreateWithFlags(&c->copy_out, cudaStreamNonBlocking) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) == cudaSuccess;
+    for (cudaEvent_t* e : {&c->ev_start, &c->ev_feat, &c->ev_gt, &c->ev_render, &c->ev_out, &c->ev_fork, &c->ev_offsets, &c->ev_tiles})
         ok = ok && cudaEventCreateWithFlags(e, cudaEventDisableTiming) == cudaSuccess;
     if (!ok) { fhgs_destroy(c); return FHGS_ERR_INTERNAL; }   // releases whatever was created
     *out = c;
@@ -43,7 +46,8 @@ extern "C" void fhgs_destroy(fhgs_ctx* ctx) {
     DeviceGuard dg(ctx);
     if (ctx->copy_in) cudaStreamDestroy(ctx->copy_in);
     if (ctx->copy_out) cudaStreamDestroy(ctx->copy_out);
-    for (cudaEvent_t e : {ctx->ev_start, ctx->ev_feat, ctx->ev_gt, ctx->ev_render, ctx->ev_out})
+    if (ctx->side) cudaStreamDestroy(ctx->side);
+    for (cudaEvent_t e : {ctx->ev_start, ctx->ev_feat, ctx->ev_gt, ctx->ev_render, ctx->ev_out, ctx->ev_fork, ctx->ev_offsets, ctx->ev_tiles})
         if (e) cudaEventDestroy(e);
     delete ctx;
 }

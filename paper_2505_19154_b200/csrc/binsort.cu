@@ -787,6 +787,7 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
     int* tile_diff = (int*)(sc + L.tile_diff);
     const size_t diff_bytes = (size_t)gw1 * gh1 * 4;
     if (grid_counts) FHGS_CUDA(ctx, cudaMemsetAsync(tile_diff, 0, diff_bytes, s));
+    const bool side_overlap = grid_counts && vs->n > 0;
     const int first_bit = full_key ? 0 : 32;
     const int npass = ((32 + tile_bits) - first_bit + 7) / 8;
     vs->sorted_buf = npass & 1;
@@ -804,6 +805,10 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
             presort_init_kernel<<<grid, 256, grid_counts ? diff_bytes : 0, s>>>(vs->n, vs->depth, vs->tiles_touched, pk[0], pv[0], hist32,
                                                                                vs->rect, gw1, gh1, grid_counts ? tile_diff : nullptr);
             FHGS_LAUNCH_CHECK(ctx);
+            if (side_overlap) {
+                FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_fork, s));
+                FHGS_CUDA(ctx, cudaStreamWaitEvent(ctx->side, ctx->ev_fork, 0));
+            }
             hist_scan_kernel<<<4, 256, 0, s>>>(hist32);
             FHGS_LAUNCH_CHECK(ctx);
             FHGS_CUDA(ctx, cudaFuncSetAttribute(onesweep_kernel<uint32_t, SORT_TILE_K32 / OS_THREADS>,
@@ -821,14 +826,26 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
                 FHGS_LAUNCH_CHECK(ctx);
             }
             perm = pv[0];   // 4 passes -> back in buffer 0
-            // `offsets` is defined in index order (C1-S step 1): a scan-only launch
+            // `offsets` is defined in index order (C1-S step 1): a scan-only launch.  With the tile-count path it and the
+            // tile scan (ranges, digit offsets of the tile-id passes, tile order) depend only on presort_init: they run on
+            // the context's side stream beside the four pre-sort passes and the depth-order scan (forked after
+            // presort_init, joined before the emission needs M and before the first tile-id pass needs the offsets).
             ScanDupArgs sa0;
             memset(&sa0, 0, sizeof(sa0));
             sa0.n = vs->n; sa0.GW = GW; sa0.tiles_touched = vs->tiles_touched;
             sa0.offsets = vs->offsets; sa0.num_instances = vs->num_instances;
             sa0.status = scan_status + L.scan_tiles; sa0.ticket = ctrl + CTRL_SCAN2_TICKET;
-            scan_dup_kernel<<<scan_grid, SCAN_THREADS, 0, s>>>(sa0);
+            cudaStream_t s0 = side_overlap ? ctx->side : s;
+            scan_dup_kernel<<<scan_grid, SCAN_THREADS, 0, s0>>>(sa0);
             FHGS_LAUNCH_CHECK(ctx);
+            if (side_overlap) {
+                FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_offsets, ctx->side));
+                FHGS_CUDA(ctx, cudaFuncSetAttribute(tile_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)diff_bytes));
+                tile_scan_kernel<<<1, TS_THREADS, diff_bytes, ctx->side>>>(tile_diff, gw1, gh1, vs->num_instances, vs->capacity, vs->ranges,
+                                                                        hist, npass, (uint32_t*)(sc + L.tile_order), ctrl + CTRL_ORDER_VALID);
+                FHGS_LAUNCH_CHECK(ctx);
+                FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_tiles, ctx->side));
+            }
         }
         if (full_key || vs->capacity == 0) {
             ScanDupArgs sa;
@@ -858,12 +875,9 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
             ea.num_instances = vs->num_instances; ea.capacity = vs->capacity;
             ea.starts = (uint32_t*)(sc + L.emit_starts); ea.units = (int)L.emit_tiles;
             ea.keys = vs->keys[0]; ea.vals = vs->vals[0]; ea.hist = hist; ea.npass = grid_counts ? 0 : npass;
-            if (grid_counts) {   // ranges and digit offsets from the per-tile counts
-                FHGS_CUDA(ctx, cudaFuncSetAttribute(tile_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)diff_bytes));
-                tile_scan_kernel<<<1, TS_THREADS, diff_bytes, s>>>(tile_diff, gw1, gh1, vs->num_instances, vs->capacity, vs->ranges, hist, npass,
-                                                                 (uint32_t*)(sc + L.tile_order), ctrl + CTRL_ORDER_VALID);
-                FHGS_LAUNCH_CHECK(ctx);
-            }
+            // grid_counts: ranges and digit offsets come from the per-tile counts (tile_scan_kernel, on the side stream);
+            // the emission needs M from the offsets scan
+            if (side_overlap) FHGS_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_offsets, 0));
             emit_partition_kernel<<<(ea.units + 1 + 255) / 256, 256, 0, s>>>(ea);
             FHGS_LAUNCH_CHECK(ctx);
             const int egrid = std::min(ea.units, ctx->num_sms * 8);
@@ -879,6 +893,7 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
             FHGS_CUDA(ctx, cudaFuncSetAttribute(onesweep_kernel<uint64_t, SORT_TILE_K64 / OS_THREADS>,
                                                 cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
             const int sort_grid = (int)((vs->capacity + SORT_TILE_K64 - 1) / SORT_TILE_K64);
+            if (side_overlap) FHGS_CUDA(ctx, cudaStreamWaitEvent(s, ctx->ev_tiles, 0));
             for (int p = 0; p < npass; ++p) {
                 FHGS_CUDA(ctx, cudaMemsetAsync(sort_status, 0, (size_t)sort_grid * 256 * 4, s));
                 OneSweepArgs<uint64_t> oa;

@@ -18,6 +18,9 @@ struct fhgs_ctx {
     // fhgs_frame_host only: copy streams / events that overlap host<->device copies with the steps
     cudaStream_t copy_in, copy_out;
     cudaEvent_t ev_start, ev_feat, ev_gt, ev_render, ev_out;
+    // fhgs_bin_sort only: the index-order offsets scan and the tile scan run beside the depth pre-sort on this stream
+    cudaStream_t side;
+    cudaEvent_t ev_fork, ev_offsets, ev_tiles;
     char err[512];
 };
 

@@ -135,6 +135,14 @@ def test_large_shape_fp16_d512():
     print(w)
 
 
+def test_fp16_storage_d256_multiview_shape():
+    """fp16 storage at D = 256 (features, GT map, feature image and fused output in fp16, fp32
+    accumulation) on the Multi-view shape: blobs, 3 orbit views accumulated, 2e-3."""
+    cfg = pu.reduced_config("multiview", n=40_000, width=216, height=168, n_views=200, log_scale_mu=-3.0, feat_dtype="f16")
+    w = run_case(cfg, [0, 67, 133], pu.TOL_F16, sort_flags=(0,))
+    print(w)
+
+
 def test_odd_d_paths():
     """D=4 and D=24 (CH=4 / CH=8 per-pixel kernels)."""
     for d in (4, 24):
