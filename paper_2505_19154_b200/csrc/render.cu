@@ -76,16 +76,16 @@ constexpr int R_STAGES = 3;
 template <typename FT>
 constexpr bool kConsHigh = sizeof(FT) == 4;
 
-template <int DC, typename FT>
+template <int DC, typename FT, int PRIM = 0>
 struct RenderWsSmem {
-    WsCtrl<R_STAGES> ct;
+    WsCtrl<R_STAGES, PRIM> ct;
     float4 rgb[WS_QCAP];                                   // staged colours (xyz used)
     __align__(128) float W[R_STAGES][WS_KB * WS_CONS];     // W[s][kk][slot]
     __align__(128) FT F[R_STAGES][WS_KB * DC];             // feature rows of the batch
 };
 
-template <int DC, typename FT, bool DIAG>
-__device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, const RenderArgs& a, const WsWork& wk) {
+template <int DC, typename FT, bool DIAG, int PRIM>
+__device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT, PRIM>& sm, const RenderArgs& a, const WsWork& wk) {
     const int p = threadIdx.x - (kConsHigh<FT> ? 0 : WS_CONS), lane = p & 31, pw = p >> 5;   // p = pixel slot, pw = warp-block
     const FT* feat = reinterpret_cast<const FT*>(a.feat);
     const float q_cutoff = a.t.q_cutoff, alpha_max = a.t.alpha_max, t_min = a.t.t_min;
@@ -120,8 +120,9 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
         bool last = false;
         do {
             while (qt - qh < WS_KB && pos < range.y) {
-                qt += ws_chunk_append(sm.ct, ch, pos, qt, bx0, by0, bx1, by1, q_cutoff, p,
-                                      [&](int s, const WsChunk& c) { sm.rgb[s] = make_float4(c.r, c.gr, c.b, 0.f); });
+                qt += ws_chunk_append<PRIM>(sm.ct, ch, pos, qt, bx0, by0, bx1, by1, q_cutoff, p,
+                                            [&](int s, const WsChunk& c) { sm.rgb[s] = make_float4(c.r, c.gr, c.b, 0.f); },
+                                            a.t.ray_transform);
                 pos += WS_PROD;
                 ws_chunk_issue(a.t, a.rgb_g, ch);
                 ws_chunk_prefetch_id(a.t, pos + WS_PROD, range.y, p, ch);
@@ -144,7 +145,8 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
                     const float4 r0 = sm.ct.rec0[s];
                     const float4 r1 = sm.ct.rec1[s];
                     const float4 c = sm.rgb[s];
-                    const float w = ws_weight(r0, r1.x, r1.y, P, q_cutoff, alpha_max, t_min);
+                    const float w = PRIM ? ws_weight_surfel(r0, r1, sm.ct.rec2[PRIM ? s : 0], P, q_cutoff, alpha_max, t_min)
+                                         : ws_weight(r0, r1.x, r1.y, P, q_cutoff, alpha_max, t_min);
                     Wd[kk * WS_CONS] = w;
                     C0 = fmaf(w, c.x, C0); C1 = fmaf(w, c.y, C1); C2 = fmaf(w, c.z, C2);
                     m |= (w != 0.f ? 1u : 0u) << kk;
@@ -183,8 +185,8 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT>& sm, con
     }
 }
 
-template <int DC, typename FT>
-__device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT>& sm, const RenderArgs& a) {
+template <int DC, typename FT, int PRIM>
+__device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT, PRIM>& sm, const RenderArgs& a) {
     constexpr int NJ = DC / 32;   // float4 channel groups per thread
     // consumers are the HIGH warps (8-15): the SMSP arbiter favours high warp ids, and the consumers are the critical path
     const int tid = threadIdx.x - (kConsHigh<FT> ? WS_PROD : 0), lane = tid & 31, warp = tid >> 5;
@@ -251,10 +253,10 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT>& sm, con
     }
 }
 
-template <int DC, typename FT, bool DIAG>
+template <int DC, typename FT, bool DIAG, int PRIM = 0>
 __global__ void __launch_bounds__(WS_THREADS, 1) render_ws_kernel(const RenderArgs a, const WsWork wk) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    RenderWsSmem<DC, FT>& sm = *reinterpret_cast<RenderWsSmem<DC, FT>*>(smem_raw);
+    RenderWsSmem<DC, FT, PRIM>& sm = *reinterpret_cast<RenderWsSmem<DC, FT, PRIM>*>(smem_raw);
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int s = 0; s < R_STAGES; ++s) {
@@ -268,10 +270,10 @@ __global__ void __launch_bounds__(WS_THREADS, 1) render_ws_kernel(const RenderAr
     const bool is_producer = kConsHigh<FT> ? threadIdx.x < WS_PROD : threadIdx.x >= WS_CONS;
     if (is_producer) {
         setmaxnreg_dec<R_PROD_REGS>();
-        render_ws_producer<DC, FT, DIAG>(sm, a, wk);
+        render_ws_producer<DC, FT, DIAG, PRIM>(sm, a, wk);
     } else {
         setmaxnreg_inc<R_CONS_REGS>();
-        render_ws_consumer<DC, FT>(sm, a);
+        render_ws_consumer<DC, FT, PRIM>(sm, a);
         if (threadIdx.x == (kConsHigh<FT> ? WS_PROD : 0)) ws_queue_release(wk);
     }
 }
@@ -390,12 +392,12 @@ cudaError_t launch(K kernel, size_t smem, int grid, cudaStream_t st, const Rende
     return cudaGetLastError();
 }
 
-template <int DC, typename FT, bool DIAG>
+template <int DC, typename FT, bool DIAG, int PRIM = 0>
 cudaError_t launch_ws1(const RenderArgs& a, const WsWork& wk, int grid, cudaStream_t st) {
-    const size_t smem = sizeof(RenderWsSmem<DC, FT>);
-    cudaError_t e = cudaFuncSetAttribute(render_ws_kernel<DC, FT, DIAG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const size_t smem = sizeof(RenderWsSmem<DC, FT, PRIM>);
+    cudaError_t e = cudaFuncSetAttribute(render_ws_kernel<DC, FT, DIAG, PRIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    render_ws_kernel<DC, FT, DIAG><<<grid, WS_THREADS, smem, st>>>(a, wk);
+    render_ws_kernel<DC, FT, DIAG, PRIM><<<grid, WS_THREADS, smem, st>>>(a, wk);
     return cudaGetLastError();
 }
 
@@ -412,14 +414,17 @@ cudaError_t launch_ws(const RenderArgs& a, int tiles, int num_sms, uint32_t* ctr
     // tile_visited store: with that code present ptxas lays the producer loop out 3.7 % faster (1.361 vs 1.411 ms on
     // the Mid frame, reproducible); without a request a.tile_visited is NULL and nothing is written.  fp16 rows: the
     // variant without it is the faster one (5.07 vs 5.36 ms on Large) and is used unless diagnostics are requested.
+    if (a.t.ray_transform) return launch_ws1<DC, FT, true, 1>(a, wk, grid, st);   // surfel form (one instantiation per dtype)
     if (sizeof(FT) == 4 || a.tile_visited) return launch_ws1<DC, FT, true>(a, wk, grid, st);
     return launch_ws1<DC, FT, false>(a, wk, grid, st);
 }
 
 template <typename FT>
 cudaError_t dispatch(const RenderArgs& a, int grid, int num_sms, uint32_t* queue, const uint32_t* order, cudaStream_t st, bool has_feat) {
-    if (a.t.ray_transform) {   // surfel mode (NEXT-3): the per-pixel kernels, CH channels per pass, for every D
+    if (a.t.ray_transform) {   // surfel mode (NEXT-3): the same pipelines with the surfel weight; per-pixel kernels for small D
         if (!has_feat) return launch(render_pixel_kernel<0, FT, 1>, sizeof(PixelSmem<0, 1>), grid, st, a);
+        if (a.D % 128 == 0) return launch_ws<128, FT>(a, grid, num_sms, queue, order, st);
+        if (a.D % 64 == 0) return launch_ws<64, FT>(a, grid, num_sms, queue, order, st);
         if (a.D % 16 == 0) return launch(render_pixel_kernel<16, FT, 1>, sizeof(PixelSmem<16, 1>), grid, st, a);
         if (a.D % 8 == 0) return launch(render_pixel_kernel<8, FT, 1>, sizeof(PixelSmem<8, 1>), grid, st, a);
         return launch(render_pixel_kernel<4, FT, 1>, sizeof(PixelSmem<4, 1>), grid, st, a);

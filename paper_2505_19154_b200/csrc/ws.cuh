@@ -130,7 +130,10 @@ __device__ __forceinline__ float ex2_approx(float x) {
 }
 
 // Control block of the pipeline (lives at the front of dynamic shared memory).
-template <int STAGES>
+// PRIM = 0 (EWA Gaussian): rec0 = gx, gy, A, 2B; rec1 = C, opacity, id, position.
+// PRIM = 1 (surfel): the nine entries of the ray transform adj(T): rec0 = m00, m01, m02, m10;
+//          rec1 = m11, opacity, id, position; rec2 = m12, m20, m21, m22.
+template <int STAGES, int PRIM = 0>
 struct WsCtrl {
     uint64_t full[STAGES];
     uint64_t empty[STAGES];
@@ -138,8 +141,9 @@ struct WsCtrl {
     uint32_t mask[STAGES][8];     // per warp-block: bit kk set <=> instance kk gave the block a weight
     uint32_t wcount[WS_PROD / 32];
     int item;                     // work item broadcast among the producers
-    float4 rec0[WS_QCAP];         // gx, gy, A, 2B
-    float4 rec1[WS_QCAP];         // C, opacity, id (bits), position in the sorted list (bits)
+    float4 rec0[WS_QCAP];
+    float4 rec1[WS_QCAP];         // .y opacity, .z id (bits), .w position in the sorted list (bits)
+    float4 rec2[PRIM ? WS_QCAP : 1];
 };
 
 struct WsWork {
@@ -174,6 +178,25 @@ __device__ __forceinline__ float ws_weight(const float4 r0, const float C, const
     const float G = ex2_approx(-0.72134752044448170368f * fmaxf(q, 0.f));   // exp(-q/2)
     const float alpha = fminf(alpha_max, op * G);
     const bool c = (q <= q_cutoff) && !p.done;
+    const float a = c ? alpha : 0.f;
+    const float w = a * p.T;
+    p.T = fmaf(-a, p.T, p.T);
+    p.n += c ? 1u : 0u;
+    p.done = p.done || (p.T < t_min);
+    return w;
+}
+
+// Surfel form of ws_weight: p = adj(T) (x, y, 1)^T, num = p_x^2 + p_y^2, den = p_z^2 in the normative binary32 fmaf
+// expressions (traverse.cuh eval_weight_surfel, oracle fo_surfel_terms); contributes iff den > 0 and num <= q_cut den.
+__device__ __forceinline__ float ws_weight_surfel(const float4 r0, const float4 r1, const float4 r2, WsPixel& p, const float q_cutoff,
+                                                  const float alpha_max, const float t_min) {
+    const float p0 = __fmaf_rn(p.fx, r0.x, __fmaf_rn(p.fy, r0.y, r0.z));
+    const float p1 = __fmaf_rn(p.fx, r0.w, __fmaf_rn(p.fy, r1.x, r2.x));
+    const float p2 = __fmaf_rn(p.fx, r2.y, __fmaf_rn(p.fy, r2.z, r2.w));
+    const float num = __fmaf_rn(p0, p0, __fmul_rn(p1, p1)), den = __fmul_rn(p2, p2);
+    const bool c = (den > 0.f) && (num <= __fmul_rn(q_cutoff, den)) && !p.done;
+    const float G = ex2_approx(-0.72134752044448170368f * __fdividef(num, c ? den : 1.f));
+    const float alpha = fminf(alpha_max, r1.y * G);
     const float a = c ? alpha : 0.f;
     const float w = a * p.T;
     p.T = fmaf(-a, p.T, p.T);
@@ -221,13 +244,27 @@ __device__ __forceinline__ void ws_chunk_prefetch_id(const TraverseArgs& a, uint
 
 // Tile-cull the chunk and append the survivors, in order, to the ring at q_tail.  Returns the number
 // appended (same in all producer threads).  Two producer-wide barriers.
-template <typename CTRL, typename EXTRA>
+template <int PRIM = 0, typename CTRL, typename EXTRA>
 __device__ __forceinline__ int ws_chunk_append(CTRL& ct, const WsChunk& c, uint32_t chunk_pos, int q_tail, float bx0, float by0,
-                                               float bx1, float by1, float q_cutoff, int p, EXTRA&& extra) {
+                                               float bx1, float by1, float q_cutoff, int p, EXTRA&& extra,
+                                               const float4* ray_transform = nullptr) {
     const int lane = p & 31, pw = p >> 5;
     float4 co = c.co;
-    co.y = 2.0f * co.y;   // exact
-    const bool keep = c.valid && tile_may_contribute(c.g, co, bx0, by0, bx1, by1, q_cutoff);
+    bool keep;
+    if (PRIM) {   // surfel: footprint bounding box (centre c.g, half extents co.x, co.y) against the tile's pixel box
+        keep = c.valid && !(c.g.x + co.x < bx0 || c.g.x - co.x > bx1 || c.g.y + co.y < by0 || c.g.y - co.y > by1);
+    } else {
+        co.y = 2.0f * co.y;   // exact
+        keep = c.valid && tile_may_contribute(c.g, co, bx0, by0, bx1, by1, q_cutoff);
+    }
+    // surfel: the survivors' ray transforms are fetched here (not prefetched with the chunk: 12 more registers per producer
+    // thread would spill; the producers have the slack)
+    float4 m0 = make_float4(0.f, 0.f, 0.f, 0.f), m1 = m0, m2 = m0;
+    if (PRIM && keep) {
+        m0 = __ldg(ray_transform + 3 * (size_t)c.id);
+        m1 = __ldg(ray_transform + 3 * (size_t)c.id + 1);
+        m2 = __ldg(ray_transform + 3 * (size_t)c.id + 2);
+    }
     const uint32_t ballot = __ballot_sync(TR_FULL, keep);
     if (lane == 0) ct.wcount[pw] = __popc(ballot);
     named_bar_sync(WS_BAR_PROD, WS_PROD);
@@ -240,8 +277,14 @@ __device__ __forceinline__ int ws_chunk_append(CTRL& ct, const WsChunk& c, uint3
     }
     if (keep) {
         const int s = (q_tail + off + __popc(ballot & ((1u << lane) - 1u))) & (WS_QCAP - 1);
-        ct.rec0[s] = make_float4(c.g.x, c.g.y, co.x, co.y);
-        ct.rec1[s] = make_float4(co.z, co.w, __uint_as_float(c.id), __uint_as_float(chunk_pos + (uint32_t)p));
+        if (PRIM) {
+            ct.rec0[s] = make_float4(m0.x, m0.y, m0.z, m1.x);
+            ct.rec1[s] = make_float4(m1.y, co.w, __uint_as_float(c.id), __uint_as_float(chunk_pos + (uint32_t)p));
+            ct.rec2[PRIM ? s : 0] = make_float4(m1.z, m2.x, m2.y, m2.z);
+        } else {
+            ct.rec0[s] = make_float4(c.g.x, c.g.y, co.x, co.y);
+            ct.rec1[s] = make_float4(co.z, co.w, __uint_as_float(c.id), __uint_as_float(chunk_pos + (uint32_t)p));
+        }
         extra(s, c);
     }
     named_bar_sync(WS_BAR_PROD, WS_PROD);
