@@ -210,9 +210,10 @@ enum { FW_FLAG_FIRST = 4 };
 template <typename GT>
 constexpr int kGBufs = sizeof(GT) == 2 ? 2 : 1;
 
-template <typename GT>
+// PRIM = 1 (surfel): three records per survivor; the ring shrinks to 288 slots (modulo wrap) to fit beside the fp32 tile
+template <typename GT, int PRIM = 0>
 struct FuseWsSmem {
-    WsCtrl<FW_STAGES> ct;
+    WsCtrl<FW_STAGES, PRIM, PRIM ? 288 : WS_QCAP> ct;
     uint64_t g_full[2], g_free[2];
     uint64_t item_full[2], item_empty[2];
     int items[2];
@@ -238,8 +239,8 @@ __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t by
                  : "memory");
 }
 
-template <typename GT>
-__device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem<GT>& sm, const FuseArgs& a, const WsWork& wk) {
+template <typename GT, int PRIM>
+__device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem<GT, PRIM>& sm, const FuseArgs& a, const WsWork& wk) {
     const int lane = threadIdx.x & 31;
     const GT* gt = reinterpret_cast<const GT*>(a.gt);
     int islot = 0, gb = 0;
@@ -284,8 +285,9 @@ __device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem<GT>& sm, const Fuse
     }
 }
 
-template <typename GT>
-__device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseArgs& a, const WsWork& wk) {
+template <typename GT, int PRIM>
+__device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT, PRIM>& sm, const FuseArgs& a, const WsWork& wk) {
+    using CT = decltype(sm.ct);
     const int p = threadIdx.x, lane = p & 31;   // producers are warps 0-7
     const float q_cutoff = a.t.q_cutoff, alpha_max = a.t.alpha_max, t_min = a.t.t_min;
     const int sx = p & 15, sy = p >> 4;   // row-major pixel slot (matches the GT tile rows)
@@ -323,7 +325,8 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseA
         bool last = false, first = true;
         do {
             while (qt - qh < WS_KB && pos < range.y) {
-                qt += ws_chunk_append(sm.ct, ch, pos, qt, bx0, by0, bx1, by1, q_cutoff, p, [](int, const WsChunk&) {});
+                qt += ws_chunk_append<PRIM>(sm.ct, ch, pos, qt, bx0, by0, bx1, by1, q_cutoff, p, [](int, const WsChunk&) {},
+                                            a.t.ray_transform);
                 pos += WS_PROD;
                 ws_chunk_issue(a.t, nullptr, ch);
                 ws_chunk_prefetch_id(a.t, pos + WS_PROD, range.y, p, ch);
@@ -333,7 +336,7 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseA
             mbar_wait_backoff(&sm.ct.empty[stage], phase ^ 1u);
             WS_TACC(2);
             WS_TCNT(5);
-            if (p < WS_KB) sm.ids[stage][p] = p < nb ? __float_as_uint(sm.ct.rec1[(qh + p) & (WS_QCAP - 1)].z) : 0u;
+            if (p < WS_KB) sm.ids[stage][p] = p < nb ? __float_as_uint(sm.ct.rec1[CT::slot(qh + p)].z) : 0u;
             float* Wd = sm.W[stage] + p * 4;
             const bool warp_done = __all_sync(TR_FULL, P.done);
 #pragma unroll 2
@@ -343,11 +346,12 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseA
 #pragma unroll
                     for (int j = 0; j < 4; ++j) {
                         const int kk = kq * 4 + j;
-                        const int s = (qh + kk) & (WS_QCAP - 1);
+                        const int s = CT::slot(qh + kk);
                         const float4 r0 = sm.ct.rec0[s];
                         const float4 r1 = sm.ct.rec1[s];
                         WsPixel Q = P;
-                        const float w = ws_weight(r0, r1.x, r1.y, Q, q_cutoff, alpha_max, t_min);
+                        const float w = PRIM ? ws_weight_surfel(r0, r1, sm.ct.rec2[PRIM ? s : 0], Q, q_cutoff, alpha_max, t_min)
+                                             : ws_weight(r0, r1.x, r1.y, Q, q_cutoff, alpha_max, t_min);
                         if (kk < nb) { P = Q; w4[j] = w; }
                     }
                 }
@@ -368,8 +372,8 @@ __device__ __forceinline__ void fuse_ws_producer(FuseWsSmem<GT>& sm, const FuseA
     (void)lane;
 }
 
-template <typename GT>
-__device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT>& sm, const FuseArgs& a) {
+template <typename GT, int PRIM>
+__device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT, PRIM>& sm, const FuseArgs& a) {
     // consumers are warps 8-15: the SMSP arbiter favours high warp ids and the consumers are the critical path
     const int tid = threadIdx.x - WS_PROD, lane = tid & 31, warp = tid >> 5;
     const int half = warp >> 2, cw = warp & 3;
@@ -483,10 +487,10 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT>& sm, const FuseA
 }
 
 
-template <typename GT>
+template <typename GT, int PRIM = 0>
 __global__ void __launch_bounds__(FW_THREADS, 1) fuse_ws_kernel(const FuseArgs a, const WsWork wk) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    FuseWsSmem<GT>& sm = *reinterpret_cast<FuseWsSmem<GT>*>(smem_raw);
+    FuseWsSmem<GT, PRIM>& sm = *reinterpret_cast<FuseWsSmem<GT, PRIM>*>(smem_raw);
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int s = 0; s < FW_STAGES; ++s) {
@@ -667,10 +671,11 @@ cudaError_t launch(K kernel, size_t smem, int grid, cudaStream_t st, const FuseA
     return cudaGetLastError();
 }
 
-template <typename GT>
+template <typename GT, int PRIM = 0>
 cudaError_t launch_fuse_ws(const FuseArgs& a, int tiles, int num_sms, uint32_t* ctrl, const uint32_t* order, cudaStream_t st) {
-    const size_t smem = sizeof(FuseWsSmem<GT>);
-    cudaError_t e = cudaFuncSetAttribute(fuse_ws_kernel<GT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const size_t smem = sizeof(FuseWsSmem<GT, PRIM>);
+    static_assert(sizeof(FuseWsSmem<GT, PRIM>) <= 232448, "fuse_ws shared memory exceeds 227 KB");
+    cudaError_t e = cudaFuncSetAttribute(fuse_ws_kernel<GT, PRIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     WsWork wk;
     wk.queue = ctrl + CTRL_FUSE_QUEUE;
@@ -679,13 +684,14 @@ cudaError_t launch_fuse_ws(const FuseArgs& a, int tiles, int num_sms, uint32_t* 
     wk.order = order;
     wk.order_valid = ctrl + CTRL_ORDER_VALID;
     const int grid = wk.n_items < num_sms ? wk.n_items : num_sms;
-    fuse_ws_kernel<GT><<<grid, FW_THREADS, smem, st>>>(a, wk);
+    fuse_ws_kernel<GT, PRIM><<<grid, FW_THREADS, smem, st>>>(a, wk);
     return cudaGetLastError();
 }
 
 template <typename GT>
 cudaError_t dispatch(const FuseArgs& a, int grid, int num_sms, uint32_t* queue, const uint32_t* order, cudaStream_t st) {
-    if (a.t.ray_transform) {   // surfel mode (NEXT-3): the tile-per-CTA kernels for every D
+    if (a.t.ray_transform) {   // surfel mode (NEXT-3): the same pipeline with the surfel weight; tile-per-CTA kernels otherwise
+        if (a.D % FW_DC == 0) return launch_fuse_ws<GT, 1>(a, grid, num_sms, queue, order, st);
         if (a.D % 64 == 0) return launch(fuse_tiled_kernel<64, GT, 1>, sizeof(FuseTiledSmem<64, 1>), grid, st, a);
         if (a.D % 16 == 0) return launch(fuse_pixel_kernel<16, GT, 1>, 0, grid, st, a);
         if (a.D % 8 == 0) return launch(fuse_pixel_kernel<8, GT, 1>, 0, grid, st, a);

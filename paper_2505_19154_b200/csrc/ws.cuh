@@ -133,17 +133,23 @@ __device__ __forceinline__ float ex2_approx(float x) {
 // PRIM = 0 (EWA Gaussian): rec0 = gx, gy, A, 2B; rec1 = C, opacity, id, position.
 // PRIM = 1 (surfel): the nine entries of the ray transform adj(T): rec0 = m00, m01, m02, m10;
 //          rec1 = m11, opacity, id, position; rec2 = m12, m20, m21, m22.
-template <int STAGES, int PRIM = 0>
+template <int STAGES, int PRIM = 0, int Q = WS_QCAP>
 struct WsCtrl {
+    // ring capacity: >= WS_KB - 1 + WS_PROD = 287 (a chunk is appended only while fewer than WS_KB survivors are queued).
+    // A power of two wraps with a mask; the surfel form of fuse_ws has no shared memory for 512 slots of three records
+    // and uses 288 with a modulo.
+    static constexpr int QCAP = Q;
+    static_assert(Q >= WS_KB - 1 + WS_PROD, "ring too small");
+    static __device__ __forceinline__ int slot(int x) { return (Q & (Q - 1)) == 0 ? (x & (Q - 1)) : (int)((unsigned)x % (unsigned)Q); }
     uint64_t full[STAGES];
     uint64_t empty[STAGES];
     WsMeta meta[STAGES];
     uint32_t mask[STAGES][8];     // per warp-block: bit kk set <=> instance kk gave the block a weight
     uint32_t wcount[WS_PROD / 32];
     int item;                     // work item broadcast among the producers
-    float4 rec0[WS_QCAP];
-    float4 rec1[WS_QCAP];         // .y opacity, .z id (bits), .w position in the sorted list (bits)
-    float4 rec2[PRIM ? WS_QCAP : 1];
+    float4 rec0[Q];
+    float4 rec1[Q];               // .y opacity, .z id (bits), .w position in the sorted list (bits)
+    float4 rec2[PRIM ? Q : 1];
 };
 
 struct WsWork {
@@ -276,7 +282,7 @@ __device__ __forceinline__ int ws_chunk_append(CTRL& ct, const WsChunk& c, uint3
         total += cnt;
     }
     if (keep) {
-        const int s = (q_tail + off + __popc(ballot & ((1u << lane) - 1u))) & (WS_QCAP - 1);
+        const int s = CTRL::slot(q_tail + off + __popc(ballot & ((1u << lane) - 1u)));
         if (PRIM) {
             ct.rec0[s] = make_float4(m0.x, m0.y, m0.z, m1.x);
             ct.rec1[s] = make_float4(m1.y, co.w, __uint_as_float(c.id), __uint_as_float(chunk_pos + (uint32_t)p));
