@@ -52,14 +52,19 @@ class Guarded:
         return self.interior().view(dtype).view(*shape)
 
 
-def guarded_view_state(fb, torch, n, W, H, cap, dev):
-    vs = fb.ViewState(n, W, H, cap, device=dev)
+def guarded_view_state(fb, torch, n, W, H, cap, dev, surfel=False):
+    vs = fb.ViewState(n, W, H, cap, device=dev, surfel=surfel)
     gw, gh = (W + 15) // 16, (H + 15) // 16
     m, c = max(n, 1), max(cap, 1)
     sizes = dict(xy=8 * m, depth=4 * m, conic_opacity=16 * m, rgb=12 * m, radius=4 * m, rect=8 * m, tiles_touched=4 * m,
                  offsets=4 * m, num_instances=8, ranges=8 * gw * gh, scratch=int(vs.c.scratch_bytes),
                  keys0=8 * c, keys1=8 * c, vals0=4 * c, vals1=4 * c)
+    if surfel:
+        sizes["ray_transform"] = 48 * m
     bufs = {k: Guarded(torch, v, dev) for k, v in sizes.items()}
+    if surfel:
+        vs.c.ray_transform = bufs["ray_transform"].ptr
+        vs.ray_transform = bufs["ray_transform"].view(torch.float32, (m, 12))
     for k in ("xy", "depth", "conic_opacity", "rgb", "radius", "rect", "tiles_touched", "offsets", "num_instances", "ranges", "scratch"):
         setattr(vs.c, k, bufs[k].ptr)
     vs.c.keys[0], vs.c.keys[1] = bufs["keys0"].ptr, bufs["keys1"].ptr
@@ -77,13 +82,13 @@ def guarded_view_state(fb, torch, n, W, H, cap, dev):
     return vs, bufs
 
 
-def run_guarded(cfg, view, tol, sort_flags=(1, 0), ndfd=False):
+def run_guarded(cfg, view, tol, sort_flags=(1, 0), ndfd=False, surfel=False):
     import torch
     from paper_2505_19154_b200 import binding as fb
     scene = inputs.make_scene(cfg)
     cam = inputs.make_camera(cfg, view)
     gt = inputs.make_gt_map(cfg, view, cam)
-    pr = pu.oracle_view(scene, cam)
+    pr = pu.oracle_view(scene, cam, fo.params(primitive=1 if surfel else 0))
     bo = fo.bins(pr, cfg.width, cfg.height)
     order = fo.global_order(pr)
     feat32 = scene.feat.astype(np.float32)
@@ -92,10 +97,10 @@ def run_guarded(cfg, view, tol, sort_flags=(1, 0), ndfd=False):
     touch = pu.Borderline(scene.n, cfg.feat_dim)
     touch.add_view(pr, np.nonzero(o["fragile"])[0], cfg.width, bo, gt)
 
-    gp = pu.GpuPath(scene, cfg.width, cfg.height, 16)
+    gp = pu.GpuPath(scene, cfg.width, cfg.height, 16, surfel=surfel)
     dev = gp.g.mean.device
     W, H, D, n = cfg.width, cfg.height, cfg.feat_dim, scene.n
-    vs, bufs = guarded_view_state(fb, torch, n, W, H, bo["M"] + 3, dev)   # capacity barely above M: a tail overrun hits the guard
+    vs, bufs = guarded_view_state(fb, torch, n, W, H, bo["M"] + 3, dev, surfel=surfel)   # capacity barely above M: a tail overrun hits the guard
     gp.vs = vs
     es = scene.feat.dtype.itemsize
     outs = dict(rgb=Guarded(torch, 12 * W * H, dev), feat=Guarded(torch, es * W * H * D, dev), T=Guarded(torch, 4 * W * H, dev),
@@ -138,10 +143,11 @@ def run_guarded(cfg, view, tol, sort_flags=(1, 0), ndfd=False):
             t_lgt, t_lcf = outs["lgt"].view(torch.float32, (H, W)), outs["lcf"].view(torch.float32, (H, W))
             outs["lgt"].poison(); outs["lcf"].poison(); outs["gop"].zero()
             fb.ndfd_forward(gp.ctx, gp.g, c, gp.prm, vs, gt_d, t_lgt, t_lcf)
-            work = fb.ndfd_backward(gp.ctx, gp.g, c, gp.prm, vs, gt_d, outs["gop"].view(torch.float32, (n,)))
+            if not surfel:   # the w-level backward is built for the EWA primitive
+                work = fb.ndfd_backward(gp.ctx, gp.g, c, gp.prm, vs, gt_d, outs["gop"].view(torch.float32, (n,)))
+                del work
             torch.cuda.synchronize()
             assert np.isfinite(t_lgt.cpu().numpy()).all() and np.isfinite(t_lcf.cpu().numpy()).all()
-            del work
     bad = [k for k, b in list(bufs.items()) + list(outs.items()) if not b.intact()]
     assert not bad, f"guard band overwritten next to: {bad}"
     return dict(M=int(bo["M"]))
@@ -169,3 +175,15 @@ def test_guards_ws_kernels_f16():
     print(run_guarded(pu.reduced_config("large", n=12_000, width=136, height=88, log_scale_mu=-3.2), 0, pu.TOL_F16, sort_flags=(0,)))
     print(run_guarded(pu.reduced_config("large", n=12_000, width=136, height=88, log_scale_mu=-3.2, feat_dim=128), 0, pu.TOL_F16,
                       sort_flags=(0,)))
+
+
+def test_guards_surfel_kernels():
+    """FHGS_PRIM_SURFEL: project_surfel_kernel, the surfel forms of render_ws<128> / fuse_ws (288-slot ring), render_ws<64> /
+    fuse_tiled<64>, the per-pixel kernels (D = 24), fp16 storage, and the surfel NDFD forward, between guard bands, on
+    poisoned buffers (ray_transform included), three times."""
+    print(run_guarded(pu.reduced_config("mid", n=20_000, width=200, height=120, log_scale_mu=-2.8), 0, pu.TOL_F32, ndfd=True, surfel=True))
+    print(run_guarded(pu.reduced_config("mid", n=8_000, width=120, height=72, log_scale_mu=-2.6, feat_dim=64), 0, pu.TOL_F32,
+                      sort_flags=(0,), surfel=True))
+    print(run_guarded(pu.reduced_config("tiny", n=3000, feat_dim=24, width=83, height=45, log_scale_mu=-2.3), 0, pu.TOL_F32, surfel=True))
+    print(run_guarded(pu.reduced_config("large", n=12_000, width=136, height=88, log_scale_mu=-2.8, feat_dim=128), 0, pu.TOL_F16,
+                      sort_flags=(0,), surfel=True))
