@@ -261,7 +261,7 @@ FHGS_API fhgs_status fhgs_ndfd_forward(fhgs_ctx* ctx, const fhgs_gaussians* g, c
  * grad_opacity [n] f32 is ACCUMULATED into (the caller zeroes it; atomic order is free).
  * work: device scratch of fhgs_ndfd_backward_work_bytes(width, height, D) bytes, 256-byte aligned (per-pixel
  * totals of the three forward traversals the first path uses).  D in {32,64,128,256}; other arguments as
- * fhgs_ndfd_forward. */
+ * fhgs_ndfd_forward.  Both NDFD calls also run in surfel mode (prm->primitive = FHGS_PRIM_SURFEL; f32 features and map). */
 FHGS_API size_t fhgs_ndfd_backward_work_bytes(int32_t width, int32_t height, int32_t feat_dim);
 FHGS_API fhgs_status fhgs_ndfd_backward(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam,
                                const fhgs_params* prm, const fhgs_view_state* vs, const void* gt,

@@ -837,9 +837,17 @@ double fo_ndfd_backward(int n_order, const uint32_t *order, int D, const float *
             for (int k = 0; k < n_order; ++k) {
                 if (T < t_min) break;
                 const uint32_t g = order[k];
-                const float q = fo_q(xy[2 * g], xy[2 * g + 1], conic_opacity[4 * g], conic_opacity[4 * g + 1], conic_opacity[4 * g + 2], x, y);
-                if (!(q <= q_cut)) continue;
-                const double G = exp(-0.5 * fmax((double)q, 0.0));
+                double G;
+                if (g_rt) {   /* surfel mode: G = exp(-(u^2+v^2)/2) from the ray transform (same decision as eval_alpha) */
+                    float pp[3], num, den;
+                    fo_surfel_terms(g_rt + 12 * (size_t)g, x, y, pp, &num, &den);
+                    if (!(den > 0.0f) || !(num <= q_cut * den)) continue;
+                    G = exp(-0.5 * ((double)num / (double)den));
+                } else {
+                    const float q = fo_q(xy[2 * g], xy[2 * g + 1], conic_opacity[4 * g], conic_opacity[4 * g + 1], conic_opacity[4 * g + 2], x, y);
+                    if (!(q <= q_cut)) continue;
+                    G = exp(-0.5 * fmax((double)q, 0.0));
+                }
                 const double a_raw = (double)conic_opacity[4 * g + 3] * G;
                 const double a = fmin((double)alpha_max, a_raw);
                 if (cnt == cap) {

@@ -256,7 +256,6 @@ def ndfd(pr, order, feat, gt, W, H, k=20.0, lam=0.5, mode=0, params=DEFAULT_PARA
 def ndfd_backward(pr, order, feat, gt, W, H, k=20.0, lam=0.5, lam1=1.0, lam2=1.0, params=DEFAULT_PARAMS, pix=None):
     """NDFD backward at the w level: returns (L, grad_opacity[n]) with
     L = sum over `pix` of lam1 L_gt + lam2 L_cf (blend-order accumulation) and grad_opacity = dL/d opacity."""
-    assert "ray_transform" not in pr, "the w-level backward is built for the EWA primitive only"
     feat32, gt32 = _f32(feat), _f32(gt)
     D = feat32.shape[1]
     n = pr["radius"].shape[0]
@@ -266,7 +265,8 @@ def ndfd_backward(pr, order, feat, gt, W, H, k=20.0, lam=0.5, lam1=1.0, lam2=1.0
     grad = np.zeros(n, np.float64)
     fn = lib().fo_ndfd_backward
     fn.restype = C.c_double
-    L = fn(C.c_int(order.shape[0]), _p(order), C.c_int(D), _p(pr["xy"]), _p(pr["conic_opacity"]), _p(feat32), _p(gt32),
-           C.c_int(W), C.c_int(H), _p(_f32(params)), C.c_double(k), C.c_double(lam), C.c_double(lam1), C.c_double(lam2),
-           C.c_int64(npix), _p(pix), _p(grad))
+    with _surfel(pr):
+        L = fn(C.c_int(order.shape[0]), _p(order), C.c_int(D), _p(pr["xy"]), _p(pr["conic_opacity"]), _p(feat32), _p(gt32),
+               C.c_int(W), C.c_int(H), _p(_f32(params)), C.c_double(k), C.c_double(lam), C.c_double(lam1), C.c_double(lam2),
+               C.c_int64(npix), _p(pix), _p(grad))
     return float(L), grad

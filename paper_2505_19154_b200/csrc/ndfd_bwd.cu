@@ -66,9 +66,9 @@ struct BwdSub {
 };
 
 // MODE 1: totals A_0, B_0, C_0.  MODE 3: gradient.
-template <int MODE, int LPP, int CPL, typename FT, typename GT>
+template <int MODE, int LPP, int CPL, typename FT, typename GT, int PRIM>
 __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel(const BwdArgs a) {
-    __shared__ TileQueue q;
+    __shared__ TileQueueT<PRIM> q;
     constexpr int PXW = 32 / LPP, ROWS = 8 * PXW / FHGS_TILE, STRIPS = FHGS_TILE / ROWS;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int tile = blockIdx.x / STRIPS, strip = blockIdx.x % STRIPS;
@@ -137,7 +137,21 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
             // pixel group, and handed round by shuffles (as in ndfd.cu)
             for (int k0 = sb * SB; k0 < k_end; k0 += LPP) {
               float a_c = 0.f, g_c = 0.f;
-              if (k0 + cgl < k_end) {
+              if (PRIM) {   // surfel: G = exp(-(u^2+v^2)/2) from the ray transform (traverse.cuh eval_weight_surfel)
+                  if (k0 + cgl < k_end) {
+                      const float4 m0 = q.m[0][PRIM ? k0 + cgl : 0], m1 = q.m[PRIM ? 1 : 0][PRIM ? k0 + cgl : 0], m2 = q.m[PRIM ? 2 : 0][PRIM ? k0 + cgl : 0];
+                      const float p0 = __fmaf_rn(fx, m0.x, __fmaf_rn(fy, m0.y, m0.z));
+                      const float p1 = __fmaf_rn(fx, m1.x, __fmaf_rn(fy, m1.y, m1.z));
+                      const float p2 = __fmaf_rn(fx, m2.x, __fmaf_rn(fy, m2.y, m2.z));
+                      const float num = __fmaf_rn(p0, p0, __fmul_rn(p1, p1)), den = __fmul_rn(p2, p2);
+                      if (den > 0.f && num <= __fmul_rn(a.t.q_cutoff, den)) {
+                          const float G = exp2f(-0.72134752044448170368f * __fdividef(num, den));
+                          const float a_raw = q.co[k0 + cgl].w * G;
+                          a_c = fminf(a.t.alpha_max, a_raw);
+                          g_c = a_raw < a.t.alpha_max ? G : 0.f;
+                      }
+                  }
+              } else if (k0 + cgl < k_end) {
                   const float2 gxy = q.xy[k0 + cgl];
                   const float4 co = q.co[k0 + cgl];
                   const float dx = __fsub_rn(gxy.x, fx), dy = __fsub_rn(gxy.y, fy);
@@ -241,30 +255,30 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
     }
 }
 
-template <int MODE, int LPP, int CPL, typename FT, typename GT>
+template <int MODE, int LPP, int CPL, typename FT, typename GT, int PRIM>
 cudaError_t launch1(const BwdArgs& a, int tiles, cudaStream_t st) {
     constexpr int STRIPS = FHGS_TILE / (8 * (32 / LPP) / FHGS_TILE);
     const size_t smem = 2 * (size_t)BwdSub<LPP * CPL, FT>::SB * BwdSub<LPP * CPL, FT>::ROW_BYTES;
-    cudaError_t e = cudaFuncSetAttribute(ndfd_bwd_kernel<MODE, LPP, CPL, FT, GT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(ndfd_bwd_kernel<MODE, LPP, CPL, FT, GT, PRIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    ndfd_bwd_kernel<MODE, LPP, CPL, FT, GT><<<tiles * STRIPS, TR_THREADS, smem, st>>>(a);
+    ndfd_bwd_kernel<MODE, LPP, CPL, FT, GT, PRIM><<<tiles * STRIPS, TR_THREADS, smem, st>>>(a);
     return cudaGetLastError();
 }
 
-template <int LPP, int CPL, typename FT, typename GT>
+template <int LPP, int CPL, typename FT, typename GT, int PRIM>
 cudaError_t launch3(const BwdArgs& a, int tiles, cudaStream_t st) {
     cudaError_t e;
-    if ((e = launch1<1, LPP, CPL, FT, GT>(a, tiles, st)) != cudaSuccess) return e;
-    return launch1<3, LPP, CPL, FT, GT>(a, tiles, st);
+    if ((e = launch1<1, LPP, CPL, FT, GT, PRIM>(a, tiles, st)) != cudaSuccess) return e;
+    return launch1<3, LPP, CPL, FT, GT, PRIM>(a, tiles, st);
 }
 
-template <typename FT, typename GT>
+template <typename FT, typename GT, int PRIM = 0>
 cudaError_t dispatch(const BwdArgs& a, int tiles, cudaStream_t st) {
     switch (a.D) {
-        case 32: return launch3<4, 8, FT, GT>(a, tiles, st);
-        case 64: return launch3<4, 16, FT, GT>(a, tiles, st);
-        case 128: return launch3<4, 32, FT, GT>(a, tiles, st);
-        case 256: return launch3<8, 32, FT, GT>(a, tiles, st);
+        case 32: return launch3<4, 8, FT, GT, PRIM>(a, tiles, st);
+        case 64: return launch3<4, 16, FT, GT, PRIM>(a, tiles, st);
+        case 128: return launch3<4, 32, FT, GT, PRIM>(a, tiles, st);
+        case 256: return launch3<8, 32, FT, GT, PRIM>(a, tiles, st);
         default: return cudaErrorInvalidValue;
     }
 }
@@ -287,7 +301,10 @@ extern "C" fhgs_status fhgs_ndfd_backward(fhgs_ctx* ctx, const fhgs_gaussians* g
     if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
     if ((st = validate_params(ctx, prm)) != FHGS_OK) return st;
     if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
-    if (prm->primitive != FHGS_PRIM_EWA) FHGS_INVALID(ctx, "the NDFD calls are built for FHGS_PRIM_EWA only");
+    const bool surfel = prm->primitive == FHGS_PRIM_SURFEL;
+    if ((st = validate_primitive(ctx, prm, vs)) != FHGS_OK) return st;
+    if (surfel && (g->feat_dtype != FHGS_F32 || gt_dtype != FHGS_F32))
+        FHGS_INVALID(ctx, "fhgs_ndfd_backward: the surfel primitive is built for f32 features and map");
     if (!g->feat) FHGS_INVALID(ctx, "fhgs_ndfd_backward: g->feat is NULL");
     if ((g->feat_dtype != FHGS_F32 && g->feat_dtype != FHGS_F16) || (gt_dtype != FHGS_F32 && gt_dtype != FHGS_F16))
         FHGS_INVALID(ctx, "fhgs_ndfd_backward: unknown dtype");
@@ -304,7 +321,7 @@ extern "C" fhgs_status fhgs_ndfd_backward(fhgs_ctx* ctx, const fhgs_gaussians* g
     a.t.xy = reinterpret_cast<const float2*>(vs->xy);
     a.t.conic_opacity = reinterpret_cast<const float4*>(vs->conic_opacity);
     a.t.q_cutoff = prm->q_cutoff; a.t.alpha_max = prm->alpha_max; a.t.t_min = prm->t_min;
-    a.t.ray_transform = nullptr;
+    a.t.ray_transform = surfel ? reinterpret_cast<const float4*>(vs->ray_transform) : nullptr;
     a.feat = g->feat; a.gt = gt; a.D = D; a.k_sig = k_sigmoid; a.lambda = lambda; a.lam1 = lam1; a.lam2 = lam2;
     const size_t px = (size_t)cam->width * cam->height;
     a.A_tot = reinterpret_cast<float*>(work);
@@ -316,7 +333,8 @@ extern "C" fhgs_status fhgs_ndfd_backward(fhgs_ctx* ctx, const fhgs_gaussians* g
     cudaStream_t s = (cudaStream_t)stream;
     cudaError_t e;
     const bool fh = g->feat_dtype == FHGS_F16, gh = gt_dtype == FHGS_F16;
-    if (fh && gh) e = dispatch<__half, __half>(a, tiles, s);
+    if (surfel) e = dispatch<float, float, 1>(a, tiles, s);
+    else if (fh && gh) e = dispatch<__half, __half>(a, tiles, s);
     else if (fh) e = dispatch<__half, float>(a, tiles, s);
     else if (gh) e = dispatch<float, __half>(a, tiles, s);
     else e = dispatch<float, float>(a, tiles, s);

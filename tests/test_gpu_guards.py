@@ -143,10 +143,9 @@ def run_guarded(cfg, view, tol, sort_flags=(1, 0), ndfd=False, surfel=False):
             t_lgt, t_lcf = outs["lgt"].view(torch.float32, (H, W)), outs["lcf"].view(torch.float32, (H, W))
             outs["lgt"].poison(); outs["lcf"].poison(); outs["gop"].zero()
             fb.ndfd_forward(gp.ctx, gp.g, c, gp.prm, vs, gt_d, t_lgt, t_lcf)
-            if not surfel:   # the w-level backward is built for the EWA primitive
-                work = fb.ndfd_backward(gp.ctx, gp.g, c, gp.prm, vs, gt_d, outs["gop"].view(torch.float32, (n,)))
-                del work
+            work = fb.ndfd_backward(gp.ctx, gp.g, c, gp.prm, vs, gt_d, outs["gop"].view(torch.float32, (n,)))
             torch.cuda.synchronize()
+            del work
             assert np.isfinite(t_lgt.cpu().numpy()).all() and np.isfinite(t_lcf.cpu().numpy()).all()
     bad = [k for k, b in list(bufs.items()) + list(outs.items()) if not b.intact()]
     assert not bad, f"guard band overwritten next to: {bad}"

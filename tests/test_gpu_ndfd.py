@@ -77,6 +77,11 @@ def test_ndfd_surfel_primitive():
     print(_run(cfg, 0, pu.TOL_F32, surfel=True))
     cfg = pu.reduced_config("mid", n=10_000, width=160, height=96, log_scale_mu=-2.6, feat_dim=32)
     print(_run(cfg, 0, pu.TOL_F32, npix=1500, surfel=True))
+    # and the opacity gradient of those losses over surfels (w-level backward)
+    cfg = pu.reduced_config("mid", n=30_000, width=200, height=120, log_scale_mu=-2.8)
+    print(_run_backward(cfg, 0, 1.0, 1.0, surfel=True))
+    cfg = pu.reduced_config("mid", n=10_000, width=160, height=96, log_scale_mu=-2.6, feat_dim=64)
+    print(_run_backward(cfg, 0, 0.3, 2.0, k=8.0, lam=0.3, surfel=True))
 
 
 def test_ndfd_multiview_blobs_and_params():
@@ -125,15 +130,15 @@ def test_ndfd_invalid_arguments():
 
 
 # ---- NEXT-2: backward at the w level --------------------------------------------------------------
-def _run_backward(cfg, view, lam1, lam2, k=20.0, lam=0.5):
+def _run_backward(cfg, view, lam1, lam2, k=20.0, lam=0.5, surfel=False):
     import torch
     from paper_2505_19154_b200 import binding as fb
     scene = inputs.make_scene(cfg)
     cam = inputs.make_camera(cfg, view)
     gt = inputs.make_gt_map(cfg, view, cam)
-    pr = pu.oracle_view(scene, cam)
+    pr = pu.oracle_view(scene, cam, fo.params(primitive=1 if surfel else 0))
     m = fo.bins(pr, cfg.width, cfg.height)["M"]
-    gp = pu.GpuPath(scene, cfg.width, cfg.height, m + 64)
+    gp = pu.GpuPath(scene, cfg.width, cfg.height, m + 64, surfel=surfel)
     c, _ = gp.project_sort(cam)
     dev = gp.g.mean.device
     grad = torch.zeros((scene.n,), dtype=torch.float32, device=dev)
@@ -144,7 +149,7 @@ def _run_backward(cfg, view, lam1, lam2, k=20.0, lam=0.5):
     g_gpu = 0.5 * grad.cpu().numpy().astype(np.float64)
     order = fo.global_order(pr)
     L, g_or = fo.ndfd_backward(pr, order, scene.feat.astype(np.float32), gt.astype(np.float32), cfg.width, cfg.height,
-                               k=k, lam=lam, lam1=lam1, lam2=lam2)
+                               k=k, lam=lam, lam1=lam1, lam2=lam2, params=fo.params(primitive=1 if surfel else 0))
     # bar: every per-(pixel, fragment) term is O(1) and is summed over the Gaussian's footprint in fp32; the error is
     # bounded relative to the sum of |terms|, for which max|grad| over the scene is a (loose) stand-in on dense scenes
     scale = np.abs(g_or).max()

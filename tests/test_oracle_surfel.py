@@ -259,3 +259,43 @@ def test_literal_equals_scatter_and_invariants():
     pe = fo.project(sc.mean, sc.scale, sc.quat, sc.opacity, sc.sh, sc.sh_degree, cam35(cam), 64, 64)
     e = fo.render_literal(pe, fo.global_order(pe), None, 64, 64)
     assert np.abs(e["T"] - a["T"]).max() > 0.05
+
+
+def test_ndfd_on_surfels_forward_identities_and_backward_finite_differences():
+    """The NDFD oracle over surfels: O(N) recurrence == explicit pair sum in both accumulation orders, k = 0 closed form
+    against the surfel renderer, and dL/d opacity == central finite differences of the forward oracle."""
+    cfg, sc, cam, pr = _tiny_surfel(3)
+    order = fo.global_order(pr)
+    rng = np.random.default_rng(31)
+    feat = rng.standard_normal((sc.n, 12)).astype(np.float32)
+    feat /= np.linalg.norm(feat, axis=1, keepdims=True)
+    gt = rng.standard_normal((64, 64, 12)).astype(np.float32)
+    gt /= np.linalg.norm(gt, axis=2, keepdims=True)
+    pix = np.arange(0, 64 * 64, 7, dtype=np.int32)
+    for mode in (0, 1):
+        lgt, lcf, pw = fo.ndfd(pr, order, feat, gt, 64, 64, mode=mode, params=SURFEL, pix=pix, pairwise=True)
+        np.testing.assert_allclose(lcf, pw, rtol=1e-9, atol=1e-12)
+    r = fo.render_literal(pr, order, feat, 64, 64, SURFEL, pix=pix)
+    lgt0, lcf0 = fo.ndfd(pr, order, feat, gt, 64, 64, k=0.0, params=SURFEL, pix=pix)
+    Ws = 1.0 - r["T"]
+    np.testing.assert_allclose(lgt0, 0.5 * Ws, atol=1e-12)
+    np.testing.assert_allclose(lcf0, 0.25 * (Ws ** 2 - (r["feat"] ** 2).sum(axis=1)), atol=2e-7)   # features are unit-norm to fp32 rounding
+    prm = SURFEL.copy()
+    prm[5] = 0.0            # t_min = 0: the fragment lists do not change under the perturbation
+    lam1, lam2 = 0.7, 1.3
+    L, grad = fo.ndfd_backward(pr, order, feat, gt, 64, 64, lam1=lam1, lam2=lam2, params=prm)
+
+    def forward_total(p):
+        a, b = fo.ndfd(p, order, feat, gt, 64, 64, params=prm)
+        return lam1 * a.sum() + lam2 * b.sum()
+
+    assert abs(L - forward_total(pr)) <= 1e-9 * abs(L)
+    probe = np.argsort(-np.abs(grad))[[0, 1, 3, 10, 40]]
+    assert np.abs(grad[probe]).min() > 0
+    for g in probe:
+        o0 = pr["conic_opacity"][g, 3]
+        hi, lo = np.float32(o0 * (1 + 2e-3)), np.float32(o0 * (1 - 2e-3))
+        p_hi = dict(pr, conic_opacity=pr["conic_opacity"].copy()); p_hi["conic_opacity"][g, 3] = hi
+        p_lo = dict(pr, conic_opacity=pr["conic_opacity"].copy()); p_lo["conic_opacity"][g, 3] = lo
+        fd = (forward_total(p_hi) - forward_total(p_lo)) / (float(hi) - float(lo))
+        assert abs(fd - grad[g]) <= 2e-4 * max(abs(grad[g]), 1e-3), (g, fd, grad[g])
