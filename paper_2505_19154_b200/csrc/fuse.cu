@@ -201,7 +201,6 @@ __global__ void __launch_bounds__(TR_THREADS, 1) fuse_tiled_kernel(const FuseArg
 constexpr int FW_STAGES = 2;
 constexpr int FW_DC = 128;
 constexpr int FW_THREADS = WS_THREADS + 32;
-constexpr int FW_BAR_CONS = 3;
 constexpr int FW_WQ = (WS_CONS + 1) * 4;   // floats per quad row: 256 pixels x float4 + 16 B pad (bank spread over quads)
 enum { FW_FLAG_FIRST = 4 };
 
@@ -216,6 +215,7 @@ struct FuseWsSmem {
     WsCtrl<FW_STAGES, PRIM, PRIM ? 288 : WS_QCAP> ct;
     uint64_t g_full[2], g_free[2];
     uint64_t item_full[2], item_empty[2];
+    uint64_t p_full;                                      // the writing half's partial sums (and den atomics) of a batch are in place
     int items[2];
     __align__(16) uint32_t ids[FW_STAGES][WS_KB];
     __align__(16) float den_s[2][WS_KB];
@@ -456,8 +456,16 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT, PRIM>& sm, const
                 *reinterpret_cast<float4*>(&sm.P[(kg * 8 + 2 * i + 1) * FW_DC + ch]) = make_float4(v0.y, v1.y, v2.y, v3.y);
             }
         }
-        named_bar_sync(FW_BAR_CONS, WS_CONS);
-        if (!writer) {
+        // The halves are not barrier-coupled: the writing half signals p_full and goes on to the next batch, the reading
+        // half waits for it (phase = batch parity), so one half's epilogue overlaps the other half's next product.
+        // P needs no second buffer: a thread writes exactly the addresses it read one batch earlier, and it cannot get two
+        // batches ahead of the other half because as next batch's reader it waits for that half's signal; den_s[b & 1]
+        // is cleared by the reader of batch b before that reader signals batch b + 1.
+        if (writer) {
+            mbar_arrive(&sm.p_full);
+        } else {
+            mbar_wait(&sm.p_full, batch & 1u);
+            asm volatile("bar.sync %0, %1;" ::"r"(4 + half), "r"(128) : "memory");   // this half's own den atomics
             const float4 d0 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][kg * 8]);
             const float4 d1 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][kg * 8 + 4]);
             const float dv[8] = {d0.x, d0.y, d0.z, d0.w, d1.x, d1.y, d1.z, d1.w};
@@ -505,6 +513,7 @@ __global__ void __launch_bounds__(FW_THREADS, 1) fuse_ws_kernel(const FuseArgs a
             mbar_init(&sm.item_full[s], 1);
             mbar_init(&sm.item_empty[s], WS_PROD);
         }
+        mbar_init(&sm.p_full, WS_CONS / 2);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     // the GT tile buffer must never hold non-finite garbage (pixels outside the image keep stale data, weight 0)
