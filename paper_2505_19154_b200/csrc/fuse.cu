@@ -213,7 +213,8 @@ constexpr int kGBufs = sizeof(GT) == 2 ? 2 : 1;
 template <typename GT, int PRIM = 0>
 struct FuseWsSmem {
     WsCtrl<FW_STAGES, PRIM, PRIM ? 288 : WS_QCAP> ct;
-    uint64_t g_full[2], g_free[2];
+    uint64_t g_full[2][8], g_free[2];                      // g_full: one barrier per pixel half ([0], [4]) or, for a streamed-in
+                                                          // tile, per 32 pixels (2 tile rows) of a GT buffer
     uint64_t item_full[2], item_empty[2];
     uint64_t p_full;                                      // the writing half's partial sums (and den atomics) of a batch are in place
     int items[2];
@@ -263,22 +264,30 @@ __device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem<GT, PRIM>& sm, cons
         }
         const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
         const int nx = min(FHGS_TILE, a.t.W - tx0), ny = min(FHGS_TILE, a.t.H - ty0);
+        const bool split = kGBufs<GT> == 1 && a.D != FW_DC;   // see fuse_ws_consumer
         if (lane == 0) {
             mbar_wait_backoff(&sm.g_free[gb], gphase ^ 1u);
-            mbar_arrive_expect_tx(&sm.g_full[gb], (uint32_t)(nx * ny * FW_DC * sizeof(GT)));
+            if (split) {   // one barrier per pair of tile rows: the consumers start on the first rows while the rest is in flight
+#pragma unroll
+                for (int b = 0; b < 8; ++b)
+                    mbar_arrive_expect_tx(&sm.g_full[gb][b], (uint32_t)(nx * min(max(ny - 2 * b, 0), 2) * FW_DC * sizeof(GT)));
+            } else {       // one barrier per pixel half
+                mbar_arrive_expect_tx(&sm.g_full[gb][0], (uint32_t)(nx * min(ny, 8) * FW_DC * sizeof(GT)));
+                mbar_arrive_expect_tx(&sm.g_full[gb][4], (uint32_t)(nx * max(ny - 8, 0) * FW_DC * sizeof(GT)));
+            }
         }
         __syncwarp();
         GT* Gd = sm.G[gb];
         if (a.D == FW_DC) {   // a tile row is one contiguous span
             if (lane < ny)
                 bulk_g2s(&Gd[lane * FHGS_TILE * FW_DC], gt + ((size_t)(ty0 + lane) * a.t.W + tx0) * FW_DC,
-                         (uint32_t)(nx * FW_DC * sizeof(GT)), &sm.g_full[gb]);
+                         (uint32_t)(nx * FW_DC * sizeof(GT)), &sm.g_full[gb][(lane >> 3) * 4]);
         } else {
             for (int pix = lane; pix < FHGS_TILE_PX; pix += 32) {
                 const int x = pix & 15, y = pix >> 4;
                 if (x < nx && y < ny)
                     bulk_g2s(&Gd[pix * FW_DC], gt + ((size_t)(ty0 + y) * a.t.W + tx0 + x) * a.D + c0, (uint32_t)(FW_DC * sizeof(GT)),
-                             &sm.g_full[gb]);
+                             &sm.g_full[gb][split ? pix >> 5 : (pix >> 7) * 4]);
             }
         }
         if (++gb == kGBufs<GT>) { gb = 0; gphase ^= 1u; }
@@ -388,9 +397,15 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT, PRIM>& sm, const
         WS_TACC(0);
         const WsMeta m = sm.ct.meta[stage];
         if (m.flags & WS_FLAG_EXIT) break;
-        if (m.flags & FW_FLAG_FIRST) {   // next item: its GT tile is in the next buffer
+        // A single-buffered tile that arrives as 256 per-pixel copies (fp32 map, D > 128) is consumed block by block as it
+        // lands (Multi-view: fuse -3.5 %); where the tile is one copy per row or double-buffered the extra waits only cost
+        // (Mid +3 %), so everything is awaited up front there.
+        const bool first = (m.flags & FW_FLAG_FIRST) != 0;
+        const bool stream_in = first && kGBufs<GT> == 1 && a.D != FW_DC;
+        if (first) {   // next item: its GT tile is in the next buffer
             if (++gb == kGBufs<GT>) { gb = 0; gphase ^= 1u; }
-            mbar_wait(&sm.g_full[gb], gphase);
+            mbar_wait(&sm.g_full[gb][half * 4], gphase);
+            if (stream_in) mbar_wait(&sm.g_full[gb][half * 4 + 1], gphase);
             Gs = sm.G[gb] + half * 128 * FW_DC + ch;
             WS_TACC(1);
         }
@@ -415,6 +430,8 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT, PRIM>& sm, const
         float4 g = ld_g4(Gs);
 #pragma unroll 1
         for (int s0 = 0; s0 < (kg * 8 < m.nb ? 128 : 0); s0 += 32) {
+            // first batch of an item: the block after this one (its first pixel is prefetched at the end of this block)
+            if (stream_in && s0 >= 32 && s0 < 96) mbar_wait(&sm.g_full[gb][half * 4 + (s0 >> 5) + 1], gphase);
             const float* Wb = Ws + s0 * 4;
             const GT* Gb = Gs + s0 * FW_DC;
 #pragma unroll
@@ -506,7 +523,7 @@ __global__ void __launch_bounds__(FW_THREADS, 1) fuse_ws_kernel(const FuseArgs a
             mbar_init(&sm.ct.empty[s], WS_CONS);
         }
         for (int s = 0; s < 2; ++s) {
-            mbar_init(&sm.g_full[s], 1);
+            for (int b = 0; b < 8; ++b) mbar_init(&sm.g_full[s][b], 1);
             mbar_init(&sm.g_free[s], WS_CONS);
         }
         for (int s = 0; s < 2; ++s) {
