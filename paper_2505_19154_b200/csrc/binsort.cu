@@ -787,7 +787,11 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
     int* tile_diff = (int*)(sc + L.tile_diff);
     const size_t diff_bytes = (size_t)gw1 * gh1 * 4;
     if (grid_counts) FHGS_CUDA(ctx, cudaMemsetAsync(tile_diff, 0, diff_bytes, s));
+#ifdef FHGS_NO_SIDE
+    const bool side_overlap = false;
+#else
     const bool side_overlap = grid_counts && vs->n > 0;
+#endif
     const int first_bit = full_key ? 0 : 32;
     const int npass = ((32 + tile_bits) - first_bit + 7) / 8;
     vs->sorted_buf = npass & 1;
@@ -838,14 +842,14 @@ extern "C" fhgs_status fhgs_bin_sort(fhgs_ctx* ctx, const fhgs_camera* cam, fhgs
             cudaStream_t s0 = side_overlap ? ctx->side : s;
             scan_dup_kernel<<<scan_grid, SCAN_THREADS, 0, s0>>>(sa0);
             FHGS_LAUNCH_CHECK(ctx);
-            if (side_overlap) {
-                FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_offsets, ctx->side));
+            if (side_overlap) FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_offsets, ctx->side));
+            if (grid_counts) {   // ranges, digit offsets of the tile-id passes and the tile order from the per-tile counts
                 FHGS_CUDA(ctx, cudaFuncSetAttribute(tile_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)diff_bytes));
-                tile_scan_kernel<<<1, TS_THREADS, diff_bytes, ctx->side>>>(tile_diff, gw1, gh1, vs->num_instances, vs->capacity, vs->ranges,
-                                                                        hist, npass, (uint32_t*)(sc + L.tile_order), ctrl + CTRL_ORDER_VALID);
+                tile_scan_kernel<<<1, TS_THREADS, diff_bytes, s0>>>(tile_diff, gw1, gh1, vs->num_instances, vs->capacity, vs->ranges,
+                                                                 hist, npass, (uint32_t*)(sc + L.tile_order), ctrl + CTRL_ORDER_VALID);
                 FHGS_LAUNCH_CHECK(ctx);
-                FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_tiles, ctx->side));
             }
+            if (side_overlap) FHGS_CUDA(ctx, cudaEventRecord(ctx->ev_tiles, ctx->side));
         }
         if (full_key || vs->capacity == 0) {
             ScanDupArgs sa;

@@ -216,7 +216,8 @@ struct FuseWsSmem {
     uint64_t g_full[2][8], g_free[2];                      // g_full: one barrier per pixel half ([0], [4]) or, for a streamed-in
                                                           // tile, per 32 pixels (2 tile rows) of a GT buffer
     uint64_t item_full[2], item_empty[2];
-    uint64_t p_full;                                      // the writing half's partial sums (and den atomics) of a batch are in place
+    uint64_t p_full[2];                                   // the writing half's partial sums (and den atomics) of batch b are in place:
+                                                          // [b & 1], phase (b >> 1) & 1 (two barriers: a warp may run one batch ahead)
     int items[2];
     __align__(16) uint32_t ids[FW_STAGES][WS_KB];
     __align__(16) float den_s[2][WS_KB];
@@ -264,7 +265,11 @@ __device__ __forceinline__ void fuse_ws_scheduler(FuseWsSmem<GT, PRIM>& sm, cons
         }
         const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
         const int nx = min(FHGS_TILE, a.t.W - tx0), ny = min(FHGS_TILE, a.t.H - ty0);
+#ifdef FHGS_NO_STREAM_IN
+        const bool split = false;
+#else
         const bool split = kGBufs<GT> == 1 && a.D != FW_DC;   // see fuse_ws_consumer
+#endif
         if (lane == 0) {
             mbar_wait_backoff(&sm.g_free[gb], gphase ^ 1u);
             if (split) {   // one barrier per pair of tile rows: the consumers start on the first rows while the rest is in flight
@@ -401,7 +406,11 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT, PRIM>& sm, const
         // lands (Multi-view: fuse -3.5 %); where the tile is one copy per row or double-buffered the extra waits only cost
         // (Mid +3 %), so everything is awaited up front there.
         const bool first = (m.flags & FW_FLAG_FIRST) != 0;
+#ifdef FHGS_NO_STREAM_IN
+        const bool stream_in = false;
+#else
         const bool stream_in = first && kGBufs<GT> == 1 && a.D != FW_DC;
+#endif
         if (first) {   // next item: its GT tile is in the next buffer
             if (++gb == kGBufs<GT>) { gb = 0; gphase ^= 1u; }
             mbar_wait(&sm.g_full[gb][half * 4], gphase);
@@ -451,6 +460,12 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT, PRIM>& sm, const
                 wa = wa_n; wb = wb_n; g = g_n;
             }
         }
+        // a warp that had no instances in the first batch skipped the loop and its waits: every warp must have seen the whole
+        // tile before it goes on (the later batches of the item do not wait)
+        if (stream_in) {
+            mbar_wait(&sm.g_full[gb][half * 4 + 2], gphase);
+            mbar_wait(&sm.g_full[gb][half * 4 + 3], gphase);
+        }
         WS_TACC(2);
         // den partial: warp (half, cw) sums pixels [128 half + 32 cw, +32) for instance kk = lane
         {
@@ -460,11 +475,13 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT, PRIM>& sm, const
             for (int j = 0; j < 32; j += 2) { d0 += Wp[j * 4]; d1 += Wp[j * 4 + 4]; }
             atomicAdd(&sm.den_s[batch & 1][lane], d0 + d1);
         }
-        mbar_arrive(&sm.ct.empty[stage]);
-        if (m.flags & WS_FLAG_LAST) mbar_arrive(&sm.g_free[gb]);
-        if (++stage == FW_STAGES) { stage = 0; phase ^= 1u; }
-        WS_TACC(3);
         const bool writer = ((batch & 1u) != 0u) == (half != 0);
+        // The reading half releases the W stage at once; the writing half releases it after it has signalled p_full (below):
+        // no consumer warp can then be two batches ahead of another one's p_full arrival (the stage it needs is refilled
+        // only after every consumer released it), so an arrival never lands in an older phase of the barrier.
+        if (!writer) mbar_arrive(&sm.ct.empty[stage]);
+        if (m.flags & WS_FLAG_LAST) mbar_arrive(&sm.g_free[gb]);   // done with the GT tile: the scheduler may load the next one
+        WS_TACC(3);
         if (writer) {
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
@@ -479,9 +496,10 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT, PRIM>& sm, const
         // batches ahead of the other half because as next batch's reader it waits for that half's signal; den_s[b & 1]
         // is cleared by the reader of batch b before that reader signals batch b + 1.
         if (writer) {
-            mbar_arrive(&sm.p_full);
+            mbar_arrive(&sm.p_full[batch & 1u]);
+            mbar_arrive(&sm.ct.empty[stage]);
         } else {
-            mbar_wait(&sm.p_full, batch & 1u);
+            mbar_wait(&sm.p_full[batch & 1u], (batch >> 1) & 1u);
             asm volatile("bar.sync %0, %1;" ::"r"(4 + half), "r"(128) : "memory");   // this half's own den atomics
             const float4 d0 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][kg * 8]);
             const float4 d1 = *reinterpret_cast<const float4*>(&sm.den_s[batch & 1][kg * 8 + 4]);
@@ -505,6 +523,7 @@ __device__ __forceinline__ void fuse_ws_consumer(FuseWsSmem<GT, PRIM>& sm, const
             asm volatile("bar.sync %0, %1;" ::"r"(4 + half), "r"(128) : "memory");
             if (cw == 0) sm.den_s[batch & 1][lane] = 0.f;
         }
+        if (++stage == FW_STAGES) { stage = 0; phase ^= 1u; }
         WS_TACC(4);
         ++batch;
     }
@@ -530,7 +549,8 @@ __global__ void __launch_bounds__(FW_THREADS, 1) fuse_ws_kernel(const FuseArgs a
             mbar_init(&sm.item_full[s], 1);
             mbar_init(&sm.item_empty[s], WS_PROD);
         }
-        mbar_init(&sm.p_full, WS_CONS / 2);
+        mbar_init(&sm.p_full[0], WS_CONS / 2);
+        mbar_init(&sm.p_full[1], WS_CONS / 2);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     // the GT tile buffer must never hold non-finite garbage (pixels outside the image keep stale data, weight 0)

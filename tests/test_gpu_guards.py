@@ -186,3 +186,34 @@ def test_guards_surfel_kernels():
     print(run_guarded(pu.reduced_config("tiny", n=3000, feat_dim=24, width=83, height=45, log_scale_mu=-2.3), 0, pu.TOL_F32, surfel=True))
     print(run_guarded(pu.reduced_config("large", n=12_000, width=136, height=88, log_scale_mu=-2.8, feat_dim=128), 0, pu.TOL_F16,
                       sort_flags=(0,), surfel=True))
+
+
+def test_fuse_ws_back_to_back_stress():
+    """The fuse pipeline hands partial sums between its pixel halves through mbarriers and, for an fp32 map with D > 128,
+    consumes the GT tile while it streams in: 60 back-to-back accumulations of the same view without a host sync (D = 128
+    and D = 256, fp32) must complete (an mbarrier over-arrival traps) and reproduce the first one up to the atomic order."""
+    import torch
+    from paper_2505_19154_b200 import binding as fb
+    for d in (128, 256):
+        cfg = pu.reduced_config("multiview", n=60_000, width=432, height=328, n_views=200, log_scale_mu=-3.0, feat_dim=d)
+        scene = inputs.make_scene(cfg)
+        cam = inputs.make_camera(cfg, 25)
+        gp = pu.GpuPath(scene, cfg.width, cfg.height, 12_000_000)
+        c, m = gp.project_sort(cam)
+        dev = gp.g.mean.device
+        gt = torch.from_numpy(inputs.make_gt_map(cfg, 25, cam)).to(dev)
+        num = torch.zeros((scene.n, d), dtype=torch.float32, device=dev)
+        den = torch.zeros((scene.n,), dtype=torch.float32, device=dev)
+        fb.fuse_features(gp.ctx, c, gp.prm, gp.vs, gt, num, den, None, fb.FHGS_FUSE_ZERO)
+        torch.cuda.synchronize()
+        num0, den0 = num.clone(), den.clone()
+        assert float(den0.sum()) > 1000.0
+        reps = 60
+        for _ in range(reps):
+            fb.project(gp.ctx, gp.g, c, gp.prm, gp.vs)
+            fb.bin_sort(gp.ctx, c, gp.vs, sync=False)
+            fb.fuse_features(gp.ctx, c, gp.prm, gp.vs, gt, num, den, None, 0)
+        torch.cuda.synchronize()
+        k = reps + 1
+        assert float((den - k * den0).abs().max()) <= 2e-5 * k * float(den0.max())
+        assert float((num - k * num0).abs().max()) <= 2e-5 * k * float(num0.abs().max())
