@@ -15,7 +15,7 @@
 // dL/dalpha_k G_k into grad_opacity: reduced over the pixels of the warp first, then one atomic per (warp, Gaussian).
 #include <cuda_fp16.h>
 
-#include "traverse.cuh"
+#include "ws.cuh"   // packed fma.rn.f32x2 helpers (and traverse.cuh)
 
 namespace {
 
@@ -58,6 +58,12 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait_group() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
+// sum of the four partial sums of a dot product kept in two packed chains
+__device__ __forceinline__ float hsum(const unsigned long long (&p)[2]) {
+    const float2 a = unpack2(p[0]), b = unpack2(p[1]);
+    return (a.x + a.y) + (b.x + b.y);
+}
+
 // survivors whose feature rows are staged together (one of two 32 KB shared-memory buffers), as in ndfd.cu
 template <int D, typename FT>
 struct BwdSub {
@@ -87,7 +93,8 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
     const int c_lo = cgl * 4;   // interleaved float4 groups cgl, cgl + LPP, ...
     const size_t pix = (size_t)py * a.t.W + px;
 
-    float g[CPL], F[CPL], Bs[CPL];   // f_gt slice; prefix sum w f; MODE 1: running sum sigma w f, else suffix B_k
+    // f_gt slice; prefix sum w f; MODE 1: running sum sigma w f, else suffix B_k -- channel pairs packed for fma.rn.f32x2
+    unsigned long long g[CPL / 2], F[CPL / 2], Bs[CPL / 2];
 #pragma unroll
     for (int j = 0; j < CPL / 4; ++j) {
         float4 v = make_float4(0.f, 0.f, 0.f, 0.f), b = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -95,9 +102,9 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
             v = ldg4<GT>(gt + pix * a.D + c_lo + 4 * LPP * j);
             if (MODE != 1) b = *reinterpret_cast<const float4*>(a.B_tot + pix * a.D + c_lo + 4 * LPP * j);
         }
-        g[4 * j] = v.x; g[4 * j + 1] = v.y; g[4 * j + 2] = v.z; g[4 * j + 3] = v.w;
-        Bs[4 * j] = b.x; Bs[4 * j + 1] = b.y; Bs[4 * j + 2] = b.z; Bs[4 * j + 3] = b.w;
-        F[4 * j] = F[4 * j + 1] = F[4 * j + 2] = F[4 * j + 3] = 0.f;
+        g[2 * j] = pack2(v.x, v.y); g[2 * j + 1] = pack2(v.z, v.w);
+        Bs[2 * j] = pack2(b.x, b.y); Bs[2 * j + 1] = pack2(b.z, b.w);
+        F[2 * j] = F[2 * j + 1] = 0ull;
     }
     float T = 1.f, Wc = 0.f;
     float As = (MODE != 1 && inside) ? a.A_tot[pix] : 0.f;      // MODE 1: running sum; else suffix A_k
@@ -179,48 +186,50 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
                 const float w = hit ? alpha * Tb : 0.f;
                 const uint32_t id = q.id[kk];
                 const FT* f = rows + (kk - sb * SB) * (CPL * LPP);
-                float fv[CPL];
+                unsigned long long fv[CPL / 2];
 #pragma unroll
                 for (int j = 0; j < CPL / 4; ++j) {
                     const float4 v = lds4<FT>(f + 4 * LPP * j);
-                    fv[4 * j] = v.x; fv[4 * j + 1] = v.y; fv[4 * j + 2] = v.z; fv[4 * j + 3] = v.w;
+                    fv[2 * j] = pack2(v.x, v.y); fv[2 * j + 1] = pack2(v.z, v.w);
                 }
-                float ph[4] = {0.f, 0.f, 0.f, 0.f};
+                unsigned long long ph[2] = {0ull, 0ull};   // 2 packed chains per dot product
 #pragma unroll
-                for (int j = 0; j < CPL; ++j) ph[j & 3] = fmaf(fv[j], g[j], ph[j & 3]);
-                float phi = (ph[0] + ph[1]) + (ph[2] + ph[3]);
+                for (int j = 0; j < CPL / 2; ++j) fma2_acc(ph[j & 1], fv[j], g[j]);
+                float phi = hsum(ph);
 #pragma unroll
                 for (int d = 1; d < LPP; d <<= 1) phi += __shfl_xor_sync(TR_FULL, phi, d);
                 const float sigma = 1.0f / (1.0f + exp2f(k2 * (phi - a.lambda)));
                 const float sw = sigma * w;
                 if (MODE == 1) {
                     // totals A_0, B_0 and the forward losses (prefix recurrence), from which C_0 follows (see the header)
-                    float fa1[4] = {0.f, 0.f, 0.f, 0.f};
+                    unsigned long long fa1[2] = {0ull, 0ull};
 #pragma unroll
-                    for (int j = 0; j < CPL; ++j) fa1[j & 3] = fmaf(fv[j], F[j], fa1[j & 3]);
-                    float Ff1 = (fa1[0] + fa1[1]) + (fa1[2] + fa1[3]);
+                    for (int j = 0; j < CPL / 2; ++j) fma2_acc(fa1[j & 1], fv[j], F[j]);
+                    float Ff1 = hsum(fa1);
 #pragma unroll
                     for (int d = 1; d < LPP; d <<= 1) Ff1 += __shfl_xor_sync(TR_FULL, Ff1, d);
                     As += sw;
                     Cs += a.lam1 * sw + 2.0f * a.lam2 * sw * (Wc - Ff1);
                     Wc += w;
+                    const unsigned long long sw2 = pack2(sw, sw), w2 = pack2(w, w);
 #pragma unroll
-                    for (int j = 0; j < CPL; ++j) {
-                        Bs[j] = fmaf(sw, fv[j], Bs[j]);
-                        F[j] = fmaf(w, fv[j], F[j]);
+                    for (int j = 0; j < CPL / 2; ++j) {
+                        fma2_acc(Bs[j], sw2, fv[j]);
+                        fma2_acc(F[j], w2, fv[j]);
                     }
                     continue;
                 }
                 // suffixes exclude k
                 As -= sw;
-                float fa[4] = {0.f, 0.f, 0.f, 0.f}, ba[4] = {0.f, 0.f, 0.f, 0.f};
+                unsigned long long fa[2] = {0ull, 0ull}, ba[2] = {0ull, 0ull};
+                const unsigned long long nsw2 = pack2(-sw, -sw);
 #pragma unroll
-                for (int j = 0; j < CPL; ++j) {
-                    Bs[j] = fmaf(-sw, fv[j], Bs[j]);
-                    fa[j & 3] = fmaf(fv[j], F[j], fa[j & 3]);
-                    ba[j & 3] = fmaf(fv[j], Bs[j], ba[j & 3]);
+                for (int j = 0; j < CPL / 2; ++j) {
+                    fma2_acc(Bs[j], nsw2, fv[j]);
+                    fma2_acc(fa[j & 1], fv[j], F[j]);
+                    fma2_acc(ba[j & 1], fv[j], Bs[j]);
                 }
-                float Ff = (fa[0] + fa[1]) + (fa[2] + fa[3]), Bf = (ba[0] + ba[1]) + (ba[2] + ba[3]);
+                float Ff = hsum(fa), Bf = hsum(ba);
 #pragma unroll
                 for (int d = 1; d < LPP; d <<= 1) {
                     Ff += __shfl_xor_sync(TR_FULL, Ff, d);
@@ -228,8 +237,11 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
                 }
                 const float gk = a.lam1 * sigma + a.lam2 * (sigma * (Wc - Ff) + (As - Bf));
                 Wc += w;
+                {
+                    const unsigned long long w2 = pack2(w, w);
 #pragma unroll
-                for (int j = 0; j < CPL; ++j) F[j] = fmaf(w, fv[j], F[j]);
+                    for (int j = 0; j < CPL / 2; ++j) fma2_acc(F[j], w2, fv[j]);
+                }
                 {
                     Cs = fmaf(-gk, w, Cs);   // suffix excludes k
                     float contrib = hit ? (Tb * gk - Cs / (1.0f - alpha)) * Ge : 0.f;
@@ -248,9 +260,10 @@ __global__ void __launch_bounds__(TR_THREADS, CPL <= 16 ? 3 : 2) ndfd_bwd_kernel
         if (MODE == 1) {
             if (cgl == 0) { a.A_tot[pix] = As; a.C_tot[pix] = Cs; }
 #pragma unroll
-            for (int j = 0; j < CPL / 4; ++j)
-                *reinterpret_cast<float4*>(a.B_tot + pix * a.D + c_lo + 4 * LPP * j) =
-                    make_float4(Bs[4 * j], Bs[4 * j + 1], Bs[4 * j + 2], Bs[4 * j + 3]);
+            for (int j = 0; j < CPL / 4; ++j) {
+                const float2 b0 = unpack2(Bs[2 * j]), b1 = unpack2(Bs[2 * j + 1]);
+                *reinterpret_cast<float4*>(a.B_tot + pix * a.D + c_lo + 4 * LPP * j) = make_float4(b0.x, b0.y, b1.x, b1.y);
+            }
         }
     }
 }
