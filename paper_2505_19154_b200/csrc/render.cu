@@ -94,11 +94,13 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT, PRIM>& s
     int sx, sy;
     slot_to_xy(p, sx, sy);
     int item = ws_pop_end(sm.ct, ws_pop_begin(wk, p), p);
+    WS_TDECL;
     while (true) {
         if (item >= wk.n_items) {
             mbar_wait(&sm.ct.empty[stage], phase ^ 1u);
             if (p == 0) sm.ct.meta[stage] = WsMeta{0, -1, 0, WS_FLAG_EXIT};
             mbar_arrive(&sm.ct.full[stage]);
+            WS_TFLUSH(16, p == 0);
             break;
         }
         const uint32_t popped = ws_pop_begin(wk, p);   // next item, consumed at the end of this one
@@ -128,7 +130,9 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT, PRIM>& s
                 ws_chunk_prefetch_id(a.t, pos + WS_PROD, range.y, p, ch);
             }
             const int nb = min(WS_KB, qt - qh);
+            WS_TACC(1);
             mbar_wait_backoff(&sm.ct.empty[stage], phase ^ 1u);
+            WS_TACC(2);
             // feature rows of the batch: one bulk async copy each, counted on full[stage]
             if (pw == 0 && lane < nb) {
                 const uint32_t id = __float_as_uint(sm.ct.rec1[(qh + lane) & (WS_QCAP - 1)].z);
@@ -155,6 +159,7 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT, PRIM>& s
             }
             if (lane == 0) sm.ct.mask[stage][pw] = m;
             qh += nb;
+            WS_TACC(3);
             const bool all_done = named_bar_and(WS_BAR_PROD_RED, WS_PROD, P.done);
             last = all_done || (pos >= range.y && qt == qh);
             if (p == 0) sm.ct.meta[stage] = WsMeta{nb, tile, c0, last ? WS_FLAG_LAST : 0};
@@ -171,6 +176,7 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT, PRIM>& s
                 }
                 a.tile_visited[tile] = visited;
             }
+            WS_TACC(4);
             if (++stage == R_STAGES) { stage = 0; phase ^= 1u; }
         } while (!last);
         if (c0 == 0 && inside) {
@@ -182,6 +188,7 @@ __device__ __forceinline__ void render_ws_producer(RenderWsSmem<DC, FT, PRIM>& s
             if (a.out_n) a.out_n[o] = P.n;
         }
         item = ws_pop_end(sm.ct, popped, p);
+        WS_TACC(0);
     }
 }
 
@@ -195,6 +202,7 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT, PRIM>& s
     FT* out_feat = reinterpret_cast<FT*>(a.out_feat);
     int stage = 0;
     uint32_t phase = 0;
+    WS_TDECL;
     while (true) {   // one iteration per work item: accumulators live exactly one item
         unsigned long long acc[NJ * 2][8];   // [channel pair][pixel], packed (fma.rn.f32x2); this index order leaves ptxas the fewest
                                            // accumulator copies in the loop below (8 instead of 21 per 64 FFMA2)
@@ -205,8 +213,10 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT, PRIM>& s
         WsMeta m;
         while (true) {   // batches of the item
             mbar_wait(&sm.ct.full[stage], phase);
+            WS_TACC(0);
             m = sm.ct.meta[stage];
-            if (m.flags & WS_FLAG_EXIT) return;
+            if (m.flags & WS_FLAG_EXIT) { WS_TFLUSH(0, tid == 0); return; }
+            WS_TCNT(5);
             uint32_t mk = sm.ct.mask[stage][warp];
             const float* Ws = sm.W[stage] + pg * 8;
             const FT* Fs = sm.F[stage] + cg * 4;
@@ -232,6 +242,7 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT, PRIM>& s
                     for (int i = 0; i < 8; ++i) fma2_acc(acc[j][i], w2[i], fv[j]);
             }
             mbar_arrive(&sm.ct.empty[stage]);
+            WS_TACC(1);
             if (++stage == R_STAGES) { stage = 0; phase ^= 1u; }
             if (m.flags & WS_FLAG_LAST) break;
         }
@@ -250,6 +261,8 @@ __device__ __forceinline__ void render_ws_consumer(RenderWsSmem<DC, FT, PRIM>& s
                 }
             }
         }
+        WS_TACC(2);
+        WS_TCNT(6);
     }
 }
 
@@ -438,6 +451,17 @@ cudaError_t dispatch(const RenderArgs& a, int grid, int num_sms, uint32_t* queue
 }
 
 }  // namespace
+
+#ifdef FHGS_WS_TIMING
+extern "C" __attribute__((visibility("default"))) int fhgs_debug_render_timing(unsigned long long* out32, int reset) {
+    if (out32 && cudaMemcpyFromSymbol(out32, g_ws_timing, sizeof(g_ws_timing)) != cudaSuccess) return 1;
+    if (reset) {
+        unsigned long long z[32] = {0};
+        if (cudaMemcpyToSymbol(g_ws_timing, z, sizeof(z)) != cudaSuccess) return 1;
+    }
+    return 0;
+}
+#endif
 
 extern "C" fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam,
                                    const fhgs_params* prm, const fhgs_view_state* vs, float* out_rgb,
