@@ -298,6 +298,22 @@ FHGS_API fhgs_status fhgs_frame_host(fhgs_ctx* ctx, const fhgs_host_frame* host,
                             const fhgs_frame_workspace* ws, uint64_t* num_instances_host,
                             void* stream);
 
+/* Allocation-free variant of step S1's prefix sum (DuplicateWithKeys needs, per Gaussian, the
+ * inclusive prefix sum of tiles_touched) for callers that cannot provide or allocate scratch memory
+ * (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  The decoupled look-back status words live in a
+ * file-scope device array of the library (32 KB + 256 B, held by every GPU that loads the library until the process
+ * exits) instead of fhgs_view_state::scratch; the call makes no cudaMalloc / cudaFree and no allocating library call.
+ *   tiles_touched  DEVICE [n] uint32 (as written by fhgs_project);  offsets  DEVICE [n] uint32, offsets[i] =
+ *   sum_{j<=i} tiles_touched[j] (mod 2^32, like fhgs_bin_sort's);  num_instances  DEVICE [1] uint64 or NULL, the total M.
+ * n must be <= fhgs_scan_offsets_static_max_n() = 4 194 304, else FHGS_ERR_INVALID with nothing enqueued (use
+ * fhgs_bin_sort with caller scratch beyond that).  n == 0 writes only *num_instances = 0.  The result is bit-identical to
+ * the offsets / num_instances fhgs_bin_sort writes.  Every call shares the one array and clears the words it uses first:
+ * calls on one device must be stream-ordered -- two calls that overlap on the GPU race on it.  Enqueues two kernels on
+ * `stream` and returns. */
+FHGS_API int32_t fhgs_scan_offsets_static_max_n(void);
+FHGS_API fhgs_status fhgs_scan_offsets_static(fhgs_ctx* ctx, const uint32_t* tiles_touched, int32_t n, uint32_t* offsets,
+                                     uint64_t* num_instances, void* stream);
+
 /* Register-resident FFMA micro-benchmark ("the builder must first run a
  * register-resident FFMA micro-benchmark"): returns the measured FP32 rate in lane-ops/s
  * (one FMA = one lane-op) in *lane_ops_per_s and the kernel time in *ms.  Synchronises. */

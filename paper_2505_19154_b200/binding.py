@@ -25,7 +25,7 @@ FHGS_NDFD_BLEND_ORDER, FHGS_NDFD_FAR_TO_NEAR = 0, 1
 
 EXPORTS = ["fhgs_create", "fhgs_destroy", "fhgs_last_error", "fhgs_version", "fhgs_default_params",
            "fhgs_scratch_bytes", "fhgs_scratch_tile_visited", "fhgs_set_diagnostics", "fhgs_project", "fhgs_bin_sort", "fhgs_render", "fhgs_fuse_features", "fhgs_ndfd_forward", "fhgs_ndfd_backward_work_bytes", "fhgs_ndfd_backward",
-           "fhgs_frame_host", "fhgs_ffma_peak"]
+           "fhgs_frame_host", "fhgs_ffma_peak", "fhgs_scan_offsets_static_max_n", "fhgs_scan_offsets_static"]
 
 
 class FhgsError(RuntimeError):
@@ -110,6 +110,9 @@ def _load():
     lib.fhgs_ndfd_backward.argtypes = [vp, C.POINTER(CGaussians), C.POINTER(CCamera), C.POINTER(CParams), C.POINTER(CViewState),
                                        vp, C.c_int32, C.c_float, C.c_float, C.c_float, C.c_float, vp, vp, C.c_size_t, vp]
     lib.fhgs_ffma_peak.argtypes = [vp, C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]
+    lib.fhgs_scan_offsets_static_max_n.restype = C.c_int32
+    lib.fhgs_scan_offsets_static_max_n.argtypes = []
+    lib.fhgs_scan_offsets_static.argtypes = [vp, vp, C.c_int32, vp, vp, vp]
     return lib
 
 
@@ -305,6 +308,14 @@ def bin_sort(ctx: Context, cam: CCamera, vs: ViewState, sync: bool = False, flag
                            C.c_uint32(flags), _stream(stream))
     ctx.check(st)
     return int(m.value) if sync else None
+
+
+def scan_offsets_static(ctx: Context, tiles_touched, offsets, num_instances=None, n=None, stream=None):
+    """fhgs_scan_offsets_static: the allocation-free prefix sum of step S1 (library-owned static scratch).
+    tiles_touched / offsets: uint32-sized device tensors [n]; num_instances: optional 8-byte device tensor [1]."""
+    n = int(tiles_touched.numel()) if n is None else int(n)
+    ctx.check(lib.fhgs_scan_offsets_static(ctx.handle, _ptr(tiles_touched), n, _ptr(offsets), _ptr(num_instances),
+                                           _stream(stream)))
 
 
 def render(ctx: Context, g: Gaussians, cam: CCamera, prm: CParams, vs: ViewState, out_rgb, out_feat=None,

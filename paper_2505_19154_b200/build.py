@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(HERE, "libfhgs.so")
 OBJ_DIR = os.path.join(HERE, "build")
-SOURCES = ["api.cu", "project.cu", "binsort.cu", "render.cu", "fuse.cu", "ndfd.cu", "ndfd_bwd.cu"]
+SOURCES = ["api.cu", "project.cu", "binsort.cu", "render.cu", "fuse.cu", "ndfd.cu", "ndfd_bwd.cu", "noalloc.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "-I", INCLUDE, "-I", CSRC]
 
