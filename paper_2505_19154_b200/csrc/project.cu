@@ -4,13 +4,15 @@
 // Arithmetic rule of this step: every +,-,*,/,sqrt is ONE IEEE binary32 operation, round to
 // nearest even, in the written order, never contracted into an FMA.  This file therefore uses
 // the __f*_rn intrinsics throughout, which ptxas never fuses, so the result does not depend on
-// compiler flags.  The step is HBM-bound (236 B read + 56 B written per visible Gaussian at SH
-// degree 3), so the un-fused arithmetic costs nothing.
+// compiler flags.  236 B read + 56 B written per visible Gaussian at SH degree 3; ~820 instructions per warp
+// (18 IEEE divisions, 4 square roots), so the kernel is bound by issue slots and load latency together.
 //
-// Layout: one thread per Gaussian.  The SH block of a CTA (256 Gaussians x K x 3 floats, one
-// contiguous span of global memory) is staged through shared memory with coalesced 16-byte
-// loads; every thread then reads its own row with a conflict-free padded stride.
+// Layout: one thread per Gaussian.  SH degree 3: every Gaussian that can be visible fetches its own 192-byte SH row with
+// one bulk async copy while its covariance is computed (project_kernel<3, true>).  Degree 0-2 and the surfel kernel: the SH
+// block of a CTA (256 Gaussians x K x 3 floats, one contiguous span of global memory) is staged through shared memory
+// with coalesced 16-byte loads; every thread then reads its own row with a conflict-free padded stride.
 #include "common.cuh"
+#include "ws.cuh"   // mbarrier / bulk-copy wrappers
 
 namespace {
 
@@ -113,18 +115,62 @@ __device__ __forceinline__ void sh_colour(const ProjectArgs& a, const float* row
     }
 }
 
-template <int DEG>
-__global__ void __launch_bounds__(PROJ_THREADS) project_kernel(const ProjectArgs a) {
+// DIRECT (rows of a multiple of 16 bytes, i.e. SH degree 1 and 3, and a 16-byte aligned sh array): no cooperative
+// staging and no CTA-wide barrier.  A thread whose Gaussian passes the z cull and a generous frame test starts ONE bulk
+// async copy (cp.async.bulk) of its own row into its own shared-memory slot (stride 208 bytes: conflict-free for the
+// 16-byte reads), counted on its warp's mbarrier; the warp does the covariance arithmetic while the rows fly and waits
+// for them only before the colour.  Rows of culled Gaussians are not fetched, and the warps of a CTA run their load and
+// arithmetic phases out of step with each other.
+template <int DEG, bool DIRECT>
+__global__ void __launch_bounds__(PROJ_THREADS, DIRECT ? 4 : 1) project_kernel(const ProjectArgs a) {
     constexpr int K = (DEG + 1) * (DEG + 1);
     constexpr int ROW = 3 * K;                 // floats per Gaussian
     constexpr int PAD = (ROW % 2 == 0) ? ROW + 1 : ROW;  // odd stride -> conflict-free rows
-    extern __shared__ float s_sh[];            // [PROJ_THREADS][PAD]
+    constexpr int DSTRIDE = ROW + 4;           // DIRECT: floats between the row slots of two threads (208 B at degree 3)
+    bool staged_row = false;
+    uint32_t warp_rows = 0;   // DIRECT: lanes of this warp with a row copy in flight
+    extern __shared__ __align__(16) float s_sh[];   // [PROJ_THREADS][PAD], or [PROJ_THREADS][DSTRIDE] in the DIRECT form
 
+    __shared__ uint64_t s_bar[PROJ_THREADS / 32];
     const int base = blockIdx.x * PROJ_THREADS;
     const int i = base + threadIdx.x;
-    const int cnt = min(PROJ_THREADS, a.n - base);
-    stage_sh_rows<DEG>(a, s_sh, base, cnt);
-    __syncthreads();
+    if (!DIRECT) {
+        const int cnt = min(PROJ_THREADS, a.n - base);
+        stage_sh_rows<DEG>(a, s_sh, base, cnt);
+        __syncthreads();
+    } else {
+        // per-warp barrier, one phase: lane 0 arrives once with the byte count of the warp's rows
+        if ((threadIdx.x & 31) == 0) {
+            mbar_init(&s_bar[threadIdx.x >> 5], 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        }
+        __syncwarp();
+        // the frame test (a hint: it decides no result) is taken by the whole warp before any lane leaves
+        bool want = false;
+        if (i < a.n) {
+            const float p0 = __ldg(a.mean + 3 * (size_t)i), p1 = __ldg(a.mean + 3 * (size_t)i + 1),
+                        p2 = __ldg(a.mean + 3 * (size_t)i + 2);
+            const float* V = a.V;
+            const float tx = V[0] * p0 + V[1] * p1 + V[2] * p2 + V[3], ty = V[4] * p0 + V[5] * p1 + V[6] * p2 + V[7],
+                        tz = V[8] * p0 + V[9] * p1 + V[10] * p2 + V[11];
+            const float hx = a.fx * tx + (a.cx - 0.5f * (float)a.W) * tz, hy = a.fy * ty + (a.cy - 0.5f * (float)a.H) * tz;
+            // centre within 15 % of the image size of the frame: |px - W/2| <= 0.65 W, written without the division
+            want = tz >= a.z_near && fabsf(hx) <= 0.65f * (float)a.W * tz && fabsf(hy) <= 0.65f * (float)a.H * tz;
+        }
+        const uint32_t ballot = __ballot_sync(0xffffffffu, want);
+        if (ballot) {
+            uint64_t* bar = &s_bar[threadIdx.x >> 5];
+            if ((threadIdx.x & 31) == 0) {
+                mbar_expect_tx(bar, (uint32_t)(__popc(ballot) * ROW * 4));
+                mbar_arrive(bar);
+            }
+            __syncwarp();
+            if (want) bulk_g2s(s_sh + threadIdx.x * DSTRIDE, a.sh + (size_t)i * ROW, ROW * 4, bar);
+        }
+        staged_row = want;
+        warp_rows = ballot;
+    }
     if (i >= a.n) return;
 
     float o_xy0 = 0.f, o_xy1 = 0.f, o_depth = 0.f;
@@ -137,6 +183,12 @@ __global__ void __launch_bounds__(PROJ_THREADS) project_kernel(const ProjectArgs
     do {
         const float p0 = __ldg(a.mean + 3 * (size_t)i), p1 = __ldg(a.mean + 3 * (size_t)i + 1),
                     p2 = __ldg(a.mean + 3 * (size_t)i + 2);
+        // every per-Gaussian input is requested up front (one DRAM round trip instead of three dependent ones; a culled
+        // Gaussian wastes 32 bytes)
+        const float4 qv = __ldg(reinterpret_cast<const float4*>(a.quat) + i);
+        const float s0 = __ldg(a.scale + 3 * (size_t)i), s1 = __ldg(a.scale + 3 * (size_t)i + 1),
+                    s2 = __ldg(a.scale + 3 * (size_t)i + 2);
+        const float op = __ldg(a.opacity + i);
         const float* V = a.V;
         // 1. camera-space position
         float t[3];
@@ -152,7 +204,6 @@ __global__ void __launch_bounds__(PROJ_THREADS) project_kernel(const ProjectArgs
         const float uc = fminf(fmaxf(u, -a.Lx), a.Lx), vc = fminf(fmaxf(v, -a.Ly), a.Ly);
         const float X = mul(uc, z), Y = mul(vc, z);
         // 4. rotation from the (normalised) quaternion
-        const float4 qv = __ldg(reinterpret_cast<const float4*>(a.quat) + i);
         float qw = qv.x, qx = qv.y, qy = qv.z, qz = qv.w;
         const float qn = sq(add(add(add(mul(qw, qw), mul(qx, qx)), mul(qy, qy)), mul(qz, qz)));
         qw = dvd(qw, qn); qx = dvd(qx, qn); qy = dvd(qy, qn); qz = dvd(qz, qn);
@@ -167,8 +218,6 @@ __global__ void __launch_bounds__(PROJ_THREADS) project_kernel(const ProjectArgs
         R[7] = mul(2.0f, add(mul(qy, qz), mul(qw, qx)));
         R[8] = sub(1.0f, mul(2.0f, add(mul(qx, qx), mul(qy, qy))));
         // 5. Sigma3D = (R S)(R S)^T
-        const float s0 = __ldg(a.scale + 3 * (size_t)i), s1 = __ldg(a.scale + 3 * (size_t)i + 1),
-                    s2 = __ldg(a.scale + 3 * (size_t)i + 2);
         float M[9];
 #pragma unroll
         for (int k = 0; k < 3; ++k) {
@@ -225,14 +274,23 @@ __global__ void __launch_bounds__(PROJ_THREADS) project_kernel(const ProjectArgs
         const int ix0 = (int)x0, ix1 = (int)x1, iy0 = (int)y0, iy1 = (int)y1;
         if (ix1 <= ix0 || iy1 <= iy0) break;
         // 10. SH colour
-        sh_colour<DEG>(a, s_sh + threadIdx.x * PAD, p0, p1, p2, o_rgb);
+        if (DIRECT && staged_row) {
+            mbar_wait(&s_bar[threadIdx.x >> 5], 0);   // the rows of this warp have landed
+            sh_colour<DEG>(a, s_sh + threadIdx.x * DSTRIDE, p0, p1, p2, o_rgb);
+        } else if (DIRECT) {
+            sh_colour<DEG>(a, a.sh + (size_t)i * ROW, p0, p1, p2, o_rgb);   // rare: scalar loads from global memory
+        } else {
+            sh_colour<DEG>(a, s_sh + threadIdx.x * PAD, p0, p1, p2, o_rgb);
+        }
         o_xy0 = px; o_xy1 = py; o_depth = z;
-        o_co = make_float4(conA, conB, conC, __ldg(a.opacity + i));
+        o_co = make_float4(conA, conB, conC, op);
         o_radius = (int)r;
         o_rect = make_ushort4((unsigned short)ix0, (unsigned short)iy0, (unsigned short)ix1, (unsigned short)iy1);
         o_tt = (uint32_t)((ix1 - ix0) * (iy1 - iy0));
     } while (0);
 
+    // no lane leaves while a copy into this CTA's shared memory may still be in flight
+    if (DIRECT && warp_rows) mbar_wait(&s_bar[threadIdx.x >> 5], 0);
     reinterpret_cast<float2*>(a.xy)[i] = make_float2(o_xy0, o_xy1);
     a.depth[i] = o_depth;
     reinterpret_cast<float4*>(a.conic_opacity)[i] = o_co;
@@ -371,15 +429,23 @@ cudaError_t launch_project(const ProjectArgs& a, cudaStream_t st) {
     constexpr int ROW = 3 * K;
     constexpr int PAD = (ROW % 2 == 0) ? ROW + 1 : ROW;
     const size_t smem = (size_t)PROJ_THREADS * PAD * sizeof(float);
-    cudaError_t e = cudaFuncSetAttribute(project_kernel<DEG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
     const int grid = (a.n + PROJ_THREADS - 1) / PROJ_THREADS;
+    // degree 3 (192-byte rows): the per-row bulk-copy form; the shorter rows of degree 0-2 measured faster staged
+    if (!a.ray_transform && DEG == 3 && aligned_to(a.sh, 16)) {
+        const size_t dsmem = (size_t)PROJ_THREADS * (ROW + 4) * sizeof(float);
+        cudaError_t e = cudaFuncSetAttribute(project_kernel<DEG, (DEG == 3)>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dsmem);
+        if (e != cudaSuccess) return e;
+        project_kernel<DEG, (DEG == 3)><<<grid, PROJ_THREADS, dsmem, st>>>(a);
+        return cudaGetLastError();
+    }
+    cudaError_t e = cudaFuncSetAttribute(project_kernel<DEG, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
     if (a.ray_transform) {
         e = cudaFuncSetAttribute(project_surfel_kernel<DEG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
         project_surfel_kernel<DEG><<<grid, PROJ_THREADS, smem, st>>>(a);
     } else {
-        project_kernel<DEG><<<grid, PROJ_THREADS, smem, st>>>(a);
+        project_kernel<DEG, false><<<grid, PROJ_THREADS, smem, st>>>(a);
     }
     return cudaGetLastError();
 }
