@@ -220,6 +220,47 @@ def test_randomized_shapes_sweep():
         print(it, base, kw, view, w)
 
 
+def test_project_sh_row_paths_agree():
+    """Step P at SH degree 3 has two ways to fetch a Gaussian's SH row: one bulk async copy per row (16-byte aligned sh
+    array) and the CTA-staged form (any alignment).  Both must give the oracle's projection, bit for bit on everything but
+    the colour, and the same colour bits as each other -- also when most of the frame test's guesses are wrong (a camera
+    that sees only part of the scene, so many staged rows belong to Gaussians that are culled later and vice versa)."""
+    import torch
+    from paper_2505_19154_b200 import binding as fb
+    cfg = inputs.scaled(inputs.CONFIGS["mid"], n=70001, width=208, height=112, log_scale_mu=-2.5, n_views=4)
+    scene = inputs.make_scene(cfg)
+    assert scene.sh_degree == 3
+    ctx = fb.Context(0)
+    prm = fb.default_params()
+    g = fb.Gaussians(scene.mean, scene.scale, scene.quat, scene.opacity, scene.sh, None, scene.sh_degree)
+    # the same coefficients at an address that is 4 (mod 16): the staged form
+    raw = torch.empty(g.sh.numel() + 4, dtype=torch.float32, device="cuda")
+    base = 1 if raw.data_ptr() % 16 == 0 else 0
+    while (raw.data_ptr() + 4 * base) % 16 == 0:
+        base += 1
+    sh_off = raw[base:base + g.sh.numel()].view_as(g.sh)
+    sh_off.copy_(g.sh)
+    g2 = fb.Gaussians(scene.mean, scene.scale, scene.quat, scene.opacity, scene.sh, None, scene.sh_degree)
+    g2.sh = sh_off
+    g2.refresh()
+    assert g.sh.data_ptr() % 16 == 0 and g2.sh.data_ptr() % 16 != 0
+    for view in (0, 1):
+        cam = inputs.make_camera(cfg, view)
+        c = fb.make_camera(cam.view, cam.proj, cam.cam_pos, cam.width, cam.height)
+        pr = pu.oracle_view(scene, cam)
+        outs = []
+        for gg in (g, g2):
+            vs = fb.ViewState(scene.n, cfg.width, cfg.height, 0)
+            vs.rgb.fill_(float("nan"))
+            fb.project(ctx, gg, c, prm, vs)
+            torch.cuda.synchronize()
+            outs.append(vs.projected())
+            pu.check_projection(pr, outs[-1])
+        for k in outs[0]:
+            assert np.array_equal(outs[0][k].view(np.uint8), outs[1][k].view(np.uint8)), f"paths differ in {k} (view {view})"
+        assert 0 < int((outs[0]["tiles_touched"] > 0).sum()) < scene.n
+
+
 def test_large_tile_grid_fallback_sort():
     """2064x1616 px -> (GW+1)*(GH+1) = 130*102 > 12288: fhgs_bin_sort leaves the shared-memory tile-count
     path and derives histograms / ranges from the instance list; both schedules, integers bit-exact."""
