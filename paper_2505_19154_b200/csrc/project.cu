@@ -146,7 +146,8 @@ __global__ void __launch_bounds__(PROJ_THREADS, DIRECT ? 4 : 1) project_kernel(c
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         }
         __syncwarp();
-        // the frame test (a hint: it decides no result) is taken by the whole warp before any lane leaves
+        // the frame test (a hint: it decides no result -- a visible Gaussian it misses reads its row from global memory in
+        // step 10) is taken by the whole warp before any lane leaves
         bool want = false;
         if (i < a.n) {
             const float p0 = __ldg(a.mean + 3 * (size_t)i), p1 = __ldg(a.mean + 3 * (size_t)i + 1),
@@ -155,8 +156,11 @@ __global__ void __launch_bounds__(PROJ_THREADS, DIRECT ? 4 : 1) project_kernel(c
             const float tx = V[0] * p0 + V[1] * p1 + V[2] * p2 + V[3], ty = V[4] * p0 + V[5] * p1 + V[6] * p2 + V[7],
                         tz = V[8] * p0 + V[9] * p1 + V[10] * p2 + V[11];
             const float hx = a.fx * tx + (a.cx - 0.5f * (float)a.W) * tz, hy = a.fy * ty + (a.cy - 0.5f * (float)a.H) * tz;
-            // centre within 15 % of the image size of the frame: |px - W/2| <= 0.65 W, written without the division
-            want = tz >= a.z_near && fabsf(hx) <= 0.65f * (float)a.W * tz && fabsf(hy) <= 0.65f * (float)a.H * tz;
+            // |px - W/2| <= W/2 + margin, written without the division; margin ~ the 3-sigma radius of the largest axis
+            // (1.4 covers the clamped perspective stretch) plus the dilation and one tile of slack
+            const float smax = fmaxf(fmaxf(__ldg(a.scale + 3 * (size_t)i), __ldg(a.scale + 3 * (size_t)i + 1)), __ldg(a.scale + 3 * (size_t)i + 2));
+            const float mz = 4.2f * smax * fmaxf(fabsf(a.fx), fabsf(a.fy)) + 18.f * tz;   // margin * tz
+            want = tz >= a.z_near && fabsf(hx) <= 0.5f * (float)a.W * tz + mz && fabsf(hy) <= 0.5f * (float)a.H * tz + mz;
         }
         const uint32_t ballot = __ballot_sync(0xffffffffu, want);
         if (ballot) {
