@@ -48,7 +48,10 @@ typedef enum {
     FHGS_ERR_CAPACITY = 3  /* instance buffers too small (only reported by a synchronous bin_sort) */
 } fhgs_status;
 
-typedef enum { FHGS_F32 = 0, FHGS_F16 = 1 } fhgs_dtype;
+/* Storage types of feature rows, ground-truth maps and feature outputs; the arithmetic is fp32 throughout.  FHGS_BF16
+ * (SURVEY 8(f) NEXT-4 iv) is accepted by fhgs_render, fhgs_fuse_features and fhgs_frame_host; the NDFD entry points take
+ * FHGS_F32 / FHGS_F16 only. */
+typedef enum { FHGS_F32 = 0, FHGS_F16 = 1, FHGS_BF16 = 2 } fhgs_dtype;
 
 /* Opaque context: device ordinal, SM count, last-error text, two copy streams + events used only by fhgs_frame_host,
  * and one side stream + events on which fhgs_bin_sort runs two small scans beside its depth pre-sort (forked from and
@@ -69,14 +72,14 @@ FHGS_API const char* fhgs_version(void);
 typedef struct {
     int32_t n;          /* number of Gaussians, >= 0 */
     int32_t sh_degree;  /* 0..3; K = (sh_degree+1)^2 coefficients per colour channel */
-    int32_t feat_dim;   /* D > 0, multiple of 4 (f32) or 8 (f16); ignored when feat == NULL */
+    int32_t feat_dim;   /* D > 0, multiple of 4 (f32) or 8 (f16, bf16); ignored when feat == NULL */
     int32_t feat_dtype; /* fhgs_dtype of `feat` */
     const float* mean;    /* [n,3] */
     const float* scale;   /* [n,3] */
     const float* quat;    /* [n,4] */
     const float* opacity; /* [n]   */
     const float* sh;      /* [n,K,3] coefficient-major, RGB-minor */
-    const void* feat;     /* [n,D] f32 or f16, 16-byte aligned; NULL for RGB-only rendering */
+    const void* feat;     /* [n,D] f32, f16 or bf16, 16-byte aligned; NULL for RGB-only rendering */
 } fhgs_gaussians;
 
 typedef struct {

@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("FHGS_LIB") or os.path.join(_HERE, "libfhgs.so")   # FHGS_LIB: load another build of the same ABI
 
 FHGS_OK, FHGS_ERR_INTERNAL, FHGS_ERR_INVALID, FHGS_ERR_CAPACITY = 0, 1, 2, 3
-FHGS_F32, FHGS_F16 = 0, 1
+FHGS_F32, FHGS_F16, FHGS_BF16 = 0, 1, 2
 FHGS_SORT_FULL_KEY = 1
 FHGS_FUSE_ZERO, FHGS_FUSE_FINALIZE, FHGS_FUSE_L2NORM, FHGS_FUSE_FINALIZE_ONLY, FHGS_FUSE_ZERO_ONLY = 1, 2, 4, 8, 16
 FHGS_FUSE_ZERO_TOUCHED = 32
@@ -165,6 +165,8 @@ def _dtype_code(t: torch.Tensor) -> int:
         return FHGS_F32
     if t.dtype == torch.float16:
         return FHGS_F16
+    if t.dtype == torch.bfloat16:
+        return FHGS_BF16   # fhgs_render / fhgs_fuse_features / fhgs_frame_host only
     raise TypeError(f"unsupported feature dtype {t.dtype}")
 
 
@@ -327,7 +329,7 @@ def render(ctx: Context, g: Gaussians, cam: CCamera, prm: CParams, vs: ViewState
 
 def fuse_features(ctx: Context, cam, prm: CParams, vs: ViewState, gt, num, den, out_feat=None, flags: int = 0,
                   stream=None):
-    """fhgs_fuse_features (step F).  gt [H,W,D] f32/f16; num [n,D] f32; den [n] f32."""
+    """fhgs_fuse_features (step F).  gt [H,W,D] f32/f16/bf16; num [n,D] f32; den [n] f32."""
     d = int(num.shape[1])
     gt_code = FHGS_F32 if gt is None else _dtype_code(gt)
     out_code = FHGS_F32 if out_feat is None else _dtype_code(out_feat)

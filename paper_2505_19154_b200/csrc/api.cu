@@ -151,15 +151,16 @@ extern "C" fhgs_status fhgs_frame_host(fhgs_ctx* ctx, const fhgs_host_frame* hos
     if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
     if (g->n != vs->n) FHGS_INVALID(ctx, "fhgs_frame_host: g->n != vs->n");
     if (!g->mean || !g->scale || !g->quat || !g->opacity || !g->sh) FHGS_INVALID(ctx, "fhgs_frame_host: NULL device Gaussian array");
-    if (g->feat_dtype != FHGS_F32 && g->feat_dtype != FHGS_F16) FHGS_INVALID(ctx, "fhgs_frame_host: unknown feat_dtype");
-    if (g->feat_dim % (g->feat_dtype == FHGS_F16 ? 8 : 4)) FHGS_INVALID(ctx, "fhgs_frame_host: feat_dim must be a multiple of 4 (f32) / 8 (f16)");
+    if (g->feat_dtype != FHGS_F32 && g->feat_dtype != FHGS_F16 && g->feat_dtype != FHGS_BF16)
+        FHGS_INVALID(ctx, "fhgs_frame_host: unknown feat_dtype");
+    if (g->feat_dim % (g->feat_dtype == FHGS_F32 ? 4 : 8)) FHGS_INVALID(ctx, "fhgs_frame_host: feat_dim must be a multiple of 4 (f32) / 8 (f16, bf16)");
     if (!aligned_to(g->feat, 16) || !aligned_to(ws->out_feat, 16) || !aligned_to(ws->gt, 16) || !aligned_to(ws->num, 16) ||
         !aligned_to(ws->den, 4) || !aligned_to(ws->fused_feat, 16))
         FHGS_INVALID(ctx, "fhgs_frame_host: feat / workspace buffers must be 16-byte aligned");
     DeviceGuard dg(ctx);
     cudaStream_t s = (cudaStream_t)stream;
     const size_t n = (size_t)g->n, K = (size_t)(g->sh_degree + 1) * (g->sh_degree + 1);
-    const size_t e = g->feat_dtype == FHGS_F16 ? 2 : 4, D = (size_t)g->feat_dim;
+    const size_t e = g->feat_dtype == FHGS_F32 ? 4 : 2, D = (size_t)g->feat_dim;
     const size_t px = (size_t)cam->width * cam->height;
     uint64_t m = 0;
     // Schedule (three streams, so that PCIe runs in both directions while the steps execute):

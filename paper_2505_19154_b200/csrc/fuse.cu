@@ -42,11 +42,10 @@ __device__ __forceinline__ float4 load_gt4(const GT* p);
 template <>
 __device__ __forceinline__ float4 load_gt4<float>(const float* p) { return __ldg(reinterpret_cast<const float4*>(p)); }
 template <>
-__device__ __forceinline__ float4 load_gt4<__half>(const __half* p) {
-    const uint2 r = __ldg(reinterpret_cast<const uint2*>(p));
-    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
-    const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
-    return make_float4(a.x, a.y, b.x, b.y);
+__device__ __forceinline__ float4 load_gt4<__half>(const __half* p) { return cvt16x4(__ldg(reinterpret_cast<const uint2*>(p)), p); }
+template <>
+__device__ __forceinline__ float4 load_gt4<__nv_bfloat16>(const __nv_bfloat16* p) {
+    return cvt16x4(__ldg(reinterpret_cast<const uint2*>(p)), p);
 }
 
 template <int DC, int PRIM>
@@ -227,14 +226,10 @@ struct FuseWsSmem {
     GT G_pad[FW_DC];                                      // target of the consumers' one-past-the-end prefetch
 };
 
-// 4 consecutive channels of the staged GT tile -> fp32 (exact for fp16 storage)
+// 4 consecutive channels of the staged GT tile -> fp32 (exact for fp16 / bf16 storage)
 __device__ __forceinline__ float4 ld_g4(const float* p) { return *reinterpret_cast<const float4*>(p); }
-__device__ __forceinline__ float4 ld_g4(const __half* p) {
-    const uint2 r = *reinterpret_cast<const uint2*>(p);
-    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
-    const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
-    return make_float4(a.x, a.y, b.x, b.y);
-}
+__device__ __forceinline__ float4 ld_g4(const __half* p) { return cvt16x4(*reinterpret_cast<const uint2*>(p), p); }
+__device__ __forceinline__ float4 ld_g4(const __nv_bfloat16* p) { return cvt16x4(*reinterpret_cast<const uint2*>(p), p); }
 
 __device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("{\n\t.reg .b64 st;\n\tmbarrier.arrive.expect_tx.shared::cta.b64 st, [%0], %1;\n\t}" ::"r"(smem_u32(bar)), "r"(bytes)
@@ -648,6 +643,11 @@ __global__ void __launch_bounds__(TR_THREADS) fuse_pixel_kernel(const FuseArgs a
 // ---------------------------------------------------------------------------------------------
 constexpr int ROWS_PER_WARP = 32, ROW_WARPS = 8;   // 256 rows per CTA
 
+// one float4 of a finalised row in the storage type of out_feat (16-bit types: round to nearest even)
+__device__ __forceinline__ void store_out4(float* out, size_t i4, float4 v) { reinterpret_cast<float4*>(out)[i4] = v; }
+__device__ __forceinline__ void store_out4(__half* out, size_t i4, float4 v) { reinterpret_cast<uint2*>(out)[i4] = pack16x4(v, out); }
+__device__ __forceinline__ void store_out4(__nv_bfloat16* out, size_t i4, float4 v) { reinterpret_cast<uint2*>(out)[i4] = pack16x4(v, out); }
+
 template <typename OT>
 __global__ void __launch_bounds__(256) finalize_kernel(int n, int D, const float* num, const float* den, float den_eps,
                                                        int l2norm, OT* out) {
@@ -678,15 +678,7 @@ __global__ void __launch_bounds__(256) finalize_kernel(int n, int D, const float
         for (int j = lane; j < n4; j += 32) {
             const float4 v = __ldg(src + j);
             const float x = v.x / d * scale, y = v.y / d * scale, z = v.z / d * scale, w = v.w / d * scale;
-            if (sizeof(OT) == 4) {
-                reinterpret_cast<float4*>(out)[(size_t)row * n4 + j] = make_float4(x, y, z, w);
-            } else {
-                const __half2 a = __floats2half2_rn(x, y), b = __floats2half2_rn(z, w);
-                uint2 rr;
-                rr.x = *reinterpret_cast<const uint32_t*>(&a);
-                rr.y = *reinterpret_cast<const uint32_t*>(&b);
-                reinterpret_cast<uint2*>(out)[(size_t)row * n4 + j] = rr;
-            }
+            store_out4(out, (size_t)row * n4 + j, make_float4(x, y, z, w));
         }
     }
 }
@@ -781,10 +773,10 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
     const bool finalize = (flags & (FHGS_FUSE_FINALIZE | FHGS_FUSE_FINALIZE_ONLY)) != 0;
     fhgs_status st;
     if ((st = validate_params(ctx, prm)) != FHGS_OK) return st;
-    if (gt_dtype != FHGS_F32 && gt_dtype != FHGS_F16) FHGS_INVALID(ctx, "fhgs_fuse_features: unknown gt_dtype");
-    if (out_dtype != FHGS_F32 && out_dtype != FHGS_F16) FHGS_INVALID(ctx, "fhgs_fuse_features: unknown out_dtype");
-    const int mult = (accumulate && gt_dtype == FHGS_F16) ? 8 : 4;
-    if (feat_dim <= 0 || feat_dim % mult) FHGS_INVALID(ctx, "fhgs_fuse_features: feat_dim must be a positive multiple of 4 (f32) / 8 (f16)");
+    if (gt_dtype != FHGS_F32 && gt_dtype != FHGS_F16 && gt_dtype != FHGS_BF16) FHGS_INVALID(ctx, "fhgs_fuse_features: unknown gt_dtype");
+    if (out_dtype != FHGS_F32 && out_dtype != FHGS_F16 && out_dtype != FHGS_BF16) FHGS_INVALID(ctx, "fhgs_fuse_features: unknown out_dtype");
+    const int mult = (accumulate && gt_dtype != FHGS_F32) ? 8 : 4;
+    if (feat_dim <= 0 || feat_dim % mult) FHGS_INVALID(ctx, "fhgs_fuse_features: feat_dim must be a positive multiple of 4 (f32) / 8 (f16, bf16)");
     if (!aligned_to(num, 16) || !aligned_to(den, 4)) FHGS_INVALID(ctx, "fhgs_fuse_features: num must be 16-byte aligned");
     if (vs->n < 0) FHGS_INVALID(ctx, "fhgs_fuse_features: vs->n < 0");
     if (accumulate) {
@@ -823,8 +815,9 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
         const ScratchLayout L = make_scratch_layout(vs->n, vs->capacity, cam->width, cam->height);
         uint32_t* queue = reinterpret_cast<uint32_t*>((char*)vs->scratch + L.ctrl);
         const uint32_t* order = reinterpret_cast<const uint32_t*>((char*)vs->scratch + L.tile_order);
-        cudaError_t e = gt_dtype == FHGS_F16 ? dispatch<__half>(a, grid, ctx->num_sms, queue, order, s)
-                                             : dispatch<float>(a, grid, ctx->num_sms, queue, order, s);
+        cudaError_t e = gt_dtype == FHGS_F16    ? dispatch<__half>(a, grid, ctx->num_sms, queue, order, s)
+                        : gt_dtype == FHGS_BF16 ? dispatch<__nv_bfloat16>(a, grid, ctx->num_sms, queue, order, s)
+                                                : dispatch<float>(a, grid, ctx->num_sms, queue, order, s);
         FHGS_CUDA(ctx, e);
     }
     if (finalize && n > 0) {
@@ -832,6 +825,8 @@ extern "C" fhgs_status fhgs_fuse_features(fhgs_ctx* ctx, const fhgs_camera* cam,
         const int l2 = (flags & FHGS_FUSE_L2NORM) ? 1 : 0;
         if (out_dtype == FHGS_F16)
             finalize_kernel<__half><<<grid, 256, 0, s>>>((int)n, feat_dim, num, den, prm->den_eps, l2, (__half*)out_feat);
+        else if (out_dtype == FHGS_BF16)
+            finalize_kernel<__nv_bfloat16><<<grid, 256, 0, s>>>((int)n, feat_dim, num, den, prm->den_eps, l2, (__nv_bfloat16*)out_feat);
         else
             finalize_kernel<float><<<grid, 256, 0, s>>>((int)n, feat_dim, num, den, prm->den_eps, l2, (float*)out_feat);
         FHGS_LAUNCH_CHECK(ctx);

@@ -42,25 +42,17 @@ template <> struct FeatIO<float> {
     // 4 consecutive channels as two packed pairs, straight from the 16-byte load (no repacking moves)
     static __device__ __forceinline__ ulonglong2 load_pairs(const float* p) { return *reinterpret_cast<const ulonglong2*>(p); }
 };
-template <> struct FeatIO<__half> {
-    static __device__ __forceinline__ float4 load4(const __half* p) {
-        const uint2 r = *reinterpret_cast<const uint2*>(p);
-        const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
-        const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
-        return make_float4(a.x, a.y, b.x, b.y);
-    }
-    static __device__ __forceinline__ void store4(__half* p, float4 v) {
-        const __half2 a = __floats2half2_rn(v.x, v.y), b = __floats2half2_rn(v.z, v.w);
-        uint2 r;
-        r.x = *reinterpret_cast<const uint32_t*>(&a);
-        r.y = *reinterpret_cast<const uint32_t*>(&b);
-        *reinterpret_cast<uint2*>(p) = r;
-    }
-    static __device__ __forceinline__ ulonglong2 load_pairs(const __half* p) {
+// 16-bit storage (fp16 or bf16): widened exactly on load, rounded to nearest even on store
+template <typename HT> struct FeatIO16 {
+    static __device__ __forceinline__ float4 load4(const HT* p) { return cvt16x4(*reinterpret_cast<const uint2*>(p), p); }
+    static __device__ __forceinline__ void store4(HT* p, float4 v) { *reinterpret_cast<uint2*>(p) = pack16x4(v, p); }
+    static __device__ __forceinline__ ulonglong2 load_pairs(const HT* p) {
         const float4 f = load4(p);
         return make_ulonglong2(pack2(f.x, f.y), pack2(f.z, f.w));
     }
 };
+template <> struct FeatIO<__half> : FeatIO16<__half> {};
+template <> struct FeatIO<__nv_bfloat16> : FeatIO16<__nv_bfloat16> {};
 
 // ---------------------------------------------------------------------------------------------
 // TILED variant (DC in {64,128}): warp-specialised persistent pipeline (ws.cuh)
@@ -477,9 +469,10 @@ extern "C" fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const
     const bool has_feat = out_feat != nullptr;
     if (has_feat) {
         if (!g->feat) FHGS_INVALID(ctx, "fhgs_render: out_feat given but g->feat is NULL");
-        if (g->feat_dtype != FHGS_F32 && g->feat_dtype != FHGS_F16) FHGS_INVALID(ctx, "fhgs_render: unknown feat_dtype");
-        const int mult = g->feat_dtype == FHGS_F16 ? 8 : 4;
-        if (g->feat_dim <= 0 || g->feat_dim % mult) FHGS_INVALID(ctx, "fhgs_render: feat_dim must be a positive multiple of 4 (f32) / 8 (f16)");
+        if (g->feat_dtype != FHGS_F32 && g->feat_dtype != FHGS_F16 && g->feat_dtype != FHGS_BF16)
+            FHGS_INVALID(ctx, "fhgs_render: unknown feat_dtype");
+        const int mult = g->feat_dtype == FHGS_F32 ? 4 : 8;
+        if (g->feat_dim <= 0 || g->feat_dim % mult) FHGS_INVALID(ctx, "fhgs_render: feat_dim must be a positive multiple of 4 (f32) / 8 (f16, bf16)");
         if (!aligned_to(g->feat, 16) || !aligned_to(out_feat, 16)) FHGS_INVALID(ctx, "fhgs_render: feat/out_feat must be 16-byte aligned");
         if (g->n != vs->n) FHGS_INVALID(ctx, "fhgs_render: g->n != vs->n");
     }
@@ -502,8 +495,9 @@ extern "C" fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const
     // tile_visited is requested with fhgs_set_diagnostics; otherwise no kernel writes into the caller's scratch
     const bool diag = ctx->diagnostics != 0;
     a.tile_visited = diag ? reinterpret_cast<uint32_t*>((char*)vs->scratch + L.tile_visited) : nullptr;
-    cudaError_t e = (has_feat && g->feat_dtype == FHGS_F16) ? dispatch<__half>(a, grid, ctx->num_sms, queue, order, s, has_feat)
-                                                            : dispatch<float>(a, grid, ctx->num_sms, queue, order, s, has_feat);
+    cudaError_t e = (has_feat && g->feat_dtype == FHGS_F16)    ? dispatch<__half>(a, grid, ctx->num_sms, queue, order, s, has_feat)
+                    : (has_feat && g->feat_dtype == FHGS_BF16) ? dispatch<__nv_bfloat16>(a, grid, ctx->num_sms, queue, order, s, has_feat)
+                                                               : dispatch<float>(a, grid, ctx->num_sms, queue, order, s, has_feat);
     FHGS_CUDA(ctx, e);
     return FHGS_OK;
 }

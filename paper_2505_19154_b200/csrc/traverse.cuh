@@ -16,6 +16,7 @@
 // Stage B (per pixel): eval_weight() -- the normative q (bit-identical to the oracle's fmaf
 // expression), cut-off, alpha, w = alpha*T, T update, stop flag.
 #pragma once
+#include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
 #include "common.cuh"
@@ -23,6 +24,26 @@
 constexpr int TR_THREADS = 256;
 constexpr int TR_QCAP = 512;           // ring capacity (power of two) >= KB + 256
 constexpr uint32_t TR_FULL = 0xffffffffu;
+
+// Four consecutive 16-bit stored values (one 8-byte load) <-> fp32.  Both directions are exact / round-to-nearest-even:
+// fp16 and bf16 widen exactly; bf16 is the upper half of the binary32 pattern.
+__device__ __forceinline__ float4 cvt16x4(uint2 r, const __half*) {
+    const float2 a = __half22float2(*reinterpret_cast<const __half2*>(&r.x));
+    const float2 b = __half22float2(*reinterpret_cast<const __half2*>(&r.y));
+    return make_float4(a.x, a.y, b.x, b.y);
+}
+__device__ __forceinline__ float4 cvt16x4(uint2 r, const __nv_bfloat16*) {
+    return make_float4(__uint_as_float(r.x << 16), __uint_as_float(r.x & 0xffff0000u), __uint_as_float(r.y << 16),
+                       __uint_as_float(r.y & 0xffff0000u));
+}
+__device__ __forceinline__ uint2 pack16x4(float4 v, const __half*) {
+    const __half2 a = __floats2half2_rn(v.x, v.y), b = __floats2half2_rn(v.z, v.w);
+    return make_uint2(*reinterpret_cast<const uint32_t*>(&a), *reinterpret_cast<const uint32_t*>(&b));
+}
+__device__ __forceinline__ uint2 pack16x4(float4 v, const __nv_bfloat16*) {
+    const __nv_bfloat162 a = __floats2bfloat162_rn(v.x, v.y), b = __floats2bfloat162_rn(v.z, v.w);
+    return make_uint2(*reinterpret_cast<const uint32_t*>(&a), *reinterpret_cast<const uint32_t*>(&b));
+}
 
 struct TraverseArgs {
     int W, H, GW;

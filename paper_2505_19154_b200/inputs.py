@@ -38,7 +38,7 @@ class Scene:
     quat: np.ndarray      # [N,4] f32 (w,x,y,z)
     opacity: np.ndarray   # [N]   f32 in [0,1]
     sh: np.ndarray        # [N,K,3] f32, K=(deg+1)^2
-    feat: np.ndarray      # [N,D] f32 or f16
+    feat: np.ndarray      # [N,D] f32 or f16 ("bf16": f32 values that are exactly representable in bfloat16)
     sh_degree: int
 
     @property
@@ -56,7 +56,7 @@ class Config:
     seed: int
     n: int
     feat_dim: int
-    feat_dtype: str          # "f32" | "f16"
+    feat_dtype: str          # "f32" | "f16" | "bf16" (numpy has no bfloat16: values are rounded, the array stays f32)
     sh_degree: int
     width: int
     height: int
@@ -75,6 +75,13 @@ CONFIGS = {
     "large": Config("large", 1004, 3_000_000, 512, "f16", 3, 1920, 1080, 1, 2.0, -4.0, 0.7, True, "unit"),
     "multiview": Config("multiview", 1005, 2_000_000, 256, "f32", 0, 1296, 968, 200, 5.0, -4.0, 0.7, True, "blobs"),
 }
+
+
+def round_to_bf16(a: np.ndarray) -> np.ndarray:
+    """fp32 -> nearest bfloat16 (ties to even), returned as fp32: what a bf16 store of `a` holds.  Finite inputs."""
+    u = np.ascontiguousarray(a, dtype=np.float32).view(np.uint32)
+    r = ((u >> np.uint32(16)) & np.uint32(1)) + np.uint32(0x7FFF)
+    return ((u + r) & np.uint32(0xFFFF0000)).view(np.float32)
 
 
 def scaled(cfg: Config, **kw) -> Config:
@@ -197,6 +204,8 @@ def make_scene(cfg: Config) -> Scene:
         feat = _unit_rows(feat)
     if cfg.feat_dtype == "f16":
         feat = feat.astype(np.float16)
+    elif cfg.feat_dtype == "bf16":
+        feat = round_to_bf16(feat)
     return Scene(mean, scale, quat, opacity, sh, feat, cfg.sh_degree)
 
 
@@ -239,6 +248,8 @@ def make_gt_map(cfg: Config, view_idx: int, cam: Camera | None = None) -> np.nda
         raise ValueError(cfg.gt_kind)
     if cfg.feat_dtype == "f16":
         g = g.astype(np.float16)
+    elif cfg.feat_dtype == "bf16":
+        g = round_to_bf16(g)
     return np.ascontiguousarray(g)
 
 

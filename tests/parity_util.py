@@ -10,6 +10,9 @@ from paper_2505_19154_b200 import inputs
 
 TOL_F32 = 1e-4      # north_star: max abs on fp32 RGB, features and fused vectors
 TOL_F16 = 2e-3      # north_star: where features are stored fp16
+# bf16 storage (NEXT-4 iv; north_star states no bar): one rounding to 8 significant bits of an output of magnitude <= 1
+# is <= 2^-9 = 1.95e-3, on top of the fp32 accumulation bound 1e-4 ("Tolerances")
+TOL_BF16 = 2.5e-3
 
 
 def cam35(cam):
@@ -25,12 +28,16 @@ def oracle_view(scene, cam, params=fo.DEFAULT_PARAMS):
 class GpuPath:
     """One scene on the device + a reusable view state."""
 
-    def __init__(self, scene, width, height, capacity, device=0, surfel=False):
+    def __init__(self, scene, width, height, capacity, device=0, surfel=False, storage=None):
+        """storage="bf16": feature rows, GT maps and feature outputs are stored as bfloat16 on the device (the numpy
+        arrays carry bf16-exact f32 values); results come back widened to f32."""
         import torch
         from paper_2505_19154_b200 import binding as fb
         self.torch, self.fb = torch, fb
         self.ctx = fb.Context(device)
-        self.g = fb.Gaussians(scene.mean, scene.scale, scene.quat, scene.opacity, scene.sh, scene.feat, scene.sh_degree)
+        self.bf16 = storage == "bf16"
+        feat = torch.from_numpy(np.ascontiguousarray(scene.feat)).to(torch.bfloat16) if self.bf16 else scene.feat
+        self.g = fb.Gaussians(scene.mean, scene.scale, scene.quat, scene.opacity, scene.sh, feat, scene.sh_degree)
         self.vs = fb.ViewState(scene.n, width, height, capacity, surfel=surfel)
         self.prm = fb.default_params(primitive=fb.FHGS_PRIM_SURFEL if surfel else fb.FHGS_PRIM_EWA)
         self.W, self.H = width, height
@@ -54,13 +61,15 @@ class GpuPath:
                    feat=t.empty((self.H, self.W, self.D), dtype=self.g.feat.dtype, device=dev) if with_feat else None)
         self.fb.render(self.ctx, self.g, c, self.prm, self.vs, out["rgb"], out["feat"], out["T"], out["n"])
         t.cuda.synchronize()
-        return {k: (None if v is None else v.cpu().numpy()) for k, v in out.items()}
+        return {k: (None if v is None else (v.float() if v.dtype == t.bfloat16 else v).cpu().numpy()) for k, v in out.items()}
 
     def fuse(self, c, gt, num=None, den=None, flags=None, out_dtype=None):
         t, fb = self.torch, self.fb
         dev = self.g.mean.device
         n = self.g.n
         gt_d = t.from_numpy(np.ascontiguousarray(gt)).to(dev)
+        if self.bf16:
+            gt_d = gt_d.to(t.bfloat16)   # exact: the map holds bf16-representable values
         if num is None:
             num = t.zeros((n, self.D), dtype=t.float32, device=dev)
             den = t.zeros((n,), dtype=t.float32, device=dev)
@@ -72,10 +81,12 @@ class GpuPath:
     def finalize(self, num, den, prev, l2norm=False):
         t, fb = self.torch, self.fb
         out = t.from_numpy(np.ascontiguousarray(prev)).to(num.device)
+        if self.bf16:
+            out = out.to(t.bfloat16)
         fl = fb.FHGS_FUSE_FINALIZE_ONLY | (fb.FHGS_FUSE_L2NORM if l2norm else 0)
         fb.fuse_features(self.ctx, None, self.prm, self.vs, None, num, den, out, fl)
         t.cuda.synchronize()
-        return out.cpu().numpy()
+        return (out.float() if self.bf16 else out).cpu().numpy()
 
 
 def check_projection(pr_o, pr_g):

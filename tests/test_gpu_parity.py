@@ -27,7 +27,7 @@ def run_case(cfg, views, tol, literal_pixels=None, sort_flags=(0, 1), capacity_s
     cap = int(max(Ms) * capacity_slack) + 16
     if fixed_capacity is not None:
         cap = fixed_capacity
-    gp = pu.GpuPath(scene, cfg.width, cfg.height, cap, surfel=bool(primitive))
+    gp = pu.GpuPath(scene, cfg.width, cfg.height, cap, surfel=bool(primitive), storage=cfg.feat_dtype)
     gp.prm.rect_mode = rect_mode
     feat32 = scene.feat.astype(np.float32)
     fabs = float(np.abs(feat32).max())
@@ -141,6 +141,29 @@ def test_fp16_storage_d256_multiview_shape():
     cfg = pu.reduced_config("multiview", n=40_000, width=216, height=168, n_views=200, log_scale_mu=-3.0, feat_dtype="f16")
     w = run_case(cfg, [0, 67, 133], pu.TOL_F16, sort_flags=(0,))
     print(w)
+
+
+def test_bf16_storage_d256_and_d64():
+    """NEXT-4 (iv): bfloat16 storage of feature rows, GT maps and feature outputs (fp32 arithmetic), on the warp-specialised
+    kernels (D = 256: two channel chunks, double-buffered 16-bit GT tile) and the tiled ones (D = 64)."""
+    cfg = pu.reduced_config("multiview", n=40_000, width=216, height=168, n_views=200, log_scale_mu=-3.0, feat_dtype="bf16")
+    w = run_case(cfg, views=[0, 100], tol=pu.TOL_BF16)
+    print("bf16 d256", w)
+    cfg = pu.reduced_config("mid", n=30_000, width=200, height=120, log_scale_mu=-3.0, feat_dim=64, feat_dtype="bf16")
+    w = run_case(cfg, views=[0], tol=pu.TOL_BF16)
+    print("bf16 d64", w)
+    # the NDFD entry points take f32 / f16 only and say so
+    import torch
+    from paper_2505_19154_b200 import binding as fb
+    scene = inputs.make_scene(cfg)
+    cam = inputs.make_camera(cfg, 0)
+    gp = pu.GpuPath(scene, cfg.width, cfg.height, 1 << 20, storage="bf16")
+    c, _ = gp.project_sort(cam)
+    gt = torch.zeros((cfg.height, cfg.width, cfg.feat_dim), dtype=torch.bfloat16, device="cuda")
+    lgt = torch.zeros((cfg.height, cfg.width), dtype=torch.float32, device="cuda")
+    with pytest.raises(fb.FhgsError) as e:
+        fb.ndfd_forward(gp.ctx, gp.g, c, gp.prm, gp.vs, gt, lgt, lgt.clone())
+    assert e.value.status == fb.FHGS_ERR_INVALID
 
 
 def test_odd_d_paths():
