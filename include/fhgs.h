@@ -14,6 +14,9 @@
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Every call
  *     only enqueues work on `stream` and returns, except fhgs_bin_sort with a non-NULL
  *     num_instances_host, fhgs_frame_host and fhgs_ffma_peak, which synchronise `stream`.
+ *     No entry point other than those three synchronises, allocates device memory or uses the legacy stream on its
+ *     own, so a sequence of calls on one stream can be captured into a CUDA graph (fhgs_bin_sort forks onto the
+ *     context's side stream and joins back with events inside the call, which capture follows).
  *   - Arrays are row-major.  Images are channel-last [H,W,C].  Tiles are 16x16 px
  *     (PAPER.md:302), tile_id = ty * GW + tx with GW = ceil(W/16), GH = ceil(H/16).
  *   - Camera: view[16] = world->camera, row-major, applied to column vectors; camera frame is
