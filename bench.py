@@ -165,7 +165,8 @@ def run_reference(args, rank: int):
             "warmup": args.warmup, "ms_per_step": 1e3 * wall / args.steps,
             "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "mid: N=1e6 SH3 D=128 f32, 1 view 1920x1080 + one 1920x1080x128 GT map",
+            "config": {"workload": (f"mid: N={scene.n} SH{scene.sh_degree} D={cfg.feat_dim} f32, 1 view {cfg.width}x{cfg.height} + one "
+                                    f"{cfg.width}x{cfg.height}x{cfg.feat_dim} GT map"),   # the same string as the cuda arm's
                        "sample": smp.desc},
             "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": smp.desc},
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
