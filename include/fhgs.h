@@ -304,6 +304,17 @@ FHGS_API fhgs_status fhgs_frame_host(fhgs_ctx* ctx, const fhgs_host_frame* host,
                             const fhgs_frame_workspace* ws, uint64_t* num_instances_host,
                             void* stream);
 
+/* Steps R and F in ONE traversal with one weight phase (SURVEY 8(f) NEXT-4 ii; the same w = alpha T serves
+ * the rendered sums and the fused sums): equivalent to fhgs_render(..., out_feat, ...) followed by
+ * fhgs_fuse_features(..., flags = 0) on the same view state -- images bit-identical, num / den equal up to the order of their
+ * floating-point atomics.  Available in the per-pixel regime only: feat_dim NOT a multiple of 64 (FHGS_ERR_INVALID otherwise;
+ * the tiled kernels cannot hold both working sets).  gt [H,W,D] has the storage type of g->feat; out_rgb,
+ * out_feat, gt, num [n,D] f32 and den [n] f32 are required and are NOT cleared (accumulation over views as in step F);
+ * out_T / out_ncontrib may be NULL. */
+FHGS_API fhgs_status fhgs_render_fuse(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam, const fhgs_params* prm,
+                             const fhgs_view_state* vs, float* out_rgb, void* out_feat, float* out_T, uint32_t* out_ncontrib,
+                             const void* gt, float* num, float* den, void* stream);
+
 /* Allocation-free variant of step S1's prefix sum (DuplicateWithKeys needs, per Gaussian, the
  * inclusive prefix sum of tiles_touched) for callers that cannot provide or allocate scratch memory
  * (CUDA graph capture, serving loops, harnesses that forbid cudaMalloc).  The decoupled look-back status words live in a

@@ -25,7 +25,7 @@ FHGS_NDFD_BLEND_ORDER, FHGS_NDFD_FAR_TO_NEAR = 0, 1
 
 EXPORTS = ["fhgs_create", "fhgs_destroy", "fhgs_last_error", "fhgs_version", "fhgs_default_params",
            "fhgs_scratch_bytes", "fhgs_scratch_tile_visited", "fhgs_set_diagnostics", "fhgs_project", "fhgs_bin_sort", "fhgs_render", "fhgs_fuse_features", "fhgs_ndfd_forward", "fhgs_ndfd_backward_work_bytes", "fhgs_ndfd_backward",
-           "fhgs_frame_host", "fhgs_ffma_peak", "fhgs_scan_offsets_static_max_n", "fhgs_scan_offsets_static"]
+           "fhgs_frame_host", "fhgs_ffma_peak", "fhgs_scan_offsets_static_max_n", "fhgs_scan_offsets_static", "fhgs_render_fuse"]
 
 
 class FhgsError(RuntimeError):
@@ -113,6 +113,8 @@ def _load():
     lib.fhgs_scan_offsets_static_max_n.restype = C.c_int32
     lib.fhgs_scan_offsets_static_max_n.argtypes = []
     lib.fhgs_scan_offsets_static.argtypes = [vp, vp, C.c_int32, vp, vp, vp]
+    lib.fhgs_render_fuse.argtypes = [vp, C.POINTER(CGaussians), C.POINTER(CCamera), C.POINTER(CParams), C.POINTER(CViewState),
+                                     vp, vp, vp, vp, vp, vp, vp, vp]
     return lib
 
 
@@ -325,6 +327,17 @@ def render(ctx: Context, g: Gaussians, cam: CCamera, prm: CParams, vs: ViewState
     """fhgs_render (step R).  Outputs are caller-allocated torch tensors."""
     ctx.check(lib.fhgs_render(ctx.handle, C.byref(g.c), C.byref(cam), C.byref(prm), C.byref(vs.c), _ptr(out_rgb),
                               _ptr(out_feat), _ptr(out_T), _ptr(out_ncontrib), _stream(stream)))
+
+
+def render_fuse(ctx: Context, g: Gaussians, cam: CCamera, prm: CParams, vs: ViewState, out_rgb, out_feat, gt, num, den,
+                out_T=None, out_ncontrib=None, stream=None):
+    """fhgs_render_fuse: steps R and F in one traversal (per-pixel regime: D not a multiple of 64).  gt has the dtype of
+    the feature rows; num / den are accumulated into, not cleared."""
+    if gt.dtype != g.feat.dtype:
+        raise TypeError("gt must have the storage type of the feature rows")
+    ctx.check(lib.fhgs_render_fuse(ctx.handle, C.byref(g.c), C.byref(cam), C.byref(prm), C.byref(vs.c), _ptr(out_rgb),
+                                   _ptr(out_feat), _ptr(out_T), _ptr(out_ncontrib), _ptr(gt), _ptr(num), _ptr(den),
+                                   _stream(stream)))
 
 
 def fuse_features(ctx: Context, cam, prm: CParams, vs: ViewState, gt, num, den, out_feat=None, flags: int = 0,

@@ -389,6 +389,158 @@ __global__ void __launch_bounds__(TR_THREADS) render_pixel_kernel(const RenderAr
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Single-traversal render + fuse (fhgs_render_fuse; SURVEY 8(f) NEXT-4 ii) for the per-pixel regime (D not a multiple of
+// 64): the pixel's thread evaluates every weight w = alpha T once and uses it twice -- for the pixel's own
+// colour / feature sums (step R) and, reduced over the warp's 32 pixels with shuffles, for num[id] += w gt(x), den[id] += w
+// (step F: one red per warp and Gaussian).  Same arithmetic and order as render_pixel_kernel and fuse.cu's pixel kernel.
+// ---------------------------------------------------------------------------------------------
+struct RenderFuseArgs {
+    RenderArgs r;
+    const void* gt;   // [H,W,D], same storage type as the feature rows
+    float* num;
+    float* den;
+};
+
+__device__ __forceinline__ void rf_red_add_v4(float* addr, float4 v) {
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+__device__ __forceinline__ void rf_red_add(float* addr, float v) {
+    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(v) : "memory");
+}
+
+template <int CH, typename FT, int PRIM>
+__global__ void __launch_bounds__(TR_THREADS) render_fuse_pixel_kernel(const RenderFuseArgs af) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    PixelSmem<CH, PRIM>& sm = *reinterpret_cast<PixelSmem<CH, PRIM>*>(smem_raw);
+    const RenderArgs& a = af.r;
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int tile = blockIdx.x;
+    const int tx0 = (tile % a.t.GW) * FHGS_TILE, ty0 = (tile / a.t.GW) * FHGS_TILE;
+    int sx, sy;
+    slot_to_xy(tid, sx, sy);
+    const int px = tx0 + sx, py = ty0 + sy;
+    const bool inside = px < a.t.W && py < a.t.H;
+    const float fx = (float)px, fy = (float)py;
+    const float bx0 = (float)tx0, by0 = (float)ty0;
+    const float bx1 = (float)min(tx0 + FHGS_TILE - 1, a.t.W - 1), by1 = (float)min(ty0 + FHGS_TILE - 1, a.t.H - 1);
+    const uint2 range = __ldg(reinterpret_cast<const uint2*>(a.t.ranges) + tile);
+    const FT* feat = reinterpret_cast<const FT*>(a.feat);
+    const FT* gt = reinterpret_cast<const FT*>(af.gt);
+    FT* out_feat = reinterpret_cast<FT*>(a.out_feat);
+
+    for (int c0 = 0; c0 < a.D; c0 += CH) {
+        float T = 1.f, C0 = 0.f, C1 = 0.f, C2 = 0.f;
+        uint32_t n = 0;
+        bool done = !inside;
+        float acc[CH], g[CH];
+#pragma unroll
+        for (int j = 0; j < CH; ++j) acc[j] = 0.f;
+#pragma unroll
+        for (int j = 0; j < CH / 4; ++j) {
+            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (inside) v = FeatIO<FT>::load4(gt + ((size_t)py * a.t.W + px) * a.D + c0 + 4 * j);
+            g[4 * j] = v.x; g[4 * j + 1] = v.y; g[4 * j + 2] = v.z; g[4 * j + 3] = v.w;
+        }
+        uint32_t pos = range.x;
+        int q_head = 0, q_count = 0;
+        while (true) {
+            while (q_count < R_KB && pos < range.y) {
+                const int tail = q_head + q_count;
+                const int added = stage_chunk(a.t, sm.q, pos, range.y, tail, bx0, by0, bx1, by1);
+                for (int k = tid; k < added; k += TR_THREADS) {
+                    const int s = (tail + k) & (TR_QCAP - 1);
+                    const uint32_t id = sm.q.id[s];
+                    sm.rgb[s] = make_float4(__ldg(a.rgb_g + 3 * (size_t)id), __ldg(a.rgb_g + 3 * (size_t)id + 1),
+                                            __ldg(a.rgb_g + 3 * (size_t)id + 2), 0.f);
+                }
+                for (int k = tid; k < added * (CH / 4); k += TR_THREADS) {
+                    const int r = k / (CH / 4), c = k % (CH / 4);
+                    const int s = (tail + r) & (TR_QCAP - 1);
+                    const uint32_t id = sm.q.id[s];
+                    *reinterpret_cast<float4*>(&sm.F[s * CH + 4 * c]) = FeatIO<FT>::load4(feat + (size_t)id * a.D + c0 + 4 * c);
+                }
+                q_count += added;
+                pos += TR_THREADS;
+            }
+            const int nb = q_count;   // drain everything staged
+            if (nb == 0) break;
+            __syncthreads();
+            for (int kk = 0; kk < nb; ++kk) {
+                const int s = (q_head + kk) & (TR_QCAP - 1);
+                const float w = eval_weight_q<PRIM>(sm.q, s, fx, fy, a.t, T, done, n);   // the one weight phase
+                if (w != 0.f) {   // step R: this pixel's sums
+                    const float4 c = sm.rgb[s];
+                    C0 = fmaf(w, c.x, C0); C1 = fmaf(w, c.y, C1); C2 = fmaf(w, c.z, C2);
+#pragma unroll
+                    for (int j = 0; j < CH / 4; ++j) {
+                        const float4 f = *reinterpret_cast<const float4*>(&sm.F[s * CH + 4 * j]);
+                        acc[4 * j] = fmaf(w, f.x, acc[4 * j]);
+                        acc[4 * j + 1] = fmaf(w, f.y, acc[4 * j + 1]);
+                        acc[4 * j + 2] = fmaf(w, f.z, acc[4 * j + 2]);
+                        acc[4 * j + 3] = fmaf(w, f.w, acc[4 * j + 3]);
+                    }
+                }
+                if (!__any_sync(TR_FULL, w != 0.f)) continue;   // step F: this Gaussian's sums over the warp's pixels
+                const uint32_t id = sm.q.id[s];
+                float v[CH + 1];
+#pragma unroll
+                for (int j = 0; j < CH; ++j) v[j] = w * g[j];
+                v[CH] = w;
+#pragma unroll
+                for (int d = 16; d >= 1; d >>= 1)
+#pragma unroll
+                    for (int j = 0; j < CH + 1; ++j) v[j] += __shfl_xor_sync(TR_FULL, v[j], d);
+                if (lane == 0) {
+                    float* dst = af.num + (size_t)id * a.D + c0;
+#pragma unroll
+                    for (int j = 0; j < CH / 4; ++j) rf_red_add_v4(dst + 4 * j, make_float4(v[4 * j], v[4 * j + 1], v[4 * j + 2], v[4 * j + 3]));
+                    if (c0 == 0) rf_red_add(af.den + id, v[CH]);
+                }
+            }
+            q_head = (q_head + nb) & (TR_QCAP - 1);
+            q_count = 0;
+            if (__syncthreads_and(done)) break;
+        }
+        if (inside) {
+            const size_t p = (size_t)py * a.t.W + px;
+            if (c0 == 0) {
+                a.out_rgb[3 * p] = fmaf(T, a.bg[0], C0);
+                a.out_rgb[3 * p + 1] = fmaf(T, a.bg[1], C1);
+                a.out_rgb[3 * p + 2] = fmaf(T, a.bg[2], C2);
+                if (a.out_T) a.out_T[p] = T;
+                if (a.out_n) a.out_n[p] = n;
+            }
+#pragma unroll
+            for (int j = 0; j < CH / 4; ++j)
+                FeatIO<FT>::store4(out_feat + p * a.D + c0 + 4 * j, make_float4(acc[4 * j], acc[4 * j + 1], acc[4 * j + 2], acc[4 * j + 3]));
+        }
+        __syncthreads();
+    }
+}
+
+template <int CH, typename FT, int PRIM>
+cudaError_t launch_render_fuse(const RenderFuseArgs& af, int grid, cudaStream_t st) {
+    const size_t smem = sizeof(PixelSmem<CH, PRIM>);
+    cudaError_t e = cudaFuncSetAttribute(render_fuse_pixel_kernel<CH, FT, PRIM>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    render_fuse_pixel_kernel<CH, FT, PRIM><<<grid, TR_THREADS, smem, st>>>(af);
+    return cudaGetLastError();
+}
+
+template <typename FT>
+cudaError_t dispatch_render_fuse(const RenderFuseArgs& af, int grid, cudaStream_t st) {
+    const int D = af.r.D;
+    if (af.r.t.ray_transform) {
+        if (D % 16 == 0) return launch_render_fuse<16, FT, 1>(af, grid, st);
+        if (D % 8 == 0) return launch_render_fuse<8, FT, 1>(af, grid, st);
+        return launch_render_fuse<4, FT, 1>(af, grid, st);
+    }
+    if (D % 16 == 0) return launch_render_fuse<16, FT, 0>(af, grid, st);
+    if (D % 8 == 0) return launch_render_fuse<8, FT, 0>(af, grid, st);
+    return launch_render_fuse<4, FT, 0>(af, grid, st);
+}
+
 template <typename K>
 cudaError_t launch(K kernel, size_t smem, int grid, cudaStream_t st, const RenderArgs& a) {
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -498,6 +650,48 @@ extern "C" fhgs_status fhgs_render(fhgs_ctx* ctx, const fhgs_gaussians* g, const
     cudaError_t e = (has_feat && g->feat_dtype == FHGS_F16)    ? dispatch<__half>(a, grid, ctx->num_sms, queue, order, s, has_feat)
                     : (has_feat && g->feat_dtype == FHGS_BF16) ? dispatch<__nv_bfloat16>(a, grid, ctx->num_sms, queue, order, s, has_feat)
                                                                : dispatch<float>(a, grid, ctx->num_sms, queue, order, s, has_feat);
+    FHGS_CUDA(ctx, e);
+    return FHGS_OK;
+}
+
+extern "C" fhgs_status fhgs_render_fuse(fhgs_ctx* ctx, const fhgs_gaussians* g, const fhgs_camera* cam, const fhgs_params* prm,
+                                        const fhgs_view_state* vs, float* out_rgb, void* out_feat, float* out_T,
+                                        uint32_t* out_ncontrib, const void* gt, float* num, float* den, void* stream) {
+    if (!ctx) return FHGS_ERR_INVALID;
+    if (!g || !cam || !prm || !vs) FHGS_INVALID(ctx, "fhgs_render_fuse: NULL argument");
+    fhgs_status st;
+    if ((st = validate_camera(ctx, cam)) != FHGS_OK) return st;
+    if ((st = validate_params(ctx, prm)) != FHGS_OK) return st;
+    if ((st = validate_view_state(ctx, vs, cam)) != FHGS_OK) return st;
+    if ((st = validate_primitive(ctx, prm, vs)) != FHGS_OK) return st;
+    if (!out_rgb || !out_feat || !gt || !num || !den || !g->feat) FHGS_INVALID(ctx, "fhgs_render_fuse: out_rgb, out_feat, gt, num, den and g->feat are required");
+    if (g->feat_dtype != FHGS_F32 && g->feat_dtype != FHGS_F16 && g->feat_dtype != FHGS_BF16) FHGS_INVALID(ctx, "fhgs_render_fuse: unknown feat_dtype");
+    const int mult = g->feat_dtype == FHGS_F32 ? 4 : 8;
+    if (g->feat_dim <= 0 || g->feat_dim % mult) FHGS_INVALID(ctx, "fhgs_render_fuse: feat_dim must be a positive multiple of 4 (f32) / 8 (f16, bf16)");
+    if (g->feat_dim % 64 == 0)
+        FHGS_INVALID(ctx, "fhgs_render_fuse: feat_dim is a multiple of 64 -- the tiled kernels have no shared-memory room for a "
+                          "shared weight phase (DESIGN.md 9e ii); call fhgs_render and fhgs_fuse_features");
+    if (!aligned_to(g->feat, 16) || !aligned_to(out_feat, 16) || !aligned_to(gt, 16) || !aligned_to(num, 16) || !aligned_to(den, 4))
+        FHGS_INVALID(ctx, "fhgs_render_fuse: feat / out_feat / gt / num must be 16-byte aligned");
+    if (g->n != vs->n) FHGS_INVALID(ctx, "fhgs_render_fuse: g->n != vs->n");
+    RenderFuseArgs af;
+    RenderArgs& a = af.r;
+    a.t.W = cam->width; a.t.H = cam->height; a.t.GW = tiles_x(cam->width);
+    a.t.ranges = vs->ranges; a.t.vals = vs->vals[vs->sorted_buf & 1];
+    a.t.xy = reinterpret_cast<const float2*>(vs->xy);
+    a.t.conic_opacity = reinterpret_cast<const float4*>(vs->conic_opacity);
+    a.t.q_cutoff = prm->q_cutoff; a.t.alpha_max = prm->alpha_max; a.t.t_min = prm->t_min;
+    a.t.ray_transform = prm->primitive == FHGS_PRIM_SURFEL ? reinterpret_cast<const float4*>(vs->ray_transform) : nullptr;
+    a.rgb_g = vs->rgb; a.feat = g->feat; a.D = g->feat_dim;
+    a.bg[0] = prm->bg[0]; a.bg[1] = prm->bg[1]; a.bg[2] = prm->bg[2];
+    a.out_rgb = out_rgb; a.out_feat = out_feat; a.out_T = out_T; a.out_n = out_ncontrib; a.tile_visited = nullptr;
+    af.gt = gt; af.num = num; af.den = den;
+    const int grid = tiles_x(cam->width) * tiles_y(cam->height);
+    DeviceGuard dg(ctx);
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e = g->feat_dtype == FHGS_F16    ? dispatch_render_fuse<__half>(af, grid, s)
+                    : g->feat_dtype == FHGS_BF16 ? dispatch_render_fuse<__nv_bfloat16>(af, grid, s)
+                                                 : dispatch_render_fuse<float>(af, grid, s);
     FHGS_CUDA(ctx, e);
     return FHGS_OK;
 }

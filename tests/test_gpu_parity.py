@@ -284,6 +284,60 @@ def test_project_sh_row_paths_agree():
         assert 0 < int((outs[0]["tiles_touched"] > 0).sum()) < scene.n
 
 
+@pytest.mark.parametrize("case", ["tiny", "small", "d48_f16", "surfel_d24"])
+def test_render_fuse_single_traversal(case):
+    """NEXT-4 (ii): fhgs_render_fuse (one traversal, one weight phase) against fhgs_render followed by fhgs_fuse_features on
+    the same view state: images and contributor counts bit for bit, accumulators (two views accumulated) up to the order
+    of their floating-point atomics; the separate calls are the ones the oracle checks element by element above."""
+    import torch
+    from paper_2505_19154_b200 import binding as fb
+    surfel = case == "surfel_d24"
+    if case == "tiny":
+        cfg = inputs.CONFIGS["tiny"]
+    elif case == "small":
+        cfg = inputs.CONFIGS["small"]
+    elif case == "d48_f16":
+        cfg = pu.reduced_config("small", n=30_000, width=200, height=120, feat_dim=48, feat_dtype="f16")
+    else:
+        cfg = pu.reduced_config("small", n=20_000, width=136, height=88, feat_dim=24)
+    scene = inputs.make_scene(cfg)
+    W, H, D, n = cfg.width, cfg.height, cfg.feat_dim, scene.n
+    gp = pu.GpuPath(scene, W, H, 64 * n + 4096, surfel=surfel)
+    dev = gp.g.mean.device
+    fdt = gp.g.feat.dtype
+    mk = lambda: dict(rgb=torch.full((H, W, 3), float("nan"), device=dev), feat=torch.zeros((H, W, D), dtype=fdt, device=dev),
+                      T=torch.full((H, W), float("nan"), device=dev), n=torch.full((H, W), -1, dtype=torch.int32, device=dev))
+    num_a, den_a = torch.zeros((n, D), device=dev), torch.zeros((n,), device=dev)
+    num_b, den_b = torch.zeros((n, D), device=dev), torch.zeros((n,), device=dev)
+    gmax = 0.0
+    for view in (0, 1):
+        cam = inputs.make_camera(cfg, view)
+        c, m = gp.project_sort(cam)
+        assert m > 0
+        gt = torch.from_numpy(np.ascontiguousarray(inputs.make_gt_map(cfg, view, cam))).to(dev)
+        gmax = max(gmax, float(gt.float().abs().max()))
+        a, b = mk(), mk()
+        fb.render(gp.ctx, gp.g, c, gp.prm, gp.vs, a["rgb"], a["feat"], a["T"], a["n"])
+        fb.fuse_features(gp.ctx, c, gp.prm, gp.vs, gt, num_a, den_a, None, 0)
+        fb.render_fuse(gp.ctx, gp.g, c, gp.prm, gp.vs, b["rgb"], b["feat"], gt, num_b, den_b, out_T=b["T"], out_ncontrib=b["n"])
+        torch.cuda.synchronize()
+        for k in a:
+            assert torch.equal(a[k], b[k]), f"{k} differs (view {view})"
+    assert bool((den_a > 0).any())
+    assert bool(((den_a - den_b).abs() <= pu.TOL_F32 * den_a.abs() + 1e-12).all())
+    assert bool(((num_a - num_b).abs().amax(dim=1) <= pu.TOL_F32 * den_a.abs() * gmax + 1e-12).all())
+    # the tiled regime is refused with a message that says why
+    if case == "tiny":
+        cfg64 = pu.reduced_config("tiny", feat_dim=64)
+        sc64 = inputs.make_scene(cfg64)
+        gp64 = pu.GpuPath(sc64, cfg64.width, cfg64.height, 1 << 16)
+        c64, _ = gp64.project_sort(inputs.make_camera(cfg64, 0))
+        z = lambda *s: torch.zeros(s, device=dev)
+        with pytest.raises(fb.FhgsError) as e:
+            fb.render_fuse(gp64.ctx, gp64.g, c64, gp64.prm, gp64.vs, z(64, 64, 3), z(64, 64, 64), z(64, 64, 64), z(sc64.n, 64), z(sc64.n))
+        assert e.value.status == fb.FHGS_ERR_INVALID and "multiple of 64" in str(e.value)
+
+
 def test_large_tile_grid_fallback_sort():
     """2064x1616 px -> (GW+1)*(GH+1) = 130*102 > 12288: fhgs_bin_sort leaves the shared-memory tile-count
     path and derives histograms / ranges from the instance list; both schedules, integers bit-exact."""
