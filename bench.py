@@ -605,6 +605,27 @@ def run_cuda_workload(args, local_rank: int):
         fb.bin_sort(ctx, cam, vs, sync=False)
         fb.render(ctx, g, cam, prm, vs, out_rgb, None, None, out_n)
         n_contrib += int(out_n.to(torch.int64).sum().item())
+    # NEXT-4 (ii), per-pixel regime only (D not a multiple of 64): steps R + F as two calls against fhgs_render_fuse
+    single = None
+    if not multiview and D % 64 != 0 and len(cams) == 1:
+        def r_then_f():
+            fb.render(ctx, g, cams[0], prm, vs, out_rgb, out_feat, None, out_n)
+            fb.fuse_features(ctx, cams[0], prm, vs, gt, num, den, None, 0)
+
+        def r_and_f():
+            fb.render_fuse(ctx, g, cams[0], prm, vs, out_rgb, out_feat, gt, num, den, out_ncontrib=out_n)
+        ms2 = []
+        for fn in (r_then_f, r_and_f):
+            for _ in range(5):
+                fn()
+            ea, eb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            ea.record(stream)
+            for _ in range(50):
+                fn()
+            eb.record(stream)
+            torch.cuda.synchronize()
+            ms2.append(ea.elapsed_time(eb) / 50)
+        single = {"render_then_fuse_ms": ms2[0], "render_fuse_ms": ms2[1], "note": "accumulate only (no clear / finalise)"}
     alu_nominal = 148 * FP32_LANES_PER_SM * peaks["sm_max_mhz"] * 1e6
     roof = {}
     if not multiview:
@@ -623,7 +644,8 @@ def run_cuda_workload(args, local_rank: int):
                        "views": views, "instances_M": Ms, "contributors_per_px": n_contrib / (W * H * len(cams)),
                        "gt": "one seeded unit-norm map reused for every view (values do not affect timing)" if multiview
                              else "inputs.make_gt_map"},
-            "ms": acc, "ms_per_view": total_ms / args.steps / len(cams), "roofline_steps": roof, "cpu_baseline": None,
+            "ms": acc, "ms_per_view": total_ms / args.steps / len(cams), "roofline_steps": roof,
+            "single_traversal": single, "cpu_baseline": None,
             "e2e": None, "gpu_launches": None, "clocks": clocks}
     print(json.dumps(line), flush=True)
 
