@@ -777,6 +777,61 @@ def run_multiview_sweep(args, rank: int, world: int, local_rank: int):
         dist.destroy_process_group()
 
 
+# --------------------------------------------------------------------------------------------------
+# NEXT-4 (v): LABELLED comparison, outside north_star's "no tensor cores" contract and outside the product path
+# --------------------------------------------------------------------------------------------------
+def run_tc_compare(args, local_rank: int):
+    """`--tc-compare`: what the per-tile products of steps R / F would cost on the tensor cores with 3xTF32 splitting
+    (SURVEY 8(f) NEXT-4 v).  Library GEMMs only (cuBLAS batched matmul through torch), on synthetic operands of the Mid
+    frame's shape: one batch entry per tile, W^T [128 instances x 256 pixels] times G [256 pixels x 128 channels] (a
+    tile's 106 tile-culled survivors on average, padded to 128).  3xTF32: x = hi + lo with hi = x truncated to 10
+    mantissa bits; W^T G ~ hi hi + lo hi + hi lo, three TF32 GEMMs with fp32 accumulation.  Reported next to the FP32
+    (CUDA-core SGEMM) form of the same batched product and to the error of each against float64.  Nothing of this is
+    called by the library; libfhgs.so contains no tensor-core instruction (profiles/r02_sass_census.md)."""
+    import torch
+    dev = torch.device("cuda", local_rank)
+    torch.manual_seed(1234)
+    tiles, n_inst, px, ch = 8160, 128, 256, 128
+    # weights: non-negative, most of them zero (a pixel blends ~70 of the tile's instances), rows sum to < 1 per pixel
+    Wt = torch.rand((tiles, n_inst, px), device=dev) * (torch.rand((tiles, n_inst, px), device=dev) < 0.55) * 0.02
+    G = torch.randn((tiles, px, ch), device=dev) / ch ** 0.5
+
+    def split(x):
+        hi = (x.view(torch.int32) & -8192).view(torch.float32)   # clear the 13 low mantissa bits: exactly a TF32 value
+        return hi, x - hi
+
+    def timed(fn, reps=5):
+        for _ in range(2):
+            fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(reps):
+            out = fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps, out
+
+    torch.backends.cuda.matmul.allow_tf32 = False
+    ms_fp32, c_fp32 = timed(lambda: torch.bmm(Wt, G))
+    torch.backends.cuda.matmul.allow_tf32 = True
+    ms_tf32, c_tf32 = timed(lambda: torch.bmm(Wt, G))
+    ms_split, parts = timed(lambda: (split(Wt), split(G)))
+    (w_hi, w_lo), (g_hi, g_lo) = parts
+    ms_3x, c_3x = timed(lambda: torch.bmm(w_hi, g_hi) + torch.bmm(w_lo, g_hi) + torch.bmm(w_hi, g_lo))
+    torch.backends.cuda.matmul.allow_tf32 = False
+    ref = torch.bmm(Wt[:64].double(), G[:64].double())
+    err = lambda c: float((c[:64].double() - ref).abs().max())
+    flop = 2.0 * tiles * n_inst * px * ch
+    line = {"experiment": "NEXT-4 (v) tensor-core comparison -- LABELLED, outside north_star's contract, library GEMMs, not a bench line",
+            "shape": {"tiles": tiles, "instances": n_inst, "pixels": px, "channels": ch, "flop_per_product": flop},
+            "fp32_sgemm": {"ms": ms_fp32, "tflops": flop / ms_fp32 / 1e9, "max_abs_err_vs_f64": err(c_fp32)},
+            "tf32_single": {"ms": ms_tf32, "tflops": flop / ms_tf32 / 1e9, "max_abs_err_vs_f64": err(c_tf32)},
+            "tf32_3x": {"ms_gemms_and_adds": ms_3x, "ms_split": ms_split, "tflops_fp32_equivalent": flop / ms_3x / 1e9,
+                        "max_abs_err_vs_f64": err(c_3x)},
+            "library_kernel_for_scale": "fuse_ws_kernel<float>: 1.57 ms for the Mid frame's W^T G including traversal, weights and atomics"}
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -791,6 +846,8 @@ def main():
     ap.add_argument("--rect", default="radius", choices=["radius", "tight"],
                     help="tile rectangle rule: north_star's scalar 3-sigma radius (default, the bench line) or the tight per-axis extents (NEXT-4 i)")
     ap.add_argument("--ndfd", action="store_true", help="mid: also time fhgs_ndfd_forward (NEXT-1 row) on the frame")
+    ap.add_argument("--tc-compare", action="store_true",
+                    help="NEXT-4 (v): labelled 3xTF32 tensor-core comparison of the per-tile products (library GEMMs; not a bench line)")
     ap.add_argument("--views", type=int, default=8, help="multiview: number of evenly spaced orbit cameras per sweep")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
@@ -798,6 +855,10 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.tc_compare:
+        if rank == 0:
+            run_tc_compare(args, local_rank)
         return
     if args.workload == "multiview" and (args.views > 8 or world > 1):
         run_multiview_sweep(args, rank, world, local_rank)      # the config as BASELINE.json states it (and its sharded form)
