@@ -139,6 +139,18 @@ def run_guarded(cfg, view, tol, sort_flags=(1, 0), ndfd=False, surfel=False):
         else:
             for k in ("rgb", "feat", "T", "n"):
                 assert np.array_equal(first[k], g[k]), f"{k} not reproducible (repetition {rep})"
+        if D % 64 != 0:
+            # the single-traversal call (per-pixel regime) on poisoned outputs and cleared accumulators: against the oracle
+            # directly, and bit for bit against the two separate calls
+            for k in ("rgb", "feat", "T", "n"):
+                outs[k].poison()
+            outs["num"].zero(); outs["den"].zero()
+            fb.render_fuse(gp.ctx, gp.g, c, gp.prm, vs, t_rgb, t_feat, gt_d, t_num, t_den, out_T=t_T, out_ncontrib=t_n)
+            torch.cuda.synchronize()
+            g2 = dict(rgb=t_rgb.cpu().numpy(), feat=t_feat.cpu().numpy(), T=t_T.cpu().numpy(), n=t_n.cpu().numpy())
+            for k in g2:
+                assert np.array_equal(g[k], g2[k]), f"fhgs_render_fuse: {k} differs from fhgs_render"
+            pu.check_fuse(num_o, den_o, t_num, t_den, float(np.abs(gt.astype(np.float32)).max()), tol, touch)
         if ndfd:
             t_lgt, t_lcf = outs["lgt"].view(torch.float32, (H, W)), outs["lcf"].view(torch.float32, (H, W))
             outs["lgt"].poison(); outs["lcf"].poison(); outs["gop"].zero()
