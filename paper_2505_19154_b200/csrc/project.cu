@@ -115,7 +115,7 @@ __device__ __forceinline__ void sh_colour(const ProjectArgs& a, const float* row
     }
 }
 
-// DIRECT (rows of a multiple of 16 bytes, i.e. SH degree 1 and 3, and a 16-byte aligned sh array): no cooperative
+// DIRECT (launched for SH degree 3 with a 16-byte aligned sh array; the rows must be a multiple of 16 bytes): no cooperative
 // staging and no CTA-wide barrier.  A thread whose Gaussian passes the z cull and a generous frame test starts ONE bulk
 // async copy (cp.async.bulk) of its own row into its own shared-memory slot (stride 208 bytes: conflict-free for the
 // 16-byte reads), counted on its warp's mbarrier; the warp does the covariance arithmetic while the rows fly and waits
@@ -157,7 +157,7 @@ __global__ void __launch_bounds__(PROJ_THREADS, DIRECT ? 4 : 1) project_kernel(c
                         tz = V[8] * p0 + V[9] * p1 + V[10] * p2 + V[11];
             const float hx = a.fx * tx + (a.cx - 0.5f * (float)a.W) * tz, hy = a.fy * ty + (a.cy - 0.5f * (float)a.H) * tz;
             // |px - W/2| <= W/2 + margin, written without the division; margin ~ the 3-sigma radius of the largest axis
-            // (1.4 covers the clamped perspective stretch) plus the dilation and one tile of slack
+            // (4.2 = 3 sigma x 1.4, the factor covering the clamped perspective stretch) plus the dilation and one tile of slack
             const float smax = fmaxf(fmaxf(__ldg(a.scale + 3 * (size_t)i), __ldg(a.scale + 3 * (size_t)i + 1)), __ldg(a.scale + 3 * (size_t)i + 2));
             const float mz = 4.2f * smax * fmaxf(fabsf(a.fx), fabsf(a.fy)) + 18.f * tz;   // margin * tz
             want = tz >= a.z_near && fabsf(hx) <= 0.5f * (float)a.W * tz + mz && fabsf(hy) <= 0.5f * (float)a.H * tz + mz;
